@@ -1,0 +1,136 @@
+/*
+ * scarf.h — C ABI of libscarf: analytic 3-D molecular scattering form factors on one B200 (sm_100a).
+ *
+ *     f_s(q) = g * sum_{mu nu} T^s_{mu nu} * Int d^3r  phi_mu(r) phi_nu(r) exp(i q.r)          (g = 2)
+ *
+ * This is the "Cartesian grid method" of arxiv 2512.18010 (SCarFFF): Eq. (35) /root/reference/PAPER.md:244,
+ * evaluated in closed form as Eq. (48)-(50) PAPER.md:326-338 (the monomial D-tensor form) for a stack of
+ * transition density matrices T^s over an arbitrary list of momentum-transfer vectors q, all in FP64.
+ * The paper defines no API (it is a script-driven Julia package); the calls below follow its
+ * statement that the method "depends only on the availability of a transition density matrix and a
+ * selection of any Gaussian basis set" plus geometry.
+ *
+ * Pipeline:
+ *   scarf_set_basis        S0 orbital normalisation, Eq. (A1)-(A5) PAPER.md:619-641;
+ *                          S1 primitive-shell-pair setup = Gaussian product, Eq. (37)-(39), (43) PAPER.md:263-300;
+ *                          S2 per-axis Hermite expansion coefficients (McMurchie-Davidson recurrences; they equal
+ *                             K_AB * C^u / i^u of Eq. (50)).            Host work + one upload.
+ *   scarf_set_transitions  S3 fold T^s into per-pair coefficients D^s (Eq. (48)-(49)), screen,
+ *                             pack the pair stream.                                  Device kernels.
+ *   scarf_form_factors     S4 the hot kernel: for every q, sum over pairs of
+ *                             exp(-q^2/4p) e^{i q.P} sum_t D^s_t (i q)^t  (Eq. (48)). Device kernel(s).
+ *
+ * Conventions
+ *   - Atomic units: positions in bohr, exponents in bohr^-2, q in bohr^-1.  No unit conversion happens here.
+ *   - Fourier sign e^{+i q.r} (Eq. 19), so f(-q) = conj f(q) for real T.
+ *   - Cartesian components of a shell of angular momentum l: (a,b,c), a+b+c = l, a descending then b
+ *     descending: p = x,y,z; d = xx,xy,xz,yy,yz,zz; f = xxx,xxy,xxz,xyy,xyz,xzz,yyy,yyz,yzz,zzz.
+ *     Every component is individually normalised to 1.  Basis functions are numbered shell by
+ *     shell in this component order.
+ *   - Contraction coefficients multiply unit-normalised primitives (Eq. A3); the contracted orbital
+ *     is then renormalised (Eq. A5).
+ *   - Every call returns SCARF_OK (0) or a negative SCARF_E* code; scarf_last_error() holds the text.  No C++
+ *     exception crosses this boundary and there is no global state.  A context is not thread-safe; distinct
+ *     contexts are independent.
+ *   - Inputs are COPIED during set_* (the caller keeps ownership and may free at once).  Outputs are caller-owned.
+ *   - "host or device" pointers are classified with cudaPointerGetAttributes: device and managed memory are used
+ *     in place; pinned or pageable host memory is staged through context-owned device buffers and the call
+ *     returns after the copy back has completed.  With device pointers the work is asynchronous on the context
+ *     stream.
+ *   - There is NO CPU fallback: without a usable CUDA device scarf_set_transitions / scarf_form_factors fail with
+ *     SCARF_ENODEVICE.
+ */
+#ifndef SCARF_H
+#define SCARF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SCARF_OK 0
+#define SCARF_EINVAL (-1)    /* bad argument, shape, l > SCARF_MAX_L, non-positive exponent, NaN/Inf in host input */
+#define SCARF_ESTATE (-2)    /* calls out of order (e.g. form_factors before set_transitions)                      */
+#define SCARF_ENOMEM (-3)    /* host or device allocation failed                                                   */
+#define SCARF_ECUDA (-4)     /* CUDA runtime error; text in scarf_last_error                                       */
+#define SCARF_ENODEVICE (-5) /* the context was created host-only (device < 0) or no device is usable              */
+
+#define SCARF_MAX_L 3        /* highest shell angular momentum (f); pair classes L = l_a + l_b <= 6                */
+#define SCARF_N_CLASSES (2 * SCARF_MAX_L + 1)
+
+typedef struct scarf_ctx scarf_ctx; /* opaque; owns every device buffer it allocates */
+
+/* Counters filled by scarf_get_stats.  "pair" = primitive shell pair (A,k) <= (B,k'). */
+typedef struct scarf_stats {
+    int32_t n_atoms, n_shells, n_prim_shells, nbf, n_states, l_max;
+    int64_t n_pairs_all;                       /* all primitive shell pairs, A <= B                                 */
+    int64_t n_pairs_prescreened;               /* after the T-independent host screen (K_AB underflow)              */
+    int64_t n_pairs_kept;                      /* after the T-dependent bound screen (set_transitions)              */
+    int64_t pairs_kept_per_class[SCARF_N_CLASSES];
+    int64_t n_herm_kept;                       /* sum over kept pairs of n_herm(L) = (L+1)(L+2)(L+3)/6              */
+    int64_t cart_term_pairs;                   /* ordered Cartesian-term pairs, the paper's N_c^2 (Eq. 68)          */
+    double stream_bytes;                       /* packed pair stream read by the hot kernel                         */
+    double slots_per_q;                        /* FP64 issue-slot model per q-point        */
+    double evals_per_q;                        /* kept pairs x states                                               */
+    double last_setup_host_ms;                 /* scarf_set_basis host time                                         */
+    double last_fold_ms, last_kernel_ms;       /* device time of the last S3 / S4 (CUDA events; 0 until queried)    */
+    int32_t last_kernel_launches;              /* kernels launched by the last scarf_form_factors                   */
+    int32_t last_fold_launches;                /* kernels launched by the last scarf_set_transitions               */
+} scarf_stats;
+
+/* device >= 0: CUDA ordinal.  device < 0: host-only context (set_basis, overlap, stats work; the rest ENODEVICE). */
+int scarf_create(scarf_ctx** out, int device);
+void scarf_destroy(scarf_ctx* ctx);
+
+/* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = the legacy default stream. */
+int scarf_set_stream(scarf_ctx* ctx, void* cuda_stream);
+
+/* Options.  "prefactor": g, default 2.0 (Eq. 18, spin sum); takes effect at the next set_transitions.
+ *           "screen_tol": default 1e-16; a pair is dropped when its rigorous bound
+ *                         B_P = max_s sum_t |D^s_t| sup_q |q|^n e^{-q^2/4p} is below screen_tol * mean(B);
+ *                         0 keeps everything.  The paper's own epsilon = 1e-6 thresholding is an
+ *                         approximation and is NOT applied.
+ *           "timing": 1 records CUDA-event times of S3/S4 into the stats (adds a stream sync per call).         */
+int scarf_set_option(scarf_ctx* ctx, const char* key, double value);
+
+/* HOST pointers.  atom_xyz [n_atoms][3].  Shell i sits on atom shell_atom[i], has angular momentum shell_l[i]
+ * (0..SCARF_MAX_L) and shell_nprim[i] >= 1 primitives taken consecutively from exponents[] / coeffs[].
+ * Invalidates any transitions set before. */
+int scarf_set_basis(scarf_ctx* ctx, int n_atoms, const double* atom_xyz, int n_shells, const int32_t* shell_atom,
+                    const int32_t* shell_l, const int32_t* shell_nprim, const double* exponents,
+                    const double* coeffs);
+
+int scarf_nbf(const scarf_ctx* ctx); /* number of contracted Cartesian basis functions, or a negative code */
+
+/* AO overlap S[nbf][nbf] (= Int phi_mu phi_nu, the q = 0 pair integral) into HOST memory, from the S1/S2 tables. */
+int scarf_overlap(scarf_ctx* ctx, double* S_host);
+
+/* T [n_states][nbf][nbf], row-major FP64, real, need not be symmetric.  Host or device pointer.
+ * May be called repeatedly on one basis. */
+int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T);
+
+/* q [n_q][3] FP64; out [n_states][n_q][2] FP64 (re, im interleaved).  Host or device pointers, independently.
+ * Any point set (no grid structure is assumed).  May be called repeatedly. */
+int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out);
+
+int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out);
+const char* scarf_last_error(const scarf_ctx* ctx);
+const char* scarf_version(void);
+
+/* Measured FP64 issue peak of the device: runs a register-only chain of dependent-free DFMAs on every SM and
+ * returns lane-level DFMA per second (1 "slot" = 2 flop) and the SM clock (MHz) observed during the run.
+ * This is the denominator of the roofline fraction bench.py reports. */
+int scarf_fp64_peak(int device, double* dfma_per_s, double* sm_clock_mhz);
+
+/* Host-side building blocks, exported so the CPU test-suite can pin them without a GPU.
+ * scarf_host_hermite_E: E[(la+1)][(lb+1)][(la+lb+1)] for one axis, McMurchie-Davidson:
+ *     (x-Ax)^i (x-Bx)^j e^{-alpha (x-Ax)^2 - beta (x-Bx)^2} = sum_t E_t^{ij} (d/dPx)^t e^{-p (x-Px)^2}.
+ * scarf_host_shell_norms: c[(component, primitive)] effective coefficients of one shell, component-major. */
+int scarf_host_hermite_E(int la, int lb, double alpha, double beta, double Ax, double Bx, double* E_out);
+int scarf_host_shell_norms(int l, int nprim, const double* exponents, const double* coeffs, double* c_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SCARF_H */

@@ -1,0 +1,244 @@
+"""Thin ctypes binding of libscarf.so (include/scarf.h).  Argument marshalling only: every step of the path
+runs inside the library.  PyTorch tensors are accepted for T, q and out (their `data_ptr()` is passed on);
+numpy arrays are passed as host pointers.  If the library has not been built the import of this module fails
+loudly — there is no fallback of any kind.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libscarf.so")
+
+SCARF_OK, SCARF_EINVAL, SCARF_ESTATE, SCARF_ENOMEM, SCARF_ECUDA, SCARF_ENODEVICE = 0, -1, -2, -3, -4, -5
+SCARF_MAX_L = 3
+SCARF_N_CLASSES = 2 * SCARF_MAX_L + 1
+_CODES = {-1: "EINVAL", -2: "ESTATE", -3: "ENOMEM", -4: "ECUDA", -5: "ENODEVICE"}
+
+EXPORTS = ["scarf_create", "scarf_destroy", "scarf_set_stream", "scarf_set_option", "scarf_set_basis", "scarf_nbf",
+           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_get_stats", "scarf_last_error",
+           "scarf_version", "scarf_fp64_peak", "scarf_host_hermite_E", "scarf_host_shell_norms"]
+
+
+class ScarfStats(C.Structure):
+    _fields_ = [("n_atoms", C.c_int32), ("n_shells", C.c_int32), ("n_prim_shells", C.c_int32), ("nbf", C.c_int32),
+                ("n_states", C.c_int32), ("l_max", C.c_int32),
+                ("n_pairs_all", C.c_int64), ("n_pairs_prescreened", C.c_int64), ("n_pairs_kept", C.c_int64),
+                ("pairs_kept_per_class", C.c_int64 * SCARF_N_CLASSES),
+                ("n_herm_kept", C.c_int64), ("cart_term_pairs", C.c_int64),
+                ("stream_bytes", C.c_double), ("slots_per_q", C.c_double), ("evals_per_q", C.c_double),
+                ("last_setup_host_ms", C.c_double), ("last_fold_ms", C.c_double), ("last_kernel_ms", C.c_double),
+                ("last_kernel_launches", C.c_int32), ("last_fold_launches", C.c_int32)]
+
+    def as_dict(self):
+        d = {}
+        for name, _t in self._fields_:
+            v = getattr(self, name)
+            d[name] = list(v) if hasattr(v, "__len__") else v
+        return d
+
+
+class ScarfError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"scarf error {_CODES.get(code, code)}: {msg}")
+        self.code = code
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2512_18010_b200.build` "
+                          "(nvcc, sm_100a).  There is no CPU fallback.")
+    L = C.CDLL(LIB_PATH)
+    dp, ip, vp = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.c_void_p
+    L.scarf_create.argtypes = [C.POINTER(vp), C.c_int]
+    L.scarf_destroy.argtypes = [vp]
+    L.scarf_destroy.restype = None
+    L.scarf_set_stream.argtypes = [vp, vp]
+    L.scarf_set_option.argtypes = [vp, C.c_char_p, C.c_double]
+    L.scarf_set_basis.argtypes = [vp, C.c_int, dp, C.c_int, ip, ip, ip, dp, dp]
+    L.scarf_nbf.argtypes = [vp]
+    L.scarf_overlap.argtypes = [vp, dp]
+    L.scarf_set_transitions.argtypes = [vp, C.c_int, vp]
+    L.scarf_form_factors.argtypes = [vp, C.c_int64, vp, vp]
+    L.scarf_get_stats.argtypes = [vp, C.POINTER(ScarfStats)]
+    L.scarf_last_error.argtypes = [vp]
+    L.scarf_last_error.restype = C.c_char_p
+    L.scarf_version.restype = C.c_char_p
+    L.scarf_fp64_peak.argtypes = [C.c_int, dp, dp]
+    L.scarf_host_hermite_E.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, dp]
+    L.scarf_host_shell_norms.argtypes = [C.c_int, C.c_int, dp, dp, dp]
+    for name in EXPORTS:      # every symbol include/scarf.h declares must resolve
+        getattr(L, name)
+    return L
+
+
+_lib = _load()
+
+
+def lib():
+    return _lib
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _ip(a):
+    return a.ctypes.data_as(C.POINTER(C.c_int32))
+
+
+def _is_torch(x) -> bool:
+    return hasattr(x, "data_ptr") and hasattr(x, "is_contiguous")
+
+
+def _ptr(x, what, n_expected=None):
+    """(pointer, keep-alive object) for a float64, C-contiguous numpy array or torch tensor."""
+    if _is_torch(x):
+        import torch
+        if x.dtype != torch.float64 or not x.is_contiguous():
+            raise ValueError(f"{what}: torch tensor must be float64 and contiguous")
+        if n_expected is not None and x.numel() != n_expected:
+            raise ValueError(f"{what}: expected {n_expected} elements, got {x.numel()}")
+        return C.c_void_p(x.data_ptr()), x
+    a = np.ascontiguousarray(x, dtype=np.float64)
+    if n_expected is not None and a.size != n_expected:
+        raise ValueError(f"{what}: expected {n_expected} elements, got {a.size}")
+    return C.c_void_p(a.ctypes.data), a
+
+
+def version() -> str:
+    return _lib.scarf_version().decode()
+
+
+def fp64_peak(device: int = 0):
+    """(lane-level DFMA per second, SM clock in MHz) measured on `device` by the library's micro-benchmark."""
+    r, m = C.c_double(0), C.c_double(0)
+    rc = _lib.scarf_fp64_peak(int(device), C.byref(r), C.byref(m))
+    if rc != SCARF_OK:
+        raise ScarfError(rc, "scarf_fp64_peak failed")
+    return r.value, m.value
+
+
+def host_hermite_E(la, lb, alpha, beta, Ax, Bx) -> np.ndarray:
+    out = np.zeros((la + 1, lb + 1, la + lb + 1))
+    rc = _lib.scarf_host_hermite_E(la, lb, alpha, beta, Ax, Bx, _dp(out))
+    if rc != SCARF_OK:
+        raise ScarfError(rc, "scarf_host_hermite_E")
+    return out
+
+
+def host_shell_norms(l, exponents, coeffs) -> np.ndarray:
+    e = np.ascontiguousarray(exponents, np.float64)
+    d = np.ascontiguousarray(coeffs, np.float64)
+    out = np.zeros(((l + 1) * (l + 2) // 2, e.size))
+    rc = _lib.scarf_host_shell_norms(int(l), int(e.size), _dp(e), _dp(d), _dp(out))
+    if rc != SCARF_OK:
+        raise ScarfError(rc, "scarf_host_shell_norms")
+    return out
+
+
+class Scarf:
+    """One libscarf context.  device=None creates a host-only context (basis setup, overlap, stats)."""
+
+    def __init__(self, device=0):
+        self._h = C.c_void_p()
+        rc = _lib.scarf_create(C.byref(self._h), -1 if device is None else int(device))
+        if rc != SCARF_OK:
+            raise ScarfError(rc, "scarf_create failed (no usable CUDA device? there is no CPU fallback)")
+        self.device = device
+        self.n_states = 0
+        self._nbf = 0
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            _lib.scarf_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def _check(self, rc):
+        if rc != SCARF_OK:
+            raise ScarfError(rc, _lib.scarf_last_error(self._h).decode())
+
+    def set_stream(self, cuda_stream: int):
+        self._check(_lib.scarf_set_stream(self._h, C.c_void_p(int(cuda_stream))))
+
+    def set_option(self, key: str, value: float):
+        self._check(_lib.scarf_set_option(self._h, key.encode(), float(value)))
+
+    def set_basis(self, basis=None, *, atom_xyz=None, shell_atom=None, shell_l=None, shell_nprim=None,
+                  exponents=None, coeffs=None):
+        if basis is not None:
+            atom_xyz, shell_atom, shell_l = basis.atom_xyz, basis.shell_atom, basis.shell_l
+            shell_nprim, exponents, coeffs = basis.shell_nprim, basis.exponents, basis.coeffs
+        xyz = np.ascontiguousarray(atom_xyz, np.float64).reshape(-1, 3)
+        sa = np.ascontiguousarray(shell_atom, np.int32)
+        sl = np.ascontiguousarray(shell_l, np.int32)
+        sn = np.ascontiguousarray(shell_nprim, np.int32)
+        e = np.ascontiguousarray(exponents, np.float64)
+        d = np.ascontiguousarray(coeffs, np.float64)
+        if not (sa.size == sl.size == sn.size) or e.size != d.size or e.size != int(sn.sum()):
+            raise ValueError("set_basis: inconsistent array lengths")
+        self._check(_lib.scarf_set_basis(self._h, xyz.shape[0], _dp(xyz), sl.size, _ip(sa), _ip(sl), _ip(sn), _dp(e), _dp(d)))
+        self._nbf = int(_lib.scarf_nbf(self._h))
+        self.n_states = 0
+
+    @property
+    def nbf(self) -> int:
+        return self._nbf
+
+    def overlap(self) -> np.ndarray:
+        S = np.zeros((self._nbf, self._nbf))
+        self._check(_lib.scarf_overlap(self._h, _dp(S)))
+        return S
+
+    def set_transitions(self, T):
+        shape = tuple(T.shape)
+        if len(shape) == 2:
+            shape = (1,) + shape
+        if len(shape) != 3 or shape[1] != self._nbf or shape[2] != self._nbf:
+            raise ValueError(f"set_transitions: T must be [n_states][{self._nbf}][{self._nbf}]")
+        p, keep = _ptr(T, "T", shape[0] * shape[1] * shape[2])
+        self._check(_lib.scarf_set_transitions(self._h, shape[0], p))
+        self.n_states = shape[0]
+
+    def form_factors(self, q, out=None):
+        """q: [n_q][3] float64 numpy (host) or torch (host or cuda).  out: optional float64 buffer
+        [n_states][n_q][2] (numpy or torch); allocated like q when omitted.  Returns complex128 [n_states][n_q]
+        (a view of `out`)."""
+        n_q = int(q.shape[0])
+        if tuple(q.shape) != (n_q, 3):
+            raise ValueError("form_factors: q must be [n_q][3]")
+        qp, qkeep = _ptr(q, "q", 3 * n_q)
+        if out is None:
+            if _is_torch(q):
+                import torch
+                out = torch.empty((self.n_states, n_q, 2), dtype=torch.float64, device=q.device)
+            else:
+                out = np.empty((self.n_states, n_q, 2))
+        op, okeep = _ptr(out, "out", self.n_states * n_q * 2)
+        if not _is_torch(out) and okeep is not out:
+            raise ValueError("form_factors: out must be a C-contiguous float64 array")
+        self._check(_lib.scarf_form_factors(self._h, n_q, qp, op))
+        if _is_torch(out):
+            import torch
+            return torch.view_as_complex(out.view(self.n_states, n_q, 2))
+        return out.reshape(self.n_states, n_q, 2).view(np.complex128)[..., 0]
+
+    def stats(self) -> dict:
+        s = ScarfStats()
+        self._check(_lib.scarf_get_stats(self._h, C.byref(s)))
+        return s.as_dict()

@@ -1,0 +1,206 @@
+// fold.cu — S3 of SURVEY.md §8(a): fold the transition matrices T^s into per-primitive-pair Hermite
+// coefficients (the paper's T M D product, Eq. (48)-(49) PAPER.md:326-334), compute the screening bound,
+// and pack the kept records.  Also the FP64 peak micro-benchmark.
+#include "kernels.cuh"
+
+namespace scarf {
+
+__constant__ unsigned char c_herm[kMaxHerm][4];              // (t,u,v,n) of Hermite index h
+__constant__ unsigned char c_comp[kMaxL + 1][kMaxCart][4];   // (a,b,c,-) of component comp of shell l
+__constant__ double c_fcomp[kMaxL + 1][kMaxCart];            // 1/sqrt((2a-1)!!(2b-1)!!(2c-1)!!)
+
+cudaError_t upload_tables()
+{
+    unsigned char herm[kMaxHerm][4];
+    int h = 0;
+    for (int n = 0; n <= kMaxClass; ++n)
+        for (int t = n; t >= 0; --t)
+            for (int u = n - t; u >= 0; --u) {
+                herm[h][0] = (unsigned char)t; herm[h][1] = (unsigned char)u;
+                herm[h][2] = (unsigned char)(n - t - u); herm[h][3] = (unsigned char)n;
+                ++h;
+            }
+    unsigned char comp[kMaxL + 1][kMaxCart][4] = {};
+    double fcomp[kMaxL + 1][kMaxCart] = {};
+    for (int l = 0; l <= kMaxL; ++l)
+        for (int c = 0; c < ncart(l); ++c) {
+            int abc[3];
+            component_powers(l, c, abc);
+            comp[l][c][0] = (unsigned char)abc[0]; comp[l][c][1] = (unsigned char)abc[1];
+            comp[l][c][2] = (unsigned char)abc[2];
+            fcomp[l][c] = component_factor(l, c);
+        }
+    cudaError_t e = cudaMemcpyToSymbol(c_herm, herm, sizeof herm);
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpyToSymbol(c_comp, comp, sizeof comp);
+    if (e != cudaSuccess) return e;
+    return cudaMemcpyToSymbol(c_fcomp, fcomp, sizeof fcomp);
+}
+
+// One warp per primitive shell pair; lanes stride over the Hermite index h.
+//   D^s_h = g * scale * sign(n) * sum_{ca,cb} f_ca f_cb (T^s[mu][nu] + T^s[nu][mu]) Ex[a][a'][t] Ey[b][b'][u] Ez[c][c'][v]
+// and the bound B_P = max_s sum_h |D^s_h| (2 p n / e)^{n/2}  (sup over q of |q|^n e^{-q^2/4p}; 1 for n = 0).
+__global__ void __launch_bounds__(128) fold_kernel(const FoldArgs a)
+{
+    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (warp >= a.n_pairs) return;
+    const PairMeta m = a.pairs[warp];
+    const int la = m.la, lb = m.lb, L = m.L, nt = L + 1, nh = nherm(L);
+    const int blk = (la + 1) * (lb + 1) * nt;
+    const double* __restrict__ Ex = a.E + m.e_off;
+    const double* __restrict__ Ey = Ex + blk;
+    const double* __restrict__ Ez = Ey + blk;
+    double* rec = reinterpret_cast<double*>(a.staging + a.cls_off[L] + (unsigned long long)(warp - a.class_first[L]) * a.rec_bytes[L]);
+    if (lane == 0) {
+        rec[0] = m.Px; rec[1] = m.Py; rec[2] = m.Pz; rec[3] = m.inv4p;
+        if ((a.NS * nh) & 1) rec[4 + a.NS * nh] = 0.0;
+    }
+    const size_t nbf = (size_t)a.nbf;
+    const double* __restrict__ T = a.T + (size_t)a.s0 * nbf * nbf;
+    double bsum[kMaxStateTile];
+#pragma unroll
+    for (int s = 0; s < kMaxStateTile; ++s) bsum[s] = 0.0;
+    const int nca = ncart(la), ncb = ncart(lb);
+    for (int h = lane; h < nh; h += 32) {
+        const int t = c_herm[h][0], u = c_herm[h][1], v = c_herm[h][2], n = c_herm[h][3];
+        double acc[kMaxStateTile];
+#pragma unroll
+        for (int s = 0; s < kMaxStateTile; ++s) acc[s] = 0.0;
+        for (int ca = 0; ca < nca; ++ca) {
+            const int a1 = c_comp[la][ca][0], b1 = c_comp[la][ca][1], c1 = c_comp[la][ca][2];
+            for (int cb = 0; cb < ncb; ++cb) {
+                const int a2 = c_comp[lb][cb][0], b2 = c_comp[lb][cb][1], c2 = c_comp[lb][cb][2];
+                if (t > a1 + a2 || u > b1 + b2 || v > c1 + c2) continue;
+                const double G = c_fcomp[la][ca] * c_fcomp[lb][cb] * Ex[(a1 * (lb + 1) + a2) * nt + t] *
+                                 Ey[(b1 * (lb + 1) + b2) * nt + u] * Ez[(c1 * (lb + 1) + c2) * nt + v];
+                const size_t mu = (size_t)(m.bf0a + ca), nu = (size_t)(m.bf0b + cb);
+                const double* t1 = T + mu * nbf + nu;
+                const double* t2 = T + nu * nbf + mu;
+#pragma unroll
+                for (int s = 0; s < kMaxStateTile; ++s)
+                    if (s < a.ns_real) acc[s] += G * (t1[(size_t)s * nbf * nbf] + t2[(size_t)s * nbf * nbf]);
+            }
+        }
+        const double sign = ((n >> 1) & 1) ? -1.0 : 1.0;
+        const double mn = n == 0 ? 1.0 : pow(2.0 * m.p * n * 0.36787944117144233, 0.5 * n);
+        const double f = a.g * m.scale * sign;
+#pragma unroll
+        for (int s = 0; s < kMaxStateTile; ++s)
+            if (s < a.NS) {
+                const double D = s < a.ns_real ? f * acc[s] : 0.0;
+                rec[4 + s * nh + h] = D;
+                bsum[s] += fabs(D) * mn;
+            }
+    }
+    double b = 0.0;
+#pragma unroll
+    for (int s = 0; s < kMaxStateTile; ++s) {
+        double x = bsum[s];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+        b = fmax(b, x);
+    }
+    if (lane == 0) a.bound[warp] = a.first_tile ? b : fmax(a.bound[warp], b);
+}
+
+cudaError_t launch_fold(const FoldArgs& a, cudaStream_t st)
+{
+    if (a.n_pairs <= 0) return cudaSuccess;
+    const int threads = 128;
+    const long long blocks = (a.n_pairs * 32 + threads - 1) / threads;
+    fold_kernel<<<(unsigned)blocks, threads, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+// One warp per kept record: copy it from the staging layout to its packed position (16-byte chunks).
+__global__ void __launch_bounds__(128) pack_kernel(const char* __restrict__ staging, char* __restrict__ packed,
+                                                   const unsigned long long* __restrict__ src_off,
+                                                   const unsigned long long* __restrict__ dst_off,
+                                                   const int* __restrict__ nbytes, long long n)
+{
+    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (warp >= n) return;
+    const uint4* s = reinterpret_cast<const uint4*>(staging + src_off[warp]);
+    uint4* d = reinterpret_cast<uint4*>(packed + dst_off[warp]);
+    const int chunks = nbytes[warp] >> 4;
+    for (int i = lane; i < chunks; i += 32) d[i] = s[i];
+}
+
+cudaError_t launch_pack(const char* staging, char* packed, const unsigned long long* src_off,
+                        const unsigned long long* dst_off, const int* nbytes, long long n, cudaStream_t st)
+{
+    if (n <= 0) return cudaSuccess;
+    const int threads = 128;
+    const long long blocks = (n * 32 + threads - 1) / threads;
+    pack_kernel<<<(unsigned)blocks, threads, 0, st>>>(staging, packed, src_off, dst_off, nbytes, n);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// FP64 issue-rate micro-benchmark: 8 independent DFMA chains per thread, registers only.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dfma_peak_kernel(double* sink, int iters, long long* cycles)
+{
+    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double m = 1.0000000001, c = 1e-12;
+    const long long t0 = clock64();
+#pragma unroll 1
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+            a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+        }
+    }
+    const long long t1 = clock64();
+    const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == 123.456) sink[0] = s;
+    if (threadIdx.x == 0 && blockIdx.x == 0) cycles[0] = t1 - t0;
+}
+
+cudaError_t run_fp64_peak(double* dfma_per_s, double* sm_clock_mhz)
+{
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    double* sink = nullptr;
+    long long* cyc = nullptr;
+    if ((e = cudaMalloc(&sink, 8)) != cudaSuccess) return e;
+    if ((e = cudaMalloc(&cyc, 8)) != cudaSuccess) { cudaFree(sink); return e; }
+    cudaEvent_t ev0, ev1;
+    cudaEventCreate(&ev0);
+    cudaEventCreate(&ev1);
+    const int blocks = sms * 4, threads = 256, iters = 20000;
+    dfma_peak_kernel<<<blocks, threads>>>(sink, 2000, cyc);  // warm-up
+    double best = 0.0, best_mhz = 0.0;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(ev0);
+        dfma_peak_kernel<<<blocks, threads>>>(sink, iters, cyc);
+        cudaEventRecord(ev1);
+        e = cudaEventSynchronize(ev1);
+        if (e != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, ev0, ev1);
+        long long c = 0;
+        cudaMemcpy(&c, cyc, 8, cudaMemcpyDeviceToHost);
+        const double rate = (double)blocks * threads * (double)iters * 64.0 / (ms * 1e-3);
+        if (rate > best) {
+            best = rate;
+            best_mhz = (double)c / (ms * 1e-3) * 1e-6;  // block 0 runs for ~the whole kernel when the grid is one wave
+        }
+    }
+    cudaEventDestroy(ev0);
+    cudaEventDestroy(ev1);
+    cudaFree(sink);
+    cudaFree(cyc);
+    if (e != cudaSuccess) return e;
+    *dfma_per_s = best;
+    *sm_clock_mhz = best_mhz;
+    return cudaGetLastError();
+}
+
+}  // namespace scarf

@@ -1,0 +1,70 @@
+// kernels.cuh — device-side data layout and launcher prototypes shared by scarf_api.cu and the kernel files.
+//
+// Pair stream ("records"), one per kept primitive shell pair, grouped by class L = la + lb, per state tile:
+//
+//     double  Px, Py, Pz, inv4p                 32-byte header (Gaussian-product centre, 1/(4p))
+//     double  D[NS][n_herm(L)]                  folded coefficients, state-major, Hermite index h fastest
+//     double  0 (only if NS*n_herm is odd)      pad to a 16-byte multiple
+//
+// Hermite index h enumerates (t,u,v) by total degree n = t+u+v ascending, then t descending, then u descending,
+// so the list for class L is a prefix of the list for class L+1.  The factor i^n of (iq)^t is folded into D:
+// even n carry (-1)^{n/2} and contribute to the real polynomial A, odd n carry (-1)^{(n-1)/2} and contribute
+// to the imaginary polynomial B;   term = e^{-q^2/4p} (cos qP + i sin qP) (A + iB).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "host_setup.hpp"
+
+namespace scarf {
+
+constexpr int kMaxStateTile = 12;  // states whose accumulators one thread keeps in registers
+
+__host__ __device__ inline constexpr int rec_doubles(int L, int NS)
+{
+    return 4 + ((NS * nherm(L) + 1) & ~1);
+}
+
+struct ClassStream {
+    long long n;               // records in this class
+    unsigned long long off;    // byte offset of the class's first record from the tile base
+    int rec_bytes;
+    int pad;
+};
+
+struct TileStream {            // one state tile of the pair stream
+    int s0, ns_real, NS;       // first state, real states, padded/templated state count
+    int pad;
+    char* base;                // device pointer
+    unsigned long long bytes;
+    ClassStream cls[kNClasses];
+};
+
+struct FoldArgs {
+    const PairMeta* pairs;
+    long long n_pairs;
+    const double* E;
+    const double* T;           // [ns_total][nbf][nbf]
+    int nbf, s0, ns_real, NS;
+    int first_tile, pad;
+    double g;
+    char* staging;             // tile stream laid out for ALL prescreened pairs
+    double* bound;             // [n_pairs] screening bound B_P
+    long long class_first[kNClasses + 1];
+    unsigned long long cls_off[kNClasses];
+    int rec_bytes[kNClasses];
+};
+
+cudaError_t launch_fold(const FoldArgs& a, cudaStream_t st);
+cudaError_t launch_pack(const char* staging, char* packed, const unsigned long long* src_off,
+                        const unsigned long long* dst_off, const int* nbytes, long long n, cudaStream_t st);
+cudaError_t upload_tables();   // constant-memory index tables; once per process
+
+// v0: one thread per q, records read straight from global memory.  accumulate != 0: out += result.
+cudaError_t launch_ff_v0(int L, const TileStream& ts, const double* q, long long n_q, double* out, int accumulate,
+                         cudaStream_t st);
+
+cudaError_t run_fp64_peak(double* dfma_per_s, double* sm_clock_mhz);
+
+}  // namespace scarf

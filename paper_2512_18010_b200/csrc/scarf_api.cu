@@ -1,0 +1,495 @@
+// scarf_api.cu — the C ABI of include/scarf.h: context, argument checking, host<->device staging, launch order.
+#include <chrono>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/scarf.h"
+#include "kernels.cuh"
+
+using namespace scarf;
+
+namespace {
+
+struct DevBuf {
+    void* p = nullptr;
+    size_t cap = 0;
+    cudaError_t ensure(size_t bytes)
+    {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) cudaFree(p);
+        p = nullptr; cap = 0;
+        cudaError_t e = cudaMalloc(&p, bytes);
+        if (e == cudaSuccess) cap = bytes;
+        return e;
+    }
+    void release()
+    {
+        if (p) cudaFree(p);
+        p = nullptr; cap = 0;
+    }
+};
+
+// FP64 issue-slot model: per (q, pair, state) W(L), per (q, pair) C_tr.
+const double kW[kNClasses] = {2, 7, 13, 23, 38, 59, 87};
+const double kCtr = 40.0;
+
+bool g_tables_uploaded_dev[64] = {};
+
+}  // namespace
+
+struct scarf_ctx {
+    int device = -1;
+    bool host_only = true;
+    cudaStream_t stream = nullptr;
+    double prefactor = 2.0, screen_tol = 1e-16;
+    bool timing = false;
+    int kernel_variant = -1;  // -1 auto, 0 force v0
+    std::string err;
+    HostSetup hs;
+    bool have_basis = false, have_T = false;
+    int n_states = 0;
+    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb;
+    std::vector<DevBuf> staging, packed;
+    std::vector<TileStream> tiles;
+    scarf_stats st = {};
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+};
+
+namespace {
+
+int fail(scarf_ctx* c, int code, const std::string& msg)
+{
+    if (c) c->err = msg;
+    return code;
+}
+
+int cuda_fail(scarf_ctx* c, cudaError_t e, const char* where)
+{
+    cudaGetLastError();
+    if (e == cudaErrorMemoryAllocation) return fail(c, SCARF_ENOMEM, std::string(where) + ": out of device memory");
+    return fail(c, SCARF_ECUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+
+#define CU(call, where)                                        \
+    do {                                                       \
+        cudaError_t e__ = (call);                              \
+        if (e__ != cudaSuccess) return cuda_fail(ctx, e__, where); \
+    } while (0)
+
+bool is_device_ptr(const void* p)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+bool all_finite(const double* x, size_t n)
+{
+    double acc = 0.0;
+    for (size_t i = 0; i < n; ++i) acc += x[i] * 0.0;  // NaN/Inf propagate: Inf*0 = NaN
+    return acc == 0.0;
+}
+
+int tile_size_for(int ns)  // smallest instantiated state tile >= ns (ns <= 12)
+{
+    static const int sizes[] = {1, 2, 4, 6, 8, 12};
+    for (int s : sizes)
+        if (s >= ns) return s;
+    return kMaxStateTile;
+}
+
+void free_device(scarf_ctx* c)
+{
+    c->d_pairs.release(); c->d_E.release(); c->d_bound.release(); c->d_T.release(); c->d_q.release();
+    c->d_out.release(); c->d_src.release(); c->d_dst.release(); c->d_nb.release();
+    for (auto& b : c->staging) b.release();
+    for (auto& b : c->packed) b.release();
+    c->staging.clear(); c->packed.clear(); c->tiles.clear();
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* scarf_version(void) { return "scarf 0.1 (sm_100a)"; }
+
+int scarf_create(scarf_ctx** out, int device)
+{
+    if (!out) return SCARF_EINVAL;
+    *out = nullptr;
+    scarf_ctx* ctx = new (std::nothrow) scarf_ctx();
+    if (!ctx) return SCARF_ENOMEM;
+    if (device >= 0) {
+        int n = 0;
+        cudaError_t e = cudaGetDeviceCount(&n);
+        if (e != cudaSuccess || device >= n) {
+            cudaGetLastError();
+            delete ctx;
+            return SCARF_ENODEVICE;
+        }
+        e = cudaSetDevice(device);
+        if (e == cudaSuccess && !(device < 64 && g_tables_uploaded_dev[device])) {
+            e = upload_tables();
+            if (e == cudaSuccess && device < 64) g_tables_uploaded_dev[device] = true;
+        }
+        if (e == cudaSuccess) e = cudaEventCreate(&ctx->ev0);
+        if (e == cudaSuccess) e = cudaEventCreate(&ctx->ev1);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            delete ctx;
+            return SCARF_ECUDA;
+        }
+        ctx->device = device;
+        ctx->host_only = false;
+    }
+    *out = ctx;
+    return SCARF_OK;
+}
+
+void scarf_destroy(scarf_ctx* ctx)
+{
+    if (!ctx) return;
+    if (!ctx->host_only) {
+        cudaSetDevice(ctx->device);
+        cudaStreamSynchronize(ctx->stream);
+        free_device(ctx);
+        if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+        if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    }
+    delete ctx;
+}
+
+int scarf_set_stream(scarf_ctx* ctx, void* cuda_stream)
+{
+    if (!ctx) return SCARF_EINVAL;
+    ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    return SCARF_OK;
+}
+
+int scarf_set_option(scarf_ctx* ctx, const char* key, double value)
+{
+    if (!ctx || !key) return SCARF_EINVAL;
+    if (!std::isfinite(value)) return fail(ctx, SCARF_EINVAL, "set_option: non-finite value");
+    const std::string k(key);
+    if (k == "prefactor") ctx->prefactor = value;
+    else if (k == "screen_tol") {
+        if (value < 0) return fail(ctx, SCARF_EINVAL, "set_option: screen_tol must be >= 0");
+        ctx->screen_tol = value;
+    } else if (k == "timing") ctx->timing = value != 0.0;
+    else if (k == "kernel_variant") ctx->kernel_variant = (int)value;
+    else return fail(ctx, SCARF_EINVAL, "set_option: unknown key '" + k + "'");
+    return SCARF_OK;
+}
+
+int scarf_set_basis(scarf_ctx* ctx, int n_atoms, const double* atom_xyz, int n_shells, const int32_t* shell_atom,
+                    const int32_t* shell_l, const int32_t* shell_nprim, const double* exponents, const double* coeffs)
+{
+    if (!ctx) return SCARF_EINVAL;
+    try {
+        const auto t0 = std::chrono::steady_clock::now();
+        ctx->have_basis = ctx->have_T = false;
+        std::string err;
+        int rc = build_setup(n_atoms, atom_xyz, n_shells, shell_atom, shell_l, shell_nprim, exponents, coeffs, ctx->hs, err);
+        if (rc != SCARF_OK) return fail(ctx, rc, err);
+        const HostSetup& hs = ctx->hs;
+        if (!ctx->host_only) {
+            CU(cudaSetDevice(ctx->device), "set_basis");
+            CU(ctx->d_pairs.ensure(std::max<size_t>(64, hs.pairs.size() * sizeof(PairMeta))), "set_basis: alloc pairs");
+            CU(ctx->d_E.ensure(std::max<size_t>(64, hs.E.size() * sizeof(double))), "set_basis: alloc E");
+            CU(cudaMemcpyAsync(ctx->d_pairs.p, hs.pairs.data(), hs.pairs.size() * sizeof(PairMeta), cudaMemcpyHostToDevice, ctx->stream), "set_basis: upload pairs");
+            CU(cudaMemcpyAsync(ctx->d_E.p, hs.E.data(), hs.E.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream), "set_basis: upload E");
+            CU(cudaStreamSynchronize(ctx->stream), "set_basis: sync");  // the host vectors may be rebuilt by the next call
+        }
+        scarf_stats& st = ctx->st;
+        st = scarf_stats();
+        st.n_atoms = hs.n_atoms; st.n_shells = hs.n_shells; st.n_prim_shells = (int32_t)hs.prim.size();
+        st.nbf = hs.nbf; st.l_max = hs.l_max;
+        st.n_pairs_all = hs.n_pairs_all;
+        st.n_pairs_prescreened = (int64_t)hs.pairs.size();
+        st.cart_term_pairs = hs.cart_term_pairs;
+        st.last_setup_host_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+        ctx->have_basis = true;
+        return SCARF_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(ctx, SCARF_ENOMEM, "set_basis: out of host memory");
+    } catch (...) {
+        return fail(ctx, SCARF_EINVAL, "set_basis: unexpected exception");
+    }
+}
+
+int scarf_nbf(const scarf_ctx* ctx)
+{
+    if (!ctx) return SCARF_EINVAL;
+    if (!ctx->have_basis) return SCARF_ESTATE;
+    return ctx->hs.nbf;
+}
+
+int scarf_overlap(scarf_ctx* ctx, double* S_host)
+{
+    if (!ctx || !S_host) return SCARF_EINVAL;
+    if (!ctx->have_basis) return fail(ctx, SCARF_ESTATE, "overlap: set_basis first");
+    overlap_from_setup(ctx->hs, S_host);
+    return SCARF_OK;
+}
+
+int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T)
+{
+    if (!ctx) return SCARF_EINVAL;
+    if (ctx->host_only) return fail(ctx, SCARF_ENODEVICE, "set_transitions: host-only context; there is no CPU fallback");
+    if (!ctx->have_basis) return fail(ctx, SCARF_ESTATE, "set_transitions: set_basis first");
+    if (n_states < 1 || !T) return fail(ctx, SCARF_EINVAL, "set_transitions: n_states < 1 or null T");
+    try {
+        ctx->have_T = false;
+        const HostSetup& hs = ctx->hs;
+        const size_t nbf = (size_t)hs.nbf, tsz = (size_t)n_states * nbf * nbf;
+        const long long np = (long long)hs.pairs.size();
+        CU(cudaSetDevice(ctx->device), "set_transitions");
+        cudaStream_t st = ctx->stream;
+        const double* dT = T;
+        if (!is_device_ptr(T)) {
+            if (!all_finite(T, tsz)) return fail(ctx, SCARF_EINVAL, "set_transitions: NaN/Inf in T");
+            CU(ctx->d_T.ensure(tsz * sizeof(double)), "set_transitions: alloc T");
+            CU(cudaMemcpyAsync(ctx->d_T.p, T, tsz * sizeof(double), cudaMemcpyHostToDevice, st), "set_transitions: upload T");
+            dT = static_cast<const double*>(ctx->d_T.p);
+        }
+        // state tiles
+        std::vector<TileStream> tiles;
+        for (int s0 = 0; s0 < n_states; s0 += kMaxStateTile) {
+            TileStream t = {};
+            t.s0 = s0;
+            t.ns_real = std::min(kMaxStateTile, n_states - s0);
+            t.NS = tile_size_for(t.ns_real);
+            tiles.push_back(t);
+        }
+        if (ctx->staging.size() < tiles.size()) ctx->staging.resize(tiles.size());
+        if (ctx->packed.size() < tiles.size()) ctx->packed.resize(tiles.size());
+        CU(ctx->d_bound.ensure(std::max<size_t>(64, (size_t)np * sizeof(double))), "set_transitions: alloc bound");
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "set_transitions: event");
+        // fold every tile into a staging stream that holds ALL prescreened pairs
+        for (size_t it = 0; it < tiles.size(); ++it) {
+            TileStream& t = tiles[it];
+            FoldArgs a = {};
+            a.pairs = static_cast<const PairMeta*>(ctx->d_pairs.p);
+            a.n_pairs = np;
+            a.E = static_cast<const double*>(ctx->d_E.p);
+            a.T = dT;
+            a.nbf = hs.nbf; a.s0 = t.s0; a.ns_real = t.ns_real; a.NS = t.NS;
+            a.first_tile = it == 0;
+            a.g = ctx->prefactor;
+            a.bound = static_cast<double*>(ctx->d_bound.p);
+            unsigned long long off = 0;
+            for (int c = 0; c < kNClasses; ++c) {
+                a.class_first[c] = hs.class_first[c];
+                a.cls_off[c] = off;
+                a.rec_bytes[c] = rec_doubles(c, t.NS) * 8;
+                off += (unsigned long long)hs.class_count[c] * a.rec_bytes[c];
+            }
+            a.class_first[kNClasses] = hs.class_first[kNClasses];
+            CU(ctx->staging[it].ensure(std::max<unsigned long long>(64, off)), "set_transitions: alloc staging");
+            a.staging = static_cast<char*>(ctx->staging[it].p);
+            CU(launch_fold(a, st), "set_transitions: fold kernel");
+            t.base = a.staging;
+            t.bytes = off;
+            for (int c = 0; c < kNClasses; ++c) {
+                t.cls[c].n = hs.class_count[c];
+                t.cls[c].off = a.cls_off[c];
+                t.cls[c].rec_bytes = a.rec_bytes[c];
+            }
+        }
+        // screening: B_P < screen_tol * mean(B) is dropped (rigorous: total dropped <= screen_tol * sum B)
+        std::vector<double> bound((size_t)np);
+        CU(cudaMemcpyAsync(bound.data(), ctx->d_bound.p, (size_t)np * sizeof(double), cudaMemcpyDeviceToHost, st), "set_transitions: read bounds");
+        CU(cudaStreamSynchronize(st), "set_transitions: sync");
+        double sumB = 0.0;
+        for (double b : bound) {
+            if (!std::isfinite(b)) return fail(ctx, SCARF_EINVAL, "set_transitions: NaN/Inf produced by T (device input not finite?)");
+            sumB += b;
+        }
+        const double thr = np > 0 ? ctx->screen_tol * sumB / (double)np : 0.0;
+        std::vector<unsigned long long> src, dst;
+        std::vector<int> nb;
+        long long kept_per_class[kNClasses] = {};
+        std::vector<long long> kept_idx;
+        kept_idx.reserve((size_t)np);
+        for (int c = 0; c < kNClasses; ++c)
+            for (long long i = hs.class_first[c]; i < hs.class_first[c + 1]; ++i)
+                if (bound[(size_t)i] > 0.0 && bound[(size_t)i] >= thr) {
+                    kept_idx.push_back(i);
+                    ++kept_per_class[c];
+                }
+        const long long n_kept = (long long)kept_idx.size();
+        if (n_kept < np) {
+            src.resize((size_t)n_kept); dst.resize((size_t)n_kept); nb.resize((size_t)n_kept);
+            CU(ctx->d_src.ensure(std::max<size_t>(64, (size_t)n_kept * 8)), "set_transitions: alloc");
+            CU(ctx->d_dst.ensure(std::max<size_t>(64, (size_t)n_kept * 8)), "set_transitions: alloc");
+            CU(ctx->d_nb.ensure(std::max<size_t>(64, (size_t)n_kept * 4)), "set_transitions: alloc");
+            for (size_t it = 0; it < tiles.size(); ++it) {
+                TileStream& t = tiles[it];
+                unsigned long long off = 0, new_off[kNClasses];
+                for (int c = 0; c < kNClasses; ++c) {
+                    new_off[c] = off;
+                    off += (unsigned long long)kept_per_class[c] * t.cls[c].rec_bytes;
+                }
+                size_t k = 0;
+                for (int c = 0; c < kNClasses; ++c) {
+                    long long j = 0;
+                    for (; k < kept_idx.size() && kept_idx[k] < hs.class_first[c + 1]; ++k, ++j) {
+                        src[k] = t.cls[c].off + (unsigned long long)(kept_idx[k] - hs.class_first[c]) * t.cls[c].rec_bytes;
+                        dst[k] = new_off[c] + (unsigned long long)j * t.cls[c].rec_bytes;
+                        nb[k] = t.cls[c].rec_bytes;
+                    }
+                }
+                CU(ctx->packed[it].ensure(std::max<unsigned long long>(64, off)), "set_transitions: alloc packed");
+                CU(cudaMemcpyAsync(ctx->d_src.p, src.data(), (size_t)n_kept * 8, cudaMemcpyHostToDevice, st), "set_transitions: upload");
+                CU(cudaMemcpyAsync(ctx->d_dst.p, dst.data(), (size_t)n_kept * 8, cudaMemcpyHostToDevice, st), "set_transitions: upload");
+                CU(cudaMemcpyAsync(ctx->d_nb.p, nb.data(), (size_t)n_kept * 4, cudaMemcpyHostToDevice, st), "set_transitions: upload");
+                CU(launch_pack(static_cast<const char*>(ctx->staging[it].p), static_cast<char*>(ctx->packed[it].p),
+                               static_cast<const unsigned long long*>(ctx->d_src.p), static_cast<const unsigned long long*>(ctx->d_dst.p),
+                               static_cast<const int*>(ctx->d_nb.p), n_kept, st), "set_transitions: pack kernel");
+                CU(cudaStreamSynchronize(st), "set_transitions: sync");  // src/dst/nb host vectors are reused per tile
+                t.base = static_cast<char*>(ctx->packed[it].p);
+                t.bytes = off;
+                for (int c = 0; c < kNClasses; ++c) {
+                    t.cls[c].n = kept_per_class[c];
+                    t.cls[c].off = new_off[c];
+                }
+            }
+        }
+        if (ctx->timing) {
+            CU(cudaEventRecord(ctx->ev1, st), "set_transitions: event");
+            CU(cudaEventSynchronize(ctx->ev1), "set_transitions: event sync");
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
+            ctx->st.last_fold_ms = ms;
+        }
+        ctx->tiles = tiles;
+        ctx->n_states = n_states;
+        scarf_stats& s = ctx->st;
+        s.n_states = n_states;
+        s.n_pairs_kept = n_kept;
+        s.n_herm_kept = 0; s.slots_per_q = 0.0; s.stream_bytes = 0.0;
+        for (int c = 0; c < kNClasses; ++c) {
+            s.pairs_kept_per_class[c] = kept_per_class[c];
+            s.n_herm_kept += kept_per_class[c] * nherm(c);
+            s.slots_per_q += (double)kept_per_class[c] * ((double)n_states * kW[c] + kCtr * (double)tiles.size());
+        }
+        for (const auto& t : tiles) s.stream_bytes += (double)t.bytes;
+        s.evals_per_q = (double)n_kept * (double)n_states;
+        s.last_fold_launches = (int32_t)(tiles.size() * (n_kept < np ? 2 : 1));
+        ctx->have_T = true;
+        return SCARF_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(ctx, SCARF_ENOMEM, "set_transitions: out of host memory");
+    } catch (...) {
+        return fail(ctx, SCARF_EINVAL, "set_transitions: unexpected exception");
+    }
+}
+
+int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out)
+{
+    if (!ctx) return SCARF_EINVAL;
+    if (ctx->host_only) return fail(ctx, SCARF_ENODEVICE, "form_factors: host-only context; there is no CPU fallback");
+    if (!ctx->have_T) return fail(ctx, SCARF_ESTATE, "form_factors: set_basis and set_transitions first");
+    if (n_q < 0) return fail(ctx, SCARF_EINVAL, "form_factors: n_q < 0");
+    if (n_q == 0) return SCARF_OK;
+    if (!q || !out) return fail(ctx, SCARF_EINVAL, "form_factors: null q or out");
+    try {
+        CU(cudaSetDevice(ctx->device), "form_factors");
+        cudaStream_t st = ctx->stream;
+        const size_t qbytes = (size_t)n_q * 3 * sizeof(double);
+        const size_t obytes = (size_t)ctx->n_states * (size_t)n_q * 2 * sizeof(double);
+        const double* dq = q;
+        double* dout = out;
+        const bool q_host = !is_device_ptr(q), out_host = !is_device_ptr(out);
+        if (q_host) {
+            if (!all_finite(q, (size_t)n_q * 3)) return fail(ctx, SCARF_EINVAL, "form_factors: NaN/Inf in q");
+            CU(ctx->d_q.ensure(qbytes), "form_factors: alloc q");
+            CU(cudaMemcpyAsync(ctx->d_q.p, q, qbytes, cudaMemcpyHostToDevice, st), "form_factors: upload q");
+            dq = static_cast<const double*>(ctx->d_q.p);
+        }
+        if (out_host) {
+            CU(ctx->d_out.ensure(obytes), "form_factors: alloc out");
+            dout = static_cast<double*>(ctx->d_out.p);
+        }
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "form_factors: event");
+        int launches = 0;
+        for (const TileStream& t : ctx->tiles) {
+            bool first = true;
+            for (int L = 0; L < kNClasses; ++L) {
+                if (t.cls[L].n <= 0) continue;
+                CU(launch_ff_v0(L, t, dq, n_q, dout, first ? 0 : 1, st), "form_factors: kernel");
+                first = false;
+                ++launches;
+            }
+            if (first)  // no pair survived (T == 0): the answer is exactly zero
+                CU(cudaMemsetAsync(dout + (size_t)t.s0 * n_q * 2, 0, (size_t)t.ns_real * n_q * 2 * sizeof(double), st), "form_factors: memset");
+        }
+        ctx->st.last_kernel_launches = launches;
+        if (ctx->timing) {
+            CU(cudaEventRecord(ctx->ev1, st), "form_factors: event");
+            CU(cudaEventSynchronize(ctx->ev1), "form_factors: event sync");
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
+            ctx->st.last_kernel_ms = ms;
+        }
+        if (out_host) {
+            CU(cudaMemcpyAsync(out, dout, obytes, cudaMemcpyDeviceToHost, st), "form_factors: download out");
+            CU(cudaStreamSynchronize(st), "form_factors: sync");
+        } else if (q_host) {
+            CU(cudaStreamSynchronize(st), "form_factors: sync");  // pageable q must not be reused before the copy ends
+        }
+        return SCARF_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(ctx, SCARF_ENOMEM, "form_factors: out of host memory");
+    } catch (...) {
+        return fail(ctx, SCARF_EINVAL, "form_factors: unexpected exception");
+    }
+}
+
+int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out)
+{
+    if (!ctx || !out) return SCARF_EINVAL;
+    *out = ctx->st;
+    return SCARF_OK;
+}
+
+const char* scarf_last_error(const scarf_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int scarf_fp64_peak(int device, double* dfma_per_s, double* sm_clock_mhz)
+{
+    if (!dfma_per_s || !sm_clock_mhz) return SCARF_EINVAL;
+    int n = 0;
+    if (cudaGetDeviceCount(&n) != cudaSuccess || device < 0 || device >= n) {
+        cudaGetLastError();
+        return SCARF_ENODEVICE;
+    }
+    if (cudaSetDevice(device) != cudaSuccess) return SCARF_ECUDA;
+    return run_fp64_peak(dfma_per_s, sm_clock_mhz) == cudaSuccess ? SCARF_OK : SCARF_ECUDA;
+}
+
+int scarf_host_hermite_E(int la, int lb, double alpha, double beta, double Ax, double Bx, double* E_out)
+{
+    if (la < 0 || lb < 0 || la > kMaxL || lb > kMaxL || !(alpha > 0) || !(beta > 0) || !E_out) return SCARF_EINVAL;
+    const double p = alpha + beta, P = (alpha * Ax + beta * Bx) / p;
+    hermite_E_axis(la, lb, p, P - Ax, P - Bx, std::exp(-alpha * beta / p * (Ax - Bx) * (Ax - Bx)), E_out);
+    return SCARF_OK;
+}
+
+int scarf_host_shell_norms(int l, int nprim, const double* exponents, const double* coeffs, double* c_out)
+{
+    if (!exponents || !coeffs || !c_out || l < 0 || l > kMaxL || nprim < 1) return SCARF_EINVAL;
+    std::vector<double> cp((size_t)nprim);
+    int rc = shell_coefficients(l, nprim, exponents, coeffs, cp.data());
+    if (rc != SCARF_OK) return rc;
+    for (int c = 0; c < ncart(l); ++c)
+        for (int k = 0; k < nprim; ++k) c_out[c * nprim + k] = cp[(size_t)k] * component_factor(l, c);
+    return SCARF_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,212 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same seeded
+inputs.  Tolerance (BASELINE.json north_star): max_q |f_gpu - f_oracle| <= 1e-10 * max_q |f_oracle| per state.
+
+Inputs are generated with the ORACLE's overlap (no oracle input ever comes from the CUDA path).
+Small configs are compared on their full grids; configs 3-5 run on the GPU at full size, in the launch
+configuration bench.py times, and are compared on a seeded sample of q-points the oracle evaluates one by one,
+plus properties that hold at any size (f(-q) = conj f(q), host/device pointer agreement).
+"""
+import numpy as np
+import pytest
+
+from paper_2512_18010_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked tests must run on the B200 box")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def Scarf():
+    from paper_2512_18010_b200 import Scarf as S
+    return S
+
+
+def gpu_form_factors(Scarf, torch, basis, T, q, **opts):
+    with Scarf(0) as sc:
+        for k, v in opts.items():
+            sc.set_option(k, v)
+        sc.set_basis(basis)
+        sc.set_transitions(torch.as_tensor(T, dtype=torch.float64, device="cuda").contiguous())
+        qd = torch.as_tensor(q, dtype=torch.float64, device="cuda").contiguous()
+        f = sc.form_factors(qd)
+        torch.cuda.synchronize()
+        return f.cpu().numpy(), sc.stats()
+
+
+def assert_parity(f_gpu, f_ref, tol=TOL):
+    assert f_gpu.shape == f_ref.shape
+    for s in range(f_ref.shape[0]):
+        scale = np.max(np.abs(f_ref[s]))
+        err = np.max(np.abs(f_gpu[s] - f_ref[s]))
+        assert err <= tol * scale, f"state {s}: max err {err:.3e} > {tol:g} * {scale:.3e}"
+
+
+def test_config1_full_grid(oracle_mod, Scarf, torch_cuda):
+    w = W.make_workload(1, oracle_mod.overlap)
+    f_ref = oracle_mod.form_factors(w.basis, w.T, w.q)
+    f_gpu, st = gpu_form_factors(Scarf, torch_cuda, w.basis, w.T, w.q)
+    assert_parity(f_gpu, f_ref)
+    assert st["n_pairs_all"] == 171 and st["nbf"] == 10
+
+
+def test_config2_strided_grid(oracle_mod, Scarf, torch_cuda):
+    w = W.make_workload(2, oracle_mod.overlap)
+    f_gpu, st = gpu_form_factors(Scarf, torch_cuda, w.basis, w.T, w.q)
+    idx = W.sample_q_indices(w.n_q, 300, seed=2)
+    f_ref = oracle_mod.form_factors(w.basis, w.T, w.q[idx])
+    assert_parity(f_gpu[:, idx], f_ref)
+    # properties on the full grid: the grid is symmetric under q -> -q (index reversal)
+    np.testing.assert_allclose(f_gpu[:, ::-1], np.conj(f_gpu), rtol=0, atol=1e-12 * np.max(np.abs(f_gpu)))
+
+
+@pytest.mark.parametrize("config,n_sample", [(3, 160), (4, 40), (5, 160)])
+def test_full_size_sampled(oracle_mod, Scarf, torch_cuda, config, n_sample):
+    w = W.make_workload(config, oracle_mod.overlap)
+    f_gpu, st = gpu_form_factors(Scarf, torch_cuda, w.basis, w.T, w.q)
+    assert f_gpu.shape == (12, w.n_q)
+    idx = W.sample_q_indices(w.n_q, n_sample, seed=config)
+    f_ref = oracle_mod.form_factors(w.basis, w.T, w.q[idx])
+    assert_parity(f_gpu[:, idx], f_ref)
+    assert np.all(np.isfinite(f_gpu.view(np.float64)))
+    if w.grid["kind"] == "cartesian":
+        np.testing.assert_allclose(f_gpu[:, ::-1], np.conj(f_gpu), rtol=0, atol=1e-12 * np.max(np.abs(f_gpu)))
+
+
+def test_unscreened_equals_screened(oracle_mod, Scarf, torch_cuda):
+    """screen_tol = 0 keeps every pair; the default screen must change nothing at the 1e-10 level."""
+    w = W.make_workload(2, oracle_mod.overlap)
+    q = w.q[::211]
+    f_a, st_a = gpu_form_factors(Scarf, torch_cuda, w.basis, w.T, q, screen_tol=0.0)
+    f_b, st_b = gpu_form_factors(Scarf, torch_cuda, w.basis, w.T, q)
+    assert st_a["n_pairs_kept"] >= st_b["n_pairs_kept"]
+    assert np.max(np.abs(f_a - f_b)) <= 1e-13 * np.max(np.abs(f_a))
+    f_ref = oracle_mod.form_factors(w.basis, w.T, q)
+    assert_parity(f_a, f_ref)
+
+
+@pytest.mark.parametrize("n_states", [1, 2, 3, 5, 7, 12, 13, 25])
+def test_state_counts_and_tiles(oracle_mod, Scarf, torch_cuda, n_states):
+    """State tiles: padded tile sizes and more than one tile of 12."""
+    w = W.make_workload(1, oracle_mod.overlap)
+    rng = np.random.default_rng(n_states)
+    T = rng.normal(size=(n_states, w.basis.nbf, w.basis.nbf))
+    q = w.q[::13]
+    f_ref = oracle_mod.form_factors(w.basis, T, q)
+    f_gpu, _ = gpu_form_factors(Scarf, torch_cuda, w.basis, T, q)
+    assert_parity(f_gpu, f_ref)
+
+
+@pytest.mark.parametrize("n_q", [1, 2, 31, 33, 127, 129, 257, 1000])
+def test_ragged_q_counts(oracle_mod, Scarf, torch_cuda, n_q):
+    w = W.make_workload(1, oracle_mod.overlap)
+    rng = np.random.default_rng(n_q)
+    q = rng.uniform(-5, 5, size=(n_q, 3))
+    q[0] = 0.0                                  # q = 0 exactly: f = g Tr(T S) = 0
+    f_ref = oracle_mod.form_factors(w.basis, w.T, q)
+    f_gpu, _ = gpu_form_factors(Scarf, torch_cuda, w.basis, w.T, q)
+    scale = max(np.max(np.abs(f_ref)), 1e-3)
+    assert np.max(np.abs(f_gpu - f_ref)) <= TOL * scale
+    assert abs(f_gpu[0, 0]) < 1e-13
+
+
+def test_high_l_classes(oracle_mod, Scarf, torch_cuda):
+    """d and f shells on two centres: classes L = 0..6 all populated."""
+    from tests.test_oracle_pins import mk_basis
+    rng = np.random.default_rng(4)
+    sh = lambda at: [(at, 0, [2.1, 0.4], [0.5, 0.6]), (at, 1, [1.3, 0.3], [0.7, 0.5]), (at, 2, [0.9], [1.0]), (at, 3, [0.7], [1.0])]
+    b = mk_basis([[0.1, 0.2, -0.9], [0.3, -0.4, 1.0]], sh(0) + sh(1))
+    T = rng.normal(size=(3, b.nbf, b.nbf))
+    q = rng.uniform(-6, 6, size=(200, 3))
+    f_ref = oracle_mod.form_factors(b, T, q)
+    f_gpu, st = gpu_form_factors(Scarf, torch_cuda, b, T, q)
+    assert all(n > 0 for n in st["pairs_kept_per_class"])
+    assert_parity(f_gpu, f_ref)
+
+
+def test_large_q_and_far_atoms(oracle_mod, Scarf, torch_cuda):
+    """Large phases q.P (argument reduction of sincos) and strong Gaussian damping (exp underflow)."""
+    from tests.test_oracle_pins import mk_basis
+    rng = np.random.default_rng(8)
+    b = mk_basis([[40.0, -35.0, 20.0], [41.5, -34.0, 21.0]],
+                 [(0, 0, [900.0, 3.0], [0.5, 0.6]), (0, 1, [50.0], [1.0]), (1, 0, [0.2], [1.0]), (1, 2, [1.1], [1.0])])
+    T = rng.normal(size=(2, b.nbf, b.nbf))
+    q = rng.uniform(-60, 60, size=(300, 3))
+    f_ref = oracle_mod.form_factors(b, T, q)
+    f_gpu, _ = gpu_form_factors(Scarf, torch_cuda, b, T, q)
+    assert_parity(f_gpu, f_ref)
+
+
+def test_host_and_device_pointers_agree(oracle_mod, Scarf, torch_cuda):
+    torch = torch_cuda
+    w = W.make_workload(1, oracle_mod.overlap)
+    q = w.q[::7].copy()
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(w.T)                                  # host T
+        f_host = sc.form_factors(q).copy()                       # host q, host out
+        qd = torch.as_tensor(q, device="cuda")
+        f_dev = sc.form_factors(qd).cpu().numpy()                # device q, device out
+        out_pinned = torch.empty((1, q.shape[0], 2), dtype=torch.float64).pin_memory()
+        f_mixed = sc.form_factors(qd, out=out_pinned).numpy().copy()   # device q, pinned host out
+    assert np.array_equal(f_host, f_dev) and np.array_equal(f_host, f_mixed)
+    assert_parity(f_host, oracle_mod.form_factors(w.basis, w.T, q))
+
+
+def test_repeated_calls_and_prefactor(oracle_mod, Scarf, torch_cuda):
+    w = W.make_workload(2, oracle_mod.overlap)
+    q = w.q[::997]
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(w.T[:4])
+        f4 = sc.form_factors(q).copy()
+        sc.set_transitions(w.T)                                  # new stack on the same basis
+        f12 = sc.form_factors(q).copy()
+        f12b = sc.form_factors(q).copy()                         # repeat
+        sc.set_option("prefactor", 1.0)
+        sc.set_transitions(w.T)
+        f12_g1 = sc.form_factors(q).copy()
+    assert np.array_equal(f12, f12b)
+    assert np.array_equal(f12[:4], f4)
+    np.testing.assert_allclose(f12_g1, 0.5 * f12, rtol=1e-14, atol=0)
+    assert_parity(f12, oracle_mod.form_factors(w.basis, w.T, q))
+
+
+def test_zero_T_and_empty_q(oracle_mod, Scarf, torch_cuda):
+    w = W.make_workload(1, oracle_mod.overlap)
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(np.zeros_like(w.T))
+        f = sc.form_factors(w.q[:100])
+        assert np.all(f == 0)
+        assert sc.form_factors(np.zeros((0, 3))).shape == (1, 0)
+
+
+def test_error_paths(oracle_mod, Scarf, torch_cuda):
+    from paper_2512_18010_b200.binding import ScarfError, SCARF_ESTATE, SCARF_EINVAL
+    w = W.make_workload(1, oracle_mod.overlap)
+    with Scarf(0) as sc:
+        with pytest.raises(ScarfError) as e:
+            sc.n_states = 1
+            sc.form_factors(w.q[:4])
+        assert e.value.code == SCARF_ESTATE
+        sc.set_basis(w.basis)
+        bad = w.T.copy()
+        bad[0, 1, 2] = np.nan
+        with pytest.raises(ScarfError) as e:
+            sc.set_transitions(bad)
+        assert e.value.code == SCARF_EINVAL
+        sc.set_transitions(w.T)
+        qbad = w.q[:4].copy()
+        qbad[2, 1] = np.inf
+        with pytest.raises(ScarfError) as e:
+            sc.form_factors(qbad)
+        assert e.value.code == SCARF_EINVAL
