@@ -174,8 +174,10 @@ def test_repeated_calls_and_prefactor(oracle_mod, Scarf, torch_cuda):
         sc.set_option("prefactor", 1.0)
         sc.set_transitions(w.T)
         f12_g1 = sc.form_factors(q).copy()
-    assert np.array_equal(f12, f12b)
-    assert np.array_equal(f12[:4], f4)
+    assert np.array_equal(f12, f12b)                             # same inputs, same launch: bit-reproducible
+    # 4 states vs 12 states: another state tile (other kernel instantiation, other screened pair set), so
+    # only agreement to round-off is guaranteed
+    assert np.max(np.abs(f12[:4] - f4)) <= 1e-13 * np.max(np.abs(f12))
     np.testing.assert_allclose(f12_g1, 0.5 * f12, rtol=1e-14, atol=0)
     assert_parity(f12, oracle_mod.form_factors(w.basis, w.T, q))
 
