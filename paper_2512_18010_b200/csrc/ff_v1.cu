@@ -1,0 +1,326 @@
+// ff_v1.cu — S4, the tuned hot kernel (Eq. (48)).
+//
+//   f_s(q) = sum_pairs e^{-q^2/4p} (cos q.P + i sin q.P) (A_s(q) + i B_s(q)),
+//   A_s = sum_{n even} D^s_h q^h,  B_s = sum_{n odd} D^s_h q^h         (i^n folded into D by the fold kernel)
+//
+// Work decomposition.  The grid is n_tiles x n_chunks CTAs.  A tile is kTile = 2 x kThreads q-points (every
+// thread keeps TWO q-points and all NS <= 12 states of both in registers: 4 NS FP64 accumulators), a chunk is a
+// cost-balanced contiguous slice of the class-sorted pair stream (it may span classes).  With one chunk the CTA
+// stores straight into `out`; with several, each chunk stores a partial [chunk][state][q] and a second kernel
+// adds the partials in chunk order (deterministic, no atomics).  Chunks exist only to give the block scheduler
+// ~20 waves of equal-cost CTAs, so that the tail of the last wave is a few per cent of the run.
+//
+// Operand delivery.  Every polynomial FMA needs its own warp-uniform coefficient.  The records of the chunk
+// are staged through shared memory by 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx), kStages
+// deep, issued by one thread; all threads then read them with broadcast LDS.128 (two coefficients per load,
+// each used for both q-points of the thread => 4 DFMA per LDS.128, a quarter of the LDS issue rate that one
+// coefficient per load and per q-point would need).  All loops over (state, Hermite index) are unrolled at
+// compile time from the class L, so monomials and accumulators are plain registers.
+//
+// FP64 budget per (q, pair): 4 (arguments) + 15 (e^{-x}) + 19 (sincos) + 2 = 40 issue slots, and per
+// (q, pair, state) n_herm + 3 (2 for L = 0) — the work model of DESIGN.md.
+#include <utility>
+
+#include "ff_math.cuh"
+#include "kernels.cuh"
+
+namespace scarf {
+
+namespace {
+
+constexpr int kThreads = 128;
+constexpr int kNQ = 2;                       // q-points per thread
+constexpr int kTile = kThreads * kNQ;        // q-points per CTA
+constexpr int kStages = 3;
+constexpr int kStageBytes = 8192;            // >= the largest record (L = 6, NS = 12: 8096 B)
+
+template <int I> using IC = std::integral_constant<int, I>;
+template <class F, int... Is>
+__device__ __forceinline__ void static_for_impl(F&& f, std::integer_sequence<int, Is...>) { (f(IC<Is>{}), ...); }
+template <int N, class F>
+__device__ __forceinline__ void static_for(F&& f) { static_for_impl(f, std::make_integer_sequence<int, N>{}); }
+
+// total degree n = t+u+v of Hermite index h (enumeration: n ascending; see kernels.cuh)
+__host__ __device__ constexpr int hdeg(int h)
+{
+    int n = 0;
+    while (nherm(n) <= h) ++n;
+    return n;
+}
+// exponents (t,u,v) of Hermite index h
+__host__ __device__ constexpr int hexp(int h, int axis)
+{
+    const int n = hdeg(h);
+    int idx = n == 0 ? 0 : nherm(n - 1);
+    for (int t = n; t >= 0; --t)
+        for (int u = n - t; u >= 0; --u) {
+            if (idx == h) return axis == 0 ? t : (axis == 1 ? u : n - t - u);
+            ++idx;
+        }
+    return 0;
+}
+// index of the monomial with one power of `axis` less (parent in the recurrence mono[h] = mono[parent] * q_axis)
+__host__ __device__ constexpr int hindex(int t, int u, int v)
+{
+    const int n = t + u + v;
+    int idx = n == 0 ? 0 : nherm(n - 1);
+    for (int tt = n; tt >= 0; --tt)
+        for (int uu = n - tt; uu >= 0; --uu) {
+            if (tt == t && uu == u) return idx;
+            ++idx;
+        }
+    return 0;
+}
+
+// ---- mbarrier / bulk-copy wrappers (PTX ISA: mbarrier, cp.async.bulk) -------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+struct Pipe {               // stage ring shared by all class segments of the CTA
+    unsigned char* buf;     // kStages x kStageBytes
+    uint64_t* full;         // kStages mbarriers
+    uint32_t it;            // stages consumed so far (all threads keep the same count)
+};
+
+// ---- one record: transcendental part, then the (state, h) loop --------------------------------------------
+template <int L, int NS, int NQA, int jq0>
+__device__ __forceinline__ void consume_record(const double2* __restrict__ r2, const double (&qv)[kNQ][4],
+                                               const double (&mono)[NQA][nherm(L)],
+                                               double (&re)[kNQ][NS], double (&im)[kNQ][NS])
+{
+    constexpr int NH = nherm(L), N = NS * NH;
+    const double2 h0 = r2[0], h1 = r2[1];   // Px, Py | Pz, 1/(4p)
+    double gc[NQA], gs[NQA];
+#pragma unroll
+    for (int j = 0; j < NQA; ++j) {
+        const double* qj = qv[jq0 + j];
+        const double ph = fma(qj[0], h0.x, fma(qj[1], h0.y, qj[2] * h1.x));
+        const double e = exp_neg(qj[3] * h1.y);
+        double sn, cs;
+        sincos_fast(ph, sn, cs);
+        gc[j] = e * cs;
+        gs[j] = e * sn;
+    }
+    const double2* __restrict__ D2 = r2 + 2;
+    double A[NQA], B[NQA];
+    static_for<(N + 1) / 2>([&](auto i2c) {
+        constexpr int i2 = decltype(i2c)::value;
+        const double2 c = D2[i2];
+        static_for<2>([&](auto halfc) {
+            constexpr int half = decltype(halfc)::value;
+            constexpr int i = 2 * i2 + half;
+            if constexpr (i < N) {
+                constexpr int s = i / NH, h = i % NH, n = hdeg(h);
+                const double cv = half ? c.y : c.x;
+#pragma unroll
+                for (int j = 0; j < NQA; ++j) {
+                    if constexpr (h == 0) A[j] = cv;
+                    else if constexpr (h == 1) B[j] = cv * mono[j][1];
+                    else if constexpr (n & 1) B[j] = fma(cv, mono[j][h], B[j]);
+                    else A[j] = fma(cv, mono[j][h], A[j]);
+                }
+                if constexpr (h == NH - 1) {
+#pragma unroll
+                    for (int j = 0; j < NQA; ++j) {
+                        re[jq0 + j][s] = fma(gc[j], A[j], re[jq0 + j][s]);
+                        im[jq0 + j][s] = fma(gs[j], A[j], im[jq0 + j][s]);
+                        if constexpr (L > 0) {
+                            re[jq0 + j][s] = fma(-gs[j], B[j], re[jq0 + j][s]);
+                            im[jq0 + j][s] = fma(gc[j], B[j], im[jq0 + j][s]);
+                        }
+                    }
+                }
+            }
+        });
+    });
+}
+
+template <int L, int NQA, int jq0>
+__device__ __forceinline__ void make_monomials(const double (&qv)[kNQ][4], double (&mono)[NQA][nherm(L)])
+{
+    constexpr int NH = nherm(L);
+#pragma unroll
+    for (int j = 0; j < NQA; ++j) {
+        mono[j][0] = 1.0;
+        static_for<NH - 1>([&](auto hc) {
+            constexpr int h = decltype(hc)::value + 1;
+            constexpr int t = hexp(h, 0), u = hexp(h, 1), v = hexp(h, 2);
+            // peel one power off the first non-zero axis
+            constexpr int ax = t > 0 ? 0 : (u > 0 ? 1 : 2);
+            constexpr int parent = hindex(t - (ax == 0), u - (ax == 1), v - (ax == 2));
+            mono[j][h] = parent == 0 ? qv[jq0 + j][ax] : mono[j][parent] * qv[jq0 + j][ax];
+        });
+    }
+}
+
+// ---- one class segment of the chunk: stream its records through the stage ring ---------------------------
+template <int L, int NS>
+__device__ __forceinline__ void run_class(Pipe& pp, const char* __restrict__ seg, int n_rec, const double (&qv)[kNQ][4],
+                                          double (&re)[kNQ][NS], double (&im)[kNQ][NS])
+{
+    constexpr int REC = rec_doubles(L, NS) * 8;
+    constexpr int SREC = kStageBytes / REC;              // records per stage (>= 1)
+    static_assert(SREC >= 1, "record larger than a stage");
+    constexpr int NQA = L <= 3 ? kNQ : 1;                // q-points evaluated together (register budget)
+    const int n_st = (n_rec + SREC - 1) / SREC;
+    const bool producer = threadIdx.x == 0;
+    auto issue = [&](int j) {                            // stage j of this segment into ring slot (it0 + j) % kStages
+        const int slot = (int)((pp.it + (uint32_t)j) % kStages);
+        const int first = j * SREC, cnt = min(SREC, n_rec - first);
+        const uint32_t bytes = (uint32_t)cnt * REC;
+        mbar_expect_tx(&pp.full[slot], bytes);
+        bulk_g2s(pp.buf + slot * kStageBytes, seg + (size_t)first * REC, bytes, &pp.full[slot]);
+    };
+    // all threads have left the previous segment's stages
+    __syncthreads();
+    if (producer)
+        for (int j = 0; j < min(kStages, n_st); ++j) issue(j);
+    // `pp.it` is only advanced after the loop so that issue() sees the segment's base
+    for (int j = 0; j < n_st; ++j) {
+        const uint32_t g = pp.it + (uint32_t)j;
+        const int slot = (int)(g % kStages);
+        mbar_wait(&pp.full[slot], (g / kStages) & 1u);
+        const int cnt = min(SREC, n_rec - j * SREC);
+        const unsigned char* sp = pp.buf + slot * kStageBytes;
+        static_for<kNQ / NQA>([&](auto jc) {
+            constexpr int jq0 = decltype(jc)::value * NQA;
+            double mono[NQA][nherm(L)];
+            make_monomials<L, NQA, jq0>(qv, mono);
+#pragma unroll 1
+            for (int k = 0; k < cnt; ++k)
+                consume_record<L, NS, NQA, jq0>(reinterpret_cast<const double2*>(sp + k * REC), qv, mono, re, im);
+        });
+        __syncthreads();                                 // the slot is free again
+        if (producer && j + kStages < n_st) issue(j + kStages);
+    }
+    pp.it += (uint32_t)n_st;
+}
+
+template <int NS>
+__global__ void __launch_bounds__(kThreads, 2) ff_v1_kernel(const V1Args a)
+{
+    __shared__ __align__(128) unsigned char stage_buf[kStages * kStageBytes];
+    __shared__ __align__(8) uint64_t full_bar[kStages];
+    const int tile = (int)(blockIdx.x % (unsigned)a.n_tiles), chunk = (int)(blockIdx.x / (unsigned)a.n_tiles);
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kStages; ++s) mbar_init(&full_bar[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    Pipe pp = {stage_buf, full_bar, 0u};
+
+    double qv[kNQ][4];
+    long long iq[kNQ];
+#pragma unroll
+    for (int j = 0; j < kNQ; ++j) {
+        iq[j] = (long long)tile * kTile + j * kThreads + threadIdx.x;
+        const bool ok = iq[j] < a.n_q;
+        qv[j][0] = ok ? a.q[3 * iq[j]] : 0.0;
+        qv[j][1] = ok ? a.q[3 * iq[j] + 1] : 0.0;
+        qv[j][2] = ok ? a.q[3 * iq[j] + 2] : 0.0;
+        qv[j][3] = qv[j][0] * qv[j][0] + qv[j][1] * qv[j][1] + qv[j][2] * qv[j][2];
+    }
+    double re[kNQ][NS], im[kNQ][NS];
+#pragma unroll
+    for (int j = 0; j < kNQ; ++j)
+#pragma unroll
+        for (int s = 0; s < NS; ++s) re[j][s] = im[j][s] = 0.0;
+
+    const V1Chunk& ck = a.chunks[chunk];
+#ifndef SCARF_V1_MAXL
+#define SCARF_V1_MAXL 6
+#endif
+#define SCARF_V1_CLASS(LV)                                                                                              \
+    if (LV <= SCARF_V1_MAXL && ck.n[LV] > 0)                                                                                                   \
+        run_class<LV, NS>(pp, a.base + a.cls_off[LV] + (size_t)ck.begin[LV] * (rec_doubles(LV, NS) * 8), ck.n[LV], qv, re, im);
+    SCARF_V1_CLASS(0)
+    SCARF_V1_CLASS(1)
+    SCARF_V1_CLASS(2)
+    SCARF_V1_CLASS(3)
+    SCARF_V1_CLASS(4)
+    SCARF_V1_CLASS(5)
+    SCARF_V1_CLASS(6)
+#undef SCARF_V1_CLASS
+
+    double2* dst = reinterpret_cast<double2*>(a.dst) + (size_t)chunk * a.chunk_stride;
+#pragma unroll
+    for (int j = 0; j < kNQ; ++j)
+        if (iq[j] < a.n_q)
+#pragma unroll
+            for (int s = 0; s < NS; ++s)
+                if (s < a.ns_real) dst[(size_t)s * a.n_q + iq[j]] = make_double2(re[j][s], im[j][s]);
+}
+
+// out[s][iq] = sum_k partial[k][s][iq], k ascending.
+__global__ void __launch_bounds__(256) reduce_partials_kernel(const double2* __restrict__ part, double2* __restrict__ out,
+                                                              long long n_elem, long long chunk_stride, int n_chunks)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_elem) return;
+    double2 acc = part[i];
+    for (int k = 1; k < n_chunks; ++k) {
+        const double2 v = part[(size_t)k * chunk_stride + i];
+        acc.x += v.x;
+        acc.y += v.y;
+    }
+    out[i] = acc;
+}
+
+}  // namespace
+
+int v1_tile_q() { return kTile; }
+
+cudaError_t launch_ff_v1(int NS, const V1Args& a, cudaStream_t st)
+{
+    if (a.n_q <= 0 || a.n_chunks <= 0) return cudaSuccess;
+    const unsigned blocks = (unsigned)a.n_tiles * (unsigned)a.n_chunks;
+    switch (NS) {
+    case 1: ff_v1_kernel<1><<<blocks, kThreads, 0, st>>>(a); break;
+    case 2: ff_v1_kernel<2><<<blocks, kThreads, 0, st>>>(a); break;
+    case 4: ff_v1_kernel<4><<<blocks, kThreads, 0, st>>>(a); break;
+    case 6: ff_v1_kernel<6><<<blocks, kThreads, 0, st>>>(a); break;
+    case 8: ff_v1_kernel<8><<<blocks, kThreads, 0, st>>>(a); break;
+    case 12: ff_v1_kernel<12><<<blocks, kThreads, 0, st>>>(a); break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_reduce_partials(const double* part, double* out, long long n_elem, long long chunk_stride, int n_chunks,
+                                   cudaStream_t st)
+{
+    if (n_elem <= 0) return cudaSuccess;
+    const unsigned blocks = (unsigned)((n_elem + 255) / 256);
+    reduce_partials_kernel<<<blocks, 256, 0, st>>>(reinterpret_cast<const double2*>(part), reinterpret_cast<double2*>(out),
+                                                   n_elem, chunk_stride, n_chunks);
+    return cudaGetLastError();
+}
+
+}  // namespace scarf

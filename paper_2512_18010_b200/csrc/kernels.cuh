@@ -65,6 +65,29 @@ cudaError_t upload_tables();   // constant-memory index tables; once per process
 cudaError_t launch_ff_v0(int L, const TileStream& ts, const double* q, long long n_q, double* out, int accumulate,
                          cudaStream_t st);
 
+// v1 (ff_v1.cu): the tuned kernel.  A chunk is a cost-balanced slice of the class-sorted stream; per class c it
+// covers records [begin[c], begin[c] + n[c]) of that class.
+constexpr int kMaxChunks = 32;
+struct V1Chunk {
+    int begin[kNClasses];
+    int n[kNClasses];
+};
+struct V1Args {
+    const char* base;                       // tile stream base
+    unsigned long long cls_off[kNClasses];  // byte offset of each class's first record
+    const double* q;                        // [n_q][3]
+    long long n_q;
+    int n_tiles, n_chunks;                  // grid = n_tiles * n_chunks CTAs, chunk-major
+    int ns_real, pad;
+    double* dst;                            // n_chunks == 1: out + s0*n_q*2; else the partial buffer
+    long long chunk_stride;                 // double2 elements between the partials of consecutive chunks
+    V1Chunk chunks[kMaxChunks];
+};
+int v1_tile_q();                            // q-points per CTA
+cudaError_t launch_ff_v1(int NS, const V1Args& a, cudaStream_t st);
+cudaError_t launch_reduce_partials(const double* part, double* out, long long n_elem, long long chunk_stride,
+                                   int n_chunks, cudaStream_t st);
+
 cudaError_t run_fp64_peak(double* dfma_per_s, double* sm_clock_mhz);
 
 }  // namespace scarf

@@ -46,12 +46,14 @@ struct scarf_ctx {
     cudaStream_t stream = nullptr;
     double prefactor = 2.0, screen_tol = 1e-16;
     bool timing = false;
-    int kernel_variant = -1;  // -1 auto, 0 force v0
+    int kernel_variant = -1;  // -1 auto (v1), 0 force the baseline kernel v0
+    int n_chunks_opt = 0;     // 0 auto, else the number of stream chunks of the v1 kernel
     std::string err;
     HostSetup hs;
     bool have_basis = false, have_T = false;
     int n_states = 0;
-    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb;
+    int sm_count = 148;
+    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb, d_partial;
     std::vector<DevBuf> staging, packed;
     std::vector<TileStream> tiles;
     scarf_stats st = {};
@@ -104,10 +106,56 @@ int tile_size_for(int ns)  // smallest instantiated state tile >= ns (ns <= 12)
     return kMaxStateTile;
 }
 
+// Split the tile's class-sorted stream into <= K chunks of (nearly) equal modelled cost; a chunk may span classes.
+// Returns the number of non-empty chunks written to `out`.
+int build_chunks(const TileStream& t, int K, V1Chunk* out)
+{
+    double w[kNClasses], total = 0.0;
+    long long nrec = 0;
+    for (int c = 0; c < kNClasses; ++c) {
+        w[c] = (double)t.ns_real * kW[c] + kCtr;
+        total += (double)t.cls[c].n * w[c];
+        nrec += t.cls[c].n;
+    }
+    if (nrec == 0) return 0;
+    K = (int)std::max<long long>(1, std::min<long long>(K, nrec));
+    int k = 0;
+    double acc = 0.0;
+    std::memset(out, 0, sizeof(V1Chunk) * (size_t)K);
+    bool cur_empty = true;
+    for (int c = 0; c < kNClasses; ++c) {
+        long long rem = t.cls[c].n, pos = 0;
+        while (rem > 0) {
+            long long take = rem;
+            if (k < K - 1) {
+                const double need = total * (double)(k + 1) / (double)K - acc;
+                take = std::min<long long>(rem, (long long)std::llround(need / w[c]));
+                if (take <= 0) {
+                    if (cur_empty) take = 1;
+                    else { ++k; cur_empty = true; continue; }
+                }
+            }
+            out[k].begin[c] = (int)pos;
+            out[k].n[c] = (int)take;
+            cur_empty = false;
+            acc += (double)take * w[c];
+            pos += take; rem -= take;
+            if (k < K - 1 && acc >= total * (double)(k + 1) / (double)K - 0.5 * w[c]) { ++k; cur_empty = true; }
+        }
+    }
+    int n = 0;                                     // compact away chunks that stayed empty
+    for (int i = 0; i < K; ++i) {
+        bool any = false;
+        for (int c = 0; c < kNClasses; ++c) any = any || out[i].n[c] > 0;
+        if (any) { if (n != i) out[n] = out[i]; ++n; }
+    }
+    return n;
+}
+
 void free_device(scarf_ctx* c)
 {
     c->d_pairs.release(); c->d_E.release(); c->d_bound.release(); c->d_T.release(); c->d_q.release();
-    c->d_out.release(); c->d_src.release(); c->d_dst.release(); c->d_nb.release();
+    c->d_out.release(); c->d_src.release(); c->d_dst.release(); c->d_nb.release(); c->d_partial.release();
     for (auto& b : c->staging) b.release();
     for (auto& b : c->packed) b.release();
     c->staging.clear(); c->packed.clear(); c->tiles.clear();
@@ -138,6 +186,7 @@ int scarf_create(scarf_ctx** out, int device)
             e = upload_tables();
             if (e == cudaSuccess && device < 64) g_tables_uploaded_dev[device] = true;
         }
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device);
         if (e == cudaSuccess) e = cudaEventCreate(&ctx->ev0);
         if (e == cudaSuccess) e = cudaEventCreate(&ctx->ev1);
         if (e != cudaSuccess) {
@@ -183,6 +232,7 @@ int scarf_set_option(scarf_ctx* ctx, const char* key, double value)
         ctx->screen_tol = value;
     } else if (k == "timing") ctx->timing = value != 0.0;
     else if (k == "kernel_variant") ctx->kernel_variant = (int)value;
+    else if (k == "n_chunks") ctx->n_chunks_opt = (int)value;
     else return fail(ctx, SCARF_EINVAL, "set_option: unknown key '" + k + "'");
     return SCARF_OK;
 }
@@ -420,15 +470,51 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
         if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "form_factors: event");
         int launches = 0;
         for (const TileStream& t : ctx->tiles) {
-            bool first = true;
-            for (int L = 0; L < kNClasses; ++L) {
-                if (t.cls[L].n <= 0) continue;
-                CU(launch_ff_v0(L, t, dq, n_q, dout, first ? 0 : 1, st), "form_factors: kernel");
-                first = false;
-                ++launches;
+            long long nrec = 0;
+            for (int L = 0; L < kNClasses; ++L) nrec += t.cls[L].n;
+            double* tile_out = dout + (size_t)t.s0 * n_q * 2;
+            if (nrec == 0) {  // no pair survived (T == 0): the answer is exactly zero
+                CU(cudaMemsetAsync(tile_out, 0, (size_t)t.ns_real * n_q * 2 * sizeof(double), st), "form_factors: memset");
+                continue;
             }
-            if (first)  // no pair survived (T == 0): the answer is exactly zero
-                CU(cudaMemsetAsync(dout + (size_t)t.s0 * n_q * 2, 0, (size_t)t.ns_real * n_q * 2 * sizeof(double), st), "form_factors: memset");
+            if (ctx->kernel_variant == 0) {  // baseline form: one launch per class, accumulating into out
+                bool first = true;
+                for (int L = 0; L < kNClasses; ++L) {
+                    if (t.cls[L].n <= 0) continue;
+                    CU(launch_ff_v0(L, t, dq, n_q, dout, first ? 0 : 1, st), "form_factors: kernel");
+                    first = false;
+                    ++launches;
+                }
+                continue;
+            }
+            V1Args a = {};
+            a.base = t.base;
+            for (int L = 0; L < kNClasses; ++L) a.cls_off[L] = t.cls[L].off;
+            a.q = dq;
+            a.n_q = n_q;
+            const long long n_tiles = (n_q + v1_tile_q() - 1) / v1_tile_q();
+            if (n_tiles > 0x7fffffffLL / kMaxChunks) return fail(ctx, SCARF_EINVAL, "form_factors: n_q too large for one call");
+            a.n_tiles = (int)n_tiles;
+            // ~24 waves of CTAs (2 resident per SM) so that the ragged last wave costs a few per cent
+            long long K = ctx->n_chunks_opt > 0 ? ctx->n_chunks_opt : (24LL * 2 * ctx->sm_count + n_tiles / 2) / n_tiles;
+            K = std::max<long long>(1, std::min<long long>(K, kMaxChunks));
+            const size_t per_chunk = (size_t)t.ns_real * (size_t)n_q * 16;
+            while (K > 1 && (double)K * (double)per_chunk > 4e9) --K;  // partial buffer <= 4 GB
+            a.n_chunks = build_chunks(t, (int)K, a.chunks);
+            a.ns_real = t.ns_real;
+            if (a.n_chunks == 1) {
+                a.dst = tile_out;
+                a.chunk_stride = 0;
+                CU(launch_ff_v1(t.NS, a, st), "form_factors: kernel");
+                ++launches;
+            } else {
+                CU(ctx->d_partial.ensure((size_t)a.n_chunks * per_chunk), "form_factors: alloc partials");
+                a.dst = static_cast<double*>(ctx->d_partial.p);
+                a.chunk_stride = (long long)t.ns_real * n_q;
+                CU(launch_ff_v1(t.NS, a, st), "form_factors: kernel");
+                CU(launch_reduce_partials(a.dst, tile_out, a.chunk_stride, a.chunk_stride, a.n_chunks, st), "form_factors: reduce kernel");
+                launches += 2;
+            }
         }
         ctx->st.last_kernel_launches = launches;
         if (ctx->timing) {
