@@ -171,11 +171,9 @@ def run_reference(args):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2512_18010_b200 import Scarf, binding, workloads as W
+    from paper_2512_18010_b200 import Scarf, binding, replicas, workloads as W
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = replicas.env_rank_world_local()
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device; the product path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -233,15 +231,9 @@ def run_ours(args):
         clocks = sampler.stop() if sampler else None
         sc.set_option("timing", 0)
     step_ms = [a.elapsed_time(b) for a, b in ev]
-    total_ms = float(sum(step_ms))
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
     st = sc.stats()
     evals_per_step = st["evals_per_q"] * w.n_q
-    ms_per_step = total_ms / args.steps
-    value = world * evals_per_step / (ms_per_step * 1e-3)
+    value, ms_per_step = replicas.whole_job_value(evals_per_step, args.steps, float(sum(step_ms)), "cuda")
 
     # ---- end to end: host buffers through the C ABI (pinned q / out, pageable T), copies inside the timed region
     q_host = torch.as_tensor(w.q).pin_memory()
@@ -262,10 +254,7 @@ def run_ours(args):
             step_host()
         barrier()
         e2e_s = (time.perf_counter() - t0) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = replicas.max_over_ranks(e2e_s, "cuda")
     e2e_value = world * evals_per_step / e2e_s
     h2d = T_host.nbytes + q_host.numel() * 8
     d2h = out_host.numel() * 8
