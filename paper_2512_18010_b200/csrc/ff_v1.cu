@@ -33,6 +33,10 @@ constexpr int kNQ = 2;                       // q-points per thread
 constexpr int kTile = kThreads * kNQ;        // q-points per CTA
 constexpr int kStages = 3;
 constexpr int kStageBytes = 8192;            // >= the largest record (L = 6, NS = 12: 8096 B)
+#ifndef SCARF_V1_SWP_MAXL
+#define SCARF_V1_SWP_MAXL 2
+#endif
+constexpr int kSwpMaxL = SCARF_V1_SWP_MAXL;   // classes whose record loop is software-pipelined (-1: none)
 
 template <int I> using IC = std::integral_constant<int, I>;
 template <class F, int... Is>
@@ -109,15 +113,15 @@ struct Pipe {               // stage ring shared by all class segments of the CT
     uint32_t it;            // stages consumed so far (all threads keep the same count)
 };
 
-// ---- one record: transcendental part, then the (state, h) loop --------------------------------------------
-template <int L, int NS, int NQA, int jq0>
-__device__ __forceinline__ void consume_record(const double2* __restrict__ r2, const double (&qv)[kNQ][4],
-                                               const double (&mono)[NQA][nherm(L)],
-                                               double (&re)[kNQ][NS], double (&im)[kNQ][NS])
+// ---- one record = transcendental part (record_trans) + the (state, h) loop (record_accum) -------------------
+// The two are separate so that run_class can software-pipeline them: the exp/sincos chains of record k+1 (low
+// ILP: two dependent Horner chains per q-point) are issued in the same basic block as the 4 NS n_herm independent
+// accumulate FMAs of record k, which fill the FP64 pipe while the chains wait on their own results.
+template <int NQA, int jq0>
+__device__ __forceinline__ void record_trans(const double2* __restrict__ r2, const double (&qv)[kNQ][4],
+                                             double (&gc)[NQA], double (&gs)[NQA])
 {
-    constexpr int NH = nherm(L), N = NS * NH;
     const double2 h0 = r2[0], h1 = r2[1];   // Px, Py | Pz, 1/(4p)
-    double gc[NQA], gs[NQA];
 #pragma unroll
     for (int j = 0; j < NQA; ++j) {
         const double* qj = qv[jq0 + j];
@@ -128,6 +132,14 @@ __device__ __forceinline__ void consume_record(const double2* __restrict__ r2, c
         gc[j] = e * cs;
         gs[j] = e * sn;
     }
+}
+
+template <int L, int NS, int NQA, int jq0>
+__device__ __forceinline__ void record_accum(const double2* __restrict__ r2, const double (&mono)[NQA][nherm(L)],
+                                             const double (&gc)[NQA], const double (&gs)[NQA],
+                                             double (&re)[kNQ][NS], double (&im)[kNQ][NS])
+{
+    constexpr int NH = nherm(L), N = NS * NH;
     const double2* __restrict__ D2 = r2 + 2;
     double A[NQA], B[NQA];
     static_for<(N + 1) / 2>([&](auto i2c) {
@@ -213,9 +225,26 @@ __device__ __forceinline__ void run_class(Pipe& pp, const char* __restrict__ seg
             constexpr int jq0 = decltype(jc)::value * NQA;
             double mono[NQA][nherm(L)];
             make_monomials<L, NQA, jq0>(qv, mono);
+            double gc[NQA], gs[NQA];
+            if constexpr (L <= kSwpMaxL) {               // software-pipelined: trans(k+1) alongside accum(k)
+                record_trans<NQA, jq0>(reinterpret_cast<const double2*>(sp), qv, gc, gs);
 #pragma unroll 1
-            for (int k = 0; k < cnt; ++k)
-                consume_record<L, NS, NQA, jq0>(reinterpret_cast<const double2*>(sp + k * REC), qv, mono, re, im);
+                for (int k = 0; k < cnt - 1; ++k) {
+                    double gcn[NQA], gsn[NQA];
+                    record_trans<NQA, jq0>(reinterpret_cast<const double2*>(sp + (k + 1) * REC), qv, gcn, gsn);
+                    record_accum<L, NS, NQA, jq0>(reinterpret_cast<const double2*>(sp + k * REC), mono, gc, gs, re, im);
+#pragma unroll
+                    for (int j = 0; j < NQA; ++j) { gc[j] = gcn[j]; gs[j] = gsn[j]; }
+                }
+                record_accum<L, NS, NQA, jq0>(reinterpret_cast<const double2*>(sp + (cnt - 1) * REC), mono, gc, gs, re, im);
+            } else {
+#pragma unroll 1
+                for (int k = 0; k < cnt; ++k) {
+                    const double2* r2 = reinterpret_cast<const double2*>(sp + k * REC);
+                    record_trans<NQA, jq0>(r2, qv, gc, gs);
+                    record_accum<L, NS, NQA, jq0>(r2, mono, gc, gs, re, im);
+                }
+            }
         });
         __syncthreads();                                 // the slot is free again
         if (producer && j + kStages < n_st) issue(j + kStages);
@@ -302,11 +331,13 @@ cudaError_t launch_ff_v1(int NS, const V1Args& a, cudaStream_t st)
     if (a.n_q <= 0 || a.n_chunks <= 0) return cudaSuccess;
     const unsigned blocks = (unsigned)a.n_tiles * (unsigned)a.n_chunks;
     switch (NS) {
+#ifndef SCARF_V1_ONLY12
     case 1: ff_v1_kernel<1><<<blocks, kThreads, 0, st>>>(a); break;
     case 2: ff_v1_kernel<2><<<blocks, kThreads, 0, st>>>(a); break;
     case 4: ff_v1_kernel<4><<<blocks, kThreads, 0, st>>>(a); break;
     case 6: ff_v1_kernel<6><<<blocks, kThreads, 0, st>>>(a); break;
     case 8: ff_v1_kernel<8><<<blocks, kThreads, 0, st>>>(a); break;
+#endif
     case 12: ff_v1_kernel<12><<<blocks, kThreads, 0, st>>>(a); break;
     default: return cudaErrorInvalidValue;
     }
