@@ -77,6 +77,7 @@ typedef struct scarf_stats {
     double last_fold_ms, last_kernel_ms;       /* device time of the last S3 / S4 (CUDA events; 0 until queried)    */
     int32_t last_kernel_launches;              /* kernels launched by the last scarf_form_factors                   */
     int32_t last_fold_launches;                /* kernels launched by the last scarf_set_transitions               */
+    double last_grid_slots;                    /* FP64 issue-slot model of the last scarf_form_factors_grid call    */
 } scarf_stats;
 
 /* device >= 0: CUDA ordinal.  device < 0: host-only context (set_basis, overlap, stats work; the rest ENODEVICE). */
@@ -113,6 +114,16 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T);
 /* q [n_q][3] FP64; out [n_states][n_q][2] FP64 (re, im interleaved).  Host or device pointers, independently.
  * Any point set (no grid structure is assumed).  May be called repeatedly. */
 int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out);
+
+/* The same f_s(q) on a Cartesian PRODUCT grid q = (qx[ix], qy[iy], qz[iz]), out index (ix*ny + iy)*nz + iz:
+ * out [n_states][nx*ny*nz][2].  On such a grid the pair factor separates per axis (the V-tensor idea of Eq. (45)-(46)
+ * PAPER.md:309-316): e^{-q^2/4p} e^{iq.P} = X_P(ix) Y_P(iy) Z_P(iz).  The three factors of every kept pair are
+ * tabulated once per call (nx+ny+nz complex numbers per pair, device memory owned by the context) and the kernel
+ * spends 2 complex multiplies per (q, pair) instead of an exp and a sincos.  Axes need not be uniform or sorted.
+ * qx, qy, qz and out: host or device pointers, independently.  Results equal scarf_form_factors on the expanded
+ * point list up to FP64 round-off.  SCARF_ENOMEM if the tables would exceed 32 GB. */
+int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_t ny, const double* qy, int32_t nz,
+                            const double* qz, double* out);
 
 int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out);
 const char* scarf_last_error(const scarf_ctx* ctx);

@@ -19,7 +19,7 @@ SCARF_N_CLASSES = 2 * SCARF_MAX_L + 1
 _CODES = {-1: "EINVAL", -2: "ESTATE", -3: "ENOMEM", -4: "ECUDA", -5: "ENODEVICE"}
 
 EXPORTS = ["scarf_create", "scarf_destroy", "scarf_set_stream", "scarf_set_option", "scarf_set_basis", "scarf_nbf",
-           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_get_stats", "scarf_last_error",
+           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_get_stats", "scarf_last_error",
            "scarf_version", "scarf_fp64_peak", "scarf_host_hermite_E", "scarf_host_shell_norms"]
 
 
@@ -31,7 +31,8 @@ class ScarfStats(C.Structure):
                 ("n_herm_kept", C.c_int64), ("cart_term_pairs", C.c_int64),
                 ("stream_bytes", C.c_double), ("slots_per_q", C.c_double), ("evals_per_q", C.c_double),
                 ("last_setup_host_ms", C.c_double), ("last_fold_ms", C.c_double), ("last_kernel_ms", C.c_double),
-                ("last_kernel_launches", C.c_int32), ("last_fold_launches", C.c_int32)]
+                ("last_kernel_launches", C.c_int32), ("last_fold_launches", C.c_int32),
+                ("last_grid_slots", C.c_double)]
 
     def as_dict(self):
         d = {}
@@ -63,6 +64,7 @@ def _load():
     L.scarf_overlap.argtypes = [vp, dp]
     L.scarf_set_transitions.argtypes = [vp, C.c_int, vp]
     L.scarf_form_factors.argtypes = [vp, C.c_int64, vp, vp]
+    L.scarf_form_factors_grid.argtypes = [vp, C.c_int32, vp, C.c_int32, vp, C.c_int32, vp, vp]
     L.scarf_get_stats.argtypes = [vp, C.POINTER(ScarfStats)]
     L.scarf_last_error.argtypes = [vp]
     L.scarf_last_error.restype = C.c_char_p
@@ -233,6 +235,29 @@ class Scarf:
         if not _is_torch(out) and okeep is not out:
             raise ValueError("form_factors: out must be a C-contiguous float64 array")
         self._check(_lib.scarf_form_factors(self._h, n_q, qp, op))
+        if _is_torch(out):
+            import torch
+            return torch.view_as_complex(out.view(self.n_states, n_q, 2))
+        return out.reshape(self.n_states, n_q, 2).view(np.complex128)[..., 0]
+
+    def form_factors_grid(self, qx, qy, qz, out=None):
+        """Product grid q = (qx[ix], qy[iy], qz[iz]), point index (ix*ny + iy)*nz + iz.  qx, qy, qz: 1-D float64
+        numpy or torch (host or cuda).  Returns complex128 [n_states][nx*ny*nz] (a view of `out`)."""
+        nx, ny, nz = int(qx.shape[0]), int(qy.shape[0]), int(qz.shape[0])
+        n_q = nx * ny * nz
+        xp, xkeep = _ptr(qx, "qx", nx)
+        yp, ykeep = _ptr(qy, "qy", ny)
+        zp, zkeep = _ptr(qz, "qz", nz)
+        if out is None:
+            if _is_torch(qx):
+                import torch
+                out = torch.empty((self.n_states, n_q, 2), dtype=torch.float64, device=qx.device)
+            else:
+                out = np.empty((self.n_states, n_q, 2))
+        op, okeep = _ptr(out, "out", self.n_states * n_q * 2)
+        if not _is_torch(out) and okeep is not out:
+            raise ValueError("form_factors_grid: out must be a C-contiguous float64 array")
+        self._check(_lib.scarf_form_factors_grid(self._h, nx, xp, ny, yp, nz, zp, op))
         if _is_torch(out):
             import torch
             return torch.view_as_complex(out.view(self.n_states, n_q, 2))

@@ -1,0 +1,235 @@
+// ff_grid.cu — S4 on a Cartesian product grid (the V-tensor idea of Eq. (45)-(46)
+// on a product grid the pair factor separates per axis).
+//
+//   q = (qx[ix], qy[iy], qz[iz]);   e^{-q^2/4p} e^{iq.P} = X_P(ix) Y_P(iy) Z_P(iz),
+//   X_P(i) = exp(-qx[i]^2/4p + i qx[i] P_x)   (same for Y, Z)
+//
+//   f_s(q) = sum_pairs X_P(ix) Y_P(iy) Z_P(iz) (A_s(q) + i B_s(q))        Eq. (48)
+//
+// grid_table_kernel evaluates the (nx + ny + nz) complex factors of every kept pair once (the exp/sincos of
+// ff_math.cuh, the same functions the general kernel uses); ff_grid_kernel then needs 12 FP64 issue slots per
+// (2 q-points, pair) for the factor — YZ = Y Z, g0 = X0 YZ, g1 = X1 YZ — instead of 2 x 40, and shares the
+// (state, Hermite index) accumulate loop with the general kernel (ff_common.cuh).
+//
+// Work decomposition: a CTA owns a 4 x 8 x 8 box of the grid and one cost-balanced chunk of the pair stream.
+// Thread t holds the points (ixl, iyl, izl) and (ixl + 2, iyl, izl), izl = t % 8, iyl = (t / 8) % 8, ixl = t / 64,
+// so a warp has one ixl (X0, X1 are broadcast loads) and writes 128-byte runs along z.  Tables are laid out
+// [box][record][point-in-box], so that the slice a CTA needs for a run of records is contiguous: per stage one
+// TMA bulk copy for the records and one for each of the three table slices, all on one mbarrier.
+#include "ff_common.cuh"
+
+namespace scarf {
+
+namespace {
+
+constexpr int kThreads = 128;
+constexpr int kStages = 3;
+constexpr int kStageBytes = 8192;             // records of one stage (>= the largest record, L = 6, NS = 12)
+constexpr int kMaxRec = 32;                   // records per stage at most (bounds the table slices)
+constexpr int kXB = kGridBX * 16, kYB = kGridBY * 16, kZB = kGridBZ * 16;   // table bytes per record and box
+constexpr int kSlotBytes = kStageBytes + kMaxRec * (kXB + kYB + kZB);
+constexpr int kSmemBytes = kStages * kSlotBytes + 64;
+static_assert(kGridBX * kGridBY * kGridBZ == kThreads * kNQ, "box = 2 points per thread");
+
+struct GPipe {
+    unsigned char* buf;     // kStages slots of kSlotBytes: records | X slice | Y slice | Z slice
+    uint64_t* full;
+    uint32_t it;
+};
+
+// ---- tables -------------------------------------------------------------------------------------------------
+// one thread per (record, padded axis point); columns [0, NXp) -> X, [NXp, NXp+NYp) -> Y, rest -> Z.
+__global__ void __launch_bounds__(256) grid_table_kernel(const GridArgs a, double2* __restrict__ tx, double2* __restrict__ ty,
+                                                         double2* __restrict__ tz)
+{
+    const int NXp = a.nbx * kGridBX, NYp = a.nby * kGridBY, NZp = a.nbz * kGridBZ, ncol = NXp + NYp + NZp;
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= a.n_rec * ncol) return;
+    const long long r = idx / ncol;
+    int col = (int)(idx - r * ncol);
+    int c = 0;
+#pragma unroll
+    for (int k = 1; k < kNClasses; ++k)
+        if (r >= a.class_first[k]) c = k;
+    const double* hdr = reinterpret_cast<const double*>(a.v.base + a.v.cls_off[c] + (size_t)(r - a.class_first[c]) * a.rec_bytes[c]);
+    const double inv4p = hdr[3];
+    int axis = 0, n = a.nx, B = kGridBX;
+    const double* ax = a.qx;
+    double2* tab = tx;
+    if (col >= NXp + NYp) { axis = 2; col -= NXp + NYp; n = a.nz; B = kGridBZ; ax = a.qz; tab = tz; }
+    else if (col >= NXp) { axis = 1; col -= NXp; n = a.ny; B = kGridBY; ax = a.qy; tab = ty; }
+    double2 v = make_double2(0.0, 0.0);
+    if (col < n) {
+        const double q = ax[col];
+        const double e = exp_neg(q * q * inv4p);
+        double sn, cs;
+        sincos_fast(q * hdr[axis], sn, cs);
+        v = make_double2(e * cs, e * sn);
+    }
+    tab[((size_t)(col / B) * a.n_rec + r) * B + (col % B)] = v;
+}
+
+__device__ __forceinline__ double2 cmul(const double2 a, const double2 b)
+{
+    return make_double2(fma(a.x, b.x, -(a.y * b.y)), fma(a.x, b.y, a.y * b.x));
+}
+
+// ---- one class segment of the chunk ----------------------------------------------------------------------------
+// r0 = stream-order index of the segment's first record (row of the tables).
+template <int L, int NS>
+__device__ __forceinline__ void run_class_grid(GPipe& pp, const GridArgs& a, const char* __restrict__ seg, long long r0, int n_rec,
+                                               int bx, int by, int bz, int ixl, int iyl, int izl,
+                                               const double (&qv)[kNQ][4], double (&re)[kNQ][NS], double (&im)[kNQ][NS])
+{
+    constexpr int REC = rec_doubles(L, NS) * 8;
+    constexpr int SREC = (kStageBytes / REC) < kMaxRec ? (kStageBytes / REC) : kMaxRec;
+    static_assert(SREC >= 1, "record larger than a stage");
+    constexpr int NQA = L <= 3 ? kNQ : 1;                // q-points evaluated together (register budget)
+    const int n_st = (n_rec + SREC - 1) / SREC;
+    const bool producer = threadIdx.x == 0;
+    auto issue = [&](int j) {
+        const int slot = (int)((pp.it + (uint32_t)j) % kStages);
+        const int first = j * SREC, cnt = min(SREC, n_rec - first);
+        unsigned char* sb = pp.buf + slot * kSlotBytes;
+        const long long r = r0 + first;
+        mbar_expect_tx(&pp.full[slot], (uint32_t)cnt * (REC + kXB + kYB + kZB));
+        bulk_g2s(sb, seg + (size_t)first * REC, (uint32_t)cnt * REC, &pp.full[slot]);
+        bulk_g2s(sb + kStageBytes, a.tx + ((size_t)bx * a.n_rec + r) * kGridBX, (uint32_t)cnt * kXB, &pp.full[slot]);
+        bulk_g2s(sb + kStageBytes + kMaxRec * kXB, a.ty + ((size_t)by * a.n_rec + r) * kGridBY, (uint32_t)cnt * kYB, &pp.full[slot]);
+        bulk_g2s(sb + kStageBytes + kMaxRec * (kXB + kYB), a.tz + ((size_t)bz * a.n_rec + r) * kGridBZ, (uint32_t)cnt * kZB,
+                 &pp.full[slot]);
+    };
+    __syncthreads();                                     // all threads have left the previous segment's stages
+    if (producer)
+        for (int j = 0; j < min(kStages, n_st); ++j) issue(j);
+    for (int j = 0; j < n_st; ++j) {
+        const uint32_t g = pp.it + (uint32_t)j;
+        const int slot = (int)(g % kStages);
+        mbar_wait(&pp.full[slot], (g / kStages) & 1u);
+        const int cnt = min(SREC, n_rec - j * SREC);
+        const unsigned char* sp = pp.buf + slot * kSlotBytes;
+        const double2* Xs = reinterpret_cast<const double2*>(sp + kStageBytes);
+        const double2* Ys = reinterpret_cast<const double2*>(sp + kStageBytes + kMaxRec * kXB);
+        const double2* Zs = reinterpret_cast<const double2*>(sp + kStageBytes + kMaxRec * (kXB + kYB));
+        static_for<kNQ / NQA>([&](auto jc) {
+            constexpr int jq0 = decltype(jc)::value * NQA;
+            double mono[NQA][nherm(L)];
+            make_monomials<L, NQA, jq0>(qv, mono);
+#pragma unroll 1
+            for (int k = 0; k < cnt; ++k) {
+                const double2 yz = cmul(Ys[k * kGridBY + iyl], Zs[k * kGridBZ + izl]);
+                double gc[NQA], gs[NQA];
+#pragma unroll
+                for (int jj = 0; jj < NQA; ++jj) {
+                    const double2 gq = cmul(Xs[k * kGridBX + ixl + 2 * (jq0 + jj)], yz);
+                    gc[jj] = gq.x;
+                    gs[jj] = gq.y;
+                }
+                record_accum<L, NS, NQA, jq0>(reinterpret_cast<const double2*>(sp + k * REC), mono, gc, gs, re, im);
+            }
+        });
+        __syncthreads();                                 // the slot is free again
+        if (producer && j + kStages < n_st) issue(j + kStages);
+    }
+    pp.it += (uint32_t)n_st;
+}
+
+template <int NS>
+__global__ void __launch_bounds__(kThreads, 2) ff_grid_kernel(const GridArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + kStages * kSlotBytes);
+    const int tile = (int)(blockIdx.x % (unsigned)a.v.n_tiles), chunk = (int)(blockIdx.x / (unsigned)a.v.n_tiles);
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kStages; ++s) mbar_init(&full_bar[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    GPipe pp = {smem, full_bar, 0u};
+
+    const int bz = tile % a.nbz, by = (tile / a.nbz) % a.nby, bx = tile / (a.nbz * a.nby);
+    const int izl = threadIdx.x % kGridBZ, iyl = (threadIdx.x / kGridBZ) % kGridBY, ixl = threadIdx.x / (kGridBZ * kGridBY);
+    const int iy = by * kGridBY + iyl, iz = bz * kGridBZ + izl;
+    double qv[kNQ][4];
+    long long iq[kNQ];
+#pragma unroll
+    for (int j = 0; j < kNQ; ++j) {
+        const int ix = bx * kGridBX + ixl + 2 * j;
+        const bool ok = ix < a.nx && iy < a.ny && iz < a.nz;
+        iq[j] = ok ? ((long long)ix * a.ny + iy) * a.nz + iz : -1;
+        qv[j][0] = ok ? a.qx[ix] : 0.0;
+        qv[j][1] = ok ? a.qy[iy] : 0.0;
+        qv[j][2] = ok ? a.qz[iz] : 0.0;
+        qv[j][3] = 0.0;
+    }
+    double re[kNQ][NS], im[kNQ][NS];
+#pragma unroll
+    for (int j = 0; j < kNQ; ++j)
+#pragma unroll
+        for (int s = 0; s < NS; ++s) re[j][s] = im[j][s] = 0.0;
+
+    const V1Chunk& ck = a.v.chunks[chunk];
+#define SCARF_GRID_CLASS(LV)                                                                                          \
+    if (ck.n[LV] > 0)                                                                                                 \
+        run_class_grid<LV, NS>(pp, a, a.v.base + a.v.cls_off[LV] + (size_t)ck.begin[LV] * (rec_doubles(LV, NS) * 8), \
+                               a.class_first[LV] + ck.begin[LV], ck.n[LV], bx, by, bz, ixl, iyl, izl, qv, re, im);
+    SCARF_GRID_CLASS(0)
+    SCARF_GRID_CLASS(1)
+    SCARF_GRID_CLASS(2)
+    SCARF_GRID_CLASS(3)
+    SCARF_GRID_CLASS(4)
+    SCARF_GRID_CLASS(5)
+    SCARF_GRID_CLASS(6)
+#undef SCARF_GRID_CLASS
+
+    double2* dst = reinterpret_cast<double2*>(a.v.dst) + (size_t)chunk * a.v.chunk_stride;
+#pragma unroll
+    for (int j = 0; j < kNQ; ++j)
+        if (iq[j] >= 0)
+#pragma unroll
+            for (int s = 0; s < NS; ++s)
+                if (s < a.v.ns_real) dst[(size_t)s * a.v.n_q + iq[j]] = make_double2(re[j][s], im[j][s]);
+}
+
+}  // namespace
+
+cudaError_t launch_grid_tables(const GridArgs& a, double2* tx, double2* ty, double2* tz, cudaStream_t st)
+{
+    const long long ncol = (long long)a.nbx * kGridBX + (long long)a.nby * kGridBY + (long long)a.nbz * kGridBZ;
+    const long long n = a.n_rec * ncol;
+    if (n <= 0) return cudaSuccess;
+    grid_table_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(a, tx, ty, tz);
+    return cudaGetLastError();
+}
+
+template <int NS>
+static cudaError_t launch_grid_ns(const GridArgs& a, unsigned blocks, cudaStream_t st)
+{
+    static bool attr_set[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev >= 0 && dev < 64 && !attr_set[dev]) {
+        cudaError_t e = cudaFuncSetAttribute(ff_grid_kernel<NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+        if (e != cudaSuccess) return e;
+        attr_set[dev] = true;
+    }
+    ff_grid_kernel<NS><<<blocks, kThreads, kSmemBytes, st>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ff_grid(int NS, const GridArgs& a, cudaStream_t st)
+{
+    if (a.v.n_q <= 0 || a.v.n_chunks <= 0) return cudaSuccess;
+    const unsigned blocks = (unsigned)a.v.n_tiles * (unsigned)a.v.n_chunks;
+    switch (NS) {
+    case 1: return launch_grid_ns<1>(a, blocks, st);
+    case 2: return launch_grid_ns<2>(a, blocks, st);
+    case 4: return launch_grid_ns<4>(a, blocks, st);
+    case 6: return launch_grid_ns<6>(a, blocks, st);
+    case 8: return launch_grid_ns<8>(a, blocks, st);
+    case 12: return launch_grid_ns<12>(a, blocks, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace scarf

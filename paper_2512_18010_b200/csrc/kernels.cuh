@@ -88,6 +88,25 @@ cudaError_t launch_ff_v1(int NS, const V1Args& a, cudaStream_t st);
 cudaError_t launch_reduce_partials(const double* part, double* out, long long n_elem, long long chunk_stride,
                                    int n_chunks, cudaStream_t st);
 
+// grid (ff_grid.cu): Cartesian product grid q = (qx[ix], qy[iy], qz[iz]), index (ix*ny + iy)*nz + iz.  The
+// Gaussian/phase factor separates, e^{-q^2/4p} e^{iq.P} = X_P(ix) Y_P(iy) Z_P(iz) (the V-tensor idea of Eq. (45)-(46)
+// PAPER.md:309-316), so it is tabulated once per (pair, axis point) and S4 needs two complex multiplies per
+// (q, pair) instead of an exp and a sincos.  A CTA owns a kGridBX x kGridBY x kGridBZ box of the grid.
+constexpr int kGridBX = 4, kGridBY = 8, kGridBZ = 8;
+struct GridArgs {
+    V1Args v;                               // stream, chunks, dst as for v1; v.q unused; v.n_q = nx*ny*nz
+    const double *qx, *qy, *qz;             // axes (device)
+    int nx, ny, nz;
+    int nbx, nby, nbz;                      // boxes per axis; v.n_tiles = nbx*nby*nbz
+    const double2 *tx, *ty, *tz;            // tables [box][record][kGridB*] of (re, im); zero beyond the axis end
+    long long n_rec;                        // records of the tile stream = rows of each table
+    long long class_first[kNClasses];       // stream-order index of each class's first record
+    int rec_bytes[kNClasses];               // record size of each class for this state tile
+    int pad;
+};
+cudaError_t launch_grid_tables(const GridArgs& a, double2* tx, double2* ty, double2* tz, cudaStream_t st);
+cudaError_t launch_ff_grid(int NS, const GridArgs& a, cudaStream_t st);
+
 cudaError_t run_fp64_peak(double* dfma_per_s, double* sm_clock_mhz);
 
 }  // namespace scarf

@@ -35,6 +35,8 @@ struct DevBuf {
 // FP64 issue-slot model: per (q, pair, state) W(L), per (q, pair) C_tr.
 const double kW[kNClasses] = {2, 7, 13, 23, 38, 59, 87};
 const double kCtr = 40.0;
+// product-grid kernel: YZ = Y Z, g0 = X0 YZ, g1 = X1 YZ: 12 slots per 2 q-points; tables: 39 per (pair, axis point)
+const double kCtrGrid = 6.0, kCtrTable = 39.0;
 
 bool g_tables_uploaded_dev[64] = {};
 
@@ -53,7 +55,7 @@ struct scarf_ctx {
     bool have_basis = false, have_T = false;
     int n_states = 0;
     int sm_count = 148;
-    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb, d_partial;
+    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb, d_partial, d_axes, d_tab;
     std::vector<DevBuf> staging, packed;
     std::vector<TileStream> tiles;
     scarf_stats st = {};
@@ -108,12 +110,12 @@ int tile_size_for(int ns)  // smallest instantiated state tile >= ns (ns <= 12)
 
 // Split the tile's class-sorted stream into <= K chunks of (nearly) equal modelled cost; a chunk may span classes.
 // Returns the number of non-empty chunks written to `out`.
-int build_chunks(const TileStream& t, int K, V1Chunk* out)
+int build_chunks(const TileStream& t, int K, V1Chunk* out, double ctr = kCtr)
 {
     double w[kNClasses], total = 0.0;
     long long nrec = 0;
     for (int c = 0; c < kNClasses; ++c) {
-        w[c] = (double)t.ns_real * kW[c] + kCtr;
+        w[c] = (double)t.ns_real * kW[c] + ctr;
         total += (double)t.cls[c].n * w[c];
         nrec += t.cls[c].n;
     }
@@ -156,6 +158,7 @@ void free_device(scarf_ctx* c)
 {
     c->d_pairs.release(); c->d_E.release(); c->d_bound.release(); c->d_T.release(); c->d_q.release();
     c->d_out.release(); c->d_src.release(); c->d_dst.release(); c->d_nb.release(); c->d_partial.release();
+    c->d_axes.release(); c->d_tab.release();
     for (auto& b : c->staging) b.release();
     for (auto& b : c->packed) b.release();
     c->staging.clear(); c->packed.clear(); c->tiles.clear();
@@ -535,6 +538,124 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
         return fail(ctx, SCARF_ENOMEM, "form_factors: out of host memory");
     } catch (...) {
         return fail(ctx, SCARF_EINVAL, "form_factors: unexpected exception");
+    }
+}
+
+int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_t ny, const double* qy, int32_t nz,
+                            const double* qz, double* out)
+{
+    if (!ctx) return SCARF_EINVAL;
+    if (ctx->host_only) return fail(ctx, SCARF_ENODEVICE, "form_factors_grid: host-only context; there is no CPU fallback");
+    if (!ctx->have_T) return fail(ctx, SCARF_ESTATE, "form_factors_grid: set_basis and set_transitions first");
+    if (nx < 0 || ny < 0 || nz < 0) return fail(ctx, SCARF_EINVAL, "form_factors_grid: negative axis length");
+    const long long n_q = (long long)nx * ny * nz;
+    if (n_q == 0) return SCARF_OK;
+    if (!qx || !qy || !qz || !out) return fail(ctx, SCARF_EINVAL, "form_factors_grid: null axis or out");
+    try {
+        CU(cudaSetDevice(ctx->device), "form_factors_grid");
+        cudaStream_t st = ctx->stream;
+        const int nbx = (nx + kGridBX - 1) / kGridBX, nby = (ny + kGridBY - 1) / kGridBY, nbz = (nz + kGridBZ - 1) / kGridBZ;
+        const long long n_tiles = (long long)nbx * nby * nbz;
+        if (n_tiles > 0x7fffffffLL / kMaxChunks) return fail(ctx, SCARF_EINVAL, "form_factors_grid: grid too large for one call");
+        // axes -> one device buffer [nx | ny | nz]
+        const double* ax_in[3] = {qx, qy, qz};
+        const int ax_n[3] = {nx, ny, nz};
+        CU(ctx->d_axes.ensure(((size_t)nx + ny + nz) * sizeof(double)), "form_factors_grid: alloc axes");
+        double* dax[3];
+        size_t off = 0;
+        bool any_host_axis = false;
+        for (int k = 0; k < 3; ++k) {
+            dax[k] = static_cast<double*>(ctx->d_axes.p) + off;
+            off += (size_t)ax_n[k];
+            const bool host = !is_device_ptr(ax_in[k]);
+            if (host && !all_finite(ax_in[k], (size_t)ax_n[k])) return fail(ctx, SCARF_EINVAL, "form_factors_grid: NaN/Inf in an axis");
+            any_host_axis = any_host_axis || host;
+            CU(cudaMemcpyAsync(dax[k], ax_in[k], (size_t)ax_n[k] * sizeof(double), host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, st),
+               "form_factors_grid: copy axis");
+        }
+        const size_t obytes = (size_t)ctx->n_states * (size_t)n_q * 2 * sizeof(double);
+        double* dout = out;
+        const bool out_host = !is_device_ptr(out);
+        if (out_host) {
+            CU(ctx->d_out.ensure(obytes), "form_factors_grid: alloc out");
+            dout = static_cast<double*>(ctx->d_out.p);
+        }
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "form_factors_grid: event");
+        int launches = 0;
+        double slots = 0.0;
+        const long long ncol = (long long)nbx * kGridBX + (long long)nby * kGridBY + (long long)nbz * kGridBZ;
+        for (const TileStream& t : ctx->tiles) {
+            GridArgs a = {};
+            long long nrec = 0;
+            for (int L = 0; L < kNClasses; ++L) {
+                a.class_first[L] = nrec;
+                a.rec_bytes[L] = t.cls[L].rec_bytes;
+                a.v.cls_off[L] = t.cls[L].off;
+                nrec += t.cls[L].n;
+                slots += (double)t.cls[L].n * ((double)n_q * ((double)t.ns_real * kW[L] + kCtrGrid) + (double)(nx + ny + nz) * kCtrTable);
+            }
+            double* tile_out = dout + (size_t)t.s0 * n_q * 2;
+            if (nrec == 0) {
+                CU(cudaMemsetAsync(tile_out, 0, (size_t)t.ns_real * n_q * 2 * sizeof(double), st), "form_factors_grid: memset");
+                continue;
+            }
+            const size_t tab_elems = (size_t)nrec * (size_t)ncol;
+            if (tab_elems * 16 > (size_t)32e9) return fail(ctx, SCARF_ENOMEM, "form_factors_grid: factor tables would exceed 32 GB");
+            CU(ctx->d_tab.ensure(tab_elems * 16), "form_factors_grid: alloc tables");
+            double2* tx = static_cast<double2*>(ctx->d_tab.p);
+            double2* ty = tx + (size_t)nrec * nbx * kGridBX;
+            double2* tz = ty + (size_t)nrec * nby * kGridBY;
+            a.v.base = t.base;
+            a.v.n_q = n_q;
+            a.v.n_tiles = (int)n_tiles;
+            a.v.ns_real = t.ns_real;
+            a.qx = dax[0]; a.qy = dax[1]; a.qz = dax[2];
+            a.nx = nx; a.ny = ny; a.nz = nz;
+            a.nbx = nbx; a.nby = nby; a.nbz = nbz;
+            a.tx = tx; a.ty = ty; a.tz = tz;
+            a.n_rec = nrec;
+            CU(launch_grid_tables(a, tx, ty, tz, st), "form_factors_grid: table kernel");
+            ++launches;
+            long long K = ctx->n_chunks_opt > 0 ? ctx->n_chunks_opt : (24LL * 2 * ctx->sm_count + n_tiles / 2) / n_tiles;
+            K = std::max<long long>(1, std::min<long long>(K, kMaxChunks));
+            const size_t per_chunk = (size_t)t.ns_real * (size_t)n_q * 16;
+            while (K > 1 && (double)K * (double)per_chunk > 4e9) --K;
+            a.v.n_chunks = build_chunks(t, (int)K, a.v.chunks, kCtrGrid);
+            if (a.v.n_chunks == 1) {
+                a.v.dst = tile_out;
+                a.v.chunk_stride = 0;
+                CU(launch_ff_grid(t.NS, a, st), "form_factors_grid: kernel");
+                ++launches;
+            } else {
+                CU(ctx->d_partial.ensure((size_t)a.v.n_chunks * per_chunk), "form_factors_grid: alloc partials");
+                a.v.dst = static_cast<double*>(ctx->d_partial.p);
+                a.v.chunk_stride = (long long)t.ns_real * n_q;
+                CU(launch_ff_grid(t.NS, a, st), "form_factors_grid: kernel");
+                CU(launch_reduce_partials(a.v.dst, tile_out, a.v.chunk_stride, a.v.chunk_stride, a.v.n_chunks, st),
+                   "form_factors_grid: reduce kernel");
+                launches += 2;
+            }
+        }
+        ctx->st.last_kernel_launches = launches;
+        ctx->st.last_grid_slots = slots;
+        if (ctx->timing) {
+            CU(cudaEventRecord(ctx->ev1, st), "form_factors_grid: event");
+            CU(cudaEventSynchronize(ctx->ev1), "form_factors_grid: event sync");
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
+            ctx->st.last_kernel_ms = ms;
+        }
+        if (out_host) {
+            CU(cudaMemcpyAsync(out, dout, obytes, cudaMemcpyDeviceToHost, st), "form_factors_grid: download out");
+            CU(cudaStreamSynchronize(st), "form_factors_grid: sync");
+        } else if (any_host_axis) {
+            CU(cudaStreamSynchronize(st), "form_factors_grid: sync");  // pageable axes must not be reused before the copy ends
+        }
+        return SCARF_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(ctx, SCARF_ENOMEM, "form_factors_grid: out of host memory");
+    } catch (...) {
+        return fail(ctx, SCARF_EINVAL, "form_factors_grid: unexpected exception");
     }
 }
 

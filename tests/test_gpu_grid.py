@@ -1,0 +1,134 @@
+"""GPU parity of the product-grid path (scarf_form_factors_grid; Eq. (45)-(46), (48)
+PAPER.md:309-330) against the CPU oracle evaluated on the expanded point list, at the north-star tolerance
+1e-10 * max|f_s|, and against the general kernel (same stream, different factor route)."""
+import numpy as np
+import pytest
+
+from paper_2512_18010_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked tests must run on the B200 box")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def Scarf():
+    from paper_2512_18010_b200 import Scarf as S
+    return S
+
+
+def expand(qx, qy, qz):
+    X, Y, Z = np.meshgrid(qx, qy, qz, indexing="ij")
+    return np.ascontiguousarray(np.stack([X.ravel(), Y.ravel(), Z.ravel()], axis=1))
+
+
+def assert_parity(f_gpu, f_ref, tol=TOL):
+    assert f_gpu.shape == f_ref.shape
+    for s in range(f_ref.shape[0]):
+        scale = np.max(np.abs(f_ref[s]))
+        err = np.max(np.abs(f_gpu[s] - f_ref[s]))
+        assert err <= tol * scale, f"state {s}: max err {err:.3e} > {tol:g} * {scale:.3e}"
+
+
+def grid_ff(Scarf, torch, basis, T, qx, qy, qz, device_axes=True):
+    with Scarf(0) as sc:
+        sc.set_basis(basis)
+        sc.set_transitions(torch.as_tensor(T, dtype=torch.float64, device="cuda").contiguous())
+        if device_axes:
+            ax = [torch.as_tensor(a, dtype=torch.float64, device="cuda").contiguous() for a in (qx, qy, qz)]
+            f = sc.form_factors_grid(*ax)
+            torch.cuda.synchronize()
+            return f.cpu().numpy(), sc.stats()
+        f = sc.form_factors_grid(np.asarray(qx), np.asarray(qy), np.asarray(qz))
+        return np.array(f), sc.stats()
+
+
+def test_grid_config1_full(oracle_mod, Scarf, torch_cuda):
+    w = W.make_workload(1, oracle_mod.overlap)
+    ax = np.linspace(-w.grid["qmax"], w.grid["qmax"], w.grid["n_per_axis"])
+    f, st = grid_ff(Scarf, torch_cuda, w.basis, w.T, ax, ax, ax)
+    assert np.array_equal(expand(ax, ax, ax), w.q)          # same point order as the config's q list
+    assert_parity(f, oracle_mod.form_factors(w.basis, w.T, w.q))
+    assert st["last_kernel_launches"] >= 2                  # table kernel + grid kernel
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 1), (1, 7, 3), (5, 1, 9), (4, 8, 8), (5, 9, 9), (13, 17, 11), (2, 3, 40)])
+def test_grid_ragged_shapes_nonuniform_axes(oracle_mod, Scarf, torch_cuda, shape):
+    """Boxes are 4 x 8 x 8: shapes below, at and above one box, ragged in every axis; unsorted, non-uniform axes."""
+    w = W.make_workload(1, oracle_mod.overlap)
+    rng = np.random.default_rng(sum(shape))
+    qx, qy, qz = (rng.uniform(-5, 5, size=n) for n in shape)
+    f, _ = grid_ff(Scarf, torch_cuda, w.basis, w.T, qx, qy, qz)
+    assert_parity(f, oracle_mod.form_factors(w.basis, w.T, expand(qx, qy, qz)))
+
+
+def test_grid_high_l_12_states_host_axes(oracle_mod, Scarf, torch_cuda):
+    """All pair classes L = 0..6 (s, p, d, f shells on two centres), 12 states, host pointers for axes and out."""
+    b = W.Basis(np.array([[0.1, 0.2, -0.9], [0.3, -0.4, 1.0]]), np.array([0, 0, 0, 0, 1, 1, 1, 1], np.int32),
+                np.array([0, 1, 2, 3, 0, 1, 2, 3], np.int32), np.array([2, 1, 1, 1, 2, 1, 1, 1], np.int32),
+                np.array([2.1, 0.4, 1.3, 0.9, 0.7, 1.9, 0.5, 1.1, 0.8, 0.6]),
+                np.array([0.5, 0.6, 1.0, 1.0, 1.0, 0.7, 0.4, 1.0, 1.0, 1.0]))
+    rng = np.random.default_rng(11)
+    T = rng.normal(size=(12, b.nbf, b.nbf))
+    qx, qy, qz = np.linspace(-6, 6, 9), np.linspace(-5, 5.5, 10), np.linspace(-4, 6, 11)
+    f, st = grid_ff(Scarf, torch_cuda, b, T, qx, qy, qz, device_axes=False)
+    assert sum(1 for n in st["pairs_kept_per_class"] if n > 0) == 7
+    assert_parity(f, oracle_mod.form_factors(b, T, expand(qx, qy, qz)))
+
+
+@pytest.mark.parametrize("n_states", [1, 3, 13])
+def test_grid_state_tiles(oracle_mod, Scarf, torch_cuda, n_states):
+    w = W.make_workload(1, oracle_mod.overlap)
+    rng = np.random.default_rng(n_states)
+    T = rng.normal(size=(n_states, w.basis.nbf, w.basis.nbf))
+    ax = np.linspace(-3, 3, 10)
+    f, _ = grid_ff(Scarf, torch_cuda, w.basis, T, ax, ax[:7], ax[:9])
+    assert_parity(f, oracle_mod.form_factors(w.basis, T, expand(ax, ax[:7], ax[:9])))
+
+
+@pytest.mark.parametrize("config,n_sample", [(2, 200), (3, 160), (4, 40)])
+def test_grid_full_size_sampled(oracle_mod, Scarf, torch_cuda, config, n_sample):
+    """Configs 2-4 are Cartesian product grids: full size on the GPU in the launch configuration bench.py times,
+    compared with the oracle on a seeded sample of points, and with the general kernel on every point."""
+    torch = torch_cuda
+    w = W.make_workload(config, oracle_mod.overlap)
+    ax = np.linspace(-w.grid["qmax"], w.grid["qmax"], w.grid["n_per_axis"])
+    idx = W.sample_q_indices(w.n_q, n_sample, seed=config)
+    f_ref = oracle_mod.form_factors(w.basis, w.T, w.q[idx])
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(torch.as_tensor(w.T, device="cuda"))
+        axd = torch.as_tensor(ax, device="cuda")
+        fg = sc.form_factors_grid(axd, axd, axd)
+        fl = sc.form_factors(torch.as_tensor(w.q, device="cuda"))
+        torch.cuda.synchronize()
+        assert_parity(fg[:, torch.as_tensor(idx, device="cuda")].cpu().numpy(), f_ref)
+        scale = fl.abs().amax(dim=1)
+        err = (fg - fl).abs().amax(dim=1)
+        assert bool((err <= 1e-11 * scale).all()), (err / scale).max().item()
+
+
+def test_grid_empty_and_errors(oracle_mod, Scarf, torch_cuda):
+    w = W.make_workload(1, oracle_mod.overlap)
+    ax = np.linspace(-1, 1, 4)
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        with pytest.raises(Exception):
+            sc.form_factors_grid(ax, ax, ax)                # no transitions yet
+        sc.set_transitions(np.zeros_like(w.T))
+        f = sc.form_factors_grid(ax, ax, ax)                # T = 0: exactly zero
+        assert f.shape == (1, 64) and not np.any(f)
+        sc.set_transitions(w.T)
+        assert sc.form_factors_grid(ax, ax[:0], ax).shape == (1, 0)
+        bad = ax.copy()
+        bad[1] = np.nan
+        with pytest.raises(Exception):
+            sc.form_factors_grid(ax, bad, ax)
