@@ -160,4 +160,130 @@ __device__ __forceinline__ void make_monomials(const double (&qv)[kNQ][4], doubl
     }
 }
 
+
+// ---- high classes (L >= 4): degree-block evaluation ---------------------------------------------------------
+// Holding all n_herm(L) monomials of two q-points in registers is impossible beyond L = 3 (35..84 doubles per
+// point).  The polynomial is therefore evaluated block by block: block 0 = Hermite indices [0, 20) (degrees <= 3),
+// then each degree shell n = 4..L in pieces of at most kBlkMax monomials.  A block's monomials are built once
+// per batch of kBlkRec records (degree-n monomials as products of two or three held degree <= 2 monomials) and
+// every block ends with its own accumulate acc += (gc + i gs)(A_blk + i B_blk) — 2 extra issue slots per state
+// and block on top of the W(L) = n_herm + 3 of the work model (a shell has one parity, so only A or only B).
+constexpr int kBlkMax = 16;
+constexpr int kBlkRec = 2;
+__host__ __device__ constexpr int blk_pieces(int n) { return (nherm(n) - nherm(n - 1) + kBlkMax - 1) / kBlkMax; }
+__host__ __device__ constexpr int blk_count(int L)
+{
+    int c = 1;
+    for (int n = 4; n <= L; ++n) c += blk_pieces(n);
+    return c;
+}
+__host__ __device__ constexpr int blk_begin(int L, int b)   // first Hermite index of block b (b == blk_count: n_herm)
+{
+    if (b == 0) return 0;
+    int c = 1;
+    for (int n = 4; n <= L; ++n) {
+        const int sz = nherm(n) - nherm(n - 1), np = blk_pieces(n), per = (sz + np - 1) / np;
+        for (int p = 0; p < np; ++p, ++c)
+            if (c == b) return nherm(n - 1) + p * per;
+    }
+    return nherm(L);
+}
+__host__ __device__ constexpr int var_at(int t, int u, int pos) { return pos < t ? 0 : (pos < t + u ? 1 : 2); }
+// k-th factor (index of a degree <= 2 monomial; 0 = the constant 1) of monomial h written as a product of pairs
+__host__ __device__ constexpr int factor_index(int h, int k)
+{
+    const int t = hexp(h, 0), u = hexp(h, 1), n = hdeg(h);
+    if (2 * k >= n) return 0;
+    int e[3] = {0, 0, 0};
+    e[var_at(t, u, 2 * k)]++;
+    if (2 * k + 1 < n) e[var_at(t, u, 2 * k + 1)]++;
+    return hindex(e[0], e[1], e[2]);
+}
+__host__ __device__ constexpr int first_of_parity(int H0, int BS, int par)
+{
+    for (int h = H0; h < H0 + BS; ++h)
+        if ((hdeg(h) & 1) == par) return h;
+    return -1;
+}
+
+template <int H0, int BS, int NQA>
+__device__ __forceinline__ void block_monomials(const double (&lo)[NQA][10], double (&mb)[NQA][BS])
+{
+#pragma unroll
+    for (int j = 0; j < NQA; ++j)
+        static_for<BS>([&](auto ic) {
+            constexpr int h = H0 + decltype(ic)::value;
+            constexpr int f0 = factor_index(h, 0), f1 = factor_index(h, 1), f2 = factor_index(h, 2);
+            double m = lo[j][f0] * lo[j][f1];
+            if constexpr (f2 != 0) m *= lo[j][f2];
+            mb[j][decltype(ic)::value] = m;
+        });
+}
+
+// acc += (gc + i gs) * sum_{h in [H0, H0+BS)} D[s][h] mono[h]      (parity of deg h routes a term to A or B)
+template <int L, int NS, int NQA, int jq0, int H0, int BS>
+__device__ __forceinline__ void record_accum_block(const double2* __restrict__ r2, const double (&mb)[NQA][BS],
+                                                   const double (&gc)[NQA], const double (&gs)[NQA],
+                                                   double (&re)[kNQ][NS], double (&im)[kNQ][NS])
+{
+    constexpr int NH = nherm(L);
+    constexpr int hA = first_of_parity(H0, BS, 0), hB = first_of_parity(H0, BS, 1);
+    const double2* __restrict__ D2 = r2 + 2;
+    static_for<NS>([&](auto sc) {
+        constexpr int s = decltype(sc)::value;
+        double A[NQA], B[NQA];
+        static_for<BS>([&](auto ic) {
+            constexpr int i = decltype(ic)::value, h = H0 + i, idx = s * NH + h;
+            const double2 c2 = D2[idx / 2];
+            const double cv = (idx & 1) ? c2.y : c2.x;
+#pragma unroll
+            for (int j = 0; j < NQA; ++j) {
+                if constexpr (h == 0) A[j] = cv;
+                else if constexpr (h == hA) A[j] = cv * mb[j][i];
+                else if constexpr (h == hB) B[j] = cv * mb[j][i];
+                else if constexpr (hdeg(h) & 1) B[j] = fma(cv, mb[j][i], B[j]);
+                else A[j] = fma(cv, mb[j][i], A[j]);
+            }
+        });
+#pragma unroll
+        for (int j = 0; j < NQA; ++j) {
+            if constexpr (hA >= 0) {
+                re[jq0 + j][s] = fma(gc[j], A[j], re[jq0 + j][s]);
+                im[jq0 + j][s] = fma(gs[j], A[j], im[jq0 + j][s]);
+            }
+            if constexpr (hB >= 0) {
+                re[jq0 + j][s] = fma(-gs[j], B[j], re[jq0 + j][s]);
+                im[jq0 + j][s] = fma(gc[j], B[j], im[jq0 + j][s]);
+            }
+        }
+    });
+}
+
+// all blocks of class L for a batch of nb <= kBlkRec records (rec0, rec0 + REC, ...) whose factors are gc/gs
+template <int L, int NS>
+__device__ __forceinline__ void accum_blocks(const unsigned char* rec0, int nb, const double (&qv)[kNQ][4],
+                                             const double (&gc)[kBlkRec][kNQ], const double (&gs)[kBlkRec][kNQ],
+                                             double (&re)[kNQ][NS], double (&im)[kNQ][NS])
+{
+    constexpr int REC = rec_doubles(L, NS) * 8;
+    static_for<blk_count(L)>([&](auto bc) {
+        constexpr int b = decltype(bc)::value;
+        constexpr int H0 = blk_begin(L, b), BS = blk_begin(L, b + 1) - H0;
+        double mb[kNQ][BS];
+        if constexpr (b == 0) {
+            static_assert(BS == nherm(3), "block 0 is the L = 3 monomial set");
+            make_monomials<3, kNQ, 0>(qv, mb);
+        } else {
+            double lo[kNQ][10];
+            make_monomials<2, kNQ, 0>(qv, lo);
+            block_monomials<H0, BS, kNQ>(lo, mb);
+        }
+        static_for<kBlkRec>([&](auto rc) {
+            constexpr int r = decltype(rc)::value;
+            if (r < nb)
+                record_accum_block<L, NS, kNQ, 0, H0, BS>(reinterpret_cast<const double2*>(rec0 + r * REC), mb, gc[r], gs[r], re, im);
+        });
+    });
+}
+
 }  // namespace scarf

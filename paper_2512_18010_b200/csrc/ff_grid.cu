@@ -111,6 +111,27 @@ __device__ __forceinline__ void run_class_grid(GPipe& pp, const GridArgs& a, con
         const double2* Xs = reinterpret_cast<const double2*>(sp + kStageBytes);
         const double2* Ys = reinterpret_cast<const double2*>(sp + kStageBytes + kMaxRec * kXB);
         const double2* Zs = reinterpret_cast<const double2*>(sp + kStageBytes + kMaxRec * (kXB + kYB));
+        if constexpr (L >= 4) {                         // degree blocks, both q-points together (ff_common.cuh)
+#pragma unroll 1
+            for (int k0 = 0; k0 < cnt; k0 += kBlkRec) {
+                const int nb = min(kBlkRec, cnt - k0);
+                double gcb[kBlkRec][kNQ], gsb[kBlkRec][kNQ];
+                static_for<kBlkRec>([&](auto rc) {
+                    constexpr int r = decltype(rc)::value;
+                    if (r < nb) {
+                        const int k = k0 + r;
+                        const double2 yz = cmul(Ys[k * kGridBY + iyl], Zs[k * kGridBZ + izl]);
+#pragma unroll
+                        for (int jj = 0; jj < kNQ; ++jj) {
+                            const double2 gq = cmul(Xs[k * kGridBX + ixl + 2 * jj], yz);
+                            gcb[r][jj] = gq.x;
+                            gsb[r][jj] = gq.y;
+                        }
+                    }
+                });
+                accum_blocks<L, NS>(sp + k0 * REC, nb, qv, gcb, gsb, re, im);
+            }
+        } else
         static_for<kNQ / NQA>([&](auto jc) {
             constexpr int jq0 = decltype(jc)::value * NQA;
             double mono[NQA][nherm(L)];

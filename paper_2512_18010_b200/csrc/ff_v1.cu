@@ -69,6 +69,18 @@ __device__ __forceinline__ void run_class(Pipe& pp, const char* __restrict__ seg
         mbar_wait(&pp.full[slot], (g / kStages) & 1u);
         const int cnt = min(SREC, n_rec - j * SREC);
         const unsigned char* sp = pp.buf + slot * kStageBytes;
+        if constexpr (L >= 4) {                         // degree blocks, both q-points together (ff_common.cuh)
+#pragma unroll 1
+            for (int k0 = 0; k0 < cnt; k0 += kBlkRec) {
+                const int nb = min(kBlkRec, cnt - k0);
+                double gcb[kBlkRec][kNQ], gsb[kBlkRec][kNQ];
+                static_for<kBlkRec>([&](auto rc) {
+                    constexpr int r = decltype(rc)::value;
+                    if (r < nb) record_trans<kNQ, 0>(reinterpret_cast<const double2*>(sp + (k0 + r) * REC), qv, gcb[r], gsb[r]);
+                });
+                accum_blocks<L, NS>(sp + k0 * REC, nb, qv, gcb, gsb, re, im);
+            }
+        } else
         static_for<kNQ / NQA>([&](auto jc) {
             constexpr int jq0 = decltype(jc)::value * NQA;
             double mono[NQA][nherm(L)];
