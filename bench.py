@@ -36,6 +36,9 @@ METRIC = "q*primitive-pair*state evaluations per second (12-form-factor job, fol
 UNIT = "evals/s"
 # FP64 lanes per SM per clock on B200 (GB100): 64 DFMA/clk/SM, as on GH100.
 DFMA_PER_CLK_PER_SM = 64
+# dram__bytes_read.sum + dram__bytes_write.sum of one ff_v1_kernel<12> launch, from the `ncu --set full` capture
+# summarised in profiles/r01b_ff_v1_ncu_full.md (config 3 only; other configs were not captured -> null).
+NCU_DRAM_BYTES_PER_LAUNCH = {3: 16.663808e6 + 293.769984e6}
 
 
 def parse():
@@ -235,6 +238,39 @@ def run_ours(args):
     evals_per_step = st["evals_per_q"] * w.n_q
     value, ms_per_step = replicas.whole_job_value(evals_per_step, args.steps, float(sum(step_ms)), "cuda")
 
+    # ---- product-grid path (NEXT-1, scarf_form_factors_grid) on the Cartesian configs: same job, same timing protocol
+    grid_path = None
+    if w.grid.get("kind") == "cartesian":
+        ax_dev = torch.as_tensor(np.linspace(-w.grid["qmax"], w.grid["qmax"], w.grid["n_per_axis"]), device="cuda")
+
+        def step_grid():
+            sc.set_transitions(T_dev)
+            sc.form_factors_grid(ax_dev, ax_dev, ax_dev, out=out_dev)
+
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                step_grid()
+            barrier()
+            gev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+            gk = []
+            sc.set_option("timing", 1)
+            for k in range(args.steps):
+                flush.fill_(k & 0xFF)
+                gev[k][0].record(stream)
+                step_grid()
+                gev[k][1].record(stream)
+                gk.append(sc.stats()["last_kernel_ms"])
+            barrier()
+            sc.set_option("timing", 0)
+        g_ms = float(np.mean([a.elapsed_time(b) for a, b in gev]))
+        g_ms = replicas.max_over_ranks(g_ms, "cuda")
+        gst = sc.stats()
+        grid_path = {"api": "scarf_form_factors_grid", "ms_per_step": g_ms, "kernel_ms": float(np.median(gk)),
+                     "value": world * evals_per_step / (g_ms * 1e-3), "unit": UNIT, "slots": gst["last_grid_slots"],
+                     "launches_per_step": int(gst["last_kernel_launches"] + gst["last_fold_launches"])}
+        step_device()   # leave the general path's result in out_dev for the parity sample below
+        torch.cuda.synchronize()
+
     # ---- end to end: host buffers through the C ABI (pinned q / out, pageable T), copies inside the timed region
     q_host = torch.as_tensor(w.q).pin_memory()
     out_host = torch.empty((w.n_states, w.n_q, 2), dtype=torch.float64).pin_memory()
@@ -274,7 +310,7 @@ def run_ours(args):
     peak_nominal = DFMA_PER_CLK_PER_SM * sms * sm_max * 1e6
     achieved = slots / (kernel_ms * 1e-3)
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_meas / 1e12, "unit": "T FP64-slot/s (1 slot = 1 DFMA lane-op = 2 flop)",
-                "frac": achieved / peak_meas, "traffic": None,
+                "frac": achieved / peak_meas, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.config),
                 "peak_source": f"measured register-only DFMA micro-benchmark (scarf_fp64_peak) at {peak_mhz:.0f} MHz; "
                                f"nominal {DFMA_PER_CLK_PER_SM}/clk/SM x {sms} SMs x {sm_max:.0f} MHz = {peak_nominal / 1e12:.2f}",
                 "frac_of_nominal": achieved / peak_nominal, "kernel": "S4 form-factor kernel(s)", "kernel_ms": kernel_ms,
@@ -294,6 +330,12 @@ def run_ours(args):
                     "job_seconds": e2e_s},
             "gpu_launches": int(args.steps * (st["last_kernel_launches"] + st["last_fold_launches"])),
             "clocks": clocks, "roofline": roofline}
+
+    if grid_path is not None:
+        g_ach = grid_path["slots"] / (grid_path["kernel_ms"] * 1e-3)
+        grid_path["roofline"] = {"bound": "alu", "achieved": g_ach / 1e12, "peak": peak_meas / 1e12, "frac": g_ach / peak_meas,
+                                 "unit": roofline["unit"]}
+        line["grid_path"] = grid_path
 
     if not args.no_cpu_baseline and world == 1:
         import oracle
