@@ -78,6 +78,7 @@ typedef struct scarf_stats {
     int32_t last_kernel_launches;              /* kernels launched by the last scarf_form_factors                   */
     int32_t last_fold_launches;                /* kernels launched by the last scarf_set_transitions               */
     double last_grid_slots;                    /* FP64 issue-slot model of the last scarf_form_factors_grid call    */
+    double dropped_bound;                      /* sum of the bounds B_P of all dropped pairs: |f_s(q) - exact| <= this, any q, s */
 } scarf_stats;
 
 /* device >= 0: CUDA ordinal.  device < 0: host-only context (set_basis, overlap, stats work; the rest ENODEVICE). */
@@ -92,6 +93,11 @@ int scarf_set_stream(scarf_ctx* ctx, void* cuda_stream);
  *                         B_P = max_s sum_t |D^s_t| sup_q |q|^n e^{-q^2/4p} is below screen_tol * mean(B);
  *                         0 keeps everything.  The paper's own epsilon = 1e-6 thresholding is an
  *                         approximation and is NOT applied.
+ *           "threshold_eps": default 0 (off).  Paper-style thresholding ("discarding all Cartesian pair
+ *                         index combinations for which |M T / (M T)_max| < epsilon"), restated on this library's unit:
+ *                         a primitive shell pair is also dropped when B_P < threshold_eps * max_P B_P (B_P already is
+ *                         the max over the states, so a pair survives if any transition needs it).  An APPROXIMATION
+ *                         whose error is bounded: scarf_stats.dropped_bound.  Takes effect at set_transitions.
  *           "timing": 1 records CUDA-event times of S3/S4 into the stats (adds a stream sync per call).         */
 int scarf_set_option(scarf_ctx* ctx, const char* key, double value);
 

@@ -32,7 +32,7 @@ class ScarfStats(C.Structure):
                 ("stream_bytes", C.c_double), ("slots_per_q", C.c_double), ("evals_per_q", C.c_double),
                 ("last_setup_host_ms", C.c_double), ("last_fold_ms", C.c_double), ("last_kernel_ms", C.c_double),
                 ("last_kernel_launches", C.c_int32), ("last_fold_launches", C.c_int32),
-                ("last_grid_slots", C.c_double)]
+                ("last_grid_slots", C.c_double), ("dropped_bound", C.c_double)]
 
     def as_dict(self):
         d = {}

@@ -46,7 +46,7 @@ struct scarf_ctx {
     int device = -1;
     bool host_only = true;
     cudaStream_t stream = nullptr;
-    double prefactor = 2.0, screen_tol = 1e-16;
+    double prefactor = 2.0, screen_tol = 1e-16, threshold_eps = 0.0;
     bool timing = false;
     int kernel_variant = -1;  // -1 auto (v1), 0 force the baseline kernel v0
     int n_chunks_opt = 0;     // 0 auto, else the number of stream chunks of the v1 kernel
@@ -234,6 +234,7 @@ int scarf_set_option(scarf_ctx* ctx, const char* key, double value)
         if (value < 0) return fail(ctx, SCARF_EINVAL, "set_option: screen_tol must be >= 0");
         ctx->screen_tol = value;
     } else if (k == "timing") ctx->timing = value != 0.0;
+    else if (k == "threshold_eps") { if (!(value >= 0.0)) return fail(ctx, SCARF_EINVAL, "set_option: threshold_eps < 0"); ctx->threshold_eps = value; }
     else if (k == "kernel_variant") ctx->kernel_variant = (int)value;
     else if (k == "n_chunks") ctx->n_chunks_opt = (int)value;
     else return fail(ctx, SCARF_EINVAL, "set_option: unknown key '" + k + "'");
@@ -364,7 +365,13 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T)
             if (!std::isfinite(b)) return fail(ctx, SCARF_EINVAL, "set_transitions: NaN/Inf produced by T (device input not finite?)");
             sumB += b;
         }
-        const double thr = np > 0 ? ctx->screen_tol * sumB / (double)np : 0.0;
+        double maxB = 0.0;
+        for (double b : bound) maxB = std::max(maxB, b);
+        // default: B_P < screen_tol * mean(B); NEXT-2 option (paper-style): B_P < threshold_eps * max(B)
+        const double thr = std::max(np > 0 ? ctx->screen_tol * sumB / (double)np : 0.0, ctx->threshold_eps * maxB);
+        double dropped_bound = 0.0;
+        for (double b : bound)
+            if (!(b > 0.0 && b >= thr)) dropped_bound += b;
         std::vector<unsigned long long> src, dst;
         std::vector<int> nb;
         long long kept_per_class[kNClasses] = {};
@@ -426,6 +433,7 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T)
         scarf_stats& s = ctx->st;
         s.n_states = n_states;
         s.n_pairs_kept = n_kept;
+        s.dropped_bound = dropped_bound;
         s.n_herm_kept = 0; s.slots_per_q = 0.0; s.stream_bytes = 0.0;
         for (int c = 0; c < kNClasses; ++c) {
             s.pairs_kept_per_class[c] = kept_per_class[c];

@@ -212,3 +212,20 @@ def test_error_paths(oracle_mod, Scarf, torch_cuda):
         with pytest.raises(ScarfError) as e:
             sc.form_factors(qbad)
         assert e.value.code == SCARF_EINVAL
+
+
+@pytest.mark.parametrize("eps", [1e-10, 1e-6, 1e-3])
+def test_threshold_eps_error_within_reported_bound(oracle_mod, Scarf, torch_cuda, eps):
+    """NEXT-2 (paper-style thresholding): an approximation whose error must stay below the bound the
+    library reports (sum of the dropped pairs' B_P), for every state and q; the exact path is the oracle."""
+    torch = torch_cuda
+    w = W.make_workload(2, oracle_mod.overlap)
+    idx = W.sample_q_indices(w.n_q, 300, seed=7)
+    q = w.q[idx]
+    f_ref = oracle_mod.form_factors(w.basis, w.T, q)
+    f0, st0 = gpu_form_factors(Scarf, torch, w.basis, w.T, q)
+    f1, st1 = gpu_form_factors(Scarf, torch, w.basis, w.T, q, threshold_eps=eps)
+    assert st1["n_pairs_kept"] < st0["n_pairs_kept"]
+    assert st1["dropped_bound"] >= st0["dropped_bound"] >= 0.0
+    err = np.max(np.abs(f1 - f_ref))
+    assert err <= st1["dropped_bound"] + TOL * np.max(np.abs(f_ref))
