@@ -38,6 +38,10 @@ def lib():
         L.oracle_hermite_He.restype = None
         L.oracle_shift_coeffs.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, dp]
         L.oracle_shift_coeffs.restype = None
+        L.oracle_sph_harm.argtypes = [C.c_int, C.c_double, C.c_double, dp]
+        L.oracle_sph_harm.restype = None
+        L.oracle_angular_moments.argtypes = [C.c_int, C.c_int, C.c_int, dp, dp, C.c_int, C.c_int, dp, dp, dp]
+        L.oracle_angular_moments.restype = C.c_int
         _lib = L
     return _lib
 
@@ -139,3 +143,28 @@ def shift_coeffs(ai, aj, u, v) -> np.ndarray:
     out = np.zeros(ai + aj + 1)
     lib().oracle_shift_coeffs(ai, aj, u, v, _dp(out))
     return out
+
+
+def sph_harm(l_max: int, cos_theta: float, phi: float) -> np.ndarray:
+    """complex128 [(l_max+1)^2], index l(l+1)+m: orthonormal Y_l^m with the Condon-Shortley phase."""
+    out = np.zeros(((l_max + 1) ** 2, 2))
+    lib().oracle_sph_harm(int(l_max), float(cos_theta), float(phi), _dp(out))
+    return out[:, 0] + 1j * out[:, 1]
+
+
+def angular_moments(f, cos_theta, w_theta, n_phi: int, l_max: int):
+    """f: complex [n_states][n_r][n_theta][n_phi] on the product grid (theta nodes/weights given, phi_k = 2 pi k/n_phi).
+    Returns (R complex [n_states][n_r][(l_max+1)^2], <f^2>_Omega real [n_states][n_r]): Eq. (57), (59)."""
+    f = np.asarray(f, np.complex128)
+    ns, nr, nt, nph = f.shape
+    if nph != n_phi or len(cos_theta) != nt or len(w_theta) != nt:
+        raise ValueError("angular_moments: shape mismatch")
+    fr = np.ascontiguousarray(np.stack([f.real, f.imag], axis=-1))
+    ct = np.ascontiguousarray(cos_theta, np.float64)
+    wt = np.ascontiguousarray(w_theta, np.float64)
+    nlm = (l_max + 1) ** 2
+    R = np.zeros((ns, nr, nlm, 2))
+    f2 = np.zeros((ns, nr))
+    if lib().oracle_angular_moments(ns, nr, nt, _dp(ct), _dp(wt), int(n_phi), int(l_max), _dp(fr), _dp(R), _dp(f2)) != 0:
+        raise ValueError("oracle_angular_moments: bad arguments")
+    return R[..., 0] + 1j * R[..., 1], f2

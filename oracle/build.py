@@ -1,4 +1,4 @@
-"""Build oracle/liboracle.so from oracle/scarf_oracle.c with gcc (plain C99 + OpenMP, libm only).
+"""Build oracle/liboracle.so from oracle/scarf_oracle.c and oracle/angular_oracle.c with gcc (plain C99 + OpenMP, libm only).
 
 TEST INFRASTRUCTURE.  `python -m oracle.build` or `oracle.build.build()`.
 """
@@ -9,14 +9,14 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(HERE, "scarf_oracle.c")
+SRCS = [os.path.join(HERE, "scarf_oracle.c"), os.path.join(HERE, "angular_oracle.c")]
 LIB = os.path.join(HERE, "liboracle.so")
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= max(os.path.getmtime(x) for x in SRCS):
         return LIB
-    cmd = ["gcc", "-std=gnu99", "-O2", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", LIB, SRC, "-lm"]
+    cmd = ["gcc", "-std=gnu99", "-O2", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", LIB] + SRCS + ["-lm"]
     if verbose:
         print(" ".join(cmd), file=sys.stderr)
     subprocess.run(cmd, check=True)
