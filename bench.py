@@ -271,6 +271,30 @@ def run_ours(args):
         step_device()   # leave the general path's result in out_dev for the parity sample below
         torch.cuda.synchronize()
 
+    # ---- angular moments of the result (NEXT-3, scarf_angular_moments) on the spherical product grid of config 5
+    angular = None
+    if w.grid.get("kind") == "spherical":
+        n_r, n_t, n_p = w.grid["n_r"], w.grid["n_theta"], w.grid["n_phi"]
+        ct, wt = np.polynomial.legendre.leggauss(n_t)
+        l_max = 24
+        f_dev = torch.view_as_complex(out_dev)
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                sc.angular_moments(f_dev, ct, wt, n_p, l_max, n_r=n_r)
+            barrier()
+            aev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+            for k in range(args.steps):
+                flush.fill_(k & 0xFF)
+                aev[k][0].record(stream)
+                sc.angular_moments(f_dev, ct, wt, n_p, l_max, n_r=n_r)
+                aev[k][1].record(stream)
+            barrier()
+        a_ms = float(np.median([a.elapsed_time(b) for a, b in aev]))
+        a_bytes = 16.0 * w.n_states * w.n_q + 16.0 * w.n_states * n_r * (l_max + 1) ** 2
+        angular = {"api": "scarf_angular_moments", "l_max": l_max, "ms_per_call": a_ms, "algorithmic_bytes": a_bytes,
+                   "achieved_gbs": a_bytes / (a_ms * 1e-3) / 1e9,
+                   "note": "includes the host-side Legendre/twiddle tables and their upload; bound: hbm"}
+
     # ---- end to end: host buffers through the C ABI (pinned q / out, pageable T), copies inside the timed region
     q_host = torch.as_tensor(w.q).pin_memory()
     out_host = torch.empty((w.n_states, w.n_q, 2), dtype=torch.float64).pin_memory()
@@ -336,6 +360,9 @@ def run_ours(args):
         grid_path["roofline"] = {"bound": "alu", "achieved": g_ach / 1e12, "peak": peak_meas / 1e12, "frac": g_ach / peak_meas,
                                  "unit": roofline["unit"]}
         line["grid_path"] = grid_path
+
+    if angular is not None:
+        line["angular_moments"] = angular
 
     if not args.no_cpu_baseline and world == 1:
         import oracle

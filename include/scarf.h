@@ -131,6 +131,21 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
 int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_t ny, const double* qy, int32_t nz,
                             const double* qz, double* out);
 
+/* Angular moments of form factors given on a spherical product grid:
+ *     f_s(q) = sum_lm Y_l^m(qhat) R_lm(q)   (Eq. 57)   =>   R_lm(q) = Int dOmega conj(Y_l^m(qhat)) f_s(q),
+ *     <f_s^2>_Omega = Int dOmega/4pi |f_s(q)|^2                       (Eq. 59),
+ * both by the grid's own quadrature: theta nodes cos_theta[j] with weights w_theta[j] (e.g. Gauss-Legendre),
+ * phi_k = 2 pi k / n_phi uniform.  Y_l^m: orthonormal, Condon-Shortley phase.
+ *   f      [n_states][n_r][n_theta][n_phi][2]  (re, im) — the layout scarf_form_factors writes for the point list
+ *          q = r_i (sin t_j cos phi_k, sin t_j sin phi_k, cos t_j), index (i*n_theta + j)*n_phi + k.  Host or device.
+ *   R_out  [n_states][n_r][(l_max+1)^2][2], index l(l+1)+m.  Host or device.
+ *   f2_out [n_states][n_r] or NULL.  Host or device.
+ *   cos_theta, w_theta: HOST.  Needs n_phi >= 2 l_max + 1 (no phi aliasing), n_phi <= 2048, l_max <= 64; exact for
+ *   band limit l + l' <= 2 n_theta - 1 with Gauss-Legendre nodes.  Independent of the basis and transitions set. */
+int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t n_theta, const double* cos_theta,
+                          const double* w_theta, int32_t n_phi, int32_t l_max, const double* f, double* R_out,
+                          double* f2_out);
+
 int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out);
 const char* scarf_last_error(const scarf_ctx* ctx);
 const char* scarf_version(void);

@@ -19,7 +19,7 @@ SCARF_N_CLASSES = 2 * SCARF_MAX_L + 1
 _CODES = {-1: "EINVAL", -2: "ESTATE", -3: "ENOMEM", -4: "ECUDA", -5: "ENODEVICE"}
 
 EXPORTS = ["scarf_create", "scarf_destroy", "scarf_set_stream", "scarf_set_option", "scarf_set_basis", "scarf_nbf",
-           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_get_stats", "scarf_last_error",
+           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_angular_moments", "scarf_get_stats", "scarf_last_error",
            "scarf_version", "scarf_fp64_peak", "scarf_host_hermite_E", "scarf_host_shell_norms"]
 
 
@@ -65,6 +65,7 @@ def _load():
     L.scarf_set_transitions.argtypes = [vp, C.c_int, vp]
     L.scarf_form_factors.argtypes = [vp, C.c_int64, vp, vp]
     L.scarf_form_factors_grid.argtypes = [vp, C.c_int32, vp, C.c_int32, vp, C.c_int32, vp, vp]
+    L.scarf_angular_moments.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, C.c_int32, C.c_int32, vp, vp, vp]
     L.scarf_get_stats.argtypes = [vp, C.POINTER(ScarfStats)]
     L.scarf_last_error.argtypes = [vp]
     L.scarf_last_error.restype = C.c_char_p
@@ -262,6 +263,45 @@ class Scarf:
             import torch
             return torch.view_as_complex(out.view(self.n_states, n_q, 2))
         return out.reshape(self.n_states, n_q, 2).view(np.complex128)[..., 0]
+
+    def angular_moments(self, f, cos_theta, w_theta, n_phi: int, l_max: int, n_r: int = None, want_f2: bool = True):
+        """f: complex128 [n_states][n_r*n_theta*n_phi] (what form_factors returns on the spherical product grid) or
+        [n_states][n_r][n_theta][n_phi]; torch (host or cuda) or numpy.  Returns (R complex [n_states][n_r][(l_max+1)^2],
+        f2 real [n_states][n_r] or None) in the same kind of memory as f."""
+        ct = np.ascontiguousarray(cos_theta, dtype=np.float64)
+        wt = np.ascontiguousarray(w_theta, dtype=np.float64)
+        n_theta = int(ct.shape[0])
+        n_states = int(f.shape[0])
+        total = 1
+        for d in f.shape[1:]:
+            total *= int(d)
+        if n_r is None:
+            n_r = total // (n_theta * int(n_phi))
+        if n_r * n_theta * int(n_phi) != total:
+            raise ValueError("angular_moments: f does not have n_r*n_theta*n_phi points per state")
+        nlm = (int(l_max) + 1) ** 2
+        if _is_torch(f):
+            import torch
+            fr = torch.view_as_real(f.contiguous()) if f.is_complex() else f
+            fp, fkeep = _ptr(fr, "f", n_states * total * 2)
+            R = torch.empty((n_states, n_r, nlm, 2), dtype=torch.float64, device=f.device)
+            f2 = torch.empty((n_states, n_r), dtype=torch.float64, device=f.device) if want_f2 else None
+            rp = C.c_void_p(R.data_ptr())
+            f2p = C.c_void_p(f2.data_ptr()) if want_f2 else None
+        else:
+            fa = np.ascontiguousarray(f, dtype=np.complex128)
+            fp, fkeep = C.c_void_p(fa.ctypes.data), fa
+            R = np.empty((n_states, n_r, nlm, 2))
+            f2 = np.empty((n_states, n_r)) if want_f2 else None
+            rp = C.c_void_p(R.ctypes.data)
+            f2p = C.c_void_p(f2.ctypes.data) if want_f2 else None
+        dp = C.POINTER(C.c_double)
+        self._check(_lib.scarf_angular_moments(self._h, n_states, n_r, n_theta, ct.ctypes.data_as(dp), wt.ctypes.data_as(dp),
+                                               int(n_phi), int(l_max), fp, rp, f2p))
+        if _is_torch(f):
+            import torch
+            return torch.view_as_complex(R), f2
+        return R.view(np.complex128)[..., 0], f2
 
     def stats(self) -> dict:
         s = ScarfStats()

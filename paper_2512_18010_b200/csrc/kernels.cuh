@@ -14,6 +14,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <vector>
 
 #include "host_setup.hpp"
 
@@ -106,6 +107,14 @@ struct GridArgs {
 };
 cudaError_t launch_grid_tables(const GridArgs& a, double2* tx, double2* ty, double2* tz, cudaStream_t st);
 cudaError_t launch_ff_grid(int NS, const GridArgs& a, cudaStream_t st);
+
+// angular moments (angular.cu, NEXT-3)
+void angular_host_tables(int l_max, int n_theta, const double* cos_theta, const double* w_theta, int n_phi,
+                         std::vector<double>& Yw, std::vector<double>& tw);
+cudaError_t launch_phi_dft(const double* f, const double* tw, long long n_rows, int n_phi, int l_max, double* F, double* rowsum2,
+                           cudaStream_t st);
+cudaError_t launch_legendre(const double* F, const double* rowsum2, const double* Yw, const double* w_theta, long long n_sr,
+                            int n_theta, int l_max, double* R, double* f2, cudaStream_t st);
 
 cudaError_t run_fp64_peak(double* dfma_per_s, double* sm_clock_mhz);
 

@@ -55,7 +55,7 @@ struct scarf_ctx {
     bool have_basis = false, have_T = false;
     int n_states = 0;
     int sm_count = 148;
-    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb, d_partial, d_axes, d_tab;
+    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb, d_partial, d_axes, d_tab, d_ang_in, d_ang_F, d_ang_tab, d_ang_out;
     std::vector<DevBuf> staging, packed;
     std::vector<TileStream> tiles;
     scarf_stats st = {};
@@ -159,6 +159,7 @@ void free_device(scarf_ctx* c)
     c->d_pairs.release(); c->d_E.release(); c->d_bound.release(); c->d_T.release(); c->d_q.release();
     c->d_out.release(); c->d_src.release(); c->d_dst.release(); c->d_nb.release(); c->d_partial.release();
     c->d_axes.release(); c->d_tab.release();
+    c->d_ang_in.release(); c->d_ang_F.release(); c->d_ang_tab.release(); c->d_ang_out.release();
     for (auto& b : c->staging) b.release();
     for (auto& b : c->packed) b.release();
     c->staging.clear(); c->packed.clear(); c->tiles.clear();
@@ -664,6 +665,82 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         return fail(ctx, SCARF_ENOMEM, "form_factors_grid: out of host memory");
     } catch (...) {
         return fail(ctx, SCARF_EINVAL, "form_factors_grid: unexpected exception");
+    }
+}
+
+int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t n_theta, const double* cos_theta,
+                          const double* w_theta, int32_t n_phi, int32_t l_max, const double* f, double* R_out, double* f2_out)
+{
+    if (!ctx) return SCARF_EINVAL;
+    if (ctx->host_only) return fail(ctx, SCARF_ENODEVICE, "angular_moments: host-only context; there is no CPU fallback");
+    if (n_states < 0 || n_r < 0 || n_theta < 1 || n_phi < 1 || l_max < 0)
+        return fail(ctx, SCARF_EINVAL, "angular_moments: bad shape");
+    if (l_max > 64) return fail(ctx, SCARF_EINVAL, "angular_moments: l_max > 64");
+    if (n_phi > 2048) return fail(ctx, SCARF_EINVAL, "angular_moments: n_phi > 2048");
+    if (n_phi < 2 * l_max + 1) return fail(ctx, SCARF_EINVAL, "angular_moments: n_phi must be >= 2 l_max + 1 (phi aliasing)");
+    const long long n_sr = (long long)n_states * n_r;
+    if (n_sr == 0) return SCARF_OK;
+    if (!cos_theta || !w_theta || !f || !R_out) return fail(ctx, SCARF_EINVAL, "angular_moments: null pointer");
+    if (!all_finite(cos_theta, (size_t)n_theta) || !all_finite(w_theta, (size_t)n_theta))
+        return fail(ctx, SCARF_EINVAL, "angular_moments: NaN/Inf in the theta nodes or weights");
+    for (int j = 0; j < n_theta; ++j)
+        if (std::fabs(cos_theta[j]) > 1.0) return fail(ctx, SCARF_EINVAL, "angular_moments: |cos theta| > 1");
+    try {
+        CU(cudaSetDevice(ctx->device), "angular_moments");
+        cudaStream_t st = ctx->stream;
+        const long long n_rows = n_sr * n_theta;
+        const int n_m = 2 * l_max + 1, nlm = (l_max + 1) * (l_max + 1), nhalf = (l_max + 1) * (l_max + 2) / 2;
+        std::vector<double> Yw, tw;
+        angular_host_tables(l_max, n_theta, cos_theta, w_theta, n_phi, Yw, tw);
+        // tables: [tw (read as double2: first, 16-byte aligned) | Yw | w_theta]
+        const size_t tab_doubles = Yw.size() + tw.size() + (size_t)n_theta;
+        CU(ctx->d_ang_tab.ensure(tab_doubles * sizeof(double)), "angular_moments: alloc tables");
+        double* dtw = static_cast<double*>(ctx->d_ang_tab.p);
+        double* dYw = dtw + tw.size();
+        double* dw = dYw + Yw.size();
+        CU(cudaMemcpyAsync(dYw, Yw.data(), Yw.size() * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
+        CU(cudaMemcpyAsync(dtw, tw.data(), tw.size() * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
+        CU(cudaMemcpyAsync(dw, w_theta, (size_t)n_theta * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
+        const size_t fbytes = (size_t)n_rows * n_phi * 2 * sizeof(double);
+        const double* df = f;
+        if (!is_device_ptr(f)) {
+            CU(ctx->d_ang_in.ensure(fbytes), "angular_moments: alloc f");
+            CU(cudaMemcpyAsync(ctx->d_ang_in.p, f, fbytes, cudaMemcpyHostToDevice, st), "angular_moments: upload f");
+            df = static_cast<const double*>(ctx->d_ang_in.p);
+        }
+        // scratch: F [n_rows][n_m] complex, rowsum2 [n_rows]
+        CU(ctx->d_ang_F.ensure(((size_t)n_rows * n_m * 2 + (size_t)n_rows) * sizeof(double)), "angular_moments: alloc scratch");
+        double* dF = static_cast<double*>(ctx->d_ang_F.p);
+        double* drow2 = dF + (size_t)n_rows * n_m * 2;
+        const size_t rbytes = (size_t)n_sr * nlm * 2 * sizeof(double), f2bytes = (size_t)n_sr * sizeof(double);
+        const bool R_host = !is_device_ptr(R_out), f2_host = f2_out && !is_device_ptr(f2_out);
+        double *dR = R_out, *df2 = f2_out;
+        if (R_host || f2_host) {
+            CU(ctx->d_ang_out.ensure(rbytes + f2bytes), "angular_moments: alloc out");
+            if (R_host) dR = static_cast<double*>(ctx->d_ang_out.p);
+            if (f2_host) df2 = static_cast<double*>(ctx->d_ang_out.p) + (size_t)n_sr * nlm * 2;
+        }
+        (void)nhalf;
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "angular_moments: event");
+        CU(launch_phi_dft(df, dtw, n_rows, n_phi, l_max, dF, drow2, st), "angular_moments: phi kernel");
+        CU(launch_legendre(dF, drow2, dYw, dw, n_sr, n_theta, l_max, dR, df2, st), "angular_moments: legendre kernel");
+        ctx->st.last_kernel_launches = 2;
+        if (ctx->timing) {
+            CU(cudaEventRecord(ctx->ev1, st), "angular_moments: event");
+            CU(cudaEventSynchronize(ctx->ev1), "angular_moments: event sync");
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
+            ctx->st.last_kernel_ms = ms;
+        }
+        if (R_host) CU(cudaMemcpyAsync(R_out, dR, rbytes, cudaMemcpyDeviceToHost, st), "angular_moments: download R");
+        if (f2_host) CU(cudaMemcpyAsync(f2_out, df2, f2bytes, cudaMemcpyDeviceToHost, st), "angular_moments: download f2");
+        // the host tables (Yw, tw) are pageable and go out of scope: the copies must have finished
+        CU(cudaStreamSynchronize(st), "angular_moments: sync");
+        return SCARF_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(ctx, SCARF_ENOMEM, "angular_moments: out of host memory");
+    } catch (...) {
+        return fail(ctx, SCARF_EINVAL, "angular_moments: unexpected exception");
     }
 }
 

@@ -1,0 +1,106 @@
+"""GPU parity of scarf_angular_moments (Eq. (57), (59), (60) PAPER.md:380-398) against the
+CPU oracle (oracle/angular_oracle.c: the plain double quadrature), element by element."""
+import numpy as np
+import pytest
+
+from paper_2512_18010_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked tests must run on the B200 box")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def Scarf():
+    from paper_2512_18010_b200 import Scarf as S
+    return S
+
+
+def assert_close(a, b, tol):
+    scale = max(np.max(np.abs(b)), 1e-300)
+    err = np.max(np.abs(a - b))
+    assert err <= tol * scale, f"max err {err:.3e} > {tol:g} * {scale:.3e}"
+
+
+@pytest.mark.parametrize("shape,l_max", [((1, 1, 1, 1), 0), ((2, 3, 5, 7), 3), ((3, 2, 10, 16), 6), ((1, 2, 33, 70), 24),
+                                         ((2, 1, 9, 130), 12), ((1, 1, 4, 1030), 8)])
+def test_random_f_matches_oracle(oracle_mod, Scarf, torch_cuda, shape, l_max):
+    """Random complex f (not band limited: the quadrature itself is what is compared), ragged shapes, n_phi around
+    the rows-per-CTA boundaries, host and device buffers."""
+    torch = torch_cuda
+    ns, nr, nt, nph = shape
+    rng = np.random.default_rng(nt * 1000 + nph)
+    f = rng.normal(size=shape) + 1j * rng.normal(size=shape)
+    ct, w = np.polynomial.legendre.leggauss(nt)
+    R_ref, f2_ref = oracle_mod.angular_moments(f, ct, w, nph, l_max)
+    with Scarf(0) as sc:
+        fd = torch.as_tensor(f, device="cuda")
+        R, f2 = sc.angular_moments(fd, ct, w, nph, l_max, n_r=nr)
+        torch.cuda.synchronize()
+        assert_close(R.cpu().numpy(), R_ref, 1e-12)
+        assert_close(f2.cpu().numpy(), f2_ref, 1e-12)
+        Rh, f2h = sc.angular_moments(f, ct, w, nph, l_max, n_r=nr)       # host pointers
+        assert np.array_equal(Rh, R.cpu().numpy()) and np.array_equal(f2h, f2.cpu().numpy())
+        Rn, none = sc.angular_moments(fd, ct, w, nph, l_max, n_r=nr, want_f2=False)
+        assert none is None and torch.equal(Rn, R)
+
+
+def test_form_factor_pipeline_on_spherical_grid(oracle_mod, Scarf, torch_cuda):
+    """S4 on a small spherical product grid, then the moments: both steps on the GPU against both oracles; Eq. (60)
+    (Parseval) approached from below as l_max grows."""
+    torch = torch_cuda
+    w = W.make_workload(1, oracle_mod.overlap)
+    n_r, n_t, n_p, l_max = 6, 24, 48, 10
+    q = W.spherical_grid(n_r, n_t, n_p, 0.05, 6.0)
+    ct, wt = np.polynomial.legendre.leggauss(n_t)
+    f_ref = oracle_mod.form_factors(w.basis, w.T, q).reshape(1, n_r, n_t, n_p)
+    R_ref, f2_ref = oracle_mod.angular_moments(f_ref, ct, wt, n_p, l_max)
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(w.T)
+        f = sc.form_factors(torch.as_tensor(q, device="cuda"))
+        R, f2 = sc.angular_moments(f, ct, wt, n_p, l_max)
+        torch.cuda.synchronize()
+    R, f2 = R.cpu().numpy(), f2.cpu().numpy()
+    assert_close(R, R_ref, 1e-10)
+    assert_close(f2, f2_ref, 1e-10)
+    parseval = np.sum(np.abs(R) ** 2, axis=-1) / (4 * np.pi)
+    assert np.all(parseval <= f2 * (1 + 1e-12))
+    assert np.all(parseval[:, :3] >= f2[:, :3] * (1 - 1e-6))     # small |q|: few harmonics suffice
+
+
+def test_argument_checks(Scarf, torch_cuda):
+    ct, w = np.polynomial.legendre.leggauss(4)
+    f = np.zeros((1, 1, 4, 8), complex)
+    with Scarf(0) as sc:
+        with pytest.raises(Exception):
+            sc.angular_moments(f, ct, w, 8, 4)          # n_phi < 2 l_max + 1
+        with pytest.raises(Exception):
+            sc.angular_moments(f, ct * 2, w, 8, 2)      # |cos theta| > 1
+        R, f2 = sc.angular_moments(f, ct, w, 8, 3)
+        assert R.shape == (1, 1, 16) and not np.any(R) and not np.any(f2)
+
+
+def test_full_size_config5_shape_sampled(oracle_mod, Scarf, torch_cuda):
+    """Config 5's grid (12 states x 128 |q| x 64 Gauss-Legendre x 128 phi, l_max = 24) at full size in the
+    launch configuration bench.py times; seeded synthetic f (no oracle input comes from the CUDA path); compared with
+    the oracle on sampled (state, |q|) pairs."""
+    torch = torch_cuda
+    ns, nr, nt, nph, l_max = 12, 128, 64, 128, 24
+    g = torch.Generator(device="cuda").manual_seed(5)
+    f = torch.randn((ns, nr, nt, nph, 2), dtype=torch.float64, device="cuda", generator=g)
+    ct, w = np.polynomial.legendre.leggauss(nt)
+    with Scarf(0) as sc:
+        R, f2 = sc.angular_moments(torch.view_as_complex(f), ct, w, nph, l_max, n_r=nr)
+        torch.cuda.synchronize()
+    for s, r in [(0, 0), (11, 127), (5, 64), (7, 3)]:
+        fs = torch.view_as_complex(f[s, r]).cpu().numpy()[None, None]
+        R_ref, f2_ref = oracle_mod.angular_moments(fs, ct, w, nph, l_max)
+        assert_close(R[s, r].cpu().numpy(), R_ref[0, 0], 1e-12)
+        assert_close(f2[s, r].cpu().numpy(), f2_ref[0, 0], 1e-12)
