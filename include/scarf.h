@@ -161,6 +161,10 @@ int scarf_fp64_peak(int device, double* dfma_per_s, double* sm_clock_mhz);
  * scarf_host_shell_norms: c[(component, primitive)] effective coefficients of one shell, component-major. */
 int scarf_host_hermite_E(int la, int lb, double alpha, double beta, double Ax, double Bx, double* E_out);
 int scarf_host_shell_norms(int l, int nprim, const double* exponents, const double* coeffs, double* c_out);
+/* scarf_host_ylm_table: the theta part of scarf_angular_moments' quadrature, Yw[j][l(l+1)/2 + m] =
+ * w_theta[j] * N_lm P_l^m(cos_theta[j]) for 0 <= m <= l <= l_max (orthonormal Y_l^m = N_lm P_l^m e^{i m phi},
+ * Condon-Shortley phase); Yw_out [n_theta][(l_max+1)(l_max+2)/2]. */
+int scarf_host_ylm_table(int l_max, int n_theta, const double* cos_theta, const double* w_theta, double* Yw_out);
 
 #ifdef __cplusplus
 }

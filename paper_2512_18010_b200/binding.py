@@ -20,7 +20,7 @@ _CODES = {-1: "EINVAL", -2: "ESTATE", -3: "ENOMEM", -4: "ECUDA", -5: "ENODEVICE"
 
 EXPORTS = ["scarf_create", "scarf_destroy", "scarf_set_stream", "scarf_set_option", "scarf_set_basis", "scarf_nbf",
            "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_angular_moments", "scarf_get_stats", "scarf_last_error",
-           "scarf_version", "scarf_fp64_peak", "scarf_host_hermite_E", "scarf_host_shell_norms"]
+           "scarf_version", "scarf_fp64_peak", "scarf_host_hermite_E", "scarf_host_shell_norms", "scarf_host_ylm_table"]
 
 
 class ScarfStats(C.Structure):
@@ -66,6 +66,7 @@ def _load():
     L.scarf_form_factors.argtypes = [vp, C.c_int64, vp, vp]
     L.scarf_form_factors_grid.argtypes = [vp, C.c_int32, vp, C.c_int32, vp, C.c_int32, vp, vp]
     L.scarf_angular_moments.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, C.c_int32, C.c_int32, vp, vp, vp]
+    L.scarf_host_ylm_table.argtypes = [C.c_int, C.c_int, dp, dp, dp]
     L.scarf_get_stats.argtypes = [vp, C.POINTER(ScarfStats)]
     L.scarf_last_error.argtypes = [vp]
     L.scarf_last_error.restype = C.c_char_p
@@ -307,3 +308,15 @@ class Scarf:
         s = ScarfStats()
         self._check(_lib.scarf_get_stats(self._h, C.byref(s)))
         return s.as_dict()
+
+
+def host_ylm_table(l_max: int, cos_theta, w_theta) -> np.ndarray:
+    """[n_theta][(l_max+1)(l_max+2)/2]: w_j N_lm P_l^m(cos theta_j), index l(l+1)/2 + m (host code of the library)."""
+    ct = np.ascontiguousarray(cos_theta, dtype=np.float64)
+    wt = np.ascontiguousarray(w_theta, dtype=np.float64)
+    out = np.zeros((ct.shape[0], (l_max + 1) * (l_max + 2) // 2))
+    dp = C.POINTER(C.c_double)
+    rc = _lib.scarf_host_ylm_table(int(l_max), int(ct.shape[0]), ct.ctypes.data_as(dp), wt.ctypes.data_as(dp), out.ctypes.data_as(dp))
+    if rc != SCARF_OK:
+        raise ScarfError(rc, "scarf_host_ylm_table failed")
+    return out

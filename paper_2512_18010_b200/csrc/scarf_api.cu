@@ -773,6 +773,17 @@ int scarf_host_hermite_E(int la, int lb, double alpha, double beta, double Ax, d
     return SCARF_OK;
 }
 
+int scarf_host_ylm_table(int l_max, int n_theta, const double* cos_theta, const double* w_theta, double* Yw_out)
+{
+    if (l_max < 0 || l_max > 64 || n_theta < 1 || !cos_theta || !w_theta || !Yw_out) return SCARF_EINVAL;
+    for (int j = 0; j < n_theta; ++j)
+        if (!(std::fabs(cos_theta[j]) <= 1.0)) return SCARF_EINVAL;
+    std::vector<double> Yw, tw;
+    angular_host_tables(l_max, n_theta, cos_theta, w_theta, 1, Yw, tw);
+    std::memcpy(Yw_out, Yw.data(), Yw.size() * sizeof(double));
+    return SCARF_OK;
+}
+
 int scarf_host_shell_norms(int l, int nprim, const double* exponents, const double* coeffs, double* c_out)
 {
     if (!exponents || !coeffs || !c_out || l < 0 || l > kMaxL || nprim < 1) return SCARF_EINVAL;

@@ -1,0 +1,111 @@
+"""CPU tests (no GPU, no compute kernels) of the C-ABI library: it loads, exports every symbol include/scarf.h declares,
+its host-side steps S0-S2 (shell normalisation, Gaussian product, McMurchie-Davidson E coefficients, overlap) and the
+host table of scarf_angular_moments agree with the oracle / quadrature / scipy, and the device entry points refuse a
+host-only context instead of falling back to the CPU."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2512_18010_b200 import workloads as W
+from tests import bruteforce as BF
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def binding():
+    from paper_2512_18010_b200 import binding as b
+    return b
+
+
+def test_every_declared_symbol_is_exported(binding):
+    hdr = open(os.path.join(ROOT, "include", "scarf.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b(scarf_[A-Za-z0-9_]+)\s*\(", hdr))
+    assert {"scarf_set_basis", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid",
+            "scarf_angular_moments"} <= names
+    lib = C.CDLL(binding.LIB_PATH)
+    for n in sorted(names):
+        assert hasattr(lib, n), f"{n} declared in include/scarf.h but not exported by libscarf.so"
+    assert names == set(binding.EXPORTS), names ^ set(binding.EXPORTS)
+    assert b"sm_100a" in binding.version().encode()
+
+
+def test_host_only_context_has_no_cpu_fallback(binding, oracle_mod):
+    w = W.make_workload(1, oracle_mod.overlap)
+    with binding.Scarf(None) as sc:
+        sc.set_basis(w.basis)
+        assert sc.nbf == w.basis.nbf
+        for call in (lambda: sc.set_transitions(w.T), lambda: sc.form_factors(w.q[:4]),
+                     lambda: sc.form_factors_grid(np.zeros(2), np.zeros(2), np.zeros(2)),
+                     lambda: sc.angular_moments(np.zeros((1, 1, 2, 4), complex), np.array([-0.5, 0.5]), np.ones(2), 4, 1)):
+            with pytest.raises(binding.ScarfError) as e:
+                call()
+            assert e.value.code in (binding.SCARF_ENODEVICE, binding.SCARF_ESTATE)
+
+
+@pytest.mark.parametrize("config", [1, 2])
+def test_host_overlap_matches_oracle(binding, oracle_mod, config):
+    """S0-S2 on the host (alpha-form, McMurchie-Davidson) against the oracle's sigma-form Eq. (38)-(46) at q = 0."""
+    w = W.make_workload(config, oracle_mod.overlap, with_q=False)
+    with binding.Scarf(None) as sc:
+        sc.set_basis(w.basis)
+        S = sc.overlap()
+        st = sc.stats()
+    assert np.max(np.abs(S - oracle_mod.overlap(w.basis))) <= 1e-12
+    assert np.allclose(np.diag(S), 1.0, atol=1e-13)
+    n = int(np.sum(w.basis.shell_nprim))
+    assert st["n_pairs_all"] == n * (n + 1) // 2 and st["nbf"] == w.basis.nbf
+
+
+def test_hermite_E_against_quadrature(binding):
+    """(x-A)^i (x-B)^j e^{-a(x-A)^2 - b(x-B)^2} = sum_t E_t^{ij} (d/dP)^t e^{-p(x-P)^2}  =>
+    Int ... e^{iqx} dx = sqrt(pi/p) e^{-q^2/4p} e^{iqP} sum_t E_t^{ij} (iq)^t; left side by trapezoid quadrature."""
+    a, b, A, B = 0.9, 1.7, -0.4, 0.55
+    p, P = a + b, (a * A + b * B) / (a + b)
+    E = binding.host_hermite_E(3, 3, a, b, A, B)
+    for q in (0.0, 0.8, -2.3):
+        for i in range(4):
+            for j in range(4):
+                lhs = BF._int1d(i, A, a, j, B, b, q)
+                rhs = np.sqrt(np.pi / p) * np.exp(-q * q / (4 * p)) * np.exp(1j * q * P) * sum(
+                    E[i, j, t] * (1j * q) ** t for t in range(i + j + 1))
+                assert abs(lhs - rhs) <= 1e-12 * max(1.0, abs(lhs)), (q, i, j)
+
+
+def test_shell_norms_against_oracle(binding, oracle_mod):
+    """Effective coefficients N_mu d_k xi_k of a contracted shell: every component has unit self-overlap."""
+    e, d = np.array([2.3, 0.7, 0.25]), np.array([0.4, 0.9, 0.6])
+    for l in range(4):
+        c = binding.host_shell_norms(l, e, d)
+        b = W.Basis(np.zeros((1, 3)), np.array([0], np.int32), np.array([l], np.int32), np.array([3], np.int32), e, d)
+        xi, N = oracle_mod.norms(b)
+        ncomp = (l + 1) * (l + 2) // 2
+        ref = (N[:, None] * d[None, :]) * xi.reshape(ncomp, 3)
+        assert np.max(np.abs(c - ref)) <= 1e-13 * np.max(np.abs(ref))
+
+
+def test_host_ylm_table_against_scipy(binding):
+    from scipy import special as sp
+    l_max = 24
+    ct, w = np.polynomial.legendre.leggauss(9)
+    Yw = binding.host_ylm_table(l_max, ct, w)
+    for l in range(l_max + 1):
+        for m in range(l + 1):
+            ref = w * sp.sph_harm_y(l, m, np.arccos(ct), 0.0).real
+            assert np.max(np.abs(Yw[:, l * (l + 1) // 2 + m] - ref)) <= 1e-15 + 2e-13 * np.max(np.abs(ref)), (l, m)
+
+
+def test_bad_arguments_are_rejected_on_the_host(binding):
+    with binding.Scarf(None) as sc:
+        good = dict(atom_xyz=np.zeros((1, 3)), shell_atom=[0], shell_l=[0], shell_nprim=[1], exponents=[1.0], coeffs=[1.0])
+        sc.set_basis(**good)
+        for bad in (dict(good, shell_l=[4]), dict(good, exponents=[-1.0]), dict(good, shell_atom=[3]),
+                    dict(good, exponents=[np.nan])):
+            with pytest.raises(binding.ScarfError):
+                sc.set_basis(**bad)
+        with pytest.raises(binding.ScarfError):
+            sc.set_option("no_such_option", 1.0)
