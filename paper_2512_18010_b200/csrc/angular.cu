@@ -40,22 +40,39 @@ __global__ void __launch_bounds__(kThreads) phi_dft_kernel(const double2* __rest
     for (int i = threadIdx.x; i < nrow * n_phi; i += kThreads) s_f[i] = src[i];
     __syncthreads();
     const double scale = 6.283185307179586476925286766559 / (double)n_phi;
-    for (int o = threadIdx.x; o < nrow * n_m; o += kThreads) {
-        const int row = o / n_m, m = o % n_m - l_max;
-        const int step = ((m % n_phi) + n_phi) % n_phi;
-        const double2* fr = s_f + row * n_phi;
-        double ar = 0.0, ai = 0.0;
+    // one work item = (pair of rows, |m|): the twiddle e^{-i m phi_k} serves +m and -m (conjugate) and both rows,
+    // 16 FMAs per 3 shared-memory loads
+    const int n_rp = (nrow + 1) / 2, n_ma = l_max + 1;
+    for (int o = threadIdx.x; o < n_rp * n_ma; o += kThreads) {
+        const int rp = o / n_ma, ma = o % n_ma;
+        const int r0 = 2 * rp, r1 = min(2 * rp + 1, nrow - 1);
+        const double2* f0 = s_f + r0 * n_phi;
+        const double2* f1 = s_f + r1 * n_phi;
+        double pr0 = 0.0, pi0 = 0.0, nr0 = 0.0, ni0 = 0.0, pr1 = 0.0, pi1 = 0.0, nr1 = 0.0, ni1 = 0.0;
         int idx = 0;
         for (int k = 0; k < n_phi; ++k) {
-            const double2 v = fr[k], t = s_tw[idx];        // t = e^{-2 pi i idx / n_phi}
-            ar = fma(v.x, t.x, ar);
-            ar = fma(-v.y, t.y, ar);
-            ai = fma(v.x, t.y, ai);
-            ai = fma(v.y, t.x, ai);
-            idx += step;
+            const double2 t = s_tw[idx];                    // (cos, -sin)(2 pi idx / n_phi) = e^{-i ma phi_k}
+            const double2 u = f0[k], v = f1[k];
+            // +ma: f * t ;  -ma: f * conj(t)
+            pr0 = fma(u.x, t.x, pr0); pr0 = fma(-u.y, t.y, pr0);
+            pi0 = fma(u.x, t.y, pi0); pi0 = fma(u.y, t.x, pi0);
+            nr0 = fma(u.x, t.x, nr0); nr0 = fma(u.y, t.y, nr0);
+            ni0 = fma(-u.x, t.y, ni0); ni0 = fma(u.y, t.x, ni0);
+            pr1 = fma(v.x, t.x, pr1); pr1 = fma(-v.y, t.y, pr1);
+            pi1 = fma(v.x, t.y, pi1); pi1 = fma(v.y, t.x, pi1);
+            nr1 = fma(v.x, t.x, nr1); nr1 = fma(v.y, t.y, nr1);
+            ni1 = fma(-v.x, t.y, ni1); ni1 = fma(v.y, t.x, ni1);
+            idx += ma;
             if (idx >= n_phi) idx -= n_phi;
         }
-        F[(size_t)(row0 + row) * n_m + (m + l_max)] = make_double2(ar * scale, ai * scale);
+        double2* F0 = F + (size_t)(row0 + r0) * n_m + l_max;
+        F0[ma] = make_double2(pr0 * scale, pi0 * scale);
+        F0[-ma] = make_double2(nr0 * scale, ni0 * scale);
+        if (r1 != r0) {
+            double2* F1 = F + (size_t)(row0 + r1) * n_m + l_max;
+            F1[ma] = make_double2(pr1 * scale, pi1 * scale);
+            F1[-ma] = make_double2(nr1 * scale, ni1 * scale);
+        }
     }
     // |f|^2 row sums: one warp per row, lanes stride over k, fixed-order shuffle tree (deterministic)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
