@@ -108,6 +108,15 @@ int scarf_set_basis(scarf_ctx* ctx, int n_atoms, const double* atom_xyz, int n_s
                     const int32_t* shell_l, const int32_t* shell_nprim, const double* exponents,
                     const double* coeffs);
 
+/* As scarf_set_basis, with shell_pure[i] != 0 marking shell i as PURE (real solid harmonics, 2l+1 functions, order
+ * m = -l..l: d = xy, yz, 2z^2-x^2-y^2, xz, x^2-y^2; f = y(3x^2-y^2), xyz, y(4z^2-x^2-y^2), z(2z^2-3x^2-3y^2),
+ * x(4z^2-x^2-y^2), z(x^2-y^2), x(x^2-3y^2); each normalised to 1) — the multi-term Cartesian orbitals of Eq. (A2)
+ * PAPER.md:625-627.  The flag is ignored for l < 2.  shell_pure == NULL: all Cartesian.  scarf_nbf, scarf_overlap
+ * and the T of scarf_set_transitions are then in that mixed basis; internally T_cart = C T C^T. */
+int scarf_set_basis_pure(scarf_ctx* ctx, int n_atoms, const double* atom_xyz, int n_shells, const int32_t* shell_atom,
+                         const int32_t* shell_l, const int32_t* shell_nprim, const double* exponents,
+                         const double* coeffs, const int32_t* shell_pure);
+
 int scarf_nbf(const scarf_ctx* ctx); /* number of contracted Cartesian basis functions, or a negative code */
 
 /* AO overlap S[nbf][nbf] (= Int phi_mu phi_nu, the q = 0 pair integral) into HOST memory, from the S1/S2 tables. */

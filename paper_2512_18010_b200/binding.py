@@ -18,7 +18,7 @@ SCARF_MAX_L = 3
 SCARF_N_CLASSES = 2 * SCARF_MAX_L + 1
 _CODES = {-1: "EINVAL", -2: "ESTATE", -3: "ENOMEM", -4: "ECUDA", -5: "ENODEVICE"}
 
-EXPORTS = ["scarf_create", "scarf_destroy", "scarf_set_stream", "scarf_set_option", "scarf_set_basis", "scarf_nbf",
+EXPORTS = ["scarf_create", "scarf_destroy", "scarf_set_stream", "scarf_set_option", "scarf_set_basis", "scarf_set_basis_pure", "scarf_nbf",
            "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_angular_moments", "scarf_get_stats", "scarf_last_error",
            "scarf_version", "scarf_fp64_peak", "scarf_host_hermite_E", "scarf_host_shell_norms", "scarf_host_ylm_table"]
 
@@ -60,6 +60,7 @@ def _load():
     L.scarf_set_stream.argtypes = [vp, vp]
     L.scarf_set_option.argtypes = [vp, C.c_char_p, C.c_double]
     L.scarf_set_basis.argtypes = [vp, C.c_int, dp, C.c_int, ip, ip, ip, dp, dp]
+    L.scarf_set_basis_pure.argtypes = [vp, C.c_int, dp, C.c_int, ip, ip, ip, dp, dp, ip]
     L.scarf_nbf.argtypes = [vp]
     L.scarf_overlap.argtypes = [vp, dp]
     L.scarf_set_transitions.argtypes = [vp, C.c_int, vp]
@@ -184,7 +185,7 @@ class Scarf:
         self._check(_lib.scarf_set_option(self._h, key.encode(), float(value)))
 
     def set_basis(self, basis=None, *, atom_xyz=None, shell_atom=None, shell_l=None, shell_nprim=None,
-                  exponents=None, coeffs=None):
+                  exponents=None, coeffs=None, shell_pure=None):
         if basis is not None:
             atom_xyz, shell_atom, shell_l = basis.atom_xyz, basis.shell_atom, basis.shell_l
             shell_nprim, exponents, coeffs = basis.shell_nprim, basis.exponents, basis.coeffs
@@ -196,7 +197,14 @@ class Scarf:
         d = np.ascontiguousarray(coeffs, np.float64)
         if not (sa.size == sl.size == sn.size) or e.size != d.size or e.size != int(sn.sum()):
             raise ValueError("set_basis: inconsistent array lengths")
-        self._check(_lib.scarf_set_basis(self._h, xyz.shape[0], _dp(xyz), sl.size, _ip(sa), _ip(sl), _ip(sn), _dp(e), _dp(d)))
+        if shell_pure is None:
+            self._check(_lib.scarf_set_basis(self._h, xyz.shape[0], _dp(xyz), sl.size, _ip(sa), _ip(sl), _ip(sn), _dp(e), _dp(d)))
+        else:
+            sp = np.ascontiguousarray(shell_pure, np.int32)
+            if sp.size != sl.size:
+                raise ValueError("set_basis: shell_pure must have one entry per shell")
+            self._check(_lib.scarf_set_basis_pure(self._h, xyz.shape[0], _dp(xyz), sl.size, _ip(sa), _ip(sl), _ip(sn), _dp(e), _dp(d),
+                                                  _ip(sp)))
         self._nbf = int(_lib.scarf_nbf(self._h))
         self.n_states = 0
 

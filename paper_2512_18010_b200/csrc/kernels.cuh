@@ -116,6 +116,14 @@ cudaError_t launch_phi_dft(const double* f, const double* tw, long long n_rows, 
 cudaError_t launch_legendre(const double* F, const double* rowsum2, const double* Yw, const double* w_theta, long long n_sr,
                             int n_theta, int l_max, double* R, double* f2, cudaStream_t st);
 
+// pure (solid-harmonic) shells (pure.cu, NEXT-5): T_cart = C T_user C^T
+constexpr int kPureMaxNnz = 4;              // user functions one Cartesian component contributes to, at most
+void pure_matrix(int l, double* C);         // [ncart(l)][2l+1]
+int build_pure_map(int n_shells, const int32_t* shell_l, const int32_t* shell_pure, std::vector<int>& nnz, std::vector<int>& uidx,
+                   std::vector<double>& ucoef);
+cudaError_t launch_transform_T(const double* Tu, double* Tc, int n_states, int nbf_u, int nbf_c, const int* nnz, const int* uidx,
+                               const double* ucoef, cudaStream_t st);
+
 cudaError_t run_fp64_peak(double* dfma_per_s, double* sm_clock_mhz);
 
 }  // namespace scarf

@@ -53,9 +53,13 @@ struct scarf_ctx {
     std::string err;
     HostSetup hs;
     bool have_basis = false, have_T = false;
+    bool any_pure = false;                 // some shell is pure: T and S are mapped through pure_*
+    int nbf_user = 0;                      // basis functions as the caller counts them
+    std::vector<int> pure_nnz, pure_uidx;
+    std::vector<double> pure_ucoef;
     int n_states = 0;
     int sm_count = 148;
-    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb, d_partial, d_axes, d_tab, d_ang_in, d_ang_F, d_ang_tab, d_ang_out;
+    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb, d_partial, d_axes, d_tab, d_ang_in, d_ang_F, d_ang_tab, d_ang_out, d_pure_map, d_Tcart;
     std::vector<DevBuf> staging, packed;
     std::vector<TileStream> tiles;
     scarf_stats st = {};
@@ -160,6 +164,7 @@ void free_device(scarf_ctx* c)
     c->d_out.release(); c->d_src.release(); c->d_dst.release(); c->d_nb.release(); c->d_partial.release();
     c->d_axes.release(); c->d_tab.release();
     c->d_ang_in.release(); c->d_ang_F.release(); c->d_ang_tab.release(); c->d_ang_out.release();
+    c->d_pure_map.release(); c->d_Tcart.release();
     for (auto& b : c->staging) b.release();
     for (auto& b : c->packed) b.release();
     c->staging.clear(); c->packed.clear(); c->tiles.clear();
@@ -245,6 +250,13 @@ int scarf_set_option(scarf_ctx* ctx, const char* key, double value)
 int scarf_set_basis(scarf_ctx* ctx, int n_atoms, const double* atom_xyz, int n_shells, const int32_t* shell_atom,
                     const int32_t* shell_l, const int32_t* shell_nprim, const double* exponents, const double* coeffs)
 {
+    return scarf_set_basis_pure(ctx, n_atoms, atom_xyz, n_shells, shell_atom, shell_l, shell_nprim, exponents, coeffs, nullptr);
+}
+
+int scarf_set_basis_pure(scarf_ctx* ctx, int n_atoms, const double* atom_xyz, int n_shells, const int32_t* shell_atom,
+                         const int32_t* shell_l, const int32_t* shell_nprim, const double* exponents, const double* coeffs,
+                         const int32_t* shell_pure)
+{
     if (!ctx) return SCARF_EINVAL;
     try {
         const auto t0 = std::chrono::steady_clock::now();
@@ -253,6 +265,19 @@ int scarf_set_basis(scarf_ctx* ctx, int n_atoms, const double* atom_xyz, int n_s
         int rc = build_setup(n_atoms, atom_xyz, n_shells, shell_atom, shell_l, shell_nprim, exponents, coeffs, ctx->hs, err);
         if (rc != SCARF_OK) return fail(ctx, rc, err);
         const HostSetup& hs = ctx->hs;
+        ctx->any_pure = false;
+        if (shell_pure)
+            for (int i = 0; i < n_shells; ++i) ctx->any_pure = ctx->any_pure || (shell_pure[i] != 0 && shell_l[i] >= 2);
+        ctx->nbf_user = build_pure_map(n_shells, shell_l, ctx->any_pure ? shell_pure : nullptr, ctx->pure_nnz, ctx->pure_uidx, ctx->pure_ucoef);
+        if (!ctx->host_only && ctx->any_pure) {
+            CU(cudaSetDevice(ctx->device), "set_basis");
+            const size_t nb = (size_t)hs.nbf, bytes = nb * 4 + nb * kPureMaxNnz * 4 + nb * kPureMaxNnz * 8 + 64;
+            CU(ctx->d_pure_map.ensure(bytes), "set_basis: alloc pure map");
+            char* base = static_cast<char*>(ctx->d_pure_map.p);   // [ucoef (8-byte aligned) | uidx | nnz]
+            CU(cudaMemcpyAsync(base, ctx->pure_ucoef.data(), nb * kPureMaxNnz * 8, cudaMemcpyHostToDevice, ctx->stream), "set_basis: upload");
+            CU(cudaMemcpyAsync(base + nb * kPureMaxNnz * 8, ctx->pure_uidx.data(), nb * kPureMaxNnz * 4, cudaMemcpyHostToDevice, ctx->stream), "set_basis: upload");
+            CU(cudaMemcpyAsync(base + nb * kPureMaxNnz * 12, ctx->pure_nnz.data(), nb * 4, cudaMemcpyHostToDevice, ctx->stream), "set_basis: upload");
+        }
         if (!ctx->host_only) {
             CU(cudaSetDevice(ctx->device), "set_basis");
             CU(ctx->d_pairs.ensure(std::max<size_t>(64, hs.pairs.size() * sizeof(PairMeta))), "set_basis: alloc pairs");
@@ -264,7 +289,7 @@ int scarf_set_basis(scarf_ctx* ctx, int n_atoms, const double* atom_xyz, int n_s
         scarf_stats& st = ctx->st;
         st = scarf_stats();
         st.n_atoms = hs.n_atoms; st.n_shells = hs.n_shells; st.n_prim_shells = (int32_t)hs.prim.size();
-        st.nbf = hs.nbf; st.l_max = hs.l_max;
+        st.nbf = ctx->nbf_user; st.l_max = hs.l_max;
         st.n_pairs_all = hs.n_pairs_all;
         st.n_pairs_prescreened = (int64_t)hs.pairs.size();
         st.cart_term_pairs = hs.cart_term_pairs;
@@ -282,14 +307,36 @@ int scarf_nbf(const scarf_ctx* ctx)
 {
     if (!ctx) return SCARF_EINVAL;
     if (!ctx->have_basis) return SCARF_ESTATE;
-    return ctx->hs.nbf;
+    return ctx->nbf_user;
 }
 
 int scarf_overlap(scarf_ctx* ctx, double* S_host)
 {
     if (!ctx || !S_host) return SCARF_EINVAL;
     if (!ctx->have_basis) return fail(ctx, SCARF_ESTATE, "overlap: set_basis first");
-    overlap_from_setup(ctx->hs, S_host);
+    if (!ctx->any_pure) {
+        overlap_from_setup(ctx->hs, S_host);
+        return SCARF_OK;
+    }
+    try {   // S_user = C^T S_cart C
+        const int nc = ctx->hs.nbf, nu = ctx->nbf_user;
+        std::vector<double> Sc((size_t)nc * nc), half((size_t)nc * nu, 0.0);
+        overlap_from_setup(ctx->hs, Sc.data());
+        for (int mu = 0; mu < nc; ++mu)
+            for (int nv = 0; nv < nc; ++nv)
+                for (int k = 0; k < ctx->pure_nnz[nv]; ++k)
+                    half[(size_t)mu * nu + ctx->pure_uidx[(size_t)nv * kPureMaxNnz + k]] +=
+                        Sc[(size_t)mu * nc + nv] * ctx->pure_ucoef[(size_t)nv * kPureMaxNnz + k];
+        std::memset(S_host, 0, sizeof(double) * (size_t)nu * nu);
+        for (int mu = 0; mu < nc; ++mu)
+            for (int k = 0; k < ctx->pure_nnz[mu]; ++k) {
+                const int a = ctx->pure_uidx[(size_t)mu * kPureMaxNnz + k];
+                const double c = ctx->pure_ucoef[(size_t)mu * kPureMaxNnz + k];
+                for (int b = 0; b < nu; ++b) S_host[(size_t)a * nu + b] += c * half[(size_t)mu * nu + b];
+            }
+    } catch (const std::bad_alloc&) {
+        return fail(ctx, SCARF_ENOMEM, "overlap: out of host memory");
+    }
     return SCARF_OK;
 }
 
@@ -302,7 +349,7 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T)
     try {
         ctx->have_T = false;
         const HostSetup& hs = ctx->hs;
-        const size_t nbf = (size_t)hs.nbf, tsz = (size_t)n_states * nbf * nbf;
+        const size_t nbf = (size_t)ctx->nbf_user, tsz = (size_t)n_states * nbf * nbf;
         const long long np = (long long)hs.pairs.size();
         CU(cudaSetDevice(ctx->device), "set_transitions");
         cudaStream_t st = ctx->stream;
@@ -312,6 +359,15 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T)
             CU(ctx->d_T.ensure(tsz * sizeof(double)), "set_transitions: alloc T");
             CU(cudaMemcpyAsync(ctx->d_T.p, T, tsz * sizeof(double), cudaMemcpyHostToDevice, st), "set_transitions: upload T");
             dT = static_cast<const double*>(ctx->d_T.p);
+        }
+        if (ctx->any_pure) {   // T_cart = C T_user C^T (pure.cu); the fold works on Cartesian components
+            const size_t nc = (size_t)hs.nbf;
+            CU(ctx->d_Tcart.ensure((size_t)n_states * nc * nc * sizeof(double)), "set_transitions: alloc T_cart");
+            const char* base = static_cast<const char*>(ctx->d_pure_map.p);
+            CU(launch_transform_T(dT, static_cast<double*>(ctx->d_Tcart.p), n_states, ctx->nbf_user, hs.nbf,
+                                  reinterpret_cast<const int*>(base + nc * kPureMaxNnz * 12), reinterpret_cast<const int*>(base + nc * kPureMaxNnz * 8),
+                                  reinterpret_cast<const double*>(base), st), "set_transitions: pure transform kernel");
+            dT = static_cast<const double*>(ctx->d_Tcart.p);
         }
         // state tiles
         std::vector<TileStream> tiles;

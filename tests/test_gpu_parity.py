@@ -229,3 +229,28 @@ def test_threshold_eps_error_within_reported_bound(oracle_mod, Scarf, torch_cuda
     assert st1["dropped_bound"] >= st0["dropped_bound"] >= 0.0
     err = np.max(np.abs(f1 - f_ref))
     assert err <= st1["dropped_bound"] + TOL * np.max(np.abs(f_ref))
+
+
+def test_pure_shells_mixed_basis(oracle_mod, Scarf, torch_cuda):
+    """NEXT-5: pure d/f shells mixed with Cartesian ones (scarf_set_basis_pure): T, nbf and the result in the mixed
+    basis; oracle = oracle/pure.py (solid harmonics from scipy's Y_lm, through the pinned Cartesian oracle)."""
+    torch = torch_cuda
+    from oracle import pure as opure
+    from tests.test_oracle_pure import mixed_basis
+    b, pure = mixed_basis()
+    rng = np.random.default_rng(21)
+    nbf = opure.basis_matrix(b, pure).shape[1]
+    T = rng.normal(size=(12, nbf, nbf))
+    q = rng.uniform(-5, 5, size=(300, 3))
+    f_ref = opure.form_factors(b, pure, T, q)
+    with Scarf(0) as sc:
+        sc.set_basis(b, shell_pure=pure)
+        assert sc.nbf == nbf
+        sc.set_transitions(torch.as_tensor(T, device="cuda"))
+        f = sc.form_factors(torch.as_tensor(q, device="cuda"))
+        torch.cuda.synchronize()
+        assert_parity(f.cpu().numpy(), f_ref)
+        sc.set_transitions(T)                                   # host pointer, same result
+        assert np.array_equal(sc.form_factors(q), f.cpu().numpy())
+        sc.set_basis(b)                                         # back to all-Cartesian on the same context
+        assert sc.nbf == b.nbf
