@@ -155,6 +155,16 @@ int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t
                           const double* w_theta, int32_t n_phi, int32_t l_max, const double* f, double* R_out,
                           double* f2_out);
 
+/* The paper's FFT method (Section III, Eq. (19)-(34) PAPER.md:140-222) as a second, APPROXIMATE
+ * route to f_s: the transition density Phi_s(x) = g sum_pq T_pq phi_q(x) phi_p(x) (Eq. 20) is tabulated at
+ * x_abc = x_min + box_len * (a/nx, b/ny, c/nz) (Eq. 25-28) and transformed (cuFFT, loaded at first use),
+ *     out[s][(ia*ny + ib)*nz + ic] = V_pix sum_abc Phi_abc exp(+i q.x_abc),  q = 2 pi ((ia - nx/2)/box_len[0], ...)
+ * (Eq. 27, 30-33; integer division; "most negative frequencies first").  Accuracy is set by the box (truncation) and
+ * the spacing (aliasing beyond pi/h), not by this library.  x_min, box_len: HOST double[3].  out [n_states][nx*ny*nz][2],
+ * host or device.  Scratch: nbf*nx*ny*nz doubles + 2 complex arrays of the output size (SCARF_ENOMEM above 64 GB). */
+int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, const double* x_min, const double* box_len,
+                           double* out);
+
 int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out);
 const char* scarf_last_error(const scarf_ctx* ctx);
 const char* scarf_version(void);

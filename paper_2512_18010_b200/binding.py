@@ -19,7 +19,7 @@ SCARF_N_CLASSES = 2 * SCARF_MAX_L + 1
 _CODES = {-1: "EINVAL", -2: "ESTATE", -3: "ENOMEM", -4: "ECUDA", -5: "ENODEVICE"}
 
 EXPORTS = ["scarf_create", "scarf_destroy", "scarf_set_stream", "scarf_set_option", "scarf_set_basis", "scarf_set_basis_pure", "scarf_nbf",
-           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_angular_moments", "scarf_get_stats", "scarf_last_error",
+           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_angular_moments", "scarf_fft_form_factors", "scarf_get_stats", "scarf_last_error",
            "scarf_version", "scarf_fp64_peak", "scarf_host_hermite_E", "scarf_host_shell_norms", "scarf_host_ylm_table"]
 
 
@@ -68,6 +68,7 @@ def _load():
     L.scarf_form_factors_grid.argtypes = [vp, C.c_int32, vp, C.c_int32, vp, C.c_int32, vp, vp]
     L.scarf_angular_moments.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, C.c_int32, C.c_int32, vp, vp, vp]
     L.scarf_host_ylm_table.argtypes = [C.c_int, C.c_int, dp, dp, dp]
+    L.scarf_fft_form_factors.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, vp]
     L.scarf_get_stats.argtypes = [vp, C.POINTER(ScarfStats)]
     L.scarf_last_error.argtypes = [vp]
     L.scarf_last_error.restype = C.c_char_p
@@ -311,6 +312,26 @@ class Scarf:
             import torch
             return torch.view_as_complex(R), f2
         return R.view(np.complex128)[..., 0], f2
+
+    def fft_form_factors(self, n, x_min, box_len, out=None, device_out=True):
+        """The paper's FFT method on an n = (nx, ny, nz) real-space grid in the box [x_min, x_min + box_len).
+        Returns complex128 [n_states][nx*ny*nz] at q = 2 pi ((ia - nx//2)/Lx, ...) (torch cuda tensor by default)."""
+        nx, ny, nz = (int(v) for v in n)
+        xm = np.ascontiguousarray(x_min, dtype=np.float64).reshape(3)
+        bl = np.ascontiguousarray(box_len, dtype=np.float64).reshape(3)
+        n_q = nx * ny * nz
+        if out is None:
+            if device_out:
+                import torch
+                out = torch.empty((self.n_states, n_q, 2), dtype=torch.float64, device=f"cuda:{self.device}")
+            else:
+                out = np.empty((self.n_states, n_q, 2))
+        op, okeep = _ptr(out, "out", self.n_states * n_q * 2)
+        self._check(_lib.scarf_fft_form_factors(self._h, nx, ny, nz, _dp(xm), _dp(bl), op))
+        if _is_torch(out):
+            import torch
+            return torch.view_as_complex(out.view(self.n_states, n_q, 2))
+        return out.reshape(self.n_states, n_q, 2).view(np.complex128)[..., 0]
 
     def stats(self) -> dict:
         s = ScarfStats()

@@ -1,0 +1,214 @@
+// fft_method.cu — the paper's FFT method as a second route to f_s(q) (Section III, Eq. (19)-(34)
+// PAPER.md:140-222): tabulate the transition density on a regular real-space grid and transform it.
+//
+//   x_abc = x_min + L (a/N_x, b/N_y, c/N_z)                                   Eq. (25)-(28)
+//   Phi_s(x) = g sum_pq T^s_pq phi_q(x) phi_p(x),  g = 2                      Eq. (20)
+//   f_s(q) ~= V_pix sum_abc Phi_abc e^{+i q.x_abc},  q = 2 pi (alpha/L_x, beta/L_y, gamma/L_z)    Eq. (27), (30)-(33)
+//   output index ia <-> alpha = ia - floor(N/2)  ("most negative frequencies first")
+//
+// Kernels: orbital_kernel (values of every contracted Cartesian orbital at every grid point, V[mu][point]),
+// density_kernel (the quadratic form v^T T^s v for up to 12 states per pass, T blocks staged in shared memory and
+// read with broadcast loads, the upper triangle only), cuFFT Z2Z (library step, loaded with dlopen at first use so that
+// libscarf.so itself has no cuFFT dependency), fft_post_kernel (V_pix, the phase e^{i q.x_min}, the reordering).
+// This is an approximation of f_s (box truncation, grid spacing); its CPU oracle is oracle/fft_method.py.
+#include <dlfcn.h>
+
+#include <cmath>
+
+#include "kernels.cuh"
+
+namespace scarf {
+
+namespace {
+
+constexpr int kPts = 128;     // points per CTA
+constexpr int kNB = 16, kMB = 8;
+
+__device__ __forceinline__ double dfo(int n)   // (2n-1)!!
+{
+    double r = 1.0;
+    for (int k = 2 * n - 1; k > 1; k -= 2) r *= k;
+    return r;
+}
+
+__global__ void __launch_bounds__(kPts) orbital_kernel(const PrimShell* __restrict__ prim, const int* __restrict__ shell_first,
+                                                       FftGrid g, double* __restrict__ V)
+{
+    const long long p = (long long)blockIdx.x * kPts + threadIdx.x;
+    if (p >= g.P) return;
+    const int sh = blockIdx.y;
+    const int k0 = shell_first[sh], k1 = shell_first[sh + 1];
+    const int ic = (int)(p % g.nz), ib = (int)((p / g.nz) % g.ny), ia = (int)(p / ((long long)g.nz * g.ny));
+    const PrimShell& ps = prim[k0];
+    const double dx = g.xmin[0] + g.len[0] * ((double)ia / g.nx) - ps.A[0];
+    const double dy = g.xmin[1] + g.len[1] * ((double)ib / g.ny) - ps.A[1];
+    const double dz = g.xmin[2] + g.len[2] * ((double)ic / g.nz) - ps.A[2];
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    double rad = 0.0;
+    for (int k = k0; k < k1; ++k) rad = fma(prim[k].cprim, exp(-prim[k].alpha * r2), rad);
+    const int l = ps.l;
+    double px[kMaxL + 1], py[kMaxL + 1], pz[kMaxL + 1];
+    px[0] = py[0] = pz[0] = 1.0;
+#pragma unroll
+    for (int i = 1; i <= kMaxL; ++i) { px[i] = px[i - 1] * dx; py[i] = py[i - 1] * dy; pz[i] = pz[i - 1] * dz; }
+    int c = 0;
+    for (int a = l; a >= 0; --a)                        // component order: a descending, then b descending
+        for (int b = l - a; b >= 0; --b) {
+            const int cc = l - a - b;
+            V[(size_t)(ps.bf0 + c) * g.P + p] = rad * px[a] * py[b] * pz[cc] * rsqrt(dfo(a) * dfo(b) * dfo(cc));
+            ++c;
+        }
+}
+
+// Phi_s(p) = g sum_{mu <= nu} c_{mu nu} v_mu v_nu,  c = T_mumu on the diagonal, T_munu + T_numu above it.
+__global__ void __launch_bounds__(kPts) density_kernel(const double* __restrict__ V, const double* __restrict__ T, int nbf, long long P,
+                                                       int s0, int ns, double g, double2* __restrict__ out)
+{
+    __shared__ __align__(16) double sT[kMaxStateTile][kMB][kNB];
+    const long long p = (long long)blockIdx.x * kPts + threadIdx.x;
+    const bool valid = p < P;
+    double acc[kMaxStateTile];
+#pragma unroll
+    for (int s = 0; s < kMaxStateTile; ++s) acc[s] = 0.0;
+    for (int nb0 = 0; nb0 < nbf; nb0 += kNB) {
+        double v[kNB];
+#pragma unroll
+        for (int i = 0; i < kNB; ++i) v[i] = (valid && nb0 + i < nbf) ? V[(size_t)(nb0 + i) * P + p] : 0.0;
+        for (int mb0 = 0; mb0 < nbf && mb0 <= nb0 + kNB - 1; mb0 += kMB) {
+            __syncthreads();
+            for (int idx = threadIdx.x; idx < kMaxStateTile * kMB * kNB; idx += kPts) {
+                const int s = idx / (kMB * kNB), m = (idx / kNB) % kMB, n = idx % kNB;
+                const int mu = mb0 + m, nu = nb0 + n;
+                double val = 0.0;
+                if (s < ns && mu < nbf && nu < nbf && nu >= mu) {
+                    const double* Ts = T + (size_t)(s0 + s) * nbf * nbf;
+                    val = Ts[(size_t)mu * nbf + nu];
+                    if (nu > mu) val += Ts[(size_t)nu * nbf + mu];
+                }
+                sT[s][m][n] = val;
+            }
+            __syncthreads();
+#pragma unroll
+            for (int m = 0; m < kMB; ++m) {
+                const double vm = (valid && mb0 + m < nbf) ? V[(size_t)(mb0 + m) * P + p] : 0.0;
+#pragma unroll
+                for (int s = 0; s < kMaxStateTile; ++s) {
+                    double w = 0.0;
+#pragma unroll
+                    for (int n = 0; n < kNB; ++n) w = fma(sT[s][m][n], v[n], w);
+                    acc[s] = fma(vm, w, acc[s]);
+                }
+            }
+        }
+    }
+    if (valid)
+#pragma unroll
+        for (int s = 0; s < kMaxStateTile; ++s)
+            if (s < ns) out[(size_t)(s0 + s) * P + p] = make_double2(g * acc[s], 0.0);
+}
+
+// out[s][(ia, ib, ic)] = V_pix e^{i q.x_min} F[s][(alpha mod N, ...)],  alpha = ia - floor(N/2)
+__global__ void __launch_bounds__(256) fft_post_kernel(const double2* __restrict__ F, FftGrid g, int ns, double2* __restrict__ out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.P * ns) return;
+    const long long p = i % g.P;
+    const int s = (int)(i / g.P);
+    const int ic = (int)(p % g.nz), ib = (int)((p / g.nz) % g.ny), ia = (int)(p / ((long long)g.nz * g.ny));
+    const int al = ia - g.nx / 2, be = ib - g.ny / 2, ga = ic - g.nz / 2;
+    const long long src = ((long long)((al + g.nx) % g.nx) * g.ny + (be + g.ny) % g.ny) * g.nz + (ga + g.nz) % g.nz;
+    const double twopi = 6.283185307179586476925286766559;
+    const double ph = twopi * (al / g.len[0] * g.xmin[0] + be / g.len[1] * g.xmin[1] + ga / g.len[2] * g.xmin[2]);
+    double sn, cs;
+    sincos(ph, &sn, &cs);
+    const double vpix = g.len[0] * g.len[1] * g.len[2] / (double)g.P;
+    const double2 f = F[(size_t)s * g.P + src];
+    out[i] = make_double2(vpix * (f.x * cs - f.y * sn), vpix * (f.x * sn + f.y * cs));
+}
+
+// ---- cuFFT through dlopen (library step; keeps libscarf.so free of a link-time cuFFT dependency) -------------------
+typedef int (*PlanFn)(int*, int, int, int, int);
+typedef int (*SetStreamFn)(int, cudaStream_t);
+typedef int (*ExecFn)(int, void*, void*, int);
+typedef int (*DestroyFn)(int);
+struct CufftApi {
+    void* h = nullptr;
+    PlanFn plan3d = nullptr;
+    SetStreamFn set_stream = nullptr;
+    ExecFn exec_z2z = nullptr;
+    DestroyFn destroy = nullptr;
+    bool tried = false;
+} g_cufft;
+
+bool load_cufft()
+{
+    if (g_cufft.tried) return g_cufft.h != nullptr;
+    g_cufft.tried = true;
+    const char* names[] = {"libcufft.so.11", "/usr/local/cuda/lib64/libcufft.so.11", "libcufft.so", "/usr/local/cuda/lib64/libcufft.so"};
+    for (const char* n : names) {
+        g_cufft.h = dlopen(n, RTLD_NOW | RTLD_LOCAL);
+        if (g_cufft.h) break;
+    }
+    if (!g_cufft.h) return false;
+    g_cufft.plan3d = (PlanFn)dlsym(g_cufft.h, "cufftPlan3d");
+    g_cufft.set_stream = (SetStreamFn)dlsym(g_cufft.h, "cufftSetStream");
+    g_cufft.exec_z2z = (ExecFn)dlsym(g_cufft.h, "cufftExecZ2Z");
+    g_cufft.destroy = (DestroyFn)dlsym(g_cufft.h, "cufftDestroy");
+    if (!g_cufft.plan3d || !g_cufft.set_stream || !g_cufft.exec_z2z || !g_cufft.destroy) {
+        dlclose(g_cufft.h);
+        g_cufft.h = nullptr;
+    }
+    return g_cufft.h != nullptr;
+}
+
+}  // namespace
+
+cudaError_t launch_orbitals(const PrimShell* prim, const int* shell_first, int n_shells, const FftGrid& g, double* V, cudaStream_t st)
+{
+    if (g.P <= 0 || n_shells <= 0) return cudaSuccess;
+    dim3 grid((unsigned)((g.P + kPts - 1) / kPts), (unsigned)n_shells);
+    orbital_kernel<<<grid, kPts, 0, st>>>(prim, shell_first, g, V);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_density(const double* V, const double* T, int nbf, long long P, int s0, int ns, double g, double* out_complex,
+                           cudaStream_t st)
+{
+    if (P <= 0 || ns <= 0) return cudaSuccess;
+    density_kernel<<<(unsigned)((P + kPts - 1) / kPts), kPts, 0, st>>>(V, T, nbf, P, s0, ns, g, reinterpret_cast<double2*>(out_complex));
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fft_post(const double* F, const FftGrid& g, int ns, double* out, cudaStream_t st)
+{
+    const long long n = g.P * ns;
+    if (n <= 0) return cudaSuccess;
+    fft_post_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const double2*>(F), g, ns, reinterpret_cast<double2*>(out));
+    return cudaGetLastError();
+}
+
+// In-place unnormalised transforms sum_abc f e^{+2 pi i (...)} of ns arrays [nx][ny][nz] of complex doubles.
+// Returns 0, -1 (cuFFT library not loadable) or a positive cufftResult.
+int cufft_inverse_batch(double* data, int nx, int ny, int nz, int ns, cudaStream_t st)
+{
+    if (!load_cufft()) return -1;
+    static int plan = -1, pnx = 0, pny = 0, pnz = 0;
+    if (plan < 0 || pnx != nx || pny != ny || pnz != nz) {
+        if (plan >= 0) g_cufft.destroy(plan);
+        plan = -1;
+        int h = 0;
+        const int rc = g_cufft.plan3d(&h, nx, ny, nz, 0x69 /* CUFFT_Z2Z */);
+        if (rc != 0) return rc;
+        plan = h; pnx = nx; pny = ny; pnz = nz;
+    }
+    int rc = g_cufft.set_stream(plan, st);
+    if (rc != 0) return rc;
+    const size_t per = (size_t)nx * ny * nz * 2;
+    for (int s = 0; s < ns; ++s) {
+        rc = g_cufft.exec_z2z(plan, data + (size_t)s * per, data + (size_t)s * per, 1 /* CUFFT_INVERSE */);
+        if (rc != 0) return rc;
+    }
+    return 0;
+}
+
+}  // namespace scarf

@@ -124,6 +124,18 @@ int build_pure_map(int n_shells, const int32_t* shell_l, const int32_t* shell_pu
 cudaError_t launch_transform_T(const double* Tu, double* Tc, int n_states, int nbf_u, int nbf_c, const int* nnz, const int* uidx,
                                const double* ucoef, cudaStream_t st);
 
+// FFT method (fft_method.cu, NEXT-4)
+struct FftGrid {
+    int nx, ny, nz, pad;
+    long long P;                            // nx*ny*nz
+    double xmin[3], len[3];
+};
+cudaError_t launch_orbitals(const PrimShell* prim, const int* shell_first, int n_shells, const FftGrid& g, double* V, cudaStream_t st);
+cudaError_t launch_density(const double* V, const double* T, int nbf, long long P, int s0, int ns, double g, double* out_complex,
+                           cudaStream_t st);
+cudaError_t launch_fft_post(const double* F, const FftGrid& g, int ns, double* out, cudaStream_t st);
+int cufft_inverse_batch(double* data, int nx, int ny, int nz, int ns, cudaStream_t st);
+
 cudaError_t run_fp64_peak(double* dfma_per_s, double* sm_clock_mhz);
 
 }  // namespace scarf

@@ -59,7 +59,8 @@ struct scarf_ctx {
     std::vector<double> pure_ucoef;
     int n_states = 0;
     int sm_count = 148;
-    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb, d_partial, d_axes, d_tab, d_ang_in, d_ang_F, d_ang_tab, d_ang_out, d_pure_map, d_Tcart;
+    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb, d_partial, d_axes, d_tab, d_ang_in, d_ang_F, d_ang_tab, d_ang_out, d_pure_map, d_Tcart, d_prim, d_V, d_fft;
+    const double* Tc_dev = nullptr;        // context-owned Cartesian T of the last set_transitions (FFT method)
     std::vector<DevBuf> staging, packed;
     std::vector<TileStream> tiles;
     scarf_stats st = {};
@@ -165,6 +166,8 @@ void free_device(scarf_ctx* c)
     c->d_axes.release(); c->d_tab.release();
     c->d_ang_in.release(); c->d_ang_F.release(); c->d_ang_tab.release(); c->d_ang_out.release();
     c->d_pure_map.release(); c->d_Tcart.release();
+    c->d_prim.release(); c->d_V.release(); c->d_fft.release();
+    c->Tc_dev = nullptr;
     for (auto& b : c->staging) b.release();
     for (auto& b : c->packed) b.release();
     c->staging.clear(); c->packed.clear(); c->tiles.clear();
@@ -368,7 +371,12 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T)
                                   reinterpret_cast<const int*>(base + nc * kPureMaxNnz * 12), reinterpret_cast<const int*>(base + nc * kPureMaxNnz * 8),
                                   reinterpret_cast<const double*>(base), st), "set_transitions: pure transform kernel");
             dT = static_cast<const double*>(ctx->d_Tcart.p);
+        } else if (dT == T) {   // caller-owned device T: keep a copy (inputs are copied; the FFT method reads T later)
+            CU(ctx->d_T.ensure(tsz * sizeof(double)), "set_transitions: alloc T");
+            CU(cudaMemcpyAsync(ctx->d_T.p, T, tsz * sizeof(double), cudaMemcpyDeviceToDevice, st), "set_transitions: copy T");
+            dT = static_cast<const double*>(ctx->d_T.p);
         }
+        ctx->Tc_dev = dT;
         // state tiles
         std::vector<TileStream> tiles;
         for (int s0 = 0; s0 < n_states; s0 += kMaxStateTile) {
@@ -797,6 +805,82 @@ int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t
         return fail(ctx, SCARF_ENOMEM, "angular_moments: out of host memory");
     } catch (...) {
         return fail(ctx, SCARF_EINVAL, "angular_moments: unexpected exception");
+    }
+}
+
+int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, const double* x_min, const double* box_len,
+                           double* out)
+{
+    if (!ctx) return SCARF_EINVAL;
+    if (ctx->host_only) return fail(ctx, SCARF_ENODEVICE, "fft_form_factors: host-only context; there is no CPU fallback");
+    if (!ctx->have_T || !ctx->Tc_dev) return fail(ctx, SCARF_ESTATE, "fft_form_factors: set_basis and set_transitions first");
+    if (nx < 1 || ny < 1 || nz < 1 || !x_min || !box_len || !out) return fail(ctx, SCARF_EINVAL, "fft_form_factors: bad grid or null pointer");
+    for (int k = 0; k < 3; ++k)
+        if (!std::isfinite(x_min[k]) || !std::isfinite(box_len[k]) || !(box_len[k] > 0))
+            return fail(ctx, SCARF_EINVAL, "fft_form_factors: box lengths must be finite and > 0");
+    try {
+        CU(cudaSetDevice(ctx->device), "fft_form_factors");
+        cudaStream_t st = ctx->stream;
+        const HostSetup& hs = ctx->hs;
+        FftGrid g = {};
+        g.nx = nx; g.ny = ny; g.nz = nz;
+        g.P = (long long)nx * ny * nz;
+        for (int k = 0; k < 3; ++k) { g.xmin[k] = x_min[k]; g.len[k] = box_len[k]; }
+        const size_t vbytes = (size_t)hs.nbf * (size_t)g.P * sizeof(double);
+        const size_t fbytes = (size_t)ctx->n_states * (size_t)g.P * 2 * sizeof(double);
+        if ((double)vbytes + 2.0 * (double)fbytes > 64e9) return fail(ctx, SCARF_ENOMEM, "fft_form_factors: grid needs more than 64 GB of scratch");
+        // primitive shells and the first primitive of every contracted shell
+        std::vector<int> first;
+        for (size_t i = 0; i < hs.prim.size(); ++i)
+            if (i == 0 || hs.prim[i].shell != hs.prim[i - 1].shell) first.push_back((int)i);
+        const int n_sh = (int)first.size();
+        first.push_back((int)hs.prim.size());
+        const size_t pbytes = hs.prim.size() * sizeof(PrimShell);
+        CU(ctx->d_prim.ensure(pbytes + first.size() * sizeof(int) + 64), "fft_form_factors: alloc basis");
+        char* pb = static_cast<char*>(ctx->d_prim.p);
+        CU(cudaMemcpyAsync(pb, hs.prim.data(), pbytes, cudaMemcpyHostToDevice, st), "fft_form_factors: upload basis");
+        CU(cudaMemcpyAsync(pb + pbytes, first.data(), first.size() * sizeof(int), cudaMemcpyHostToDevice, st), "fft_form_factors: upload basis");
+        CU(ctx->d_V.ensure(vbytes), "fft_form_factors: alloc orbital values");
+        CU(ctx->d_fft.ensure(fbytes), "fft_form_factors: alloc transform buffer");
+        const bool out_host = !is_device_ptr(out);
+        double* dout = out;
+        if (out_host) {
+            CU(ctx->d_out.ensure(fbytes), "fft_form_factors: alloc out");
+            dout = static_cast<double*>(ctx->d_out.p);
+        }
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "fft_form_factors: event");
+        double* dV = static_cast<double*>(ctx->d_V.p);
+        double* dF = static_cast<double*>(ctx->d_fft.p);
+        CU(launch_orbitals(reinterpret_cast<const PrimShell*>(pb), reinterpret_cast<const int*>(pb + pbytes), n_sh, g, dV, st),
+           "fft_form_factors: orbital kernel");
+        int launches = 1;
+        for (int s0 = 0; s0 < ctx->n_states; s0 += kMaxStateTile) {
+            CU(launch_density(dV, ctx->Tc_dev, hs.nbf, g.P, s0, std::min(kMaxStateTile, ctx->n_states - s0), ctx->prefactor, dF, st),
+               "fft_form_factors: density kernel");
+            ++launches;
+        }
+        CU(cudaStreamSynchronize(st), "fft_form_factors: sync");   // `first` (pageable) goes out of scope; cuFFT plans below
+        const int frc = cufft_inverse_batch(dF, nx, ny, nz, ctx->n_states, st);
+        if (frc < 0) return fail(ctx, SCARF_ECUDA, "fft_form_factors: the cuFFT library (libcufft.so.11) could not be loaded");
+        if (frc > 0) return fail(ctx, frc == 2 ? SCARF_ENOMEM : SCARF_ECUDA, "fft_form_factors: cuFFT error " + std::to_string(frc));
+        CU(launch_fft_post(dF, g, ctx->n_states, dout, st), "fft_form_factors: post kernel");
+        ctx->st.last_kernel_launches = launches + 1;
+        if (ctx->timing) {
+            CU(cudaEventRecord(ctx->ev1, st), "fft_form_factors: event");
+            CU(cudaEventSynchronize(ctx->ev1), "fft_form_factors: event sync");
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
+            ctx->st.last_kernel_ms = ms;
+        }
+        if (out_host) {
+            CU(cudaMemcpyAsync(out, dout, fbytes, cudaMemcpyDeviceToHost, st), "fft_form_factors: download out");
+            CU(cudaStreamSynchronize(st), "fft_form_factors: sync");
+        }
+        return SCARF_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(ctx, SCARF_ENOMEM, "fft_form_factors: out of host memory");
+    } catch (...) {
+        return fail(ctx, SCARF_EINVAL, "fft_form_factors: unexpected exception");
     }
 }
 

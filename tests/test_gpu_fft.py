@@ -1,0 +1,92 @@
+"""GPU parity of scarf_fft_form_factors (the paper's FFT method, Eq. (19)-(34) PAPER.md:140-222)
+against its CPU oracle (oracle/fft_method.py) on the same grid, and convergence to the analytic kernel's result."""
+import numpy as np
+import pytest
+
+from paper_2512_18010_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked tests must run on the B200 box")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def Scarf():
+    from paper_2512_18010_b200 import Scarf as S
+    return S
+
+
+def assert_parity(f_gpu, f_ref, tol=1e-10):
+    assert f_gpu.shape == f_ref.shape
+    for s in range(f_ref.shape[0]):
+        scale = np.max(np.abs(f_ref[s]))
+        err = np.max(np.abs(f_gpu[s] - f_ref[s]))
+        assert err <= tol * scale, f"state {s}: max err {err:.3e} > {tol:g} * {scale:.3e}"
+
+
+@pytest.mark.parametrize("n,n_states", [((8, 8, 8), 1), ((24, 20, 28), 3), ((15, 9, 21), 13), ((1, 5, 2), 2)])
+def test_fft_method_matches_oracle(oracle_mod, Scarf, torch_cuda, n, n_states):
+    """Even, odd and ragged grid sizes (several CTAs and a tail), one and two state tiles, an off-centre box;
+    basis with s, p, d, f shells and contractions (config-1 atoms plus a d/f centre)."""
+    torch = torch_cuda
+    from oracle import fft_method as offt
+    b = W.Basis(np.array([[0.0, 0.0, 0.7], [0.0, 0.0, -0.7], [0.9, -0.5, 0.1]]), np.array([0, 0, 1, 1, 2, 2], np.int32),
+                np.array([0, 1, 0, 2, 3, 1], np.int32), np.array([3, 2, 1, 1, 1, 2], np.int32),
+                np.array([5.0, 1.2, 0.3, 2.0, 0.6, 0.9, 1.1, 0.8, 1.5, 0.4]),
+                np.array([0.3, 0.6, 0.4, 0.7, 0.5, 1.0, 1.0, 1.0, 0.6, 0.8]))
+    rng = np.random.default_rng(sum(n) + n_states)
+    T = rng.normal(size=(n_states, b.nbf, b.nbf))
+    x_min, L = np.array([-5.0, -4.5, -6.0]), np.array([10.5, 9.0, 11.0])
+    f_ref = offt.form_factors(b, T, n, x_min, L)
+    with Scarf(0) as sc:
+        sc.set_basis(b)
+        sc.set_transitions(torch.as_tensor(T, device="cuda"))
+        f = sc.fft_form_factors(n, x_min, L)
+        torch.cuda.synchronize()
+        assert_parity(f.cpu().numpy(), f_ref)
+        fh = sc.fft_form_factors(n, x_min, L, device_out=False)          # host output buffer
+        assert np.array_equal(fh, f.cpu().numpy())
+        sc.set_transitions(T)                                            # host T
+        assert np.array_equal(sc.fft_form_factors(n, x_min, L, device_out=False), fh)
+
+
+def test_fft_method_converges_to_the_analytic_kernel(oracle_mod, Scarf, torch_cuda):
+    """Soft basis, 64^3 grid of spacing 0.25 bohr: the two GPU routes (tabulate-and-transform vs Eq. 48 in closed form)
+    agree to 1e-8 away from the Nyquist faces; pure d shell included (T in the mixed basis)."""
+    torch = torch_cuda
+    from oracle import fft_method as offt
+    from tests.test_oracle_fft import soft_basis
+    b = soft_basis()
+    pure = np.array([0, 0, 1, 0, 0], np.int32)
+    nbf = b.nbf - 1
+    rng = np.random.default_rng(8)
+    T = rng.normal(size=(2, nbf, nbf))
+    n, x_min, L = (64, 64, 64), np.array([-8.0] * 3), np.array([16.0] * 3)
+    q = offt.q_points(n, L)
+    idx = np.flatnonzero(np.max(np.abs(q), axis=1) < 9.0)[::97]
+    with Scarf(0) as sc:
+        sc.set_basis(b, shell_pure=pure)
+        sc.set_transitions(T)
+        f_fft = sc.fft_form_factors(n, x_min, L)[:, torch.as_tensor(idx, device="cuda")].cpu().numpy()
+        f_ana = sc.form_factors(q[idx])
+    for s in range(2):
+        assert np.max(np.abs(f_fft[s] - f_ana[s])) <= 1e-8 * np.max(np.abs(f_ana[s]))
+
+
+def test_fft_method_argument_checks(oracle_mod, Scarf, torch_cuda):
+    w = W.make_workload(1, oracle_mod.overlap)
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        with pytest.raises(Exception):
+            sc.fft_form_factors((4, 4, 4), np.zeros(3), np.ones(3))       # no transitions yet
+        sc.set_transitions(w.T)
+        with pytest.raises(Exception):
+            sc.fft_form_factors((4, 4, 4), np.zeros(3), np.array([1.0, 0.0, 1.0]))
+        with pytest.raises(Exception):
+            sc.fft_form_factors((4, 0, 4), np.zeros(3), np.ones(3))
