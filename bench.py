@@ -271,6 +271,31 @@ def run_ours(args):
         step_device()   # leave the general path's result in out_dev for the parity sample below
         torch.cuda.synchronize()
 
+    # ---- the paper's FFT method (NEXT-4, scarf_fft_form_factors) on a real-space grid of the same size: box = atoms + 5 bohr
+    fft_path = None
+    if w.grid.get("kind") == "cartesian":
+        n_ax = int(w.grid["n_per_axis"])
+        lo = w.basis.atom_xyz.min(axis=0) - 5.0
+        box = w.basis.atom_xyz.max(axis=0) + 5.0 - lo
+        fft_out = torch.empty((w.n_states, n_ax ** 3, 2), dtype=torch.float64, device="cuda")
+        with torch.cuda.stream(stream):
+            sc.set_transitions(T_dev)
+            for _ in range(2):
+                sc.fft_form_factors((n_ax,) * 3, lo, box, out=fft_out)
+            barrier()
+            fev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+            for k in range(args.steps):
+                flush.fill_(k & 0xFF)
+                fev[k][0].record(stream)
+                sc.fft_form_factors((n_ax,) * 3, lo, box, out=fft_out)
+                fev[k][1].record(stream)
+            barrier()
+        f_ms = float(np.median([a.elapsed_time(b) for a, b in fev]))
+        fma = 0.5 * w.n_states * float(w.basis.nbf) ** 2 * n_ax ** 3
+        fft_path = {"api": "scarf_fft_form_factors", "grid": [n_ax] * 3, "box_bohr": [float(x) for x in box], "ms_per_call": f_ms,
+                    "density_fma": fma, "note": "approximate method (box truncation, grid spacing); timing only"}
+        del fft_out
+
     # ---- angular moments of the result (NEXT-3, scarf_angular_moments) on the spherical product grid of config 5
     angular = None
     if w.grid.get("kind") == "spherical":
@@ -363,6 +388,8 @@ def run_ours(args):
 
     if angular is not None:
         line["angular_moments"] = angular
+    if fft_path is not None:
+        line["fft_path"] = fft_path
 
     if not args.no_cpu_baseline and world == 1:
         import oracle
