@@ -21,6 +21,12 @@ namespace scarf {
 
 namespace {
 
+#ifndef SCARF_MMA_VOLATILE
+#define SCARF_MMA_VOLATILE volatile
+#endif
+#ifndef SCARF_MMA_UNROLL
+#define SCARF_MMA_UNROLL 1
+#endif
 constexpr int kPts = 128;     // points per CTA
 constexpr int kNB = 16, kMB = 8;
 
@@ -107,6 +113,91 @@ __global__ void __launch_bounds__(kPts) density_kernel(const double* __restrict_
             if (s < ns) out[(size_t)(s0 + s) * P + p] = make_double2(g * acc[s], 0.0);
 }
 
+// ---- the same quadratic form on the FP64 tensor cores (DMMA m8n8k4) ---------------------------------------------------
+// W[p][mu] = sum_{nu >= mu} C_s[mu][nu] v_nu(p) is a dense contraction [points x nbf] . [nbf x nbf]: A = V tile (8 points x
+// 4 nu), B = C_s^T tile (4 nu x 8 mu), D = W tile (8 points x 8 mu) accumulated over nu; then Phi_s(p) = sum_mu W[p][mu] v_mu(p)
+// in the epilogue of every mu-chunk.  A warp owns 16 points (two M tiles share every B fragment) and all 12 states of the
+// pass; fragments are read straight from global memory / L1 (V is [mu][point], C_s is the zero-padded upper-triangular
+// matrix written by symmetrize_kernel: T_mumu on the diagonal, T_munu + T_numu above, 0 below).  DMMA holds the FP64 pipe
+// at its full rate with 4 register reads per 8 lane-FMAs, so it is free of the read-port bound of the SIMT form.
+__global__ void __launch_bounds__(256) symmetrize_kernel(const double* __restrict__ T, int nbf, int nbf_pad, int s0, int ns,
+                                                         double* __restrict__ C)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long per = (long long)nbf_pad * nbf_pad;
+    if (i >= per * kMaxStateTile) return;
+    const int s = (int)(i / per), mu = (int)((i % per) / nbf_pad), nu = (int)(i % nbf_pad);
+    double v = 0.0;
+    if (s < ns && mu < nbf && nu < nbf && nu >= mu) {
+        const double* Ts = T + (size_t)(s0 + s) * nbf * nbf;
+        v = Ts[(size_t)mu * nbf + nu];
+        if (nu > mu) v += Ts[(size_t)nu * nbf + mu];
+    }
+    C[i] = v;
+}
+
+__device__ __forceinline__ void dmma884(double (&d)[2], double a, double b)
+{
+    asm SCARF_MMA_VOLATILE("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
+}
+
+constexpr int kMmaWarps = 4;
+__global__ void __launch_bounds__(kMmaWarps * 32) density_mma_kernel(const double* __restrict__ V, const double* __restrict__ C, int nbf,
+                                                                     int nbf_pad, long long P, int s0, int ns, double g,
+                                                                     double2* __restrict__ out)
+{
+    const int lane = threadIdx.x & 31, gid = lane >> 2, tig = lane & 3;
+    const long long p0 = ((long long)blockIdx.x * kMmaWarps + (threadIdx.x >> 5)) * 16;
+    if (p0 >= P) return;
+    const long long pa = p0 + gid, pb = p0 + 8 + gid;
+    const bool va = pa < P, vb = pb < P;
+    const size_t per = (size_t)nbf_pad * nbf_pad;
+    double phi[2][kMaxStateTile];
+#pragma unroll
+    for (int s = 0; s < kMaxStateTile; ++s) phi[0][s] = phi[1][s] = 0.0;
+    for (int mu0 = 0; mu0 < nbf_pad; mu0 += 8) {
+        double D[2][kMaxStateTile][2];
+#pragma unroll
+        for (int s = 0; s < kMaxStateTile; ++s) D[0][s][0] = D[0][s][1] = D[1][s][0] = D[1][s][1] = 0.0;
+        const double* Cb = C + (size_t)(mu0 + gid) * nbf_pad + tig;       // B[k = tig][n = gid] = C[mu0 + gid][nu0 + tig]
+#pragma unroll SCARF_MMA_UNROLL
+        for (int nu0 = mu0; nu0 < nbf_pad; nu0 += 4) {
+            const int nu = nu0 + tig;
+            const double a0 = (va && nu < nbf) ? V[(size_t)nu * P + pa] : 0.0;   // A[row = gid][k = tig] = v_nu(point)
+            const double a1 = (vb && nu < nbf) ? V[(size_t)nu * P + pb] : 0.0;
+#pragma unroll
+            for (int s = 0; s < kMaxStateTile; ++s) {
+                const double b = Cb[(size_t)s * per + nu0];
+                dmma884(D[0][s], a0, b);
+                dmma884(D[1][s], a1, b);
+            }
+        }
+        // D[row = gid][col = 2 tig + i] = W[point][mu0 + 2 tig + i]
+        const int m0 = mu0 + 2 * tig, m1 = m0 + 1;
+        const double v00 = (va && m0 < nbf) ? V[(size_t)m0 * P + pa] : 0.0, v01 = (va && m1 < nbf) ? V[(size_t)m1 * P + pa] : 0.0;
+        const double v10 = (vb && m0 < nbf) ? V[(size_t)m0 * P + pb] : 0.0, v11 = (vb && m1 < nbf) ? V[(size_t)m1 * P + pb] : 0.0;
+#pragma unroll
+        for (int s = 0; s < kMaxStateTile; ++s) {
+            phi[0][s] = fma(D[0][s][0], v00, fma(D[0][s][1], v01, phi[0][s]));
+            phi[1][s] = fma(D[1][s][0], v10, fma(D[1][s][1], v11, phi[1][s]));
+        }
+    }
+#pragma unroll
+    for (int s = 0; s < kMaxStateTile; ++s) {
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            double x = phi[t][s];
+            x += __shfl_xor_sync(0xffffffffu, x, 1);
+            x += __shfl_xor_sync(0xffffffffu, x, 2);
+            phi[t][s] = x;
+        }
+        if (tig == 0 && s < ns) {
+            if (va) out[(size_t)(s0 + s) * P + pa] = make_double2(g * phi[0][s], 0.0);
+            if (vb) out[(size_t)(s0 + s) * P + pb] = make_double2(g * phi[1][s], 0.0);
+        }
+    }
+}
+
 // out[s][(ia, ib, ic)] = V_pix e^{i q.x_min} F[s][(alpha mod N, ...)],  alpha = ia - floor(N/2)
 __global__ void __launch_bounds__(256) fft_post_kernel(const double2* __restrict__ F, FftGrid g, int ns, double2* __restrict__ out)
 {
@@ -176,6 +267,18 @@ cudaError_t launch_density(const double* V, const double* T, int nbf, long long 
 {
     if (P <= 0 || ns <= 0) return cudaSuccess;
     density_kernel<<<(unsigned)((P + kPts - 1) / kPts), kPts, 0, st>>>(V, T, nbf, P, s0, ns, g, reinterpret_cast<double2*>(out_complex));
+    return cudaGetLastError();
+}
+
+cudaError_t launch_density_mma(const double* V, const double* T, double* Csym, int nbf, int nbf_pad, long long P, int s0, int ns,
+                               double g, double* out_complex, cudaStream_t st)
+{
+    if (P <= 0 || ns <= 0) return cudaSuccess;
+    const long long nsym = (long long)kMaxStateTile * nbf_pad * nbf_pad;
+    symmetrize_kernel<<<(unsigned)((nsym + 255) / 256), 256, 0, st>>>(T, nbf, nbf_pad, s0, ns, Csym);
+    const long long per_cta = 16LL * kMmaWarps;
+    density_mma_kernel<<<(unsigned)((P + per_cta - 1) / per_cta), kMmaWarps * 32, 0, st>>>(V, Csym, nbf, nbf_pad, P, s0, ns, g,
+                                                                                       reinterpret_cast<double2*>(out_complex));
     return cudaGetLastError();
 }
 

@@ -133,6 +133,8 @@ struct FftGrid {
 cudaError_t launch_orbitals(const PrimShell* prim, const int* shell_first, int n_shells, const FftGrid& g, double* V, cudaStream_t st);
 cudaError_t launch_density(const double* V, const double* T, int nbf, long long P, int s0, int ns, double g, double* out_complex,
                            cudaStream_t st);
+cudaError_t launch_density_mma(const double* V, const double* T, double* Csym, int nbf, int nbf_pad, long long P, int s0, int ns,
+                               double g, double* out_complex, cudaStream_t st);
 cudaError_t launch_fft_post(const double* F, const FftGrid& g, int ns, double* out, cudaStream_t st);
 int cufft_inverse_batch(double* data, int nx, int ny, int nz, int ns, cudaStream_t st);
 

@@ -50,6 +50,7 @@ struct scarf_ctx {
     bool timing = false;
     int kernel_variant = -1;  // -1 auto (v1), 0 force the baseline kernel v0
     int n_chunks_opt = 0;     // 0 auto, else the number of stream chunks of the v1 kernel
+    int fft_density_variant = 1;  // 1: DMMA kernel, 0: SIMT kernel (fft_method.cu)
     std::string err;
     HostSetup hs;
     bool have_basis = false, have_T = false;
@@ -59,7 +60,7 @@ struct scarf_ctx {
     std::vector<double> pure_ucoef;
     int n_states = 0;
     int sm_count = 148;
-    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb, d_partial, d_axes, d_tab, d_ang_in, d_ang_F, d_ang_tab, d_ang_out, d_pure_map, d_Tcart, d_prim, d_V, d_fft;
+    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb, d_partial, d_axes, d_tab, d_ang_in, d_ang_F, d_ang_tab, d_ang_out, d_pure_map, d_Tcart, d_prim, d_V, d_fft, d_Csym;
     const double* Tc_dev = nullptr;        // context-owned Cartesian T of the last set_transitions (FFT method)
     std::vector<DevBuf> staging, packed;
     std::vector<TileStream> tiles;
@@ -166,7 +167,7 @@ void free_device(scarf_ctx* c)
     c->d_axes.release(); c->d_tab.release();
     c->d_ang_in.release(); c->d_ang_F.release(); c->d_ang_tab.release(); c->d_ang_out.release();
     c->d_pure_map.release(); c->d_Tcart.release();
-    c->d_prim.release(); c->d_V.release(); c->d_fft.release();
+    c->d_prim.release(); c->d_V.release(); c->d_fft.release(); c->d_Csym.release();
     c->Tc_dev = nullptr;
     for (auto& b : c->staging) b.release();
     for (auto& b : c->packed) b.release();
@@ -246,6 +247,7 @@ int scarf_set_option(scarf_ctx* ctx, const char* key, double value)
     else if (k == "threshold_eps") { if (!(value >= 0.0)) return fail(ctx, SCARF_EINVAL, "set_option: threshold_eps < 0"); ctx->threshold_eps = value; }
     else if (k == "kernel_variant") ctx->kernel_variant = (int)value;
     else if (k == "n_chunks") ctx->n_chunks_opt = (int)value;
+    else if (k == "fft_density_variant") ctx->fft_density_variant = (int)value;
     else return fail(ctx, SCARF_EINVAL, "set_option: unknown key '" + k + "'");
     return SCARF_OK;
 }
@@ -855,9 +857,17 @@ int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, c
            "fft_form_factors: orbital kernel");
         int launches = 1;
         for (int s0 = 0; s0 < ctx->n_states; s0 += kMaxStateTile) {
-            CU(launch_density(dV, ctx->Tc_dev, hs.nbf, g.P, s0, std::min(kMaxStateTile, ctx->n_states - s0), ctx->prefactor, dF, st),
-               "fft_form_factors: density kernel");
-            ++launches;
+            const int ns_t = std::min(kMaxStateTile, ctx->n_states - s0);
+            if (ctx->fft_density_variant == 0) {
+                CU(launch_density(dV, ctx->Tc_dev, hs.nbf, g.P, s0, ns_t, ctx->prefactor, dF, st), "fft_form_factors: density kernel");
+                ++launches;
+            } else {
+                const int nbf_pad = (hs.nbf + 7) & ~7;
+                CU(ctx->d_Csym.ensure((size_t)kMaxStateTile * nbf_pad * nbf_pad * sizeof(double)), "fft_form_factors: alloc C");
+                CU(launch_density_mma(dV, ctx->Tc_dev, static_cast<double*>(ctx->d_Csym.p), hs.nbf, nbf_pad, g.P, s0, ns_t,
+                                      ctx->prefactor, dF, st), "fft_form_factors: density kernel (DMMA)");
+                launches += 2;
+            }
         }
         CU(cudaStreamSynchronize(st), "fft_form_factors: sync");   // `first` (pageable) goes out of scope; cuFFT plans below
         const int frc = cufft_inverse_batch(dF, nx, ny, nz, ctx->n_states, st);

@@ -54,6 +54,8 @@ def test_fft_method_matches_oracle(oracle_mod, Scarf, torch_cuda, n, n_states):
         assert np.array_equal(fh, f.cpu().numpy())
         sc.set_transitions(T)                                            # host T
         assert np.array_equal(sc.fft_form_factors(n, x_min, L, device_out=False), fh)
+        sc.set_option("fft_density_variant", 0)                          # SIMT density kernel instead of the DMMA one
+        assert_parity(sc.fft_form_factors(n, x_min, L, device_out=False), f_ref)
 
 
 def test_fft_method_converges_to_the_analytic_kernel(oracle_mod, Scarf, torch_cuda):
