@@ -142,6 +142,7 @@ __device__ __forceinline__ void dmma884(double (&d)[2], double a, double b)
 }
 
 constexpr int kMmaWarps = 4;
+constexpr int kMmaUnroll = SCARF_MMA_UNROLL;
 __global__ void __launch_bounds__(kMmaWarps * 32) density_mma_kernel(const double* __restrict__ V, const double* __restrict__ C, int nbf,
                                                                      int nbf_pad, long long P, int s0, int ns, double g,
                                                                      double2* __restrict__ out)
@@ -160,7 +161,7 @@ __global__ void __launch_bounds__(kMmaWarps * 32) density_mma_kernel(const doubl
 #pragma unroll
         for (int s = 0; s < kMaxStateTile; ++s) D[0][s][0] = D[0][s][1] = D[1][s][0] = D[1][s][1] = 0.0;
         const double* Cb = C + (size_t)(mu0 + gid) * nbf_pad + tig;       // B[k = tig][n = gid] = C[mu0 + gid][nu0 + tig]
-#pragma unroll SCARF_MMA_UNROLL
+#pragma unroll kMmaUnroll
         for (int nu0 = mu0; nu0 < nbf_pad; nu0 += 4) {
             const int nu = nu0 + tig;
             const double a0 = (va && nu < nbf) ? V[(size_t)nu * P + pa] : 0.0;   // A[row = gid][k = tig] = v_nu(point)
