@@ -30,6 +30,10 @@ namespace {
 constexpr int kPts = 128;     // points per CTA
 constexpr int kNB = 16, kMB = 8;
 
+// orbital values are stored in tiles of 8 points: V[(p / 8)][mu][p % 8], so that the 4 nu x 8 points of a DMMA A fragment
+// are 256 contiguous bytes (the plain [mu][point] layout costs 4 cache lines per fragment load and made L1 the limiter)
+__device__ __forceinline__ size_t vidx(int mu, long long p, int nbf) { return ((size_t)(p >> 3) * nbf + mu) * 8 + (size_t)(p & 7); }
+
 __device__ __forceinline__ double dfo(int n)   // (2n-1)!!
 {
     double r = 1.0;
@@ -38,7 +42,7 @@ __device__ __forceinline__ double dfo(int n)   // (2n-1)!!
 }
 
 __global__ void __launch_bounds__(kPts) orbital_kernel(const PrimShell* __restrict__ prim, const int* __restrict__ shell_first,
-                                                       FftGrid g, double* __restrict__ V)
+                                                       FftGrid g, int nbf, double* __restrict__ V)
 {
     const long long p = (long long)blockIdx.x * kPts + threadIdx.x;
     if (p >= g.P) return;
@@ -61,7 +65,7 @@ __global__ void __launch_bounds__(kPts) orbital_kernel(const PrimShell* __restri
     for (int a = l; a >= 0; --a)                        // component order: a descending, then b descending
         for (int b = l - a; b >= 0; --b) {
             const int cc = l - a - b;
-            V[(size_t)(ps.bf0 + c) * g.P + p] = rad * px[a] * py[b] * pz[cc] * rsqrt(dfo(a) * dfo(b) * dfo(cc));
+            V[vidx(ps.bf0 + c, p, nbf)] = rad * px[a] * py[b] * pz[cc] * rsqrt(dfo(a) * dfo(b) * dfo(cc));
             ++c;
         }
 }
@@ -79,7 +83,7 @@ __global__ void __launch_bounds__(kPts) density_kernel(const double* __restrict_
     for (int nb0 = 0; nb0 < nbf; nb0 += kNB) {
         double v[kNB];
 #pragma unroll
-        for (int i = 0; i < kNB; ++i) v[i] = (valid && nb0 + i < nbf) ? V[(size_t)(nb0 + i) * P + p] : 0.0;
+        for (int i = 0; i < kNB; ++i) v[i] = (valid && nb0 + i < nbf) ? V[vidx(nb0 + i, p, nbf)] : 0.0;
         for (int mb0 = 0; mb0 < nbf && mb0 <= nb0 + kNB - 1; mb0 += kMB) {
             __syncthreads();
             for (int idx = threadIdx.x; idx < kMaxStateTile * kMB * kNB; idx += kPts) {
@@ -96,7 +100,7 @@ __global__ void __launch_bounds__(kPts) density_kernel(const double* __restrict_
             __syncthreads();
 #pragma unroll
             for (int m = 0; m < kMB; ++m) {
-                const double vm = (valid && mb0 + m < nbf) ? V[(size_t)(mb0 + m) * P + p] : 0.0;
+                const double vm = (valid && mb0 + m < nbf) ? V[vidx(mb0 + m, p, nbf)] : 0.0;
 #pragma unroll
                 for (int s = 0; s < kMaxStateTile; ++s) {
                     double w = 0.0;
@@ -117,16 +121,23 @@ __global__ void __launch_bounds__(kPts) density_kernel(const double* __restrict_
 // W[p][mu] = sum_{nu >= mu} C_s[mu][nu] v_nu(p) is a dense contraction [points x nbf] . [nbf x nbf]: A = V tile (8 points x
 // 4 nu), B = C_s^T tile (4 nu x 8 mu), D = W tile (8 points x 8 mu) accumulated over nu; then Phi_s(p) = sum_mu W[p][mu] v_mu(p)
 // in the epilogue of every mu-chunk.  A warp owns 16 points (two M tiles share every B fragment) and all 12 states of the
-// pass; fragments are read straight from global memory / L1 (V is [mu][point], C_s is the zero-padded upper-triangular
-// matrix written by symmetrize_kernel: T_mumu on the diagonal, T_munu + T_numu above, 0 below).  DMMA holds the FP64 pipe
+// pass; fragments are read straight from global memory / L1, both stored in fragment order (256 contiguous bytes per
+// load).  C_s is the zero-padded upper-triangular matrix written by symmetrize_kernel: T_mumu on the diagonal,
+// T_munu + T_numu above, 0 below.  DMMA holds the FP64 pipe
 // at its full rate with 4 register reads per 8 lane-FMAs, so it is free of the read-port bound of the SIMT form.
+// C in DMMA B-fragment order: Cf[s][mu-chunk][nu-chunk][lane], lane = (gid, tig) <-> C_s[8 mc + gid][4 kc + tig]
+// (a fragment load is then 256 contiguous bytes instead of 8 rows)
 __global__ void __launch_bounds__(256) symmetrize_kernel(const double* __restrict__ T, int nbf, int nbf_pad, int s0, int ns,
                                                          double* __restrict__ C)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long per = (long long)nbf_pad * nbf_pad;
     if (i >= per * kMaxStateTile) return;
-    const int s = (int)(i / per), mu = (int)((i % per) / nbf_pad), nu = (int)(i % nbf_pad);
+    const int s = (int)(i / per);
+    const long long r = i % per;
+    const int lane = (int)(r & 31), n_kc = nbf_pad / 4;
+    const int kc = (int)((r >> 5) % n_kc), mc = (int)((r >> 5) / n_kc);
+    const int mu = 8 * mc + (lane >> 2), nu = 4 * kc + (lane & 3);
     double v = 0.0;
     if (s < ns && mu < nbf && nu < nbf && nu >= mu) {
         const double* Ts = T + (size_t)(s0 + s) * nbf * nbf;
@@ -143,60 +154,71 @@ __device__ __forceinline__ void dmma884(double (&d)[2], double a, double b)
 
 constexpr int kMmaWarps = 4;
 constexpr int kMmaUnroll = SCARF_MMA_UNROLL;
+#ifndef SCARF_MMA_NSP
+#define SCARF_MMA_NSP 12
+#endif
+#ifndef SCARF_MMA_MT
+#define SCARF_MMA_MT 2
+#endif
+constexpr int kMmaMT = SCARF_MMA_MT;      // 8-point M tiles per warp (they share every B fragment)
+constexpr int kMmaNSP = SCARF_MMA_NSP;    // states per pass: 4 NSP + 2 NSP accumulator doubles per lane (occupancy vs B-fragment reuse)
+static_assert(kMaxStateTile % kMmaNSP == 0, "states per pass must divide the state tile");
+// s_off: first state (within the tile) of this pass
 __global__ void __launch_bounds__(kMmaWarps * 32) density_mma_kernel(const double* __restrict__ V, const double* __restrict__ C, int nbf,
-                                                                     int nbf_pad, long long P, int s0, int ns, double g,
+                                                                     int nbf_pad, long long P, int s0, int ns, int s_off, double g,
                                                                      double2* __restrict__ out)
 {
     const int lane = threadIdx.x & 31, gid = lane >> 2, tig = lane & 3;
-    const long long p0 = ((long long)blockIdx.x * kMmaWarps + (threadIdx.x >> 5)) * 16;
+    const long long p0 = ((long long)blockIdx.x * kMmaWarps + (threadIdx.x >> 5)) * (8 * kMmaMT);
     if (p0 >= P) return;
-    const long long pa = p0 + gid, pb = p0 + 8 + gid;
-    const bool va = pa < P, vb = pb < P;
+    long long pt[kMmaMT];
+    bool ok[kMmaMT];
+#pragma unroll
+    for (int t = 0; t < kMmaMT; ++t) { pt[t] = p0 + 8 * t + gid; ok[t] = pt[t] < P; }
     const size_t per = (size_t)nbf_pad * nbf_pad;
-    double phi[2][kMaxStateTile];
+    double phi[kMmaMT][kMmaNSP];
 #pragma unroll
-    for (int s = 0; s < kMaxStateTile; ++s) phi[0][s] = phi[1][s] = 0.0;
+    for (int t = 0; t < kMmaMT; ++t)
+#pragma unroll
+        for (int s = 0; s < kMmaNSP; ++s) phi[t][s] = 0.0;
     for (int mu0 = 0; mu0 < nbf_pad; mu0 += 8) {
-        double D[2][kMaxStateTile][2];
+        double D[kMmaMT][kMmaNSP][2];
 #pragma unroll
-        for (int s = 0; s < kMaxStateTile; ++s) D[0][s][0] = D[0][s][1] = D[1][s][0] = D[1][s][1] = 0.0;
-        const double* Cb = C + (size_t)(mu0 + gid) * nbf_pad + tig;       // B[k = tig][n = gid] = C[mu0 + gid][nu0 + tig]
+        for (int t = 0; t < kMmaMT; ++t)
+#pragma unroll
+            for (int s = 0; s < kMmaNSP; ++s) D[t][s][0] = D[t][s][1] = 0.0;
+        const double* Cb = C + (size_t)s_off * per + (size_t)(mu0 / 8) * (nbf_pad / 4) * 32 + lane;   // + 32 * k-chunk
 #pragma unroll kMmaUnroll
         for (int nu0 = mu0; nu0 < nbf_pad; nu0 += 4) {
             const int nu = nu0 + tig;
-            const double a0 = (va && nu < nbf) ? V[(size_t)nu * P + pa] : 0.0;   // A[row = gid][k = tig] = v_nu(point)
-            const double a1 = (vb && nu < nbf) ? V[(size_t)nu * P + pb] : 0.0;
+            double av[kMmaMT];                                               // A[row = gid][k = tig] = v_nu(point)
 #pragma unroll
-            for (int s = 0; s < kMaxStateTile; ++s) {
-                const double b = Cb[(size_t)s * per + nu0];
-                dmma884(D[0][s], a0, b);
-                dmma884(D[1][s], a1, b);
+            for (int t = 0; t < kMmaMT; ++t) av[t] = (ok[t] && nu < nbf) ? V[vidx(nu, pt[t], nbf)] : 0.0;
+#pragma unroll
+            for (int s = 0; s < kMmaNSP; ++s) {
+                const double bf = Cb[(size_t)s * per + (size_t)(nu0 / 4) * 32];
+#pragma unroll
+                for (int t = 0; t < kMmaMT; ++t) dmma884(D[t][s], av[t], bf);
             }
         }
         // D[row = gid][col = 2 tig + i] = W[point][mu0 + 2 tig + i]
         const int m0 = mu0 + 2 * tig, m1 = m0 + 1;
-        const double v00 = (va && m0 < nbf) ? V[(size_t)m0 * P + pa] : 0.0, v01 = (va && m1 < nbf) ? V[(size_t)m1 * P + pa] : 0.0;
-        const double v10 = (vb && m0 < nbf) ? V[(size_t)m0 * P + pb] : 0.0, v11 = (vb && m1 < nbf) ? V[(size_t)m1 * P + pb] : 0.0;
 #pragma unroll
-        for (int s = 0; s < kMaxStateTile; ++s) {
-            phi[0][s] = fma(D[0][s][0], v00, fma(D[0][s][1], v01, phi[0][s]));
-            phi[1][s] = fma(D[1][s][0], v10, fma(D[1][s][1], v11, phi[1][s]));
+        for (int t = 0; t < kMmaMT; ++t) {
+            const double v0 = (ok[t] && m0 < nbf) ? V[vidx(m0, pt[t], nbf)] : 0.0, v1 = (ok[t] && m1 < nbf) ? V[vidx(m1, pt[t], nbf)] : 0.0;
+#pragma unroll
+            for (int s = 0; s < kMmaNSP; ++s) phi[t][s] = fma(D[t][s][0], v0, fma(D[t][s][1], v1, phi[t][s]));
         }
     }
 #pragma unroll
-    for (int s = 0; s < kMaxStateTile; ++s) {
+    for (int s = 0; s < kMmaNSP; ++s)
 #pragma unroll
-        for (int t = 0; t < 2; ++t) {
+        for (int t = 0; t < kMmaMT; ++t) {
             double x = phi[t][s];
             x += __shfl_xor_sync(0xffffffffu, x, 1);
             x += __shfl_xor_sync(0xffffffffu, x, 2);
-            phi[t][s] = x;
+            if (tig == 0 && s_off + s < ns && ok[t]) out[(size_t)(s0 + s_off + s) * P + pt[t]] = make_double2(g * x, 0.0);
         }
-        if (tig == 0 && s < ns) {
-            if (va) out[(size_t)(s0 + s) * P + pa] = make_double2(g * phi[0][s], 0.0);
-            if (vb) out[(size_t)(s0 + s) * P + pb] = make_double2(g * phi[1][s], 0.0);
-        }
-    }
 }
 
 // out[s][(ia, ib, ic)] = V_pix e^{i q.x_min} F[s][(alpha mod N, ...)],  alpha = ia - floor(N/2)
@@ -255,11 +277,11 @@ bool load_cufft()
 
 }  // namespace
 
-cudaError_t launch_orbitals(const PrimShell* prim, const int* shell_first, int n_shells, const FftGrid& g, double* V, cudaStream_t st)
+cudaError_t launch_orbitals(const PrimShell* prim, const int* shell_first, int n_shells, int nbf, const FftGrid& g, double* V, cudaStream_t st)
 {
     if (g.P <= 0 || n_shells <= 0) return cudaSuccess;
     dim3 grid((unsigned)((g.P + kPts - 1) / kPts), (unsigned)n_shells);
-    orbital_kernel<<<grid, kPts, 0, st>>>(prim, shell_first, g, V);
+    orbital_kernel<<<grid, kPts, 0, st>>>(prim, shell_first, g, nbf, V);
     return cudaGetLastError();
 }
 
@@ -277,9 +299,10 @@ cudaError_t launch_density_mma(const double* V, const double* T, double* Csym, i
     if (P <= 0 || ns <= 0) return cudaSuccess;
     const long long nsym = (long long)kMaxStateTile * nbf_pad * nbf_pad;
     symmetrize_kernel<<<(unsigned)((nsym + 255) / 256), 256, 0, st>>>(T, nbf, nbf_pad, s0, ns, Csym);
-    const long long per_cta = 16LL * kMmaWarps;
-    density_mma_kernel<<<(unsigned)((P + per_cta - 1) / per_cta), kMmaWarps * 32, 0, st>>>(V, Csym, nbf, nbf_pad, P, s0, ns, g,
-                                                                                       reinterpret_cast<double2*>(out_complex));
+    const long long per_cta = 8LL * kMmaMT * kMmaWarps;
+    for (int s_off = 0; s_off < ns; s_off += kMmaNSP)
+        density_mma_kernel<<<(unsigned)((P + per_cta - 1) / per_cta), kMmaWarps * 32, 0, st>>>(V, Csym, nbf, nbf_pad, P, s0, ns, s_off, g,
+                                                                                           reinterpret_cast<double2*>(out_complex));
     return cudaGetLastError();
 }
 

@@ -130,7 +130,8 @@ struct FftGrid {
     long long P;                            // nx*ny*nz
     double xmin[3], len[3];
 };
-cudaError_t launch_orbitals(const PrimShell* prim, const int* shell_first, int n_shells, const FftGrid& g, double* V, cudaStream_t st);
+cudaError_t launch_orbitals(const PrimShell* prim, const int* shell_first, int n_shells, int nbf, const FftGrid& g, double* V,
+                            cudaStream_t st);   // V in tiles of 8 points: [(P+7)/8][nbf][8]
 cudaError_t launch_density(const double* V, const double* T, int nbf, long long P, int s0, int ns, double g, double* out_complex,
                            cudaStream_t st);
 cudaError_t launch_density_mma(const double* V, const double* T, double* Csym, int nbf, int nbf_pad, long long P, int s0, int ns,

@@ -828,7 +828,7 @@ int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, c
         g.nx = nx; g.ny = ny; g.nz = nz;
         g.P = (long long)nx * ny * nz;
         for (int k = 0; k < 3; ++k) { g.xmin[k] = x_min[k]; g.len[k] = box_len[k]; }
-        const size_t vbytes = (size_t)hs.nbf * (size_t)g.P * sizeof(double);
+        const size_t vbytes = (size_t)hs.nbf * (size_t)((g.P + 7) / 8 * 8) * sizeof(double);
         const size_t fbytes = (size_t)ctx->n_states * (size_t)g.P * 2 * sizeof(double);
         if ((double)vbytes + 2.0 * (double)fbytes > 64e9) return fail(ctx, SCARF_ENOMEM, "fft_form_factors: grid needs more than 64 GB of scratch");
         // primitive shells and the first primitive of every contracted shell
@@ -853,7 +853,7 @@ int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, c
         if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "fft_form_factors: event");
         double* dV = static_cast<double*>(ctx->d_V.p);
         double* dF = static_cast<double*>(ctx->d_fft.p);
-        CU(launch_orbitals(reinterpret_cast<const PrimShell*>(pb), reinterpret_cast<const int*>(pb + pbytes), n_sh, g, dV, st),
+        CU(launch_orbitals(reinterpret_cast<const PrimShell*>(pb), reinterpret_cast<const int*>(pb + pbytes), n_sh, hs.nbf, g, dV, st),
            "fft_form_factors: orbital kernel");
         int launches = 1;
         for (int s0 = 0; s0 < ctx->n_states; s0 += kMaxStateTile) {
