@@ -52,6 +52,7 @@ def parse():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target wall time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel-variant", type=int, default=None)
+    ap.add_argument("--fft-grid", type=int, default=None, help="points per axis of the FFT-method grid (default: the config's q grid size)")
     return ap.parse_args()
 
 
@@ -274,7 +275,7 @@ def run_ours(args):
     # ---- the paper's FFT method (NEXT-4, scarf_fft_form_factors) on a real-space grid of the same size: box = atoms + 5 bohr
     fft_path = None
     if w.grid.get("kind") == "cartesian":
-        n_ax = int(w.grid["n_per_axis"])
+        n_ax = int(args.fft_grid or w.grid["n_per_axis"])
         lo = w.basis.atom_xyz.min(axis=0) - 5.0
         box = w.basis.atom_xyz.max(axis=0) + 5.0 - lo
         fft_out = torch.empty((w.n_states, n_ax ** 3, 2), dtype=torch.float64, device="cuda")
