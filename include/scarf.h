@@ -140,6 +140,14 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
 int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_t ny, const double* qy, int32_t nz,
                             const double* qz, double* out);
 
+/* Separable integrals (Eq. (64)-(65) PAPER.md:481-487): the weighted sum of f_s over a Cartesian product grid,
+ *     out[s] = sum_{ix,iy,iz} fx[ix] gy[iy] hz[iz] f_s(qx[ix], qy[iy], qz[iz])        (fx = quadrature weight x f(qx), ...),
+ * i.e. a quadrature of I_sep = Int d^3q f(q_x) g(q_y) h(q_z) f_s(q), evaluated WITHOUT forming f_s on the grid: per pair
+ * the three 1-D moments sum_i fx[i] qx[i]^t X_P(i) are contracted with the folded coefficients, so the cost is linear in
+ * nx + ny + nz (the paper's use of the V-tensors).  All pointers HOST; out [n_states][2]. */
+int scarf_separable_integral(scarf_ctx* ctx, int32_t nx, const double* qx, const double* fx, int32_t ny, const double* qy,
+                             const double* gy, int32_t nz, const double* qz, const double* hz, double* out);
+
 /* Angular moments of form factors given on a spherical product grid:
  *     f_s(q) = sum_lm Y_l^m(qhat) R_lm(q)   (Eq. 57)   =>   R_lm(q) = Int dOmega conj(Y_l^m(qhat)) f_s(q),
  *     <f_s^2>_Omega = Int dOmega/4pi |f_s(q)|^2                       (Eq. 59),

@@ -19,7 +19,7 @@ SCARF_N_CLASSES = 2 * SCARF_MAX_L + 1
 _CODES = {-1: "EINVAL", -2: "ESTATE", -3: "ENOMEM", -4: "ECUDA", -5: "ENODEVICE"}
 
 EXPORTS = ["scarf_create", "scarf_destroy", "scarf_set_stream", "scarf_set_option", "scarf_set_basis", "scarf_set_basis_pure", "scarf_nbf",
-           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_angular_moments", "scarf_fft_form_factors", "scarf_get_stats", "scarf_last_error",
+           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_separable_integral", "scarf_angular_moments", "scarf_fft_form_factors", "scarf_get_stats", "scarf_last_error",
            "scarf_version", "scarf_fp64_peak", "scarf_host_hermite_E", "scarf_host_shell_norms", "scarf_host_ylm_table"]
 
 
@@ -66,6 +66,7 @@ def _load():
     L.scarf_set_transitions.argtypes = [vp, C.c_int, vp]
     L.scarf_form_factors.argtypes = [vp, C.c_int64, vp, vp]
     L.scarf_form_factors_grid.argtypes = [vp, C.c_int32, vp, C.c_int32, vp, C.c_int32, vp, vp]
+    L.scarf_separable_integral.argtypes = [vp, C.c_int32, dp, dp, C.c_int32, dp, dp, C.c_int32, dp, dp, dp]
     L.scarf_angular_moments.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, C.c_int32, C.c_int32, vp, vp, vp]
     L.scarf_host_ylm_table.argtypes = [C.c_int, C.c_int, dp, dp, dp]
     L.scarf_fft_form_factors.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, vp]
@@ -332,6 +333,17 @@ class Scarf:
             import torch
             return torch.view_as_complex(out.view(self.n_states, n_q, 2))
         return out.reshape(self.n_states, n_q, 2).view(np.complex128)[..., 0]
+
+    def separable_integral(self, qx, fx, qy, gy, qz, hz) -> np.ndarray:
+        """sum_{ix,iy,iz} fx[ix] gy[iy] hz[iz] f_s(qx[ix], qy[iy], qz[iz]) for every state (complex128 [n_states]),
+        in O(pairs * (nx+ny+nz)): Eq. (64)-(65).  All arguments 1-D host arrays (weights x function samples)."""
+        arrs = [np.ascontiguousarray(a, dtype=np.float64) for a in (qx, fx, qy, gy, qz, hz)]
+        if arrs[0].shape != arrs[1].shape or arrs[2].shape != arrs[3].shape or arrs[4].shape != arrs[5].shape:
+            raise ValueError("separable_integral: each weight array must match its axis")
+        out = np.zeros((self.n_states, 2))
+        self._check(_lib.scarf_separable_integral(self._h, arrs[0].size, _dp(arrs[0]), _dp(arrs[1]), arrs[2].size, _dp(arrs[2]),
+                                                  _dp(arrs[3]), arrs[4].size, _dp(arrs[4]), _dp(arrs[5]), _dp(out)))
+        return out[:, 0] + 1j * out[:, 1]
 
     def stats(self) -> dict:
         s = ScarfStats()

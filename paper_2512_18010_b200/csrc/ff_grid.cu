@@ -254,3 +254,105 @@ cudaError_t launch_ff_grid(int NS, const GridArgs& a, cudaStream_t st)
 }
 
 }  // namespace scarf
+
+// ---- separable integrals (Eq. (64)-(65) PAPER.md:481-487) --------------------------------------------------------------
+//   I_s = sum_{ix,iy,iz} fx[ix] gy[iy] hz[iz] f_s(qx[ix], qy[iy], qz[iz])
+//       = sum_pairs sum_h D^s_h i^{n_h} Mx_P[t_h] My_P[u_h] Mz_P[v_h],    Mx_P[t] = sum_i fx[i] qx[i]^t X_P(i)
+// — linear in the axis lengths instead of their product (the paper's point about the V-tensors).  (-1)^{n/2} resp.
+// (-1)^{(n-1)/2} of i^n are already folded into D; odd n contribute through i.
+namespace scarf {
+
+namespace {
+
+// one thread per (record, axis): 7 complex moments  Mom[record][axis][t], t = 0..kMaxClass
+__global__ void __launch_bounds__(128) sep_moments_kernel(const GridArgs a, const double* __restrict__ wx, const double* __restrict__ wy,
+                                                          const double* __restrict__ wz, double2* __restrict__ mom)
+{
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= a.n_rec * 3) return;
+    const long long r = idx / 3;
+    const int axis = (int)(idx % 3);
+    int c = 0;
+#pragma unroll
+    for (int k = 1; k < kNClasses; ++k)
+        if (r >= a.class_first[k]) c = k;
+    const double* hdr = reinterpret_cast<const double*>(a.v.base + a.v.cls_off[c] + (size_t)(r - a.class_first[c]) * a.rec_bytes[c]);
+    const double inv4p = hdr[3], Pa = hdr[axis];
+    const int n = axis == 0 ? a.nx : (axis == 1 ? a.ny : a.nz);
+    const double* q = axis == 0 ? a.qx : (axis == 1 ? a.qy : a.qz);
+    const double* w = axis == 0 ? wx : (axis == 1 ? wy : wz);
+    double mr[kNClasses], mi[kNClasses];
+#pragma unroll
+    for (int t = 0; t < kNClasses; ++t) mr[t] = mi[t] = 0.0;
+    for (int i = 0; i < n; ++i) {
+        const double qi = q[i];
+        const double e = exp_neg(qi * qi * inv4p) * w[i];
+        double sn, cs;
+        sincos_fast(qi * Pa, sn, cs);
+        double pr = e * cs, pi = e * sn;
+#pragma unroll
+        for (int t = 0; t < kNClasses; ++t) {
+            mr[t] += pr;
+            mi[t] += pi;
+            pr *= qi;
+            pi *= qi;
+        }
+    }
+#pragma unroll
+    for (int t = 0; t < kNClasses; ++t) mom[(r * 3 + axis) * kNClasses + t] = make_double2(mr[t], mi[t]);
+}
+
+// block b sums records [b * per_block, ...) for every state of the tile: part[b][s]; fixed order, no atomics
+__global__ void __launch_bounds__(128) sep_contract_kernel(const GridArgs a, int NS, const double2* __restrict__ mom, int per_block,
+                                                           double2* __restrict__ part)
+{
+    __shared__ double2 red[128];
+    const int s = threadIdx.x % 16, lane_r = threadIdx.x / 16;      // 16 state slots x 8 record lanes
+    const long long r0 = (long long)blockIdx.x * per_block, r1 = min(a.n_rec, r0 + per_block);
+    double accr = 0.0, acci = 0.0;
+    if (s < a.v.ns_real)
+        for (long long r = r0 + lane_r; r < r1; r += 8) {
+            int c = 0;
+#pragma unroll
+            for (int k = 1; k < kNClasses; ++k)
+                if (r >= a.class_first[k]) c = k;
+            const double* rec = reinterpret_cast<const double*>(a.v.base + a.v.cls_off[c] + (size_t)(r - a.class_first[c]) * a.rec_bytes[c]);
+            const int NH = nherm(c);
+            const double* D = rec + 4 + (size_t)s * NH;
+            const double2* M = mom + (size_t)r * 3 * kNClasses;
+            int h = 0;
+            for (int n = 0; n <= c; ++n)
+                for (int t = n; t >= 0; --t)
+                    for (int u = n - t; u >= 0; --u, ++h) {
+                        const double2 xy = cmul(M[t], M[kNClasses + u]);
+                        const double2 m = cmul(xy, M[2 * kNClasses + (n - t - u)]);
+                        const double d = D[h];
+                        if (n & 1) { accr -= d * m.y; acci += d * m.x; }       // i * d * m
+                        else { accr += d * m.x; acci += d * m.y; }
+                    }
+        }
+    (void)NS;
+    red[threadIdx.x] = make_double2(accr, acci);
+    __syncthreads();
+    if (lane_r == 0) {
+        double2 t = red[s];
+        for (int k = 1; k < 8; ++k) { t.x += red[k * 16 + s].x; t.y += red[k * 16 + s].y; }
+        part[(size_t)blockIdx.x * 16 + s] = t;
+    }
+}
+
+}  // namespace
+
+// mom: [n_rec][3][kNClasses] complex scratch; part: [n_blocks][16] complex scratch.  Returns the number of blocks.
+cudaError_t launch_separable(const GridArgs& a, int NS, const double* wx, const double* wy, const double* wz, double* mom, double* part,
+                             int per_block, cudaStream_t st)
+{
+    if (a.n_rec <= 0) return cudaSuccess;
+    const long long n = a.n_rec * 3;
+    sep_moments_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(a, wx, wy, wz, reinterpret_cast<double2*>(mom));
+    const unsigned blocks = (unsigned)((a.n_rec + per_block - 1) / per_block);
+    sep_contract_kernel<<<blocks, 128, 0, st>>>(a, NS, reinterpret_cast<const double2*>(mom), per_block, reinterpret_cast<double2*>(part));
+    return cudaGetLastError();
+}
+
+}  // namespace scarf

@@ -107,6 +107,8 @@ struct GridArgs {
 };
 cudaError_t launch_grid_tables(const GridArgs& a, double2* tx, double2* ty, double2* tz, cudaStream_t st);
 cudaError_t launch_ff_grid(int NS, const GridArgs& a, cudaStream_t st);
+cudaError_t launch_separable(const GridArgs& a, int NS, const double* wx, const double* wy, const double* wz, double* mom, double* part,
+                             int per_block, cudaStream_t st);
 
 // angular moments (angular.cu, NEXT-3)
 void angular_host_tables(int l_max, int n_theta, const double* cos_theta, const double* w_theta, int n_phi,

@@ -734,6 +734,73 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
     }
 }
 
+int scarf_separable_integral(scarf_ctx* ctx, int32_t nx, const double* qx, const double* fx, int32_t ny, const double* qy,
+                             const double* gy, int32_t nz, const double* qz, const double* hz, double* out)
+{
+    if (!ctx) return SCARF_EINVAL;
+    if (ctx->host_only) return fail(ctx, SCARF_ENODEVICE, "separable_integral: host-only context; there is no CPU fallback");
+    if (!ctx->have_T) return fail(ctx, SCARF_ESTATE, "separable_integral: set_basis and set_transitions first");
+    if (nx < 1 || ny < 1 || nz < 1 || !qx || !fx || !qy || !gy || !qz || !hz || !out)
+        return fail(ctx, SCARF_EINVAL, "separable_integral: empty axis or null pointer");
+    const double* in[6] = {qx, qy, qz, fx, gy, hz};
+    const int len[6] = {nx, ny, nz, nx, ny, nz};
+    for (int k = 0; k < 6; ++k)
+        if (!all_finite(in[k], (size_t)len[k])) return fail(ctx, SCARF_EINVAL, "separable_integral: NaN/Inf in an axis or weight array");
+    try {
+        CU(cudaSetDevice(ctx->device), "separable_integral");
+        cudaStream_t st = ctx->stream;
+        CU(ctx->d_axes.ensure(2 * ((size_t)nx + ny + nz) * sizeof(double)), "separable_integral: alloc axes");
+        double* d[6];
+        size_t off = 0;
+        for (int k = 0; k < 6; ++k) {
+            d[k] = static_cast<double*>(ctx->d_axes.p) + off;
+            off += (size_t)len[k];
+            CU(cudaMemcpyAsync(d[k], in[k], (size_t)len[k] * sizeof(double), cudaMemcpyHostToDevice, st), "separable_integral: upload");
+        }
+        const int per_block = 64;
+        int launches = 0;
+        for (const TileStream& t : ctx->tiles) {
+            GridArgs a = {};
+            long long nrec = 0;
+            for (int L = 0; L < kNClasses; ++L) {
+                a.class_first[L] = nrec;
+                a.rec_bytes[L] = t.cls[L].rec_bytes;
+                a.v.cls_off[L] = t.cls[L].off;
+                nrec += t.cls[L].n;
+            }
+            for (int k = 0; k < t.ns_real; ++k) out[2 * (t.s0 + k)] = out[2 * (t.s0 + k) + 1] = 0.0;
+            if (nrec == 0) continue;
+            a.v.base = t.base;
+            a.v.ns_real = t.ns_real;
+            a.qx = d[0]; a.qy = d[1]; a.qz = d[2];
+            a.nx = nx; a.ny = ny; a.nz = nz;
+            a.n_rec = nrec;
+            const size_t n_blocks = (size_t)((nrec + per_block - 1) / per_block);
+            const size_t mom_bytes = (size_t)nrec * 3 * kNClasses * 16, part_bytes = n_blocks * 16 * 16;
+            CU(ctx->d_tab.ensure(mom_bytes + part_bytes), "separable_integral: alloc scratch");
+            double* mom = static_cast<double*>(ctx->d_tab.p);
+            double* part = mom + mom_bytes / 8;
+            CU(launch_separable(a, t.NS, d[3], d[4], d[5], mom, part, per_block, st), "separable_integral: kernels");
+            launches += 2;
+            std::vector<double> hp(n_blocks * 32);
+            CU(cudaMemcpyAsync(hp.data(), part, part_bytes, cudaMemcpyDeviceToHost, st), "separable_integral: download");
+            CU(cudaStreamSynchronize(st), "separable_integral: sync");
+            for (size_t b = 0; b < n_blocks; ++b)           // block order: deterministic
+                for (int k = 0; k < t.ns_real; ++k) {
+                    out[2 * (t.s0 + k)] += hp[(b * 16 + k) * 2];
+                    out[2 * (t.s0 + k) + 1] += hp[(b * 16 + k) * 2 + 1];
+                }
+        }
+        ctx->st.last_kernel_launches = launches;
+        CU(cudaStreamSynchronize(st), "separable_integral: sync");
+        return SCARF_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(ctx, SCARF_ENOMEM, "separable_integral: out of host memory");
+    } catch (...) {
+        return fail(ctx, SCARF_EINVAL, "separable_integral: unexpected exception");
+    }
+}
+
 int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t n_theta, const double* cos_theta,
                           const double* w_theta, int32_t n_phi, int32_t l_max, const double* f, double* R_out, double* f2_out)
 {

@@ -132,3 +132,46 @@ def test_grid_empty_and_errors(oracle_mod, Scarf, torch_cuda):
         bad[1] = np.nan
         with pytest.raises(Exception):
             sc.form_factors_grid(ax, bad, ax)
+
+
+@pytest.mark.parametrize("n_states", [1, 12, 14])
+def test_separable_integral_equals_weighted_grid_sum(oracle_mod, Scarf, torch_cuda, n_states):
+    """Eq. (64)-(65) PAPER.md:481-487: I_sep by 1-D moments per pair (linear in nx+ny+nz) against the plain weighted sum
+    of the ORACLE's f_s over the product grid; all classes L = 0..6 present."""
+    b = W.Basis(np.array([[0.1, 0.2, -0.9], [0.3, -0.4, 1.0]]), np.array([0, 0, 0, 0, 1, 1, 1, 1], np.int32),
+                np.array([0, 1, 2, 3, 0, 1, 2, 3], np.int32), np.array([2, 1, 1, 1, 2, 1, 1, 1], np.int32),
+                np.array([2.1, 0.4, 1.3, 0.9, 0.7, 1.9, 0.5, 1.1, 0.8, 0.6]),
+                np.array([0.5, 0.6, 1.0, 1.0, 1.0, 0.7, 0.4, 1.0, 1.0, 1.0]))
+    rng = np.random.default_rng(40 + n_states)
+    T = rng.normal(size=(n_states, b.nbf, b.nbf))
+    qx, qy, qz = np.linspace(-4, 4, 9), rng.uniform(-3, 3, 7), np.linspace(-5, 2, 11)
+    fx, gy, hz = rng.normal(size=9), np.exp(-qy ** 2), rng.uniform(0.1, 1, 11)
+    f = oracle_mod.form_factors(b, T, expand(qx, qy, qz)).reshape(n_states, 9, 7, 11)
+    ref = np.einsum("sxyz,x,y,z->s", f, fx, gy, hz)
+    with Scarf(0) as sc:
+        sc.set_basis(b)
+        sc.set_transitions(T)
+        got = sc.separable_integral(qx, fx, qy, gy, qz, hz)
+        assert np.array_equal(got, sc.separable_integral(qx, fx, qy, gy, qz, hz))      # deterministic
+    scale = np.einsum("sxyz,x,y,z->s", np.abs(f), np.abs(fx), np.abs(gy), np.abs(hz))
+    assert np.all(np.abs(got - ref) <= 1e-12 * scale), np.max(np.abs(got - ref) / scale)
+
+
+def test_separable_integral_full_size_config3(oracle_mod, Scarf, torch_cuda):
+    """Config 3 at full size (64^3, 9141 pairs, 12 states): the moment route against the weighted sum of the grid path's
+    own output (itself parity-checked against the oracle above) — a property that holds at any size."""
+    torch = torch_cuda
+    w = W.make_workload(3, oracle_mod.overlap)
+    ax = np.linspace(-w.grid["qmax"], w.grid["qmax"], w.grid["n_per_axis"])
+    wt = np.full_like(ax, ax[1] - ax[0])
+    fx, gy, hz = wt * np.exp(-0.05 * ax ** 2), wt * np.cos(0.3 * ax), wt / (1.0 + ax ** 2)
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(torch.as_tensor(w.T, device="cuda"))
+        axd = torch.as_tensor(ax, device="cuda")
+        f = sc.form_factors_grid(axd, axd, axd).view(w.n_states, 64, 64, 64)
+        W3 = torch.as_tensor(np.einsum("x,y,z->xyz", fx, gy, hz), device="cuda")
+        ref = (f * W3).sum(dim=(1, 2, 3)).cpu().numpy()
+        scale = (f.abs() * W3.abs()).sum(dim=(1, 2, 3)).cpu().numpy()
+        got = sc.separable_integral(ax, fx, ax, gy, ax, hz)
+    assert np.all(np.abs(got - ref) <= 1e-11 * scale), np.max(np.abs(got - ref) / scale)
