@@ -104,3 +104,33 @@ def test_full_size_config5_shape_sampled(oracle_mod, Scarf, torch_cuda):
         R_ref, f2_ref = oracle_mod.angular_moments(fs, ct, w, nph, l_max)
         assert_close(R[s, r].cpu().numpy(), R_ref[0, 0], 1e-12)
         assert_close(f2[s, r].cpu().numpy(), f2_ref[0, 0], 1e-12)
+
+
+def test_oscillator_strength_fit_small_q(oracle_mod, Scarf, torch_cuda):
+    """Eq. (81)-(82) PAPER.md:590-596: <|f_s|^2>_Omega ~ A + B q^2 + C q^4 at small |q| with B = |mu|^2 / 3, mu the
+    transition dipole (f_s -> i q.mu, Eq. 76-80).  GPU pipeline (S4 on a spherical grid + angular moments) for <f^2>;
+    mu from central differences of the ORACLE's Im f_s at q -> 0."""
+    torch = torch_cuda
+    w = W.make_workload(1, oracle_mod.overlap)
+    h = 1e-4
+    dq = np.concatenate([h * np.eye(3), -h * np.eye(3)])
+    fo = oracle_mod.form_factors(w.basis, w.T, dq)[0]
+    mu = (fo[:3].imag - fo[3:].imag) / (2 * h)
+    n_r, n_t, n_p = 12, 12, 24
+    r = np.linspace(0.01, 0.12, n_r)
+    ct, wt = np.polynomial.legendre.leggauss(n_t)
+    st = np.sqrt(1 - ct ** 2)
+    ph = 2 * np.pi * np.arange(n_p) / n_p
+    R, CT, PH = np.meshgrid(r, ct, ph, indexing="ij")
+    ST = np.broadcast_to(st[None, :, None], R.shape)
+    q = np.stack([R * ST * np.cos(PH), R * ST * np.sin(PH), R * CT], axis=-1).reshape(-1, 3)
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(w.T)
+        f = sc.form_factors(torch.as_tensor(q, device="cuda"))
+        _, f2 = sc.angular_moments(f, ct, wt, n_p, 4, n_r=n_r)
+        f2 = f2.cpu().numpy()[0]
+    A = np.stack([np.ones_like(r), r ** 2, r ** 4], axis=1)
+    coef, *_ = np.linalg.lstsq(A, f2, rcond=None)
+    assert abs(coef[1] - mu @ mu / 3) <= 1e-4 * (mu @ mu / 3)      # the paper's own level of agreement (PAPER.md:596)
+    assert abs(coef[0]) <= 1e-12 * (mu @ mu)          # f_s(0) = g Tr(T S) = 0 for S-orthonormal orbitals
