@@ -65,7 +65,8 @@ struct scarf_ctx {
     std::vector<DevBuf> staging, packed;
     std::vector<TileStream> tiles;
     scarf_stats st = {};
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev_slice = nullptr;
+    cudaStream_t copy_stream = nullptr;    // device->host copies of form_factors' output slices
 };
 
 namespace {
@@ -223,6 +224,8 @@ void scarf_destroy(scarf_ctx* ctx)
         free_device(ctx);
         if (ctx->ev0) cudaEventDestroy(ctx->ev0);
         if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+        if (ctx->ev_slice) cudaEventDestroy(ctx->ev_slice);
+        if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     }
     delete ctx;
 }
@@ -547,6 +550,8 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
         }
         if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "form_factors: event");
         int launches = 0;
+        // all state tiles for the q range [dq, dq + 3 n_q) into dout [n_states][n_q]
+        auto run_range = [&](const double* dq, long long n_q, double* dout) -> int {
         for (const TileStream& t : ctx->tiles) {
             long long nrec = 0;
             for (int L = 0; L < kNClasses; ++L) nrec += t.cls[L].n;
@@ -594,6 +599,29 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
                 launches += 2;
             }
         }
+        return SCARF_OK;
+        };
+        // Host output: the q range is cut into slices whose device->host copies (second stream) overlap the kernels of
+        // the next slice; each slice is computed into its own contiguous [n_states][slice] scratch and copied with a 2-D copy.
+        const int n_slices = (out_host && ctx->kernel_variant != 0 && n_q >= 4 * 16384) ? 4 : 1;
+        if (n_slices == 1) {
+            const int rc = run_range(dq, n_q, dout);
+            if (rc != SCARF_OK) return rc;
+        } else {
+            if (!ctx->copy_stream) CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking), "form_factors: copy stream");
+            if (!ctx->ev_slice) CU(cudaEventCreateWithFlags(&ctx->ev_slice, cudaEventDisableTiming), "form_factors: event");
+            const long long per = ((n_q + n_slices - 1) / n_slices + 255) & ~255LL;
+            for (long long q0 = 0; q0 < n_q; q0 += per) {
+                const long long nq_s = std::min(per, n_q - q0);
+                double* d_s = dout + (size_t)ctx->n_states * (size_t)q0 * 2;      // slice k occupies [n_states][nq_s] at this offset
+                const int rc = run_range(dq + 3 * q0, nq_s, d_s);
+                if (rc != SCARF_OK) return rc;
+                CU(cudaEventRecord(ctx->ev_slice, st), "form_factors: event");
+                CU(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_slice, 0), "form_factors: wait");
+                CU(cudaMemcpy2DAsync(out + 2 * q0, (size_t)n_q * 16, d_s, (size_t)nq_s * 16, (size_t)nq_s * 16, (size_t)ctx->n_states,
+                                     cudaMemcpyDeviceToHost, ctx->copy_stream), "form_factors: download slice");
+            }
+        }
         ctx->st.last_kernel_launches = launches;
         if (ctx->timing) {
             CU(cudaEventRecord(ctx->ev1, st), "form_factors: event");
@@ -602,7 +630,10 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
             cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
             ctx->st.last_kernel_ms = ms;
         }
-        if (out_host) {
+        if (out_host && n_slices > 1) {
+            CU(cudaStreamSynchronize(ctx->copy_stream), "form_factors: sync copies");
+            CU(cudaStreamSynchronize(st), "form_factors: sync");
+        } else if (out_host) {
             CU(cudaMemcpyAsync(out, dout, obytes, cudaMemcpyDeviceToHost, st), "form_factors: download out");
             CU(cudaStreamSynchronize(st), "form_factors: sync");
         } else if (q_host) {

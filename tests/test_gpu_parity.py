@@ -254,3 +254,23 @@ def test_pure_shells_mixed_basis(oracle_mod, Scarf, torch_cuda):
         assert np.array_equal(sc.form_factors(q), f.cpu().numpy())
         sc.set_basis(b)                                         # back to all-Cartesian on the same context
         assert sc.nbf == b.nbf
+
+
+def test_host_output_sliced_download_matches_device_output(oracle_mod, Scarf, torch_cuda):
+    """Host `out` with n_q >= 65536 is computed in q slices whose downloads overlap the next slice's kernels: same
+    values as the device-output path (different chunking, so equal to round-off, not bitwise) and as the oracle on a sample;
+    ragged n_q (not a multiple of the slice or tile size)."""
+    torch = torch_cuda
+    w = W.make_workload(1, oracle_mod.overlap)
+    rng = np.random.default_rng(77)
+    T = rng.normal(size=(3, w.basis.nbf, w.basis.nbf))
+    q = rng.uniform(-4, 4, size=(70001, 3))
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(T)
+        f_host = sc.form_factors(q)                                       # numpy in -> host out, sliced
+        f_dev = sc.form_factors(torch.as_tensor(q, device="cuda")).cpu().numpy()
+    scale = np.max(np.abs(f_dev), axis=1, keepdims=True)
+    assert np.max(np.abs(f_host - f_dev) / scale) <= 1e-13
+    idx = W.sample_q_indices(q.shape[0], 300, seed=3)
+    assert_parity(f_host[:, idx], oracle_mod.form_factors(w.basis, T, q[idx]))
