@@ -9,7 +9,7 @@ scarf_form_factors over the whole q grid.  Default workload: BASELINE.json confi
 is quoted on.  Metric: q.primitive-pair.state evaluations per second.
 
 `value`   : inputs resident in HBM, CUDA events on the library's stream, L2 flushed between steps.
-`e2e`     : the same job through the C ABI with HOST buffers (pinned q and out, pageable T): H2D/D2H inside.
+`e2e`     : the same job through the C ABI with HOST buffers (pinned T, q and out): H2D/D2H inside.
 `roofline`: FP64-ALU bound ("alu"): algorithmic FP64 issue slots / kernel time against the DFMA peak.
 `cpu_baseline`: the oracle, as it stands, on the host cores, on a bounded sample of the same q grid.
 
@@ -321,10 +321,10 @@ def run_ours(args):
                    "achieved_gbs": a_bytes / (a_ms * 1e-3) / 1e9,
                    "note": "includes the host-side Legendre/twiddle tables and their upload; bound: hbm"}
 
-    # ---- end to end: host buffers through the C ABI (pinned q / out, pageable T), copies inside the timed region
+    # ---- end to end: host buffers through the C ABI (pinned T, q and out), copies inside the timed region
     q_host = torch.as_tensor(w.q).pin_memory()
     out_host = torch.empty((w.n_states, w.n_q, 2), dtype=torch.float64).pin_memory()
-    T_host = np.ascontiguousarray(w.T)
+    T_host = torch.as_tensor(np.ascontiguousarray(w.T)).pin_memory()
 
     def step_host():
         sc.set_transitions(T_host)
@@ -342,7 +342,7 @@ def run_ours(args):
         e2e_s = (time.perf_counter() - t0) / e2e_steps
     e2e_s = replicas.max_over_ranks(e2e_s, "cuda")
     e2e_value = world * evals_per_step / e2e_s
-    h2d = T_host.nbytes + q_host.numel() * 8
+    h2d = T_host.numel() * 8 + q_host.numel() * 8
     d2h = out_host.numel() * 8
 
     if rank != 0:

@@ -102,9 +102,15 @@ bool is_device_ptr(const void* p)
 
 bool all_finite(const double* x, size_t n)
 {
-    double acc = 0.0;
-    for (size_t i = 0; i < n; ++i) acc += x[i] * 0.0;  // NaN/Inf propagate: Inf*0 = NaN
-    return acc == 0.0;
+    // exponent field all ones <=> NaN or Inf; integer test so that the loop vectorises (a serial FP sum cost 1.6 ms per call on
+    // config 3's q and T, inside the end-to-end step)
+    uint64_t bad = 0;
+    for (size_t i = 0; i < n; ++i) {
+        uint64_t b;
+        std::memcpy(&b, x + i, sizeof(b));
+        bad |= (uint64_t)((~b & 0x7ff0000000000000ULL) == 0);
+    }
+    return bad == 0;
 }
 
 int tile_size_for(int ns)  // smallest instantiated state tile >= ns (ns <= 12)
