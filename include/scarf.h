@@ -19,6 +19,10 @@
  *                             pack the pair stream.                                  Device kernels.
  *   scarf_form_factors     S4 the hot kernel: for every q, sum over pairs of
  *                             exp(-q^2/4p) e^{i q.P} sum_t D^s_t (i q)^t  (Eq. (48)). Device kernel(s).
+ * Around it: scarf_form_factors_grid / scarf_separable_integral (product grids: per-axis factor
+ * tables, Eq. (45)-(46), (64)-(65)), scarf_angular_moments (R_lm and <f^2>_Omega, Eq. (57)-(60)),
+ * scarf_fft_form_factors (the paper's FFT method, Eq. (19)-(34); approximate), scarf_set_basis_pure (solid-harmonic
+ * d/f shells, Eq. (A2)), option "threshold_eps" (paper-style thresholding).
  *
  * Conventions
  *   - Atomic units: positions in bohr, exponents in bohr^-2, q in bohr^-1.  No unit conversion happens here.
