@@ -51,7 +51,6 @@ def parse():
     ap.add_argument("--seed", type=int, default=None)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target wall time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--kernel-variant", type=int, default=None)
     ap.add_argument("--fft-grid", type=int, default=None, help="points per axis of the FFT-method grid (default: the config's q grid size)")
     return ap.parse_args()
 
@@ -110,7 +109,7 @@ class ClockSampler:
 def oracle_sample(w, target_s: float, seed: int = 0):
     """Time the oracle (as it stands) on a bounded, seeded sample of the workload's q grid."""
     import oracle
-    from paper_2512_18010_b200 import workloads as W
+    import workloads as W
     threads = oracle.max_threads()
     n0 = max(2, min(w.n_q, threads))
     idx = W.sample_q_indices(w.n_q, n0, seed)
@@ -140,7 +139,7 @@ def run_reference(args):
     if rank != 0:
         return
     import oracle
-    from paper_2512_18010_b200 import workloads as W
+    import workloads as W
     w = W.make_workload(args.config, oracle.overlap, seed=args.seed)
     threads = oracle.max_threads()
     # size one step at ~ cpu_seconds / (steps + warmup), at least `threads` q-points
@@ -175,7 +174,8 @@ def run_reference(args):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2512_18010_b200 import Scarf, binding, replicas, workloads as W
+    import workloads as W
+    from paper_2512_18010_b200 import Scarf, binding, replicas
 
     rank, world, local = replicas.env_rank_world_local()
     if not torch.cuda.is_available():
@@ -187,8 +187,6 @@ def run_ours(args):
     sc = Scarf(local)
     stream = torch.cuda.Stream()
     sc.set_stream(stream.cuda_stream)
-    if args.kernel_variant is not None:
-        sc.set_option("kernel_variant", args.kernel_variant)
 
     # The workload generator needs the AO overlap to orthonormalise the random MOs: the PRODUCT's own
     # (scarf_overlap, host tables) here; the oracle's in the tests.
@@ -242,7 +240,7 @@ def run_ours(args):
     # ---- product-grid path (NEXT-1, scarf_form_factors_grid) on the Cartesian configs: same job, same timing protocol
     grid_path = None
     if w.grid.get("kind") == "cartesian":
-        ax_dev = torch.as_tensor(np.linspace(-w.grid["qmax"], w.grid["qmax"], w.grid["n_per_axis"]), device="cuda")
+        ax_dev = torch.as_tensor(W.cartesian_axis(w.grid["n_per_axis"], w.grid["qmax"]), device="cuda")
 
         def step_grid():
             sc.set_transitions(T_dev)

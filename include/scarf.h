@@ -34,8 +34,14 @@
  *   - Contraction coefficients multiply unit-normalised primitives (Eq. A3); the contracted orbital
  *     is then renormalised (Eq. A5).
  *   - Every call returns SCARF_OK (0) or a negative SCARF_E* code; scarf_last_error() holds the text.  No C++
- *     exception crosses this boundary and there is no global state.  A context is not thread-safe; distinct
- *     contexts are independent.
+ *     exception crosses this boundary.  There is no mutable process-wide state: device constant tables are
+ *     compile-time initialised, kernel attributes are set per context at scarf_create, the cuFFT plan belongs to
+ *     the context (the only process-wide object is the immutable cuFFT function table, loaded once under
+ *     std::call_once).  A context is not thread-safe; distinct contexts are independent and may be driven from
+ *     different threads and on different devices.
+ *   - Argument range: |q . P| <= 2^30 for every Gaussian-product centre P (i.e. |q| * molecular extent < 1e9);
+ *     full accuracy of the phase needs |q . P| <~ 1e5.  e^{-q^2/4p} underflows to (effectively) 0 for large |q|, any
+ *     finite q is safe there.  Host q arrays are checked for NaN/Inf; device arrays are not.
  *   - Inputs are COPIED during set_* (the caller keeps ownership and may free at once).  Outputs are caller-owned.
  *   - "host or device" pointers are classified with cudaPointerGetAttributes: device and managed memory are used
  *     in place; pinned or pageable host memory is staged through context-owned device buffers and the call
@@ -102,7 +108,13 @@ int scarf_set_stream(scarf_ctx* ctx, void* cuda_stream);
  *                         a primitive shell pair is also dropped when B_P < threshold_eps * max_P B_P (B_P already is
  *                         the max over the states, so a pair survives if any transition needs it).  An APPROXIMATION
  *                         whose error is bounded: scarf_stats.dropped_bound.  Takes effect at set_transitions.
- *           "timing": 1 records CUDA-event times of S3/S4 into the stats (adds a stream sync per call).         */
+ *           "timing": 1 records CUDA-event times of S3/S4 into the stats (adds a stream sync per call).
+ *           "n_chunks": default 0 (automatic).  1..32 forces the number of cost-balanced slices the pair stream is cut
+ *                         into (the S4 grid is q-tiles x chunks; results agree to FP64 round-off for any value: the
+ *                         partial sums are added in chunk order).  A tuning/testing knob, not a numerical option.
+ *           "fft_density_variant": default 1 = FP64 tensor-core (DMMA) density kernel of scarf_fft_form_factors,
+ *                         0 = SIMT kernel (same result to round-off; slower).
+ *           Unknown keys and out-of-range values: SCARF_EINVAL.                                                      */
 int scarf_set_option(scarf_ctx* ctx, const char* key, double value);
 
 /* HOST pointers.  atom_xyz [n_atoms][3].  Shell i sits on atom shell_atom[i], has angular momentum shell_l[i]

@@ -2,7 +2,7 @@
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this
 package.  It never imports paper_2512_18010_b200's CUDA binding; it accepts the plain-array `Basis`
-container of paper_2512_18010_b200.workloads (the shared, arithmetic-free input generator) by duck typing.
+container of the top-level `workloads` module (the shared, arithmetic-free input generator) by duck typing.
 """
 from __future__ import annotations
 

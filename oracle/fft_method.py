@@ -27,7 +27,7 @@ from __future__ import annotations
 import numpy as np
 
 import oracle
-from paper_2512_18010_b200 import workloads as W
+import workloads as W
 
 
 def orbital_values(basis, pts) -> np.ndarray:

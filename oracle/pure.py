@@ -18,7 +18,7 @@ l only), so one primitive suffices for the fit; tests/test_oracle_pure.py pins t
     f_s(q) [mixed basis] = oracle.form_factors(basis, C T C^T, q),   C = blockdiag(C_l or identity).
 
 Shares no code, table or constant with paper_2512_18010_b200/csrc/pure.cu (which tabulates the monomial
-coefficients of S_lm); only the arithmetic-free helpers of paper_2512_18010_b200.workloads are used.
+coefficients of S_lm); only the arithmetic-free helpers of the top-level `workloads` module are used.
 """
 from __future__ import annotations
 
@@ -26,7 +26,7 @@ import numpy as np
 from scipy import special as sp
 
 import oracle
-from paper_2512_18010_b200 import workloads as W
+import workloads as W
 
 
 def real_sph_harm(l: int, m: int, theta, phi):

@@ -151,6 +151,11 @@ void angular_host_tables(int l_max, int n_theta, const double* cos_theta, const 
     }
 }
 
+cudaError_t angular_init_device()
+{
+    return cudaFuncSetAttribute(phi_dft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+}
+
 int angular_rows_per_cta(int n_phi) { return std::max(1, std::min(8, 2048 / std::max(1, n_phi))); }
 
 cudaError_t launch_phi_dft(const double* f, const double* tw, long long n_rows, int n_phi, int l_max, double* F, double* rowsum2,
@@ -159,14 +164,6 @@ cudaError_t launch_phi_dft(const double* f, const double* tw, long long n_rows, 
     if (n_rows <= 0) return cudaSuccess;
     const int rpc = angular_rows_per_cta(n_phi);
     const size_t smem = ((size_t)rpc * n_phi + n_phi) * sizeof(double2);
-    static bool attr_set[64] = {};
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (smem > 48 * 1024 && dev >= 0 && dev < 64 && !attr_set[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(phi_dft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
-        if (e != cudaSuccess) return e;
-        attr_set[dev] = true;
-    }
     const unsigned blocks = (unsigned)((n_rows + rpc - 1) / rpc);
     phi_dft_kernel<<<blocks, kThreads, smem, st>>>(reinterpret_cast<const double2*>(f), reinterpret_cast<const double2*>(tw), n_rows,
                                                    n_phi, l_max, rpc, reinterpret_cast<double2*>(F), rowsum2);

@@ -226,16 +226,20 @@ cudaError_t launch_grid_tables(const GridArgs& a, double2* tx, double2* ty, doub
 template <int NS>
 static cudaError_t launch_grid_ns(const GridArgs& a, unsigned blocks, cudaStream_t st)
 {
-    static bool attr_set[64] = {};
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (dev >= 0 && dev < 64 && !attr_set[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(ff_grid_kernel<NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-        if (e != cudaSuccess) return e;
-        attr_set[dev] = true;
-    }
     ff_grid_kernel<NS><<<blocks, kThreads, kSmemBytes, st>>>(a);
     return cudaGetLastError();
+}
+
+// The kernels need more than 48 KB of dynamic shared memory: an attribute of the function on the CURRENT device.
+// Called by scarf_create for the context's device (idempotent, no process-wide flag).
+cudaError_t ff_grid_init_device()
+{
+    cudaError_t e = cudaSuccess;
+#define SCARF_GRID_ATTR(NSV) \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(ff_grid_kernel<NSV>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    SCARF_GRID_ATTR(1) SCARF_GRID_ATTR(2) SCARF_GRID_ATTR(4) SCARF_GRID_ATTR(6) SCARF_GRID_ATTR(8) SCARF_GRID_ATTR(12)
+#undef SCARF_GRID_ATTR
+    return e;
 }
 
 cudaError_t launch_ff_grid(int NS, const GridArgs& a, cudaStream_t st)

@@ -29,10 +29,7 @@ constexpr int kThreads = 128;
 constexpr int kTile = kThreads * kNQ;        // q-points per CTA
 constexpr int kStages = 3;
 constexpr int kStageBytes = 8192;            // >= the largest record (L = 6, NS = 12: 8096 B)
-#ifndef SCARF_V1_SWP_MAXL
-#define SCARF_V1_SWP_MAXL 2
-#endif
-constexpr int kSwpMaxL = SCARF_V1_SWP_MAXL;   // classes whose record loop is software-pipelined (-1: none)
+constexpr int kSwpMaxL = 2;                  // classes whose record loop is software-pipelined
 
 struct Pipe {               // stage ring shared by all class segments of the CTA
     unsigned char* buf;     // kStages x kStageBytes
@@ -143,11 +140,8 @@ __global__ void __launch_bounds__(kThreads, 2) ff_v1_kernel(const V1Args a)
         for (int s = 0; s < NS; ++s) re[j][s] = im[j][s] = 0.0;
 
     const V1Chunk& ck = a.chunks[chunk];
-#ifndef SCARF_V1_MAXL
-#define SCARF_V1_MAXL 6
-#endif
 #define SCARF_V1_CLASS(LV)                                                                                              \
-    if (LV <= SCARF_V1_MAXL && ck.n[LV] > 0)                                                                                                   \
+    if (ck.n[LV] > 0)                                                                                             \
         run_class<LV, NS>(pp, a.base + a.cls_off[LV] + (size_t)ck.begin[LV] * (rec_doubles(LV, NS) * 8), ck.n[LV], qv, re, im);
     SCARF_V1_CLASS(0)
     SCARF_V1_CLASS(1)
@@ -191,13 +185,11 @@ cudaError_t launch_ff_v1(int NS, const V1Args& a, cudaStream_t st)
     if (a.n_q <= 0 || a.n_chunks <= 0) return cudaSuccess;
     const unsigned blocks = (unsigned)a.n_tiles * (unsigned)a.n_chunks;
     switch (NS) {
-#ifndef SCARF_V1_ONLY12
     case 1: ff_v1_kernel<1><<<blocks, kThreads, 0, st>>>(a); break;
     case 2: ff_v1_kernel<2><<<blocks, kThreads, 0, st>>>(a); break;
     case 4: ff_v1_kernel<4><<<blocks, kThreads, 0, st>>>(a); break;
     case 6: ff_v1_kernel<6><<<blocks, kThreads, 0, st>>>(a); break;
     case 8: ff_v1_kernel<8><<<blocks, kThreads, 0, st>>>(a); break;
-#endif
     case 12: ff_v1_kernel<12><<<blocks, kThreads, 0, st>>>(a); break;
     default: return cudaErrorInvalidValue;
     }

@@ -6,14 +6,17 @@
 //   f_s(q) ~= V_pix sum_abc Phi_abc e^{+i q.x_abc},  q = 2 pi (alpha/L_x, beta/L_y, gamma/L_z)    Eq. (27), (30)-(33)
 //   output index ia <-> alpha = ia - floor(N/2)  ("most negative frequencies first")
 //
-// Kernels: orbital_kernel (values of every contracted Cartesian orbital at every grid point, V[mu][point]),
-// density_kernel (the quadratic form v^T T^s v for up to 12 states per pass, T blocks staged in shared memory and
-// read with broadcast loads, the upper triangle only), cuFFT Z2Z (library step, loaded with dlopen at first use so that
-// libscarf.so itself has no cuFFT dependency), fft_post_kernel (V_pix, the phase e^{i q.x_min}, the reordering).
+// Kernels: orbital_kernel (values of every contracted Cartesian orbital at every grid point, in tiles of 8 points),
+// symmetrize_kernel + density_mma_kernel (the quadratic form v^T T^s v for up to 12 states per pass on the FP64 tensor
+// cores, mma.sync.m8n8k4.f64; the method of the product), density_kernel (the same form with SIMT FMAs, T blocks in
+// shared memory; kept as option "fft_density_variant" = 0 and as a second implementation the tests compare with),
+// cuFFT Z2Z (library step, loaded with dlopen at first use so that libscarf.so itself has no cuFFT dependency; the plan
+// belongs to the context), fft_post_kernel (V_pix, the phase e^{i q.x_min}, the reordering).
 // This is an approximation of f_s (box truncation, grid spacing); its CPU oracle is oracle/fft_method.py.
 #include <dlfcn.h>
 
 #include <cmath>
+#include <mutex>
 
 #include "kernels.cuh"
 
@@ -21,12 +24,6 @@ namespace scarf {
 
 namespace {
 
-#ifndef SCARF_MMA_VOLATILE
-#define SCARF_MMA_VOLATILE volatile
-#endif
-#ifndef SCARF_MMA_UNROLL
-#define SCARF_MMA_UNROLL 1
-#endif
 constexpr int kPts = 128;     // points per CTA
 constexpr int kNB = 16, kMB = 8;
 
@@ -149,19 +146,12 @@ __global__ void __launch_bounds__(256) symmetrize_kernel(const double* __restric
 
 __device__ __forceinline__ void dmma884(double (&d)[2], double a, double b)
 {
-    asm SCARF_MMA_VOLATILE("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
 }
 
 constexpr int kMmaWarps = 4;
-constexpr int kMmaUnroll = SCARF_MMA_UNROLL;
-#ifndef SCARF_MMA_NSP
-#define SCARF_MMA_NSP 12
-#endif
-#ifndef SCARF_MMA_MT
-#define SCARF_MMA_MT 2
-#endif
-constexpr int kMmaMT = SCARF_MMA_MT;      // 8-point M tiles per warp (they share every B fragment)
-constexpr int kMmaNSP = SCARF_MMA_NSP;    // states per pass: 4 NSP + 2 NSP accumulator doubles per lane (occupancy vs B-fragment reuse)
+constexpr int kMmaMT = 2;       // 8-point M tiles per warp (they share every B fragment)
+constexpr int kMmaNSP = 12;     // states per pass: 4 NSP + 2 NSP accumulator doubles per lane (occupancy vs B-fragment reuse)
 static_assert(kMaxStateTile % kMmaNSP == 0, "states per pass must divide the state tile");
 // s_off: first state (within the tile) of this pass
 __global__ void __launch_bounds__(kMmaWarps * 32) density_mma_kernel(const double* __restrict__ V, const double* __restrict__ C, int nbf,
@@ -188,7 +178,7 @@ __global__ void __launch_bounds__(kMmaWarps * 32) density_mma_kernel(const doubl
 #pragma unroll
             for (int s = 0; s < kMmaNSP; ++s) D[t][s][0] = D[t][s][1] = 0.0;
         const double* Cb = C + (size_t)s_off * per + (size_t)(mu0 / 8) * (nbf_pad / 4) * 32 + lane;   // + 32 * k-chunk
-#pragma unroll kMmaUnroll
+#pragma unroll 1
         for (int nu0 = mu0; nu0 < nbf_pad; nu0 += 4) {
             const int nu = nu0 + tig;
             double av[kMmaMT];                                               // A[row = gid][k = tig] = v_nu(point)
@@ -241,6 +231,7 @@ __global__ void __launch_bounds__(256) fft_post_kernel(const double2* __restrict
 }
 
 // ---- cuFFT through dlopen (library step; keeps libscarf.so free of a link-time cuFFT dependency) -------------------
+// The function table is immutable once loaded (std::call_once); plans are owned by the calling context (CufftPlan).
 typedef int (*PlanFn)(int*, int, int, int, int);
 typedef int (*SetStreamFn)(int, cudaStream_t);
 typedef int (*ExecFn)(int, void*, void*, int);
@@ -251,28 +242,31 @@ struct CufftApi {
     SetStreamFn set_stream = nullptr;
     ExecFn exec_z2z = nullptr;
     DestroyFn destroy = nullptr;
-    bool tried = false;
-} g_cufft;
+};
 
-bool load_cufft()
+const CufftApi* cufft_api()
 {
-    if (g_cufft.tried) return g_cufft.h != nullptr;
-    g_cufft.tried = true;
-    const char* names[] = {"libcufft.so.11", "/usr/local/cuda/lib64/libcufft.so.11", "libcufft.so", "/usr/local/cuda/lib64/libcufft.so"};
-    for (const char* n : names) {
-        g_cufft.h = dlopen(n, RTLD_NOW | RTLD_LOCAL);
-        if (g_cufft.h) break;
-    }
-    if (!g_cufft.h) return false;
-    g_cufft.plan3d = (PlanFn)dlsym(g_cufft.h, "cufftPlan3d");
-    g_cufft.set_stream = (SetStreamFn)dlsym(g_cufft.h, "cufftSetStream");
-    g_cufft.exec_z2z = (ExecFn)dlsym(g_cufft.h, "cufftExecZ2Z");
-    g_cufft.destroy = (DestroyFn)dlsym(g_cufft.h, "cufftDestroy");
-    if (!g_cufft.plan3d || !g_cufft.set_stream || !g_cufft.exec_z2z || !g_cufft.destroy) {
-        dlclose(g_cufft.h);
-        g_cufft.h = nullptr;
-    }
-    return g_cufft.h != nullptr;
+    static CufftApi api;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        const char* names[] = {"libcufft.so.11", "/usr/local/cuda/lib64/libcufft.so.11", "libcufft.so", "/usr/local/cuda/lib64/libcufft.so"};
+        void* h = nullptr;
+        for (const char* n : names) {
+            h = dlopen(n, RTLD_NOW | RTLD_LOCAL);
+            if (h) break;
+        }
+        if (!h) return;
+        api.plan3d = (PlanFn)dlsym(h, "cufftPlan3d");
+        api.set_stream = (SetStreamFn)dlsym(h, "cufftSetStream");
+        api.exec_z2z = (ExecFn)dlsym(h, "cufftExecZ2Z");
+        api.destroy = (DestroyFn)dlsym(h, "cufftDestroy");
+        if (!api.plan3d || !api.set_stream || !api.exec_z2z || !api.destroy) {
+            dlclose(h);
+            return;
+        }
+        api.h = h;
+    });
+    return api.h ? &api : nullptr;
 }
 
 }  // namespace
@@ -314,28 +308,35 @@ cudaError_t launch_fft_post(const double* F, const FftGrid& g, int ns, double* o
     return cudaGetLastError();
 }
 
-// In-place unnormalised transforms sum_abc f e^{+2 pi i (...)} of ns arrays [nx][ny][nz] of complex doubles.
+// In-place unnormalised transforms sum_abc f e^{+2 pi i (...)} of ns arrays [nx][ny][nz] of complex doubles with the
+// context's plan (created on the device that is current, i.e. the context's; re-planned when the grid changes).
 // Returns 0, -1 (cuFFT library not loadable) or a positive cufftResult.
-int cufft_inverse_batch(double* data, int nx, int ny, int nz, int ns, cudaStream_t st)
+int cufft_inverse_batch(CufftPlan& pl, double* data, int nx, int ny, int nz, int ns, cudaStream_t st)
 {
-    if (!load_cufft()) return -1;
-    static int plan = -1, pnx = 0, pny = 0, pnz = 0;
-    if (plan < 0 || pnx != nx || pny != ny || pnz != nz) {
-        if (plan >= 0) g_cufft.destroy(plan);
-        plan = -1;
+    const CufftApi* api = cufft_api();
+    if (!api) return -1;
+    if (pl.handle < 0 || pl.nx != nx || pl.ny != ny || pl.nz != nz) {
+        cufft_plan_release(pl);
         int h = 0;
-        const int rc = g_cufft.plan3d(&h, nx, ny, nz, 0x69 /* CUFFT_Z2Z */);
+        const int rc = api->plan3d(&h, nx, ny, nz, 0x69 /* CUFFT_Z2Z */);
         if (rc != 0) return rc;
-        plan = h; pnx = nx; pny = ny; pnz = nz;
+        pl.handle = h; pl.nx = nx; pl.ny = ny; pl.nz = nz;
     }
-    int rc = g_cufft.set_stream(plan, st);
+    int rc = api->set_stream(pl.handle, st);
     if (rc != 0) return rc;
     const size_t per = (size_t)nx * ny * nz * 2;
     for (int s = 0; s < ns; ++s) {
-        rc = g_cufft.exec_z2z(plan, data + (size_t)s * per, data + (size_t)s * per, 1 /* CUFFT_INVERSE */);
+        rc = api->exec_z2z(pl.handle, data + (size_t)s * per, data + (size_t)s * per, 1 /* CUFFT_INVERSE */);
         if (rc != 0) return rc;
     }
     return 0;
+}
+
+void cufft_plan_release(CufftPlan& pl)
+{
+    const CufftApi* api = cufft_api();
+    if (api && pl.handle >= 0) api->destroy(pl.handle);
+    pl = CufftPlan();
 }
 
 }  // namespace scarf

@@ -5,37 +5,39 @@
 
 namespace scarf {
 
-__constant__ unsigned char c_herm[kMaxHerm][4];              // (t,u,v,n) of Hermite index h
-__constant__ unsigned char c_comp[kMaxL + 1][kMaxCart][4];   // (a,b,c,-) of component comp of shell l
-__constant__ double c_fcomp[kMaxL + 1][kMaxCart];            // 1/sqrt((2a-1)!!(2b-1)!!(2c-1)!!)
-
-cudaError_t upload_tables()
-{
+// Index tables in the constant bank, initialised at compile time (no per-process upload step, no mutable global state):
+//   herm[h] = (t,u,v,n) of Hermite index h;  comp[l][c] = (a,b,c, (2a-1)!!(2b-1)!!(2c-1)!! ) of component c of shell l.
+struct IndexTables {
     unsigned char herm[kMaxHerm][4];
+    unsigned short comp[kMaxL + 1][kMaxCart][4];
+};
+constexpr IndexTables make_index_tables()
+{
+    IndexTables t{};
     int h = 0;
     for (int n = 0; n <= kMaxClass; ++n)
-        for (int t = n; t >= 0; --t)
-            for (int u = n - t; u >= 0; --u) {
-                herm[h][0] = (unsigned char)t; herm[h][1] = (unsigned char)u;
-                herm[h][2] = (unsigned char)(n - t - u); herm[h][3] = (unsigned char)n;
+        for (int a = n; a >= 0; --a)
+            for (int b = n - a; b >= 0; --b) {
+                t.herm[h][0] = (unsigned char)a; t.herm[h][1] = (unsigned char)b;
+                t.herm[h][2] = (unsigned char)(n - a - b); t.herm[h][3] = (unsigned char)n;
                 ++h;
             }
-    unsigned char comp[kMaxL + 1][kMaxCart][4] = {};
-    double fcomp[kMaxL + 1][kMaxCart] = {};
-    for (int l = 0; l <= kMaxL; ++l)
-        for (int c = 0; c < ncart(l); ++c) {
-            int abc[3];
-            component_powers(l, c, abc);
-            comp[l][c][0] = (unsigned char)abc[0]; comp[l][c][1] = (unsigned char)abc[1];
-            comp[l][c][2] = (unsigned char)abc[2];
-            fcomp[l][c] = component_factor(l, c);
-        }
-    cudaError_t e = cudaMemcpyToSymbol(c_herm, herm, sizeof herm);
-    if (e != cudaSuccess) return e;
-    e = cudaMemcpyToSymbol(c_comp, comp, sizeof comp);
-    if (e != cudaSuccess) return e;
-    return cudaMemcpyToSymbol(c_fcomp, fcomp, sizeof fcomp);
+    for (int l = 0; l <= kMaxL; ++l) {
+        int c = 0;
+        for (int a = l; a >= 0; --a)
+            for (int b = l - a; b >= 0; --b) {
+                const int e[3] = {a, b, l - a - b};
+                int df = 1;                                  // (2a-1)!!(2b-1)!!(2c-1)!! <= 11!! = 10395 for l <= 6
+                for (int k = 0; k < 3; ++k)
+                    for (int j = 2 * e[k] - 1; j > 1; j -= 2) df *= j;
+                t.comp[l][c][0] = (unsigned short)a; t.comp[l][c][1] = (unsigned short)b;
+                t.comp[l][c][2] = (unsigned short)(l - a - b); t.comp[l][c][3] = (unsigned short)df;
+                ++c;
+            }
+    }
+    return t;
 }
+__constant__ IndexTables c_tab = make_index_tables();
 
 // One warp per primitive shell pair; lanes stride over the Hermite index h.
 //   D^s_h = g * scale * sign(n) * sum_{ca,cb} f_ca f_cb (T^s[mu][nu] + T^s[nu][mu]) Ex[a][a'][t] Ey[b][b'][u] Ez[c][c'][v]
@@ -63,16 +65,17 @@ __global__ void __launch_bounds__(128) fold_kernel(const FoldArgs a)
     for (int s = 0; s < kMaxStateTile; ++s) bsum[s] = 0.0;
     const int nca = ncart(la), ncb = ncart(lb);
     for (int h = lane; h < nh; h += 32) {
-        const int t = c_herm[h][0], u = c_herm[h][1], v = c_herm[h][2], n = c_herm[h][3];
+        const int t = c_tab.herm[h][0], u = c_tab.herm[h][1], v = c_tab.herm[h][2], n = c_tab.herm[h][3];
         double acc[kMaxStateTile];
 #pragma unroll
         for (int s = 0; s < kMaxStateTile; ++s) acc[s] = 0.0;
         for (int ca = 0; ca < nca; ++ca) {
-            const int a1 = c_comp[la][ca][0], b1 = c_comp[la][ca][1], c1 = c_comp[la][ca][2];
+            const int a1 = c_tab.comp[la][ca][0], b1 = c_tab.comp[la][ca][1], c1 = c_tab.comp[la][ca][2];
+            const double fa = 1.0 / sqrt((double)c_tab.comp[la][ca][3]);   // = component_factor(la, ca) of the host code, bit for bit
             for (int cb = 0; cb < ncb; ++cb) {
-                const int a2 = c_comp[lb][cb][0], b2 = c_comp[lb][cb][1], c2 = c_comp[lb][cb][2];
+                const int a2 = c_tab.comp[lb][cb][0], b2 = c_tab.comp[lb][cb][1], c2 = c_tab.comp[lb][cb][2];
                 if (t > a1 + a2 || u > b1 + b2 || v > c1 + c2) continue;
-                const double G = c_fcomp[la][ca] * c_fcomp[lb][cb] * Ex[(a1 * (lb + 1) + a2) * nt + t] *
+                const double G = fa * (1.0 / sqrt((double)c_tab.comp[lb][cb][3])) * Ex[(a1 * (lb + 1) + a2) * nt + t] *
                                  Ey[(b1 * (lb + 1) + b2) * nt + u] * Ez[(c1 * (lb + 1) + c2) * nt + v];
                 const size_t mu = (size_t)(m.bf0a + ca), nu = (size_t)(m.bf0b + cb);
                 const double* t1 = T + mu * nbf + nu;

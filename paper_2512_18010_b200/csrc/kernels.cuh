@@ -60,11 +60,6 @@ struct FoldArgs {
 cudaError_t launch_fold(const FoldArgs& a, cudaStream_t st);
 cudaError_t launch_pack(const char* staging, char* packed, const unsigned long long* src_off,
                         const unsigned long long* dst_off, const int* nbytes, long long n, cudaStream_t st);
-cudaError_t upload_tables();   // constant-memory index tables; once per process
-
-// v0: one thread per q, records read straight from global memory.  accumulate != 0: out += result.
-cudaError_t launch_ff_v0(int L, const TileStream& ts, const double* q, long long n_q, double* out, int accumulate,
-                         cudaStream_t st);
 
 // v1 (ff_v1.cu): the tuned kernel.  A chunk is a cost-balanced slice of the class-sorted stream; per class c it
 // covers records [begin[c], begin[c] + n[c]) of that class.
@@ -107,12 +102,14 @@ struct GridArgs {
 };
 cudaError_t launch_grid_tables(const GridArgs& a, double2* tx, double2* ty, double2* tz, cudaStream_t st);
 cudaError_t launch_ff_grid(int NS, const GridArgs& a, cudaStream_t st);
+cudaError_t ff_grid_init_device();           // per-device function attributes (dynamic shared memory); idempotent
 cudaError_t launch_separable(const GridArgs& a, int NS, const double* wx, const double* wy, const double* wz, double* mom, double* part,
                              int per_block, cudaStream_t st);
 
 // angular moments (angular.cu, NEXT-3)
 void angular_host_tables(int l_max, int n_theta, const double* cos_theta, const double* w_theta, int n_phi,
                          std::vector<double>& Yw, std::vector<double>& tw);
+cudaError_t angular_init_device();           // per-device function attributes; idempotent
 cudaError_t launch_phi_dft(const double* f, const double* tw, long long n_rows, int n_phi, int l_max, double* F, double* rowsum2,
                            cudaStream_t st);
 cudaError_t launch_legendre(const double* F, const double* rowsum2, const double* Yw, const double* w_theta, long long n_sr,
@@ -139,7 +136,9 @@ cudaError_t launch_density(const double* V, const double* T, int nbf, long long 
 cudaError_t launch_density_mma(const double* V, const double* T, double* Csym, int nbf, int nbf_pad, long long P, int s0, int ns,
                                double g, double* out_complex, cudaStream_t st);
 cudaError_t launch_fft_post(const double* F, const FftGrid& g, int ns, double* out, cudaStream_t st);
-int cufft_inverse_batch(double* data, int nx, int ny, int nz, int ns, cudaStream_t st);
+struct CufftPlan { int handle = -1, nx = 0, ny = 0, nz = 0; };   // owned by a context, tied to its device
+int cufft_inverse_batch(CufftPlan& pl, double* data, int nx, int ny, int nz, int ns, cudaStream_t st);
+void cufft_plan_release(CufftPlan& pl);
 
 cudaError_t run_fp64_peak(double* dfma_per_s, double* sm_clock_mhz);
 

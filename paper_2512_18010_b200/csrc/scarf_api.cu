@@ -38,8 +38,6 @@ const double kCtr = 40.0;
 // product-grid kernel: YZ = Y Z, g0 = X0 YZ, g1 = X1 YZ: 12 slots per 2 q-points; tables: 39 per (pair, axis point)
 const double kCtrGrid = 6.0, kCtrTable = 39.0;
 
-bool g_tables_uploaded_dev[64] = {};
-
 }  // namespace
 
 struct scarf_ctx {
@@ -48,8 +46,7 @@ struct scarf_ctx {
     cudaStream_t stream = nullptr;
     double prefactor = 2.0, screen_tol = 1e-16, threshold_eps = 0.0;
     bool timing = false;
-    int kernel_variant = -1;  // -1 auto (v1), 0 force the baseline kernel v0
-    int n_chunks_opt = 0;     // 0 auto, else the number of stream chunks of the v1 kernel
+    int n_chunks_opt = 0;     // 0 auto, else the number of stream chunks of the S4 kernels
     int fft_density_variant = 1;  // 1: DMMA kernel, 0: SIMT kernel (fft_method.cu)
     std::string err;
     HostSetup hs;
@@ -67,6 +64,7 @@ struct scarf_ctx {
     scarf_stats st = {};
     cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev_slice = nullptr;
     cudaStream_t copy_stream = nullptr;    // device->host copies of form_factors' output slices
+    CufftPlan fft_plan;                    // cuFFT plan of the last scarf_fft_form_factors grid (this context's device)
 };
 
 namespace {
@@ -185,7 +183,7 @@ void free_device(scarf_ctx* c)
 
 extern "C" {
 
-const char* scarf_version(void) { return "scarf 0.1 (sm_100a)"; }
+const char* scarf_version(void) { return "scarf 0.2 (sm_100a)"; }
 
 int scarf_create(scarf_ctx** out, int device)
 {
@@ -202,10 +200,9 @@ int scarf_create(scarf_ctx** out, int device)
             return SCARF_ENODEVICE;
         }
         e = cudaSetDevice(device);
-        if (e == cudaSuccess && !(device < 64 && g_tables_uploaded_dev[device])) {
-            e = upload_tables();
-            if (e == cudaSuccess && device < 64) g_tables_uploaded_dev[device] = true;
-        }
+        // per-device function attributes (idempotent; set for every context so that no process-wide flag is needed)
+        if (e == cudaSuccess) e = ff_grid_init_device();
+        if (e == cudaSuccess) e = angular_init_device();
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device);
         if (e == cudaSuccess) e = cudaEventCreate(&ctx->ev0);
         if (e == cudaSuccess) e = cudaEventCreate(&ctx->ev1);
@@ -228,6 +225,7 @@ void scarf_destroy(scarf_ctx* ctx)
         cudaSetDevice(ctx->device);
         cudaStreamSynchronize(ctx->stream);
         free_device(ctx);
+        cufft_plan_release(ctx->fft_plan);
         if (ctx->ev0) cudaEventDestroy(ctx->ev0);
         if (ctx->ev1) cudaEventDestroy(ctx->ev1);
         if (ctx->ev_slice) cudaEventDestroy(ctx->ev_slice);
@@ -254,9 +252,13 @@ int scarf_set_option(scarf_ctx* ctx, const char* key, double value)
         ctx->screen_tol = value;
     } else if (k == "timing") ctx->timing = value != 0.0;
     else if (k == "threshold_eps") { if (!(value >= 0.0)) return fail(ctx, SCARF_EINVAL, "set_option: threshold_eps < 0"); ctx->threshold_eps = value; }
-    else if (k == "kernel_variant") ctx->kernel_variant = (int)value;
-    else if (k == "n_chunks") ctx->n_chunks_opt = (int)value;
-    else if (k == "fft_density_variant") ctx->fft_density_variant = (int)value;
+    else if (k == "n_chunks") {
+        if (value < 0 || value > kMaxChunks) return fail(ctx, SCARF_EINVAL, "set_option: n_chunks outside 0..32");
+        ctx->n_chunks_opt = (int)value;
+    } else if (k == "fft_density_variant") {
+        if (value != 0.0 && value != 1.0) return fail(ctx, SCARF_EINVAL, "set_option: fft_density_variant must be 0 or 1");
+        ctx->fft_density_variant = (int)value;
+    }
     else return fail(ctx, SCARF_EINVAL, "set_option: unknown key '" + k + "'");
     return SCARF_OK;
 }
@@ -566,16 +568,6 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
                 CU(cudaMemsetAsync(tile_out, 0, (size_t)t.ns_real * n_q * 2 * sizeof(double), st), "form_factors: memset");
                 continue;
             }
-            if (ctx->kernel_variant == 0) {  // baseline form: one launch per class, accumulating into out
-                bool first = true;
-                for (int L = 0; L < kNClasses; ++L) {
-                    if (t.cls[L].n <= 0) continue;
-                    CU(launch_ff_v0(L, t, dq, n_q, dout, first ? 0 : 1, st), "form_factors: kernel");
-                    first = false;
-                    ++launches;
-                }
-                continue;
-            }
             V1Args a = {};
             a.base = t.base;
             for (int L = 0; L < kNClasses; ++L) a.cls_off[L] = t.cls[L].off;
@@ -609,7 +601,7 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
         };
         // Host output: the q range is cut into slices whose device->host copies (second stream) overlap the kernels of
         // the next slice; each slice is computed into its own contiguous [n_states][slice] scratch and copied with a 2-D copy.
-        const int n_slices = (out_host && ctx->kernel_variant != 0 && n_q >= 4 * 16384) ? 4 : 1;
+        const int n_slices = (out_host && n_q >= 4 * 16384) ? 4 : 1;
         if (n_slices == 1) {
             const int rc = run_range(dq, n_q, dout);
             if (rc != SCARF_OK) return rc;
@@ -617,15 +609,21 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
             if (!ctx->copy_stream) CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking), "form_factors: copy stream");
             if (!ctx->ev_slice) CU(cudaEventCreateWithFlags(&ctx->ev_slice, cudaEventDisableTiming), "form_factors: event");
             const long long per = ((n_q + n_slices - 1) / n_slices + 255) & ~255LL;
+            // On any failure the copies already queued into the caller's `out` must have landed before we return
+            // (the caller may free `out` as soon as it sees the error code).
+            auto drain = [&](int rc) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamSynchronize(st); return rc; };
             for (long long q0 = 0; q0 < n_q; q0 += per) {
                 const long long nq_s = std::min(per, n_q - q0);
                 double* d_s = dout + (size_t)ctx->n_states * (size_t)q0 * 2;      // slice k occupies [n_states][nq_s] at this offset
                 const int rc = run_range(dq + 3 * q0, nq_s, d_s);
-                if (rc != SCARF_OK) return rc;
-                CU(cudaEventRecord(ctx->ev_slice, st), "form_factors: event");
-                CU(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_slice, 0), "form_factors: wait");
-                CU(cudaMemcpy2DAsync(out + 2 * q0, (size_t)n_q * 16, d_s, (size_t)nq_s * 16, (size_t)nq_s * 16, (size_t)ctx->n_states,
-                                     cudaMemcpyDeviceToHost, ctx->copy_stream), "form_factors: download slice");
+                if (rc != SCARF_OK) return drain(rc);
+                cudaError_t e = cudaEventRecord(ctx->ev_slice, st);
+                if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_slice, 0);
+                // one contiguous copy per state (a 2-D copy would need a pitch of n_q*16 bytes, beyond memPitch for n_q >= 2^27)
+                for (int s = 0; s < ctx->n_states && e == cudaSuccess; ++s)
+                    e = cudaMemcpyAsync(out + ((size_t)s * (size_t)n_q + (size_t)q0) * 2, d_s + (size_t)s * (size_t)nq_s * 2,
+                                        (size_t)nq_s * 16, cudaMemcpyDeviceToHost, ctx->copy_stream);
+                if (e != cudaSuccess) return drain(cuda_fail(ctx, e, "form_factors: download slice"));
             }
         }
         ctx->st.last_kernel_launches = launches;
@@ -974,7 +972,7 @@ int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, c
             }
         }
         CU(cudaStreamSynchronize(st), "fft_form_factors: sync");   // `first` (pageable) goes out of scope; cuFFT plans below
-        const int frc = cufft_inverse_batch(dF, nx, ny, nz, ctx->n_states, st);
+        const int frc = cufft_inverse_batch(ctx->fft_plan, dF, nx, ny, nz, ctx->n_states, st);
         if (frc < 0) return fail(ctx, SCARF_ECUDA, "fft_form_factors: the cuFFT library (libcufft.so.11) could not be loaded");
         if (frc > 0) return fail(ctx, frc == 2 ? SCARF_ENOMEM : SCARF_ECUDA, "fft_form_factors: cuFFT error " + std::to_string(frc));
         CU(launch_fft_post(dF, g, ctx->n_states, dout, st), "fft_form_factors: post kernel");

@@ -3,7 +3,7 @@ CPU oracle (oracle/angular_oracle.c: the plain double quadrature), element by el
 import numpy as np
 import pytest
 
-from paper_2512_18010_b200 import workloads as W
+import workloads as W
 
 pytestmark = pytest.mark.gpu
 

@@ -3,7 +3,7 @@ against its CPU oracle (oracle/fft_method.py) on the same grid, and convergence 
 import numpy as np
 import pytest
 
-from paper_2512_18010_b200 import workloads as W
+import workloads as W
 
 pytestmark = pytest.mark.gpu
 
@@ -92,3 +92,55 @@ def test_fft_method_argument_checks(oracle_mod, Scarf, torch_cuda):
             sc.fft_form_factors((4, 4, 4), np.zeros(3), np.array([1.0, 0.0, 1.0]))
         with pytest.raises(Exception):
             sc.fft_form_factors((4, 0, 4), np.zeros(3), np.ones(3))
+
+
+@pytest.mark.parametrize("config,n,extra_states", [(3, (20, 12, 28), 0), (3, (10, 6, 14), 1), (4, (10, 6, 14), 0), (4, (5, 6, 7), 1)])
+def test_fft_density_at_config_basis_sizes(oracle_mod, Scarf, torch_cuda, config, n, extra_states):
+    """The DMMA density kernel at the basis sizes bench.py times: config 3's basis (nbf = 190 -> padded
+    to 192: the last mu/nu fragments are partly zero padding, 24 mu-chunks) and config 4's (nbf = 600, f shells), 12 states
+    (one pass) and 13 (two state tiles), on a small ragged real-space grid (several CTAs and a partial warp) against the
+    oracle's orbital-product einsum; both density kernels."""
+    torch = torch_cuda
+    from oracle import fft_method as offt
+    w = W.make_workload(config, oracle_mod.overlap, with_q=False)
+    T = w.T
+    if extra_states:
+        rng = np.random.default_rng(config)
+        T = np.concatenate([T, 0.05 * rng.normal(size=(extra_states, w.basis.nbf, w.basis.nbf))], axis=0)
+    lo = w.basis.atom_xyz.min(axis=0) - 1.5
+    L = w.basis.atom_xyz.max(axis=0) + 1.5 - lo
+    f_ref = offt.form_factors(w.basis, T, n, lo, L)
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(torch.as_tensor(T, device="cuda"))
+        for variant in (1, 0):
+            sc.set_option("fft_density_variant", variant)
+            f = sc.fft_form_factors(n, lo, L)
+            torch.cuda.synchronize()
+            assert_parity(f.cpu().numpy(), f_ref)
+
+
+@pytest.mark.parametrize("n_s", [1, 2, 3, 4, 5, 6, 7, 8])
+def test_fft_density_padded_fragments(oracle_mod, Scarf, torch_cuda, n_s):
+    """nbf = 24 + n_s: every residue of nbf mod 8 (and mod 4), so the zero-padded rows/columns of the last DMMA fragments are
+    exercised against the oracle (not only GPU against GPU)."""
+    torch = torch_cuda
+    from oracle import fft_method as offt
+    rng = np.random.default_rng(100 + n_s)
+    atoms = np.array([[0.0, 0.0, 0.7], [0.0, 0.0, -0.7], [0.9, -0.5, 0.1]])
+    sa = [0, 0, 1, 1, 2, 2] + [int(i % 3) for i in range(n_s)]
+    sl = [0, 1, 0, 2, 3, 1] + [0] * n_s
+    sn = [3, 2, 1, 1, 1, 2] + [1] * n_s
+    ex = [5.0, 1.2, 0.3, 2.0, 0.6, 0.9, 1.1, 0.8, 1.5, 0.4] + list(0.25 * 1.7 ** np.arange(n_s))
+    co = [0.3, 0.6, 0.4, 0.7, 0.5, 1.0, 1.0, 1.0, 0.6, 0.8] + [1.0] * n_s
+    b = W.Basis(atoms, np.array(sa, np.int32), np.array(sl, np.int32), np.array(sn, np.int32), np.array(ex), np.array(co))
+    assert b.nbf == 24 + n_s
+    T = rng.normal(size=(5, b.nbf, b.nbf))
+    n, x_min, L = (9, 11, 7), np.array([-5.0, -4.5, -6.0]), np.array([10.5, 9.0, 11.0])
+    f_ref = offt.form_factors(b, T, n, x_min, L)
+    with Scarf(0) as sc:
+        sc.set_basis(b)
+        sc.set_transitions(T)
+        for variant in (1, 0):
+            sc.set_option("fft_density_variant", variant)
+            assert_parity(sc.fft_form_factors(n, x_min, L, device_out=False), f_ref)

@@ -4,7 +4,7 @@ PAPER.md:309-330) against the CPU oracle evaluated on the expanded point list, a
 import numpy as np
 import pytest
 
-from paper_2512_18010_b200 import workloads as W
+import workloads as W
 
 pytestmark = pytest.mark.gpu
 
@@ -53,7 +53,7 @@ def grid_ff(Scarf, torch, basis, T, qx, qy, qz, device_axes=True):
 
 def test_grid_config1_full(oracle_mod, Scarf, torch_cuda):
     w = W.make_workload(1, oracle_mod.overlap)
-    ax = np.linspace(-w.grid["qmax"], w.grid["qmax"], w.grid["n_per_axis"])
+    ax = W.cartesian_axis(w.grid["n_per_axis"], w.grid["qmax"])
     f, st = grid_ff(Scarf, torch_cuda, w.basis, w.T, ax, ax, ax)
     assert np.array_equal(expand(ax, ax, ax), w.q)          # same point order as the config's q list
     assert_parity(f, oracle_mod.form_factors(w.basis, w.T, w.q))
@@ -100,7 +100,7 @@ def test_grid_full_size_sampled(oracle_mod, Scarf, torch_cuda, config, n_sample)
     compared with the oracle on a seeded sample of points, and with the general kernel on every point."""
     torch = torch_cuda
     w = W.make_workload(config, oracle_mod.overlap)
-    ax = np.linspace(-w.grid["qmax"], w.grid["qmax"], w.grid["n_per_axis"])
+    ax = W.cartesian_axis(w.grid["n_per_axis"], w.grid["qmax"])
     idx = W.sample_q_indices(w.n_q, n_sample, seed=config)
     f_ref = oracle_mod.form_factors(w.basis, w.T, w.q[idx])
     with Scarf(0) as sc:
@@ -162,7 +162,7 @@ def test_separable_integral_full_size_config3(oracle_mod, Scarf, torch_cuda):
     own output (itself parity-checked against the oracle above) — a property that holds at any size."""
     torch = torch_cuda
     w = W.make_workload(3, oracle_mod.overlap)
-    ax = np.linspace(-w.grid["qmax"], w.grid["qmax"], w.grid["n_per_axis"])
+    ax = W.cartesian_axis(w.grid["n_per_axis"], w.grid["qmax"])
     wt = np.full_like(ax, ax[1] - ax[0])
     fx, gy, hz = wt * np.exp(-0.05 * ax ** 2), wt * np.cos(0.3 * ax), wt / (1.0 + ax ** 2)
     with Scarf(0) as sc:

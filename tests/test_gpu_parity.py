@@ -9,7 +9,7 @@ plus properties that hold at any size (f(-q) = conj f(q), host/device pointer ag
 import numpy as np
 import pytest
 
-from paper_2512_18010_b200 import workloads as W
+import workloads as W
 
 pytestmark = pytest.mark.gpu
 

@@ -9,7 +9,7 @@ import re
 import numpy as np
 import pytest
 
-from paper_2512_18010_b200 import workloads as W
+import workloads as W
 from tests import bruteforce as BF
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))

@@ -2,7 +2,7 @@
 import numpy as np
 import pytest
 
-from paper_2512_18010_b200 import workloads as W
+import workloads as W
 
 
 @pytest.fixture(scope="module")

@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 from scipy.special import eval_hermitenorm
 
-from paper_2512_18010_b200 import workloads as W
+import workloads as W
 from tests import bruteforce as bf
 
 HERE = os.path.dirname(os.path.abspath(__file__))

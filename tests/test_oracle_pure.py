@@ -4,7 +4,7 @@ import numpy as np
 import pytest
 from scipy import special as sp
 
-from paper_2512_18010_b200 import workloads as W
+import workloads as W
 
 
 @pytest.fixture(scope="module")

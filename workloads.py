@@ -1,6 +1,7 @@
 """Seeded synthetic workloads shaped like the paper's (BASELINE.json `configs`).
 
-This module is the ONLY code shared by the CUDA path and the CPU oracle.  It holds none of the
+This module (top level, outside both `paper_2512_18010_b200/` and `oracle/`) is the ONLY code shared by the CUDA
+path and the CPU oracle.  It holds none of the
 method's arithmetic: no Gaussian integrals, no normalisation constants, no form factors.  The one
 place a workload needs the method (the AO overlap matrix S, used to Löwdin-orthonormalise the
 random molecular orbitals and for the cond(S) guard) is passed in by the caller as `overlap_fn`:
@@ -90,8 +91,16 @@ def cartesian_components(l: int):
 # --------------------------------------------------------------------------------------------
 # q grids
 # --------------------------------------------------------------------------------------------
-def cartesian_grid(n: int, qmax: float) -> np.ndarray:
+def cartesian_axis(n: int, qmax: float) -> np.ndarray:
+    """linspace(-qmax, qmax, n), made EXACTLY inversion-symmetric: ax[i] == -ax[n-1-i] bit for bit.  The grid of
+    reading #13 is symmetric under q -> -q; numpy's linspace rounds the two halves differently (a few ulp), which
+    would hide that symmetry from a bitwise test.  (ax - ax[::-1])/2 is antisymmetric by construction."""
     ax = np.linspace(-qmax, qmax, n)
+    return 0.5 * (ax - ax[::-1])
+
+
+def cartesian_grid(n: int, qmax: float) -> np.ndarray:
+    ax = cartesian_axis(n, qmax)
     qx, qy, qz = np.meshgrid(ax, ax, ax, indexing="ij")
     return np.ascontiguousarray(np.stack([qx.ravel(), qy.ravel(), qz.ravel()], axis=1))
 
