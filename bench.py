@@ -1,12 +1,16 @@
 #!/usr/bin/env python
 """bench.py — throughput of the hot path (S3 fold + S4 form-factor kernel, include/scarf.h) on synthetic input.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--path auto|grid|list] [--impl ours|reference]
 
-One "step" = one 12-form-factor job on the workload: scarf_set_transitions (fold T^s into the pair stream) +
-scarf_form_factors over the whole q grid.  Default workload: BASELINE.json configs[2] = config 3 of DESIGN.md
-(10 heavy atoms + 8 H, 190 basis functions, 12 transitions, 64^3 q grid), the configuration the headline metric
-is quoted on.  Metric: q.primitive-pair.state evaluations per second.
+One "step" = one 12-form-factor job on the workload: scarf_set_transitions (fold T^s into the pair stream, screen and
+pack it on the device) + the S4 call a user makes for that q set: scarf_form_factors_grid for the Cartesian product
+grids of configs 1-4 (per-axis factor tables; f(-q) = conj f(q) on the inversion-symmetric grid), scarf_form_factors
+(arbitrary point list) for config 5 — `--path` forces one or the other; the other path is timed as well and reported
+beside the headline (`list_path` / `grid_path`).  Default workload: BASELINE.json configs[2] = config 3 of DESIGN.md
+(10 heavy atoms + 8 H, 190 basis functions, 12 transitions, 64^3 q grid), the configuration the headline metric is
+quoted on.  Metric: q.primitive-pair.state evaluations per second, one evaluation = one (q-point, kept pair, state)
+triple actually EXECUTED by S4 (mirror points filled by conjugation are not counted; `job_seconds` is the job time).
 
 `value`   : inputs resident in HBM, CUDA events on the library's stream, L2 flushed between steps.
 `e2e`     : the same job through the C ABI with HOST buffers (pinned T, q and out): H2D/D2H inside.
@@ -36,9 +40,46 @@ METRIC = "q*primitive-pair*state evaluations per second (12-form-factor job, fol
 UNIT = "evals/s"
 # FP64 lanes per SM per clock on B200 (GB100): 64 DFMA/clk/SM, as on GH100.
 DFMA_PER_CLK_PER_SM = 64
-# dram__bytes_read.sum + dram__bytes_write.sum of one ff_v1_kernel<12> launch, from the `ncu --set full` capture
-# summarised in profiles/r01b_ff_v1_ncu_full.md (config 3 only; other configs were not captured -> null).
-NCU_DRAM_BYTES_PER_LAUNCH = {3: 16.663808e6 + 293.769984e6}
+# roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, looked up BY NAME
+# (config, kernel) in the table written from the committed `ncu --set full` captures; null when there is no capture.
+TRAFFIC_TABLE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "dram_traffic_per_launch.csv")
+
+
+def traffic_from_profiles(config: int, kernel: str):
+    try:
+        with open(TRAFFIC_TABLE) as f:
+            rows = [l.strip().split(",") for l in f if l.strip() and not l.startswith("#")]
+    except OSError:
+        return None, None
+    hdr = rows[0]
+    best = None
+    for r in rows[1:]:
+        d = dict(zip(hdr, r))
+        if int(d["config"]) == config and d["kernel"] == kernel:
+            best = d                       # the last matching row = the latest capture
+    if best is None:
+        return None, None
+    return float(best["dram_bytes_read"]) + float(best["dram_bytes_write"]), best["source"]
+
+
+def measured_hbm_peak():
+    """(GB/s, source): the driver-written MEASURED_PEAKS.json, else the fallback B200_PROFILING.md states."""
+    try:
+        with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (copy bandwidth, burst)"
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "of fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def parse():
@@ -51,6 +92,8 @@ def parse():
     ap.add_argument("--seed", type=int, default=None)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target wall time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--path", default="auto", choices=["auto", "grid", "list"],
+                    help="S4 entry point of the headline step: product-grid API or arbitrary point list (auto: grid on the Cartesian configs)")
     ap.add_argument("--fft-grid", type=int, default=None, help="points per axis of the FFT-method grid (default: the config's q grid size)")
     return ap.parse_args()
 
@@ -164,7 +207,8 @@ def run_reference(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "config": args.config, "n_q": w.n_q, "n_states": w.n_states,
                        "nbf": w.basis.nbf, "n_pairs_all": n_pairs_all(w.basis), "sample": sample},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "cpu_model": cpu_model(), "kind": "oracle", "sample": sample,
+                             "unit_note": "evaluations counted on ALL primitive shell pairs (the oracle screens nothing)",
                              "job_seconds_extrapolated": dt * w.n_q / len(idx)},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -196,83 +240,106 @@ def run_ours(args):
 
     w = W.make_workload(args.config, overlap, seed=args.seed)
     sc.set_basis(w.basis)
+    cartesian = w.grid.get("kind") == "cartesian"
+    path = args.path if args.path != "auto" else ("grid" if cartesian else "list")
+    if path == "grid" and not cartesian:
+        raise SystemExit("--path grid needs a Cartesian product grid (configs 1-4)")
     T_dev = torch.as_tensor(w.T, device="cuda")
     q_dev = torch.as_tensor(w.q, device="cuda")
     out_dev = torch.empty((w.n_states, w.n_q, 2), dtype=torch.float64, device="cuda")
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+    ax_host = W.cartesian_axis(w.grid["n_per_axis"], w.grid["qmax"]) if cartesian else None   # host axes: fully asynchronous call
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def step_device():
+    def step_list():
         sc.set_transitions(T_dev)
         sc.form_factors(q_dev, out=out_dev)
 
-    # ---- resident-input timing: CUDA events on the library's stream, L2 flushed between steps (untimed)
-    with torch.cuda.stream(stream):
-        for _ in range(max(3, args.warmup)):
-            step_device()
-        barrier()
-        sampler = ClockSampler(local) if rank == 0 else None
-        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-        kern_ms = []
-        sc.set_option("timing", 1)
-        barrier()
-        t_wall0 = time.perf_counter()
-        for k in range(args.steps):
-            flush.fill_(k & 0xFF)
-            ev[k][0].record(stream)
-            step_device()
-            ev[k][1].record(stream)
-            st_k = sc.stats()
-            kern_ms.append((st_k["last_fold_ms"], st_k["last_kernel_ms"]))
-        barrier()
-        t_wall = time.perf_counter() - t_wall0
-        clocks = sampler.stop() if sampler else None
-        sc.set_option("timing", 0)
-    step_ms = [a.elapsed_time(b) for a, b in ev]
-    st = sc.stats()
-    evals_per_step = st["evals_per_q"] * w.n_q
-    value, ms_per_step = replicas.whole_job_value(evals_per_step, args.steps, float(sum(step_ms)), "cuda")
+    def step_grid():
+        sc.set_transitions(T_dev)
+        sc.form_factors_grid(ax_host, ax_host, ax_host, out=out_dev)
 
-    # ---- product-grid path (NEXT-1, scarf_form_factors_grid) on the Cartesian configs: same job, same timing protocol
-    grid_path = None
-    if w.grid.get("kind") == "cartesian":
-        ax_dev = torch.as_tensor(W.cartesian_axis(w.grid["n_per_axis"], w.grid["qmax"]), device="cuda")
+    def step_grid_plain():
+        sc.set_option("grid_symmetry", 0)
+        step_grid()
+        sc.set_option("grid_symmetry", 1)
 
-        def step_grid():
-            sc.set_transitions(T_dev)
-            sc.form_factors_grid(ax_dev, ax_dev, ax_dev, out=out_dev)
-
+    def run_timed(step, steps, warmup, sample_clocks=False):
+        """W untimed steps, then `steps` steps timed with CUDA events on the library's stream (L2 flushed before each,
+        outside the events), asynchronous (no per-call sync); then the same steps again with the library's per-kernel
+        events ("timing" option) for the kernel-only durations.  Returns a dict."""
         with torch.cuda.stream(stream):
-            for _ in range(3):
-                step_grid()
+            for _ in range(warmup):
+                step()
             barrier()
-            gev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-            gk = []
-            sc.set_option("timing", 1)
-            for k in range(args.steps):
+            sampler = ClockSampler(local) if (sample_clocks and rank == 0) else None
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+            barrier()
+            t0 = time.perf_counter()
+            for k in range(steps):
                 flush.fill_(k & 0xFF)
-                gev[k][0].record(stream)
-                step_grid()
-                gev[k][1].record(stream)
-                gk.append(sc.stats()["last_kernel_ms"])
+                ev[k][0].record(stream)
+                step()
+                ev[k][1].record(stream)
             barrier()
+            wall = time.perf_counter() - t0
+            clocks = sampler.stop() if sampler else None
+            st = sc.stats()
+            ms = [a.elapsed_time(b) for a, b in ev]
+            # instrumented pass: per-kernel CUDA events inside the library (one stream sync per call)
+            sc.set_option("timing", 1)
+            fold, kern, main = [], [], []
+            for k in range(steps):
+                flush.fill_(k & 0xFF)
+                step()
+                s2 = sc.stats()
+                fold.append(s2["last_fold_ms"]); kern.append(s2["last_kernel_ms"]); main.append(s2["last_main_kernel_ms"])
             sc.set_option("timing", 0)
-        g_ms = float(np.mean([a.elapsed_time(b) for a, b in gev]))
-        g_ms = replicas.max_over_ranks(g_ms, "cuda")
-        gst = sc.stats()
-        grid_path = {"api": "scarf_form_factors_grid", "ms_per_step": g_ms, "kernel_ms": float(np.median(gk)),
-                     "value": world * evals_per_step / (g_ms * 1e-3), "unit": UNIT, "slots": gst["last_grid_slots"],
-                     "launches_per_step": int(gst["last_kernel_launches"] + gst["last_fold_launches"])}
-        step_device()   # leave the general path's result in out_dev for the parity sample below
+            barrier()
+        return {"ms": ms, "sum_ms": float(sum(ms)), "wall_s": wall, "clocks": clocks, "stats": st,
+                "fold_ms": float(np.median(fold)), "kernel_ms": float(np.median(kern)), "main_kernel_ms": float(np.median(main)),
+                "main_kernel_ms_mean": float(np.mean(main))}
+
+    steps, warmup = args.steps, max(3, args.warmup)
+    head = run_timed(step_grid if path == "grid" else step_list, steps, warmup, sample_clocks=True)
+    st = head["stats"]
+    n_eval_q = w.n_q
+    if path == "grid" and st["last_grid_symmetric"]:
+        n_ax = w.grid["n_per_axis"]
+        n_eval_q = ((n_ax + 1) // 2) * n_ax * n_ax
+    evals_per_step = st["evals_per_q"] * n_eval_q                      # executed (q, kept pair, state) triples
+    value, ms_per_step = replicas.whole_job_value(evals_per_step, steps, head["sum_ms"], "cuda")
+    clocks = head["clocks"]
+
+    # ---- the other S4 entry point (and the product grid without the symmetry), same job, same protocol
+    def side(step, n_q_exec, slots_key):
+        r = run_timed(step, steps, 3)
+        s2 = r["stats"]
+        ms = replicas.max_over_ranks(float(np.mean(r["ms"])), "cuda")
+        slots = s2["last_grid_kernel_slots"] if slots_key == "grid" else s2["slots_per_q"] * w.n_q
+        return {"ms_per_step": ms, "job_seconds": ms * 1e-3, "kernel_ms": r["kernel_ms"], "main_kernel_ms": r["main_kernel_ms"],
+                "fold_ms": r["fold_ms"], "value": world * s2["evals_per_q"] * n_q_exec / (ms * 1e-3), "unit": UNIT,
+                "slots_main_kernel": slots, "n_chunks": s2["last_n_chunks"],
+                "launches_per_step": int(s2["last_kernel_launches"] + s2["last_fold_launches"])}
+
+    list_path = grid_path = grid_plain = None
+    if cartesian:
+        if path == "grid":
+            list_path = dict(side(step_list, w.n_q, "list"), api="scarf_form_factors")
+        else:
+            n_ax = w.grid["n_per_axis"]
+            grid_path = dict(side(step_grid, ((n_ax + 1) // 2) * n_ax * n_ax, "grid"), api="scarf_form_factors_grid", symmetric=True)
+        grid_plain = dict(side(step_grid_plain, w.n_q, "grid"), api="scarf_form_factors_grid", symmetric=False)
+        (step_grid if path == "grid" else step_list)()        # leave the headline path's result in out_dev for the parity sample
         torch.cuda.synchronize()
 
     # ---- the paper's FFT method (NEXT-4, scarf_fft_form_factors) on a real-space grid of the same size: box = atoms + 5 bohr
     fft_path = None
-    if w.grid.get("kind") == "cartesian":
+    if cartesian:
         n_ax = int(args.fft_grid or w.grid["n_per_axis"])
         lo = w.basis.atom_xyz.min(axis=0) - 5.0
         box = w.basis.atom_xyz.max(axis=0) + 5.0 - lo
@@ -282,8 +349,8 @@ def run_ours(args):
             for _ in range(2):
                 sc.fft_form_factors((n_ax,) * 3, lo, box, out=fft_out)
             barrier()
-            fev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-            for k in range(args.steps):
+            fev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+            for k in range(steps):
                 flush.fill_(k & 0xFF)
                 fev[k][0].record(stream)
                 sc.fft_form_factors((n_ax,) * 3, lo, box, out=fft_out)
@@ -292,7 +359,16 @@ def run_ours(args):
         f_ms = float(np.median([a.elapsed_time(b) for a, b in fev]))
         fma = 0.5 * w.n_states * float(w.basis.nbf) ** 2 * n_ax ** 3
         fft_path = {"api": "scarf_fft_form_factors", "grid": [n_ax] * 3, "box_bohr": [float(x) for x in box], "ms_per_call": f_ms,
-                    "density_fma": fma, "note": "approximate method (box truncation, grid spacing); timing only"}
+                    "density_fma": fma, "note": "approximate method (box truncation, grid spacing)"}
+        if rank == 0 and world == 1 and not args.no_cpu_baseline:
+            # sampled parity against the FFT-method oracle: the same basis, T and box on a small ragged grid the oracle's
+            # einsum finishes in seconds (the density kernel's launch shape depends on nbf, not on the grid size)
+            from oracle import fft_method as offt
+            n_small = (10, 6, 14)
+            f_ref = offt.form_factors(w.basis, w.T, n_small, lo, box)
+            f_gpu = sc.fft_form_factors(n_small, lo, box).cpu().numpy()
+            err = max(float(np.max(np.abs(f_gpu[s] - f_ref[s])) / np.max(np.abs(f_ref[s]))) for s in range(w.n_states))
+            fft_path["parity"] = {"grid": list(n_small), "max_rel_err_vs_fft_oracle": err, "tolerance": 1e-10, "ok": bool(err <= 1e-10)}
         del fft_out
 
     # ---- angular moments of the result (NEXT-3, scarf_angular_moments) on the spherical product grid of config 5
@@ -306,33 +382,39 @@ def run_ours(args):
             for _ in range(3):
                 sc.angular_moments(f_dev, ct, wt, n_p, l_max, n_r=n_r)
             barrier()
-            aev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-            for k in range(args.steps):
+            aev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+            for k in range(steps):
                 flush.fill_(k & 0xFF)
                 aev[k][0].record(stream)
                 sc.angular_moments(f_dev, ct, wt, n_p, l_max, n_r=n_r)
                 aev[k][1].record(stream)
             barrier()
         a_ms = float(np.median([a.elapsed_time(b) for a, b in aev]))
-        a_bytes = 16.0 * w.n_states * w.n_q + 16.0 * w.n_states * n_r * (l_max + 1) ** 2
+        a_bytes = 16.0 * w.n_states * w.n_q + 16.0 * w.n_states * n_r * (l_max + 1) ** 2 + 8.0 * w.n_states * n_r
+        hbm_peak, hbm_src = measured_hbm_peak()
+        a_traffic, a_src = traffic_from_profiles(args.config, "angular_fused_kernel")
         angular = {"api": "scarf_angular_moments", "l_max": l_max, "ms_per_call": a_ms, "algorithmic_bytes": a_bytes,
-                   "achieved_gbs": a_bytes / (a_ms * 1e-3) / 1e9,
-                   "note": "includes the host-side Legendre/twiddle tables and their upload; bound: hbm"}
+                   "roofline": {"bound": "hbm", "achieved": a_bytes / (a_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                                "frac": a_bytes / (a_ms * 1e-3) / 1e9 / hbm_peak, "traffic": a_traffic, "traffic_source": a_src,
+                                "peak_source": hbm_src}}
 
-    # ---- end to end: host buffers through the C ABI (pinned T, q and out), copies inside the timed region
+    # ---- end to end: host buffers through the C ABI (pinned T, q/axes and out), copies inside the timed region
     q_host = torch.as_tensor(w.q).pin_memory()
     out_host = torch.empty((w.n_states, w.n_q, 2), dtype=torch.float64).pin_memory()
     T_host = torch.as_tensor(np.ascontiguousarray(w.T)).pin_memory()
 
     def step_host():
         sc.set_transitions(T_host)
-        sc.form_factors(q_host, out=out_host)
+        if path == "grid":
+            sc.form_factors_grid(ax_host, ax_host, ax_host, out=out_host)
+        else:
+            sc.form_factors(q_host, out=out_host)
 
     with torch.cuda.stream(stream):
         for _ in range(2):
             step_host()
         barrier()
-        e2e_steps = max(3, min(args.steps, 10))
+        e2e_steps = max(3, min(steps, 10))
         t0 = time.perf_counter()
         for _ in range(e2e_steps):
             step_host()
@@ -340,7 +422,7 @@ def run_ours(args):
         e2e_s = (time.perf_counter() - t0) / e2e_steps
     e2e_s = replicas.max_over_ranks(e2e_s, "cuda")
     e2e_value = world * evals_per_step / e2e_s
-    h2d = T_host.numel() * 8 + q_host.numel() * 8
+    h2d = T_host.numel() * 8 + (3 * ax_host.size * 8 if path == "grid" else q_host.numel() * 8)
     d2h = out_host.numel() * 8
 
     if rank != 0:
@@ -349,42 +431,66 @@ def run_ours(args):
         return
 
     # ---- roofline of the dominant kernel (S4): algorithmic FP64 issue slots / its CUDA-event time
-    fold_ms = float(np.median([a for a, _ in kern_ms]))
-    kernel_ms = float(np.median([b for _, b in kern_ms]))
-    slots = st["slots_per_q"] * w.n_q
     peak_meas, peak_mhz = binding.fp64_peak(local)
     sms = torch.cuda.get_device_properties(local).multi_processor_count
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     peak_nominal = DFMA_PER_CLK_PER_SM * sms * sm_max * 1e6
-    achieved = slots / (kernel_ms * 1e-3)
-    roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_meas / 1e12, "unit": "T FP64-slot/s (1 slot = 1 DFMA lane-op = 2 flop)",
-                "frac": achieved / peak_meas, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.config),
-                "peak_source": f"measured register-only DFMA micro-benchmark (scarf_fp64_peak) at {peak_mhz:.0f} MHz; "
-                               f"nominal {DFMA_PER_CLK_PER_SM}/clk/SM x {sms} SMs x {sm_max:.0f} MHz = {peak_nominal / 1e12:.2f}",
-                "frac_of_nominal": achieved / peak_nominal, "kernel": "S4 form-factor kernel(s)", "kernel_ms": kernel_ms,
-                "fold_ms": fold_ms, "slots_per_launch_set": slots, "kernel_share_of_step": kernel_ms / ms_per_step,
-                "algorithmic_bytes": st["stream_bytes"] + 16.0 * w.n_states * w.n_q + 24.0 * w.n_q}
+    unit_slots = "T FP64-slot/s (1 slot = 1 DFMA lane-op = 2 flop)"
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+    def alu_roofline(slots, kernel_ms, kernel_name, poly_slots=None):
+        ach = slots / (kernel_ms * 1e-3)
+        traffic, tsrc = traffic_from_profiles(args.config, kernel_name)
+        r = {"bound": "alu", "achieved": ach / 1e12, "peak": peak_meas / 1e12, "unit": unit_slots, "frac": ach / peak_meas,
+             "traffic": traffic, "traffic_source": tsrc, "kernel": kernel_name, "kernel_ms": kernel_ms,
+             "slots_per_launch": slots, "frac_of_nominal": ach / peak_nominal}
+        if poly_slots is not None:       # the model without the per-(q, pair) transcendental / factor slots
+            r["frac_poly_only"] = poly_slots / (kernel_ms * 1e-3) / peak_meas
+        return r
+
+    kW = [2, 7, 13, 23, 38, 59, 87] + [0] * 6
+    poly_per_q = float(sum(n * w.n_states * kW[c] for c, n in enumerate(st["pairs_kept_per_class"])))
+    if path == "grid":
+        slots = st["last_grid_kernel_slots"]
+        roofline = alu_roofline(slots, head["main_kernel_ms"], "ff_grid_kernel<12>", poly_per_q * n_eval_q)
+        alg_bytes = st["stream_bytes"] + 16.0 * w.n_states * w.n_q + 32.0 * st["n_pairs_kept"] * (n_eval_q ** (1 / 3))
+    else:
+        slots = st["slots_per_q"] * w.n_q
+        roofline = alu_roofline(slots, head["main_kernel_ms"], "ff_v1_kernel<12>", poly_per_q * w.n_q)
+        alg_bytes = st["stream_bytes"] + 16.0 * w.n_states * w.n_q + 24.0 * w.n_q
+    roofline.update({"peak_source": f"measured register-only DFMA micro-benchmark (scarf_fp64_peak) at {peak_mhz:.0f} MHz; "
+                                    f"nominal {DFMA_PER_CLK_PER_SM}/clk/SM x {sms} SMs x {sm_max:.0f} MHz = {peak_nominal / 1e12:.2f}",
+                     "fold_ms": head["fold_ms"], "s4_call_ms": head["kernel_ms"],
+                     "kernel_share_of_step": head["main_kernel_ms"] / ms_per_step, "algorithmic_bytes": alg_bytes,
+                     "n_chunks": st["last_n_chunks"],
+                     "timing": "kernel_ms = median of the library's CUDA events around this kernel alone over the same K steps, "
+                               "repeated with option timing=1 right after the asynchronous timed region"})
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "config": args.config, "seed": w.seed, "n_q": w.n_q, "n_states": w.n_states,
                        "nbf": w.basis.nbf, "n_pairs_all": st["n_pairs_all"], "n_pairs_kept": st["n_pairs_kept"],
                        "pairs_kept_per_class": st["pairs_kept_per_class"], "cond_S": w.cond_S,
+                       "s4_api": "scarf_form_factors_grid" if path == "grid" else "scarf_form_factors",
+                       "inversion_symmetry_used": bool(path == "grid" and st["last_grid_symmetric"]),
+                       "q_points_evaluated": int(n_eval_q),
                        "l2": "flushed between timed steps (256 MB write, untimed)",
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
-            "job_seconds": ms_per_step * 1e-3, "wall_s_timed_region": t_wall,
+            "job_seconds": ms_per_step * 1e-3, "wall_s_timed_region": head["wall_s"],
+            "delivered_evals_per_s": world * st["evals_per_q"] * w.n_q / (ms_per_step * 1e-3),
+            "paper_unit": {"cartesian_term_pairs": st["cart_term_pairs"],
+                           "term_pair_q_state_per_s": world * float(st["cart_term_pairs"]) * w.n_q * w.n_states / (ms_per_step * 1e-3),
+                           "note": "ordered Cartesian-term pairs N_c^2 of Eq. (68) PAPER.md:505-508 x q-points x states delivered per second"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "job_seconds": e2e_s},
-            "gpu_launches": int(args.steps * (st["last_kernel_launches"] + st["last_fold_launches"])),
+            "gpu_launches": int(steps * (st["last_kernel_launches"] + st["last_fold_launches"])),
             "clocks": clocks, "roofline": roofline}
 
-    if grid_path is not None:
-        g_ach = grid_path["slots"] / (grid_path["kernel_ms"] * 1e-3)
-        grid_path["roofline"] = {"bound": "alu", "achieved": g_ach / 1e12, "peak": peak_meas / 1e12, "frac": g_ach / peak_meas,
-                                 "unit": roofline["unit"]}
-        line["grid_path"] = grid_path
-
+    for name, obj, kname, nq_exec in (("list_path", list_path, "ff_v1_kernel<12>", w.n_q), ("grid_path", grid_path, "ff_grid_kernel<12>", None),
+                                      ("grid_path_no_symmetry", grid_plain, "ff_grid_kernel<12>", w.n_q)):
+        if obj is not None:
+            obj["roofline"] = alu_roofline(obj["slots_main_kernel"], obj["main_kernel_ms"], kname)
+            line[name] = obj
     if angular is not None:
         line["angular_moments"] = angular
     if fft_path is not None:
@@ -396,11 +502,24 @@ def run_ours(args):
         f_gpu = torch.view_as_complex(out_dev)[:, torch.as_tensor(idx, device="cuda")].cpu().numpy()
         err = max(float(np.max(np.abs(f_gpu[s] - f_ref[s])) / np.max(np.abs(f_ref[s]))) for s in range(w.n_states))
         cpu_evals = float(len(idx)) * st["n_pairs_all"] * w.n_states
-        line["cpu_baseline"] = {"value": cpu_evals / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+        line["cpu_baseline"] = {"value": cpu_evals / dt, "unit": UNIT, "cores": threads, "cpu_model": cpu_model(), "kind": "oracle",
                                 "sample": f"{len(idx)} of {w.n_q} q-points (seeded sample), all {w.n_states} states, "
                                           f"every primitive pair ({st['n_pairs_all']}, unscreened)",
-                                "seconds": dt, "job_seconds_extrapolated": dt * w.n_q / len(idx)}
+                                "seconds": dt, "job_seconds_extrapolated": dt * w.n_q / len(idx),
+                                "unit_note": "the oracle loops over ordered basis-function x primitive pairs and screens nothing; its "
+                                             "evaluations are counted on ALL primitive shell pairs, the GPU's on the kept ones: compare "
+                                             "job_seconds_extrapolated with job_seconds, not the two evals/s"}
         line["parity"] = {"max_rel_err_vs_oracle_on_sample": err, "tolerance": 1e-10, "ok": bool(err <= 1e-10)}
+        # kappa_s = max_q sum_{mu nu} |g T_mu_nu I_mu_nu(q)| / max_q |f_s(q)| (SURVEY.md §8(c) "achievable tolerance"), from the
+        # oracle's pair integrals on a few sampled q: round-off of any summation order is ~ 1e-16 * kappa
+        kq = idx[:: max(1, len(idx) // 24)][:24]
+        num = np.zeros(w.n_states)
+        for i in kq:
+            I = oracle.pair_matrix(w.basis, w.q[i])
+            num = np.maximum(num, 2.0 * np.sum(np.abs(w.T * I[None]), axis=(1, 2)))
+        kap = num / np.max(np.abs(f_ref), axis=1)
+        line["kappa"] = {"max_over_states": float(np.max(kap)), "median": float(np.median(kap)), "q_points": int(len(kq)),
+                         "note": "max over sampled q of sum|term| over max over the oracle sample of |f_s|"}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -76,7 +76,8 @@ typedef struct scarf_stats {
     int32_t n_atoms, n_shells, n_prim_shells, nbf, n_states, l_max;
     int64_t n_pairs_all;                       /* all primitive shell pairs, A <= B                                 */
     int64_t n_pairs_prescreened;               /* after the T-independent host screen (K_AB underflow)              */
-    int64_t n_pairs_kept;                      /* after the T-dependent bound screen (set_transitions)              */
+    int64_t n_pairs_kept;                      /* after the T-dependent bound screen (set_transitions); the screening
+                                                * runs on the device and scarf_get_stats WAITS for its result        */
     int64_t pairs_kept_per_class[SCARF_N_CLASSES];
     int64_t n_herm_kept;                       /* sum over kept pairs of n_herm(L) = (L+1)(L+2)(L+3)/6              */
     int64_t cart_term_pairs;                   /* ordered Cartesian-term pairs, the paper's N_c^2 (Eq. 68)          */
@@ -89,6 +90,10 @@ typedef struct scarf_stats {
     int32_t last_fold_launches;                /* kernels launched by the last scarf_set_transitions               */
     double last_grid_slots;                    /* FP64 issue-slot model of the last scarf_form_factors_grid call    */
     double dropped_bound;                      /* sum of the bounds B_P of all dropped pairs: |f_s(q) - exact| <= this, any q, s */
+    int32_t last_grid_symmetric;               /* 1 if the last scarf_form_factors_grid call used f(-q) = conj f(q)  */
+    int32_t last_n_chunks;                     /* stream chunks (= cluster size) of the last S4 launch                */
+    double last_main_kernel_ms;                /* "timing": device time of the S4 kernel(s) alone (no tables/planning)*/
+    double last_grid_kernel_slots;             /* FP64 issue-slot model of the product-grid S4 kernel alone (no tables)*/
 } scarf_stats;
 
 /* device >= 0: CUDA ordinal.  device < 0: host-only context (set_basis, overlap, stats work; the rest ENODEVICE). */
@@ -110,10 +115,17 @@ int scarf_set_stream(scarf_ctx* ctx, void* cuda_stream);
  *                         whose error is bounded: scarf_stats.dropped_bound.  Takes effect at set_transitions.
  *           "timing": 1 records CUDA-event times of S3/S4 into the stats (adds a stream sync per call).
  *           "n_chunks": default 0 (automatic).  1..32 forces the number of cost-balanced slices the pair stream is cut
- *                         into (the S4 grid is q-tiles x chunks; results agree to FP64 round-off for any value: the
- *                         partial sums are added in chunk order).  A tuning/testing knob, not a numerical option.
+ *                         into (the S4 grid is q-tiles x chunks; the chunks of one q tile add their partial sums into
+ *                         `out` in chunk order, so results agree to FP64 round-off for any value).  A tuning/testing knob.
+ *           "grid_symmetry": default 1.  scarf_form_factors_grid evaluates only one half of a product grid whose three
+ *                         axes are antisymmetric bit for bit (ax[i] == -ax[n-1-i]) and stores conj f for the mirror
+ *                         points (f(-q) = conj f(q), exact for real T); 0 always evaluates every point.
  *           "fft_density_variant": default 1 = FP64 tensor-core (DMMA) density kernel of scarf_fft_form_factors,
  *                         0 = SIMT kernel (same result to round-off; slower).
+ *           "check_parseval": default 0.  1: scarf_fft_form_factors also evaluates both sides of Parseval's relation
+ *                         (Eq. 75, the paper's check_parseval flag); read them with scarf_fft_parseval.
+ *           "angular_variant": default 1 = fused FP64 tensor-core kernel of scarf_angular_moments, 0 = SIMT kernels
+ *                         (same result to round-off; slower).
  *           Unknown keys and out-of-range values: SCARF_EINVAL.                                                      */
 int scarf_set_option(scarf_ctx* ctx, const char* key, double value);
 
@@ -139,7 +151,11 @@ int scarf_nbf(const scarf_ctx* ctx); /* number of contracted Cartesian basis fun
 int scarf_overlap(scarf_ctx* ctx, double* S_host);
 
 /* T [n_states][nbf][nbf], row-major FP64, real, need not be symmetric.  Host or device pointer.
- * May be called repeatedly on one basis. */
+ * May be called repeatedly on one basis.  Everything runs on the context stream without a device->host round trip:
+ * fold, screening (threshold, stable compaction), packing and the stream descriptor stay on the device; the kept-pair
+ * counts reach the host only through scarf_get_stats.  Host T is checked for NaN/Inf here (SCARF_EINVAL); device T is
+ * checked on the device: a non-finite T keeps every pair (the NaN reaches the output) and SCARF_EINVAL is returned by
+ * scarf_get_stats and by the next S4 call that finds the screening result already on the host. */
 int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T);
 
 /* q [n_q][3] FP64; out [n_states][n_q][2] FP64 (re, im interleaved).  Host or device pointers, independently.
@@ -152,7 +168,10 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
  * tabulated once per call (nx+ny+nz complex numbers per pair, device memory owned by the context) and the kernel
  * spends 2 complex multiplies per (q, pair) instead of an exp and a sincos.  Axes need not be uniform or sorted.
  * qx, qy, qz and out: host or device pointers, independently.  Results equal scarf_form_factors on the expanded
- * point list up to FP64 round-off.  SCARF_ENOMEM if the tables would exceed 32 GB. */
+ * point list up to FP64 round-off.  SCARF_ENOMEM if the tables would exceed 32 GB.
+ * Inversion symmetry (option "grid_symmetry", default on): the axes are inspected on the host; HOST axes cost nothing,
+ * DEVICE axes are read back first (a few hundred bytes and one stream synchronisation per call) — pass the axes from
+ * host memory when the call must stay asynchronous.  scarf_stats.last_grid_symmetric says which path ran. */
 int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_t ny, const double* qy, int32_t nz,
                             const double* qz, double* out);
 
@@ -174,10 +193,19 @@ int scarf_separable_integral(scarf_ctx* ctx, int32_t nx, const double* qx, const
  *   R_out  [n_states][n_r][(l_max+1)^2][2], index l(l+1)+m.  Host or device.
  *   f2_out [n_states][n_r] or NULL.  Host or device.
  *   cos_theta, w_theta: HOST.  Needs n_phi >= 2 l_max + 1 (no phi aliasing), n_phi <= 2048, l_max <= 64; exact for
- *   band limit l + l' <= 2 n_theta - 1 with Gauss-Legendre nodes.  Independent of the basis and transitions set. */
+ *   band limit l + l' <= 2 n_theta - 1 with Gauss-Legendre nodes.  Independent of the basis and transitions set.
+ *   The quadrature tables are cached in the context (rebuilt only when nodes, weights, n_phi or l_max change); with
+ *   device pointers for f, R_out and f2_out the call is asynchronous on the context stream. */
 int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t n_theta, const double* cos_theta,
                           const double* w_theta, int32_t n_phi, int32_t l_max, const double* f, double* R_out,
                           double* f2_out);
+
+/* Oscillator-strength fit, Eq. (81)-(82) PAPER.md:591-596: least squares of  <|f_s|^2>_Omega(q) ~ A + B q^2 + C q^4  over the
+ * radial points with |q_abs[i]| <= q_max (q_max <= 0: all of them; at least three distinct |q| are needed).  f2 is the
+ * [n_states][n_r] array scarf_angular_moments returns, q_abs [n_r] the radii; coef_out [n_states][3] = (A, B, C).
+ * B = |g mu|^2 / 3 with mu the transition dipole of Eq. (77) and g the prefactor the form factors were computed with
+ * (f_s -> i g q.mu, Eq. 76); A absorbs a non-zero f(0), C the finite-q curvature.  HOST pointers; no device work. */
+int scarf_oscillator_fit(int32_t n_states, int32_t n_r, const double* q_abs, const double* f2, double q_max, double* coef_out);
 
 /* The paper's FFT method (Section III, Eq. (19)-(34) PAPER.md:140-222) as a second, APPROXIMATE
  * route to f_s: the transition density Phi_s(x) = g sum_pq T_pq phi_q(x) phi_p(x) (Eq. 20) is tabulated at
@@ -188,6 +216,14 @@ int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t
  * host or device.  Scratch: nbf*nx*ny*nz doubles + 2 complex arrays of the output size (SCARF_ENOMEM above 64 GB). */
 int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, const double* x_min, const double* box_len,
                            double* out);
+
+/* Parseval check of the FFT method, Eq. (75):  Int d^3r |Phi_s(r)|^2 = Int d^3q/(2 pi)^3 |f_s(q)|^2, on the grids
+ * of the last scarf_fft_form_factors call made with option "check_parseval" = 1:
+ *     out[s][0] = V_pix sum_abc |Phi_abc|^2,      out[s][1] = (1 / (Lx Ly Lz)) sum_q |f_s(q)|^2      (d^3q/(2 pi)^3 = 1/V_box per point).
+ * The two agree to round-off for ANY box (discrete Parseval), so a mismatch flags a broken transform/normalisation, while
+ * comparing out[s][0] across boxes/spacings shows truncation and aliasing ("grids with insufficient extent or resolution").
+ * out: HOST [n_states][2].  Synchronises the context stream.  SCARF_ESTATE if no checked call was made. */
+int scarf_fft_parseval(scarf_ctx* ctx, double* out_host);
 
 int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out);
 const char* scarf_last_error(const scarf_ctx* ctx);

@@ -19,7 +19,7 @@ SCARF_N_CLASSES = 2 * SCARF_MAX_L + 1
 _CODES = {-1: "EINVAL", -2: "ESTATE", -3: "ENOMEM", -4: "ECUDA", -5: "ENODEVICE"}
 
 EXPORTS = ["scarf_create", "scarf_destroy", "scarf_set_stream", "scarf_set_option", "scarf_set_basis", "scarf_set_basis_pure", "scarf_nbf",
-           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_separable_integral", "scarf_angular_moments", "scarf_fft_form_factors", "scarf_get_stats", "scarf_last_error",
+           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_separable_integral", "scarf_angular_moments", "scarf_oscillator_fit", "scarf_fft_form_factors", "scarf_fft_parseval", "scarf_get_stats", "scarf_last_error",
            "scarf_version", "scarf_fp64_peak", "scarf_host_hermite_E", "scarf_host_shell_norms", "scarf_host_ylm_table"]
 
 
@@ -32,7 +32,9 @@ class ScarfStats(C.Structure):
                 ("stream_bytes", C.c_double), ("slots_per_q", C.c_double), ("evals_per_q", C.c_double),
                 ("last_setup_host_ms", C.c_double), ("last_fold_ms", C.c_double), ("last_kernel_ms", C.c_double),
                 ("last_kernel_launches", C.c_int32), ("last_fold_launches", C.c_int32),
-                ("last_grid_slots", C.c_double), ("dropped_bound", C.c_double)]
+                ("last_grid_slots", C.c_double), ("dropped_bound", C.c_double),
+                ("last_grid_symmetric", C.c_int32), ("last_n_chunks", C.c_int32),
+                ("last_main_kernel_ms", C.c_double), ("last_grid_kernel_slots", C.c_double)]
 
     def as_dict(self):
         d = {}
@@ -68,8 +70,10 @@ def _load():
     L.scarf_form_factors_grid.argtypes = [vp, C.c_int32, vp, C.c_int32, vp, C.c_int32, vp, vp]
     L.scarf_separable_integral.argtypes = [vp, C.c_int32, dp, dp, C.c_int32, dp, dp, C.c_int32, dp, dp, dp]
     L.scarf_angular_moments.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, C.c_int32, C.c_int32, vp, vp, vp]
+    L.scarf_oscillator_fit.argtypes = [C.c_int32, C.c_int32, dp, dp, C.c_double, dp]
     L.scarf_host_ylm_table.argtypes = [C.c_int, C.c_int, dp, dp, dp]
     L.scarf_fft_form_factors.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, vp]
+    L.scarf_fft_parseval.argtypes = [vp, dp]
     L.scarf_get_stats.argtypes = [vp, C.POINTER(ScarfStats)]
     L.scarf_last_error.argtypes = [vp]
     L.scarf_last_error.restype = C.c_char_p
@@ -334,6 +338,12 @@ class Scarf:
             return torch.view_as_complex(out.view(self.n_states, n_q, 2))
         return out.reshape(self.n_states, n_q, 2).view(np.complex128)[..., 0]
 
+    def fft_parseval(self) -> np.ndarray:
+        """[n_states][2]: (V_pix sum |Phi|^2, sum |f|^2 / V_box) of the last fft_form_factors call (option check_parseval = 1)."""
+        out = np.zeros((self.n_states, 2))
+        self._check(_lib.scarf_fft_parseval(self._h, _dp(out)))
+        return out
+
     def separable_integral(self, qx, fx, qy, gy, qz, hz) -> np.ndarray:
         """sum_{ix,iy,iz} fx[ix] gy[iy] hz[iz] f_s(qx[ix], qy[iy], qz[iz]) for every state (complex128 [n_states]),
         in O(pairs * (nx+ny+nz)): Eq. (64)-(65).  All arguments 1-D host arrays (weights x function samples)."""
@@ -349,6 +359,17 @@ class Scarf:
         s = ScarfStats()
         self._check(_lib.scarf_get_stats(self._h, C.byref(s)))
         return s.as_dict()
+
+
+def oscillator_fit(q_abs, f2, q_max: float = 0.0) -> np.ndarray:
+    """[n_states][3] = (A, B, C) of <|f_s|^2>_Omega(q) ~ A + B q^2 + C q^4 (Eq. 81-82); f2 [n_states][n_r] host array."""
+    q = np.ascontiguousarray(q_abs, dtype=np.float64)
+    y = np.ascontiguousarray(f2, dtype=np.float64).reshape(-1, q.shape[0])
+    out = np.zeros((y.shape[0], 3))
+    rc = _lib.scarf_oscillator_fit(int(y.shape[0]), int(q.shape[0]), _dp(q), _dp(y), float(q_max), _dp(out))
+    if rc != SCARF_OK:
+        raise ScarfError(rc, "scarf_oscillator_fit failed (fewer than three usable |q|, or NaN/Inf)")
+    return out
 
 
 def host_ylm_table(l_max: int, cos_theta, w_theta) -> np.ndarray:

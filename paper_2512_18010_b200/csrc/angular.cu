@@ -10,9 +10,15 @@
 //                              and rowsum2(row) = (2 pi/n_phi) sum_k |f(row, k)|^2          (row = state, r, theta)
 //   step 2 (legendre_kernel):  R_lm(state, r) = sum_j w_j Ybar_lm(theta_j) F_m(state, r, j),
 //                              <f^2>(state, r) = 1/(4 pi) sum_j w_j rowsum2(state, r, j).
-// Step 1 reads f once (the only large array: 201 MB on config 5) and is a small dense contraction
-// [2 l_max + 1] x [n_phi] per row, done in FP64 FMAs from shared memory; step 2 is tiny.  Ybar (host, fully
-// normalised three-term recurrence) and the twiddles are tabulated once per call.
+// Step 1 is a dense contraction and runs on the FP64 tensor cores (angular_fused_kernel, mma.sync.m8n8k4.f64): with
+//   C_m = sum_k f_k cos(m phi_k),  S_m = sum_k f_k sin(m phi_k)   (m = 0..l_max; real tables, complex f)
+// F_{+m} = C_m - i S_m and F_{-m} = C_m + i S_m, so the real GEMM [rows x n_phi] . [n_phi x 2(l_max+1)] is done once for
+// the real parts and once for the imaginary parts of the SAME loaded f (half the flops of the 2 l_max + 1 complex DFT
+// columns).  One CTA owns one (state, r): its n_theta rows of F stay in shared memory and step 2 (the Legendre
+// contraction) and the |f|^2 sums finish in the same kernel, so f is read once (201 MB on config 5) and nothing but
+// R and <f^2> is written.  Tables (Ybar: host, fully normalised three-term recurrence; cos/sin in B-fragment order) are
+// cached in the context.  phi_dft_kernel + legendre_kernel (SIMT) remain as the route for shapes whose F does not fit
+// in shared memory.
 #include <cmath>
 #include <vector>
 
@@ -116,6 +122,166 @@ __global__ void __launch_bounds__(kThreads) legendre_kernel(const double2* __res
     }
 }
 
+// ---- fused tensor-core kernel -------------------------------------------------------------------------------------------
+// DMMA m8n8k4 fragments: A[row = gid][k = tig] (one double per lane), B[k = tig][col = gid], D[row = gid][col = 2 tig + i].
+// Rows = theta nodes of this (state, r); k = phi index; columns 2m (cos) and 2m+1 (sin), m = 4 nt + tig for n-tile nt.
+constexpr int kFusedWarps = 4;
+constexpr int kFusedMT = 2;            // 8-row tiles per warp and sweep (they share every B fragment)
+constexpr int kFusedKG = 4;            // k-steps per software-pipeline group (loads of the next group overlap this group's DMMAs)
+constexpr int kFusedNT = 7;            // n-tiles per pass: m = 0..27 in one pass (l_max <= 27); more passes beyond
+
+__device__ __forceinline__ void dmma884(double (&d)[2], double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
+}
+
+// Bf: [n_nt][n_ks][32] doubles (fragment order), scale 2 pi / n_phi folded in.  F_glob != nullptr: write F and rowsum2 to
+// global memory and stop (unfused route for large shapes); else finish R and f2 here.
+__global__ void __launch_bounds__(kFusedWarps * 32) angular_fused_kernel(const double2* __restrict__ f, const double* __restrict__ Bf,
+                                                                        const double* __restrict__ YwT, const double* __restrict__ w_theta,
+                                                                        int n_theta, int n_phi, int l_max, int n_nt, int n_ks,
+                                                                        double2* __restrict__ R, double* __restrict__ f2,
+                                                                        double2* __restrict__ F_glob, double* __restrict__ row2_glob)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const long long sr = blockIdx.x;
+    const int n_m = 2 * l_max + 1;
+    double* s_B = reinterpret_cast<double*>(smem_raw);                               // n_nt * n_ks * 32
+    double2* s_F = reinterpret_cast<double2*>(s_B + (size_t)n_nt * n_ks * 32);       // n_theta * n_m      (fused route only)
+    double* s_row2 = reinterpret_cast<double*>(s_F + (F_glob ? 0 : (size_t)n_theta * n_m));   // n_theta
+    {   // cos/sin fragments -> shared memory: 16-byte loads, 8 in flight per thread (the table is a multiple of 32 doubles)
+        const double2* src = reinterpret_cast<const double2*>(Bf);
+        double2* dstB = reinterpret_cast<double2*>(s_B);
+        const int n2 = n_nt * n_ks * 16;
+#pragma unroll 8
+        for (int i = threadIdx.x; i < n2; i += kFusedWarps * 32) dstB[i] = __ldg(src + i);
+    }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gid = lane >> 2, tig = lane & 3;
+    const double2* fr = f + (size_t)sr * n_theta * n_phi;
+    const double scale = 6.283185307179586476925286766559 / (double)n_phi;
+    for (int row0 = warp * 8 * kFusedMT; row0 < n_theta; row0 += kFusedWarps * 8 * kFusedMT) {
+        int row[kFusedMT];
+        bool ok[kFusedMT];
+#pragma unroll
+        for (int t = 0; t < kFusedMT; ++t) { row[t] = row0 + 8 * t + gid; ok[t] = row[t] < n_theta; }
+        double sq[kFusedMT];
+#pragma unroll
+        for (int t = 0; t < kFusedMT; ++t) sq[t] = 0.0;
+        for (int nt0 = 0; nt0 < n_nt; nt0 += kFusedNT) {
+            double aR[kFusedMT][kFusedNT][2], aI[kFusedMT][kFusedNT][2];
+#pragma unroll
+            for (int t = 0; t < kFusedMT; ++t)
+#pragma unroll
+                for (int n = 0; n < kFusedNT; ++n) aR[t][n][0] = aR[t][n][1] = aI[t][n][0] = aI[t][n][1] = 0.0;
+            // k loop in groups of kFusedKG steps, software-pipelined: the global loads of group g + 1 are in flight while the
+            // 4 kFusedNT kFusedKG DMMAs of group g run (f comes straight from HBM: ~1 us of latency to cover per load)
+            auto load_group = [&](int ks0, double2 (&a)[kFusedKG][kFusedMT]) {
+#pragma unroll
+                for (int u = 0; u < kFusedKG; ++u) {
+                    const int k = 4 * (ks0 + u) + tig;
+#pragma unroll
+                    for (int t = 0; t < kFusedMT; ++t)
+                        a[u][t] = (ok[t] && k < n_phi) ? __ldg(fr + (size_t)row[t] * n_phi + k) : make_double2(0.0, 0.0);
+                }
+            };
+            double2 cur[kFusedKG][kFusedMT], nxt[kFusedKG][kFusedMT];
+            load_group(0, cur);
+#pragma unroll 1
+            for (int ks0 = 0; ks0 < n_ks; ks0 += kFusedKG) {
+                if (ks0 + kFusedKG < n_ks) load_group(ks0 + kFusedKG, nxt);
+#pragma unroll
+                for (int u = 0; u < kFusedKG; ++u) {
+                    const int ks = ks0 + u;
+                    if (ks < n_ks) {
+#pragma unroll
+                        for (int t = 0; t < kFusedMT; ++t)
+                            if (nt0 == 0) sq[t] = fma(cur[u][t].x, cur[u][t].x, fma(cur[u][t].y, cur[u][t].y, sq[t]));
+#pragma unroll
+                        for (int n = 0; n < kFusedNT; ++n)
+                            if (nt0 + n < n_nt) {
+                                const double b = s_B[((size_t)(nt0 + n) * n_ks + ks) * 32 + lane];
+#pragma unroll
+                                for (int t = 0; t < kFusedMT; ++t) {
+                                    dmma884(aR[t][n], cur[u][t].x, b);
+                                    dmma884(aI[t][n], cur[u][t].y, b);
+                                }
+                            }
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < kFusedKG; ++u)
+#pragma unroll
+                    for (int t = 0; t < kFusedMT; ++t) cur[u][t] = nxt[u][t];
+            }
+            // lane (gid, tig) holds, for row gid and m = 4 (nt0 + n) + tig:  C_re, S_re (aR), C_im, S_im (aI)
+#pragma unroll
+            for (int t = 0; t < kFusedMT; ++t)
+#pragma unroll
+                for (int n = 0; n < kFusedNT; ++n) {
+                    const int m = 4 * (nt0 + n) + tig;
+                    if (ok[t] && nt0 + n < n_nt && m <= l_max) {
+                        const double2 Fp = make_double2(aR[t][n][0] + aI[t][n][1], aI[t][n][0] - aR[t][n][1]);   // C - i S
+                        const double2 Fn = make_double2(aR[t][n][0] - aI[t][n][1], aI[t][n][0] + aR[t][n][1]);   // C + i S
+                        double2* dstF = F_glob ? F_glob + ((size_t)sr * n_theta + row[t]) * n_m : s_F + (size_t)row[t] * n_m;
+                        dstF[l_max + m] = Fp;
+                        dstF[l_max - m] = Fn;
+                    }
+                }
+        }
+#pragma unroll
+        for (int t = 0; t < kFusedMT; ++t) {
+            double x = sq[t];
+            x += __shfl_xor_sync(0xffffffffu, x, 1);
+            x += __shfl_xor_sync(0xffffffffu, x, 2);
+            if (tig == 0 && ok[t]) {
+                if (F_glob) row2_glob[(size_t)sr * n_theta + row[t]] = x * scale;
+                else s_row2[row[t]] = x * scale;
+            }
+        }
+    }
+    if (F_glob) return;
+    __syncthreads();
+    // step 2: R[l(l+1) +- m] = (-1)^{m for -m} sum_j Yw[j][l(l+1)/2 + m] F[j][+-m + l_max].  One work item = (l, m >= 0): the
+    // weight serves +m and -m; YwT is the transposed table [l(l+1)/2 + m][n_theta_pad], so a thread streams its row with
+    // 16-byte loads, 8 in flight (the j loop was one dependent 8-byte L2 load per FMA pair before: 20 us per CTA).
+    const int nlm = (l_max + 1) * (l_max + 1), nhalf = (l_max + 1) * (l_max + 2) / 2, ntp = (n_theta + 1) & ~1;
+    for (int o = threadIdx.x; o < nhalf; o += blockDim.x) {
+        int l = (int)((sqrt(8.0 * o + 1.0) - 1.0) * 0.5);
+        while (l * (l + 1) / 2 > o) --l;
+        while ((l + 1) * (l + 2) / 2 <= o) ++l;
+        const int m = o - l * (l + 1) / 2;
+        const double2* yrow = reinterpret_cast<const double2*>(YwT + (size_t)o * ntp);
+        double pr = 0.0, pi = 0.0, nr = 0.0, ni = 0.0;
+        constexpr int kYB = 16;                             // 16-byte loads issued back to back before their values are used
+        for (int jb = 0; jb < ntp / 2; jb += kYB) {
+            double2 y[kYB];
+#pragma unroll
+            for (int u = 0; u < kYB; ++u) y[u] = jb + u < ntp / 2 ? __ldg(yrow + jb + u) : make_double2(0.0, 0.0);
+#pragma unroll
+            for (int u = 0; u < kYB; ++u) {
+                const int j = 2 * (jb + u);
+                if (j < n_theta) {
+                    const double2 p0 = s_F[(size_t)j * n_m + (l_max + m)], q0 = s_F[(size_t)j * n_m + (l_max - m)];
+                    pr = fma(y[u].x, p0.x, pr); pi = fma(y[u].x, p0.y, pi); nr = fma(y[u].x, q0.x, nr); ni = fma(y[u].x, q0.y, ni);
+                }
+                if (j + 1 < n_theta) {
+                    const double2 p1 = s_F[(size_t)(j + 1) * n_m + (l_max + m)], q1 = s_F[(size_t)(j + 1) * n_m + (l_max - m)];
+                    pr = fma(y[u].y, p1.x, pr); pi = fma(y[u].y, p1.y, pi); nr = fma(y[u].y, q1.x, nr); ni = fma(y[u].y, q1.y, ni);
+                }
+            }
+        }
+        const double sgn = (m & 1) ? -1.0 : 1.0;
+        R[(size_t)sr * nlm + l * (l + 1) + m] = make_double2(pr, pi);
+        if (m > 0) R[(size_t)sr * nlm + l * (l + 1) - m] = make_double2(sgn * nr, sgn * ni);
+    }
+    if (f2 != nullptr && threadIdx.x == 0) {
+        double acc = 0.0;
+        for (int j = 0; j < n_theta; ++j) acc = fma(w_theta[j], s_row2[j], acc);
+        f2[sr] = acc / 12.566370614359172953850573533118;
+    }
+}
+
 }  // namespace
 
 // Yw[j][l(l+1)/2 + m] = w_j * N_lm P_l^m(x_j), 0 <= m <= l <= l_max: fully normalised recurrence (orthonormal Y_l^m,
@@ -153,7 +319,9 @@ void angular_host_tables(int l_max, int n_theta, const double* cos_theta, const 
 
 cudaError_t angular_init_device()
 {
-    return cudaFuncSetAttribute(phi_dft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(phi_dft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(angular_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kAngularMaxSmem);
+    return e;
 }
 
 int angular_rows_per_cta(int n_phi) { return std::max(1, std::min(8, 2048 / std::max(1, n_phi))); }
@@ -176,6 +344,53 @@ cudaError_t launch_legendre(const double* F, const double* rowsum2, const double
     if (n_sr <= 0) return cudaSuccess;
     legendre_kernel<<<(unsigned)n_sr, kThreads, 0, st>>>(reinterpret_cast<const double2*>(F), rowsum2, Yw, w_theta, n_theta, l_max,
                                                         reinterpret_cast<double2*>(R), f2);
+    return cudaGetLastError();
+}
+
+// B-fragment table of the fused kernel: Bf[nt][ks][lane], lane = (gid, tig) <-> B[k = 4 ks + tig][col = 8 nt + gid],
+// col = 2 m + {0: cos, 1: sin}(m phi_k) * 2 pi / n_phi, phi_k = 2 pi k / n_phi; zero beyond n_phi or l_max.  The angle is
+// reduced exactly on integers (m k mod n_phi) before the call to cos/sin.  HOST.
+void angular_fragment_table(int l_max, int n_phi, std::vector<double>& Bf, int& n_nt, int& n_ks)
+{
+    n_nt = (2 * (l_max + 1) + 7) / 8;
+    n_ks = (n_phi + 3) / 4;
+    Bf.assign((size_t)n_nt * n_ks * 32, 0.0);
+    const double pi = 3.14159265358979323846264338327950288;
+    const double scale = 2.0 * pi / (double)n_phi;
+    for (int nt = 0; nt < n_nt; ++nt)
+        for (int ks = 0; ks < n_ks; ++ks)
+            for (int lane = 0; lane < 32; ++lane) {
+                const int gid = lane >> 2, tig = lane & 3, k = 4 * ks + tig, col = 8 * nt + gid, m = col / 2;
+                if (k >= n_phi || m > l_max) continue;
+                const long long idx = ((long long)m * k) % n_phi;
+                const double a = 2.0 * pi * (double)idx / (double)n_phi;
+                Bf[((size_t)nt * n_ks + ks) * 32 + lane] = scale * ((col & 1) ? std::sin(a) : std::cos(a));
+            }
+}
+
+// YwT[l(l+1)/2 + m][n_theta_pad]: the transpose of Yw, rows padded with zeros to an even length (16-byte row loads).  HOST.
+void angular_transpose_table(int l_max, int n_theta, const std::vector<double>& Yw, std::vector<double>& YwT)
+{
+    const int nhalf = (l_max + 1) * (l_max + 2) / 2, ntp = (n_theta + 1) & ~1;
+    YwT.assign((size_t)nhalf * ntp, 0.0);
+    for (int j = 0; j < n_theta; ++j)
+        for (int p = 0; p < nhalf; ++p) YwT[(size_t)p * ntp + j] = Yw[(size_t)j * nhalf + p];
+}
+
+size_t angular_fused_smem(int n_theta, int l_max, int n_nt, int n_ks, bool fused)
+{
+    return (size_t)n_nt * n_ks * 32 * 8 + (fused ? (size_t)n_theta * (2 * l_max + 1) * 16 : 0) + (size_t)n_theta * 8;
+}
+
+cudaError_t launch_angular_fused(const double* f, const double* Bf, const double* YwT, const double* w_theta, long long n_sr, int n_theta,
+                                 int n_phi, int l_max, int n_nt, int n_ks, double* R, double* f2, double* F_glob, double* row2_glob,
+                                 cudaStream_t st)
+{
+    if (n_sr <= 0) return cudaSuccess;
+    const size_t smem = angular_fused_smem(n_theta, l_max, n_nt, n_ks, F_glob == nullptr);
+    angular_fused_kernel<<<(unsigned)n_sr, kFusedWarps * 32, smem, st>>>(reinterpret_cast<const double2*>(f), Bf, YwT, w_theta, n_theta, n_phi,
+                                                                        l_max, n_nt, n_ks, reinterpret_cast<double2*>(R), f2,
+                                                                        reinterpret_cast<double2*>(F_glob), row2_glob);
     return cudaGetLastError();
 }
 

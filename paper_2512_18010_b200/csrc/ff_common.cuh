@@ -81,6 +81,25 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u
                  : "memory");
 }
 
+// ---- ordered fix-up tickets: the chunks of one q tile add into `out` in chunk order --------------------------------------
+// ticket[tile] holds the chunk whose turn it is (0 at launch; the last chunk puts 0 back).  Whole-CTA calls.
+__device__ __forceinline__ void ticket_wait(int* ticket, int turn)
+{
+    if (threadIdx.x == 0) {
+        int v;
+        do {
+            asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(ticket) : "memory");
+        } while (v != turn);
+    }
+    __syncthreads();
+}
+__device__ __forceinline__ void ticket_pass(int* ticket, int next)
+{
+    __threadfence();                                      // this thread's stores to `out` are visible device-wide ...
+    __syncthreads();                                      // ... for every thread of the CTA, before the ticket moves on
+    if (threadIdx.x == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(ticket), "r"(next) : "memory");
+}
+
 // ---- one record = transcendental part (record_trans) + the (state, h) loop (record_accum) -------------------
 // The two are separate so that run_class can software-pipeline them: the exp/sincos chains of record k+1 (low
 // ILP: two dependent Horner chains per q-point) are issued in the same basic block as the 4 NS n_herm independent

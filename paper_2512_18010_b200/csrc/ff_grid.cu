@@ -11,7 +11,14 @@
 // (2 q-points, pair) for the factor — YZ = Y Z, g0 = X0 YZ, g1 = X1 YZ — instead of 2 x 40, and shares the
 // (state, Hermite index) accumulate loop with the general kernel (ff_common.cuh).
 //
-// Work decomposition: a CTA owns a 4 x 8 x 8 box of the grid and one cost-balanced chunk of the pair stream.
+// Inversion symmetry.  f_s(-q) = conj f_s(q) for real T and real orbitals (Fourier sign e^{+iq.r}, Eq. (19)).
+// When every axis is antisymmetric bit for bit (ax[i] == -ax[n-1-i]; the host checks) the grid maps onto itself under
+// q -> -q: only the half ix < ceil(nx/2) is evaluated and the mirror point (nx-1-ix, ny-1-iy, nz-1-iz) receives the
+// conjugate in the same epilogue — half the work, no approximation (tables, monomials and sums are exactly odd/even, so the
+// stored value is what a direct evaluation at -q would give).
+//
+// Work decomposition: a CTA owns a 4 x 8 x 8 box of the grid and one cost-balanced chunk of the pair stream; the chunks of
+// one box add into `out` in chunk order through the box's ticket (as in ff_v1.cu); the last chunk also stores the mirror.
 // Thread t holds the points (ixl, iyl, izl) and (ixl + 2, iyl, izl), izl = t % 8, iyl = (t / 8) % 8, ixl = t / 64,
 // so a warp has one ixl (X0, X1 are broadcast loads) and writes 128-byte runs along z.  Tables are laid out
 // [box][record][point-in-box], so that the slice a CTA needs for a run of records is contiguous: per stage one
@@ -38,22 +45,24 @@ struct GPipe {
 };
 
 // ---- tables -------------------------------------------------------------------------------------------------
-// one thread per (record, padded axis point); columns [0, NXp) -> X, [NXp, NXp+NYp) -> Y, rest -> Z.
+// one thread per (record, padded axis point); columns [0, NXp) -> X, [NXp, NXp+NYp) -> Y, rest -> Z.  The launch is sized for
+// a.n_rows records (all prescreened pairs); rows beyond the kept count exit.
 __global__ void __launch_bounds__(256) grid_table_kernel(const GridArgs a, double2* __restrict__ tx, double2* __restrict__ ty,
                                                          double2* __restrict__ tz)
 {
+    const StreamDesc& d = *a.v.desc;
     const int NXp = a.nbx * kGridBX, NYp = a.nby * kGridBY, NZp = a.nbz * kGridBZ, ncol = NXp + NYp + NZp;
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= a.n_rec * ncol) return;
+    if (idx >= d.n_kept * ncol) return;
     const long long r = idx / ncol;
     int col = (int)(idx - r * ncol);
     int c = 0;
 #pragma unroll
     for (int k = 1; k < kNClasses; ++k)
-        if (r >= a.class_first[k]) c = k;
-    const double* hdr = reinterpret_cast<const double*>(a.v.base + a.v.cls_off[c] + (size_t)(r - a.class_first[c]) * a.rec_bytes[c]);
+        if (r >= d.cls_first[k]) c = k;
+    const double* hdr = reinterpret_cast<const double*>(a.v.base + d.cls_off[c] + (size_t)(r - d.cls_first[c]) * d.rec_bytes[c]);
     const double inv4p = hdr[3];
-    int axis = 0, n = a.nx, B = kGridBX;
+    int axis = 0, n = a.nx_eval, B = kGridBX;
     const double* ax = a.qx;
     double2* tab = tx;
     if (col >= NXp + NYp) { axis = 2; col -= NXp + NYp; n = a.nz; B = kGridBZ; ax = a.qz; tab = tz; }
@@ -66,7 +75,7 @@ __global__ void __launch_bounds__(256) grid_table_kernel(const GridArgs a, doubl
         sincos_fast(q * hdr[axis], sn, cs);
         v = make_double2(e * cs, e * sn);
     }
-    tab[((size_t)(col / B) * a.n_rec + r) * B + (col % B)] = v;
+    tab[((size_t)(col / B) * a.n_rows + r) * B + (col % B)] = v;
 }
 
 __device__ __forceinline__ double2 cmul(const double2 a, const double2 b)
@@ -94,9 +103,9 @@ __device__ __forceinline__ void run_class_grid(GPipe& pp, const GridArgs& a, con
         const long long r = r0 + first;
         mbar_expect_tx(&pp.full[slot], (uint32_t)cnt * (REC + kXB + kYB + kZB));
         bulk_g2s(sb, seg + (size_t)first * REC, (uint32_t)cnt * REC, &pp.full[slot]);
-        bulk_g2s(sb + kStageBytes, a.tx + ((size_t)bx * a.n_rec + r) * kGridBX, (uint32_t)cnt * kXB, &pp.full[slot]);
-        bulk_g2s(sb + kStageBytes + kMaxRec * kXB, a.ty + ((size_t)by * a.n_rec + r) * kGridBY, (uint32_t)cnt * kYB, &pp.full[slot]);
-        bulk_g2s(sb + kStageBytes + kMaxRec * (kXB + kYB), a.tz + ((size_t)bz * a.n_rec + r) * kGridBZ, (uint32_t)cnt * kZB,
+        bulk_g2s(sb + kStageBytes, a.tx + ((size_t)bx * a.n_rows + r) * kGridBX, (uint32_t)cnt * kXB, &pp.full[slot]);
+        bulk_g2s(sb + kStageBytes + kMaxRec * kXB, a.ty + ((size_t)by * a.n_rows + r) * kGridBY, (uint32_t)cnt * kYB, &pp.full[slot]);
+        bulk_g2s(sb + kStageBytes + kMaxRec * (kXB + kYB), a.tz + ((size_t)bz * a.n_rows + r) * kGridBZ, (uint32_t)cnt * kZB,
                  &pp.full[slot]);
     };
     __syncthreads();                                     // all threads have left the previous segment's stages
@@ -160,7 +169,7 @@ __global__ void __launch_bounds__(kThreads, 2) ff_grid_kernel(const GridArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + kStages * kSlotBytes);
-    const int tile = (int)(blockIdx.x % (unsigned)a.v.n_tiles), chunk = (int)(blockIdx.x / (unsigned)a.v.n_tiles);
+    const int tile = (int)blockIdx.x, chunk = (int)blockIdx.y;
     if (threadIdx.x == 0) {
         for (int s = 0; s < kStages; ++s) mbar_init(&full_bar[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -172,12 +181,10 @@ __global__ void __launch_bounds__(kThreads, 2) ff_grid_kernel(const GridArgs a)
     const int izl = threadIdx.x % kGridBZ, iyl = (threadIdx.x / kGridBZ) % kGridBY, ixl = threadIdx.x / (kGridBZ * kGridBY);
     const int iy = by * kGridBY + iyl, iz = bz * kGridBZ + izl;
     double qv[kNQ][4];
-    long long iq[kNQ];
 #pragma unroll
     for (int j = 0; j < kNQ; ++j) {
         const int ix = bx * kGridBX + ixl + 2 * j;
-        const bool ok = ix < a.nx && iy < a.ny && iz < a.nz;
-        iq[j] = ok ? ((long long)ix * a.ny + iy) * a.nz + iz : -1;
+        const bool ok = ix < a.nx_eval && iy < a.ny && iz < a.nz;
         qv[j][0] = ok ? a.qx[ix] : 0.0;
         qv[j][1] = ok ? a.qy[iy] : 0.0;
         qv[j][2] = ok ? a.qz[iz] : 0.0;
@@ -189,11 +196,12 @@ __global__ void __launch_bounds__(kThreads, 2) ff_grid_kernel(const GridArgs a)
 #pragma unroll
         for (int s = 0; s < NS; ++s) re[j][s] = im[j][s] = 0.0;
 
-    const V1Chunk& ck = a.v.chunks[chunk];
+    const StreamDesc& d = *a.v.desc;
+    const V1Chunk& ck = d.chunks[chunk];
 #define SCARF_GRID_CLASS(LV)                                                                                          \
     if (ck.n[LV] > 0)                                                                                                 \
-        run_class_grid<LV, NS>(pp, a, a.v.base + a.v.cls_off[LV] + (size_t)ck.begin[LV] * (rec_doubles(LV, NS) * 8), \
-                               a.class_first[LV] + ck.begin[LV], ck.n[LV], bx, by, bz, ixl, iyl, izl, qv, re, im);
+        run_class_grid<LV, NS>(pp, a, a.v.base + d.cls_off[LV] + (size_t)ck.begin[LV] * (rec_doubles(LV, NS) * 8), \
+                               d.cls_first[LV] + ck.begin[LV], ck.n[LV], bx, by, bz, ixl, iyl, izl, qv, re, im);
     SCARF_GRID_CLASS(0)
     SCARF_GRID_CLASS(1)
     SCARF_GRID_CLASS(2)
@@ -203,13 +211,33 @@ __global__ void __launch_bounds__(kThreads, 2) ff_grid_kernel(const GridArgs a)
     SCARF_GRID_CLASS(6)
 #undef SCARF_GRID_CLASS
 
-    double2* dst = reinterpret_cast<double2*>(a.v.dst) + (size_t)chunk * a.v.chunk_stride;
+    // ---- epilogue: store (one chunk) or add into `out` in chunk order (several); the LAST chunk holds the final value and
+    // also stores its conjugate at the mirror point when the grid is inversion-symmetric
+    double2* dst = reinterpret_cast<double2*>(a.v.dst);
+    const bool first = chunk == 0, last = chunk + 1 == a.v.n_chunks;
+    if (a.v.n_chunks > 1) ticket_wait(a.v.tickets + tile, chunk);
 #pragma unroll
-    for (int j = 0; j < kNQ; ++j)
-        if (iq[j] >= 0)
+    for (int j = 0; j < kNQ; ++j) {
+        const int ix = bx * kGridBX + ixl + 2 * j;
+        if (ix < a.nx_eval && iy < a.ny && iz < a.nz) {
+            const long long i = ((long long)ix * a.ny + iy) * a.nz + iz;
+            const bool mirror = last && a.sym && 2 * ix < a.nx - 1;
 #pragma unroll
             for (int s = 0; s < NS; ++s)
-                if (s < a.v.ns_real) dst[(size_t)s * a.v.n_q + iq[j]] = make_double2(re[j][s], im[j][s]);
+                if (s < a.v.ns_real) {
+                    double2* o = dst + (size_t)s * a.v.n_q;
+                    double2 v = make_double2(re[j][s], im[j][s]);
+                    if (!first) {
+                        const double2 p = __ldcg(o + i);
+                        v.x += p.x;
+                        v.y += p.y;
+                    }
+                    o[i] = v;
+                    if (mirror) o[a.v.n_q - 1 - i] = make_double2(v.x, -v.y);   // f(-q) = conj f(q)
+                }
+        }
+    }
+    if (a.v.n_chunks > 1) ticket_pass(a.v.tickets + tile, last ? 0 : chunk + 1);
 }
 
 }  // namespace
@@ -217,21 +245,21 @@ __global__ void __launch_bounds__(kThreads, 2) ff_grid_kernel(const GridArgs a)
 cudaError_t launch_grid_tables(const GridArgs& a, double2* tx, double2* ty, double2* tz, cudaStream_t st)
 {
     const long long ncol = (long long)a.nbx * kGridBX + (long long)a.nby * kGridBY + (long long)a.nbz * kGridBZ;
-    const long long n = a.n_rec * ncol;
+    const long long n = a.n_rows * ncol;
     if (n <= 0) return cudaSuccess;
     grid_table_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(a, tx, ty, tz);
     return cudaGetLastError();
 }
 
 template <int NS>
-static cudaError_t launch_grid_ns(const GridArgs& a, unsigned blocks, cudaStream_t st)
+static cudaError_t launch_grid_ns(const GridArgs& a, cudaStream_t st)
 {
-    ff_grid_kernel<NS><<<blocks, kThreads, kSmemBytes, st>>>(a);
+    const dim3 grid((unsigned)a.v.n_tiles, (unsigned)a.v.n_chunks, 1);   // dispatched x fastest: chunk-major
+    ff_grid_kernel<NS><<<grid, kThreads, kSmemBytes, st>>>(a);
     return cudaGetLastError();
 }
 
-// The kernels need more than 48 KB of dynamic shared memory: an attribute of the function on the CURRENT device.
-// Called by scarf_create for the context's device (idempotent, no process-wide flag).
+// The kernels need more than 48 KB of dynamic shared memory: an attribute of the function on the CURRENT device.  Called by scarf_create for the context's device (idempotent, no process-wide flag).
 cudaError_t ff_grid_init_device()
 {
     cudaError_t e = cudaSuccess;
@@ -244,15 +272,14 @@ cudaError_t ff_grid_init_device()
 
 cudaError_t launch_ff_grid(int NS, const GridArgs& a, cudaStream_t st)
 {
-    if (a.v.n_q <= 0 || a.v.n_chunks <= 0) return cudaSuccess;
-    const unsigned blocks = (unsigned)a.v.n_tiles * (unsigned)a.v.n_chunks;
+    if (a.v.n_q <= 0 || a.v.n_chunks <= 0 || a.v.n_tiles <= 0) return cudaSuccess;
     switch (NS) {
-    case 1: return launch_grid_ns<1>(a, blocks, st);
-    case 2: return launch_grid_ns<2>(a, blocks, st);
-    case 4: return launch_grid_ns<4>(a, blocks, st);
-    case 6: return launch_grid_ns<6>(a, blocks, st);
-    case 8: return launch_grid_ns<8>(a, blocks, st);
-    case 12: return launch_grid_ns<12>(a, blocks, st);
+    case 1: return launch_grid_ns<1>(a, st);
+    case 2: return launch_grid_ns<2>(a, st);
+    case 4: return launch_grid_ns<4>(a, st);
+    case 6: return launch_grid_ns<6>(a, st);
+    case 8: return launch_grid_ns<8>(a, st);
+    case 12: return launch_grid_ns<12>(a, st);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -272,15 +299,16 @@ namespace {
 __global__ void __launch_bounds__(128) sep_moments_kernel(const GridArgs a, const double* __restrict__ wx, const double* __restrict__ wy,
                                                           const double* __restrict__ wz, double2* __restrict__ mom)
 {
+    const StreamDesc& d = *a.v.desc;
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= a.n_rec * 3) return;
+    if (idx >= d.n_kept * 3) return;
     const long long r = idx / 3;
     const int axis = (int)(idx % 3);
     int c = 0;
 #pragma unroll
     for (int k = 1; k < kNClasses; ++k)
-        if (r >= a.class_first[k]) c = k;
-    const double* hdr = reinterpret_cast<const double*>(a.v.base + a.v.cls_off[c] + (size_t)(r - a.class_first[c]) * a.rec_bytes[c]);
+        if (r >= d.cls_first[k]) c = k;
+    const double* hdr = reinterpret_cast<const double*>(a.v.base + d.cls_off[c] + (size_t)(r - d.cls_first[c]) * d.rec_bytes[c]);
     const double inv4p = hdr[3], Pa = hdr[axis];
     const int n = axis == 0 ? a.nx : (axis == 1 ? a.ny : a.nz);
     const double* q = axis == 0 ? a.qx : (axis == 1 ? a.qy : a.qz);
@@ -307,20 +335,21 @@ __global__ void __launch_bounds__(128) sep_moments_kernel(const GridArgs a, cons
 }
 
 // block b sums records [b * per_block, ...) for every state of the tile: part[b][s]; fixed order, no atomics
-__global__ void __launch_bounds__(128) sep_contract_kernel(const GridArgs a, int NS, const double2* __restrict__ mom, int per_block,
+__global__ void __launch_bounds__(128) sep_contract_kernel(const GridArgs a, const double2* __restrict__ mom, int per_block,
                                                            double2* __restrict__ part)
 {
     __shared__ double2 red[128];
     const int s = threadIdx.x % 16, lane_r = threadIdx.x / 16;      // 16 state slots x 8 record lanes
-    const long long r0 = (long long)blockIdx.x * per_block, r1 = min(a.n_rec, r0 + per_block);
+    const StreamDesc& d = *a.v.desc;
+    const long long r0 = (long long)blockIdx.x * per_block, r1 = min(d.n_kept, r0 + per_block);   // blocks past the kept count write zeros
     double accr = 0.0, acci = 0.0;
     if (s < a.v.ns_real)
         for (long long r = r0 + lane_r; r < r1; r += 8) {
             int c = 0;
 #pragma unroll
             for (int k = 1; k < kNClasses; ++k)
-                if (r >= a.class_first[k]) c = k;
-            const double* rec = reinterpret_cast<const double*>(a.v.base + a.v.cls_off[c] + (size_t)(r - a.class_first[c]) * a.rec_bytes[c]);
+                if (r >= d.cls_first[k]) c = k;
+            const double* rec = reinterpret_cast<const double*>(a.v.base + d.cls_off[c] + (size_t)(r - d.cls_first[c]) * d.rec_bytes[c]);
             const int NH = nherm(c);
             const double* D = rec + 4 + (size_t)s * NH;
             const double2* M = mom + (size_t)r * 3 * kNClasses;
@@ -335,7 +364,6 @@ __global__ void __launch_bounds__(128) sep_contract_kernel(const GridArgs a, int
                         else { accr += d * m.x; acci += d * m.y; }
                     }
         }
-    (void)NS;
     red[threadIdx.x] = make_double2(accr, acci);
     __syncthreads();
     if (lane_r == 0) {
@@ -347,15 +375,16 @@ __global__ void __launch_bounds__(128) sep_contract_kernel(const GridArgs a, int
 
 }  // namespace
 
-// mom: [n_rec][3][kNClasses] complex scratch; part: [n_blocks][16] complex scratch.  Returns the number of blocks.
-cudaError_t launch_separable(const GridArgs& a, int NS, const double* wx, const double* wy, const double* wz, double* mom, double* part,
+// mom: [n_rows][3][kNClasses] complex scratch; part: [ceil(n_rows / per_block)][16] complex scratch.  The launches are sized
+// for a.n_rows records (all prescreened pairs); the kernels stop at the kept count they read from the descriptor.
+cudaError_t launch_separable(const GridArgs& a, const double* wx, const double* wy, const double* wz, double* mom, double* part,
                              int per_block, cudaStream_t st)
 {
-    if (a.n_rec <= 0) return cudaSuccess;
-    const long long n = a.n_rec * 3;
+    if (a.n_rows <= 0) return cudaSuccess;
+    const long long n = a.n_rows * 3;
     sep_moments_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(a, wx, wy, wz, reinterpret_cast<double2*>(mom));
-    const unsigned blocks = (unsigned)((a.n_rec + per_block - 1) / per_block);
-    sep_contract_kernel<<<blocks, 128, 0, st>>>(a, NS, reinterpret_cast<const double2*>(mom), per_block, reinterpret_cast<double2*>(part));
+    const unsigned blocks = (unsigned)((a.n_rows + per_block - 1) / per_block);
+    sep_contract_kernel<<<blocks, 128, 0, st>>>(a, reinterpret_cast<const double2*>(mom), per_block, reinterpret_cast<double2*>(part));
     return cudaGetLastError();
 }
 

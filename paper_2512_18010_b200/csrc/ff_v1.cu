@@ -1,21 +1,25 @@
-// ff_v1.cu — S4, the tuned hot kernel (Eq. (48)).
+// ff_v1.cu — S4, the general-q hot kernel (Eq. (48)).
 //
 //   f_s(q) = sum_pairs e^{-q^2/4p} (cos q.P + i sin q.P) (A_s(q) + i B_s(q)),
 //   A_s = sum_{n even} D^s_h q^h,  B_s = sum_{n odd} D^s_h q^h         (i^n folded into D by the fold kernel)
 //
 // Work decomposition.  The grid is n_tiles x n_chunks CTAs.  A tile is kTile = 2 x kThreads q-points (every
 // thread keeps TWO q-points and all NS <= 12 states of both in registers: 4 NS FP64 accumulators), a chunk is a
-// cost-balanced contiguous slice of the class-sorted pair stream (it may span classes).  With one chunk the CTA
-// stores straight into `out`; with several, each chunk stores a partial [chunk][state][q] and a second kernel
-// adds the partials in chunk order (deterministic, no atomics).  Chunks exist only to give the block scheduler
-// ~20 waves of equal-cost CTAs, so that the tail of the last wave is a few per cent of the run.
+// cost-balanced contiguous slice of the class-sorted pair stream (it may span classes; planned on the device,
+// fold.cu: plan_chunks_kernel).  Chunks exist only to give the block scheduler enough equal-cost CTAs for an even
+// last wave.  The n_chunks CTAs of one tile add their partial sums INTO `out` in chunk order (ff_common.cuh:
+// ordered_fixup): chunk 0 stores, chunk k waits for the tile's ticket to reach k, adds and passes the ticket on —
+// deterministic, no partial buffer in HBM and no second kernel (in round 1 the partials were 5 x the algorithmic
+// bytes); the read-modify-write of a 48 KB tile goes through L2.  CTAs are dispatched in blockIdx order (chunk-major
+// grid), so the CTA a ticket waits for is always already running.  (Measured alternative, not kept: the chunks of a
+// tile as a thread-block cluster reducing through distributed shared memory — gang scheduling of 7-CTA clusters cost
+// 30 % of the kernel time on config 3.)
 //
 // Operand delivery.  Every polynomial FMA needs its own warp-uniform coefficient.  The records of the chunk
 // are staged through shared memory by 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx), kStages
 // deep, issued by one thread; all threads then read them with broadcast LDS.128 (two coefficients per load,
-// each used for both q-points of the thread => 4 DFMA per LDS.128, a quarter of the LDS issue rate that one
-// coefficient per load and per q-point would need).  All loops over (state, Hermite index) are unrolled at
-// compile time from the class L, so monomials and accumulators are plain registers.
+// each used for both q-points of the thread => 4 DFMA per LDS.128).  All loops over (state, Hermite index) are
+// unrolled at compile time from the class L, so monomials and accumulators are plain registers.
 //
 // FP64 budget per (q, pair): 4 (arguments) + 15 (e^{-x}) + 19 (sincos) + 2 = 40 issue slots, and per
 // (q, pair, state) n_herm + 3 (2 for L = 0) — the work model of DESIGN.md.
@@ -30,6 +34,10 @@ constexpr int kTile = kThreads * kNQ;        // q-points per CTA
 constexpr int kStages = 3;
 constexpr int kStageBytes = 8192;            // >= the largest record (L = 6, NS = 12: 8096 B)
 constexpr int kSwpMaxL = 2;                  // classes whose record loop is software-pipelined
+// records whose transcendentals are in flight together in the pipelined loop: two for the short bodies of L <= 1
+// (measured on the B200: L = 0 74.4 -> 78.1 %, L = 1 76.8 -> 78.1 % of the DFMA peak; L = 2 loses registers to it)
+__host__ __device__ constexpr int swp_records(int L) { return L <= 1 ? 2 : 1; }
+
 
 struct Pipe {               // stage ring shared by all class segments of the CTA
     unsigned char* buf;     // kStages x kStageBytes
@@ -82,24 +90,40 @@ __device__ __forceinline__ void run_class(Pipe& pp, const char* __restrict__ seg
             constexpr int jq0 = decltype(jc)::value * NQA;
             double mono[NQA][nherm(L)];
             make_monomials<L, NQA, jq0>(qv, mono);
-            double gc[NQA], gs[NQA];
-            if constexpr (L <= kSwpMaxL) {               // software-pipelined: trans(k+1) alongside accum(k)
-                record_trans<NQA, jq0>(reinterpret_cast<const double2*>(sp), qv, gc, gs);
-#pragma unroll 1
-                for (int k = 0; k < cnt - 1; ++k) {
-                    double gcn[NQA], gsn[NQA];
-                    record_trans<NQA, jq0>(reinterpret_cast<const double2*>(sp + (k + 1) * REC), qv, gcn, gsn);
-                    record_accum<L, NS, NQA, jq0>(reinterpret_cast<const double2*>(sp + k * REC), mono, gc, gs, re, im);
+            auto rec = [&](int k) { return reinterpret_cast<const double2*>(sp + k * REC); };
+            if constexpr (L <= kSwpMaxL) {               // software-pipelined: trans(group k+1) alongside accum(group k)
+                constexpr int U = swp_records(L);
+                const int n_full = cnt / U * U;
+                double gc[U][NQA], gs[U][NQA];
+                if (n_full > 0) {
 #pragma unroll
-                    for (int j = 0; j < NQA; ++j) { gc[j] = gcn[j]; gs[j] = gsn[j]; }
+                    for (int u = 0; u < U; ++u) record_trans<NQA, jq0>(rec(u), qv, gc[u], gs[u]);
+#pragma unroll 1
+                    for (int k = 0; k + U < n_full; k += U) {
+                        double gcn[U][NQA], gsn[U][NQA];
+#pragma unroll
+                        for (int u = 0; u < U; ++u) record_trans<NQA, jq0>(rec(k + U + u), qv, gcn[u], gsn[u]);
+#pragma unroll
+                        for (int u = 0; u < U; ++u) record_accum<L, NS, NQA, jq0>(rec(k + u), mono, gc[u], gs[u], re, im);
+#pragma unroll
+                        for (int u = 0; u < U; ++u)
+#pragma unroll
+                            for (int jj = 0; jj < NQA; ++jj) { gc[u][jj] = gcn[u][jj]; gs[u][jj] = gsn[u][jj]; }
+                    }
+#pragma unroll
+                    for (int u = 0; u < U; ++u) record_accum<L, NS, NQA, jq0>(rec(n_full - U + u), mono, gc[u], gs[u], re, im);
                 }
-                record_accum<L, NS, NQA, jq0>(reinterpret_cast<const double2*>(sp + (cnt - 1) * REC), mono, gc, gs, re, im);
+#pragma unroll 1
+                for (int k = n_full; k < cnt; ++k) {     // fewer than U records left over
+                    record_trans<NQA, jq0>(rec(k), qv, gc[0], gs[0]);
+                    record_accum<L, NS, NQA, jq0>(rec(k), mono, gc[0], gs[0], re, im);
+                }
             } else {
+                double gc[NQA], gs[NQA];
 #pragma unroll 1
                 for (int k = 0; k < cnt; ++k) {
-                    const double2* r2 = reinterpret_cast<const double2*>(sp + k * REC);
-                    record_trans<NQA, jq0>(r2, qv, gc, gs);
-                    record_accum<L, NS, NQA, jq0>(r2, mono, gc, gs, re, im);
+                    record_trans<NQA, jq0>(rec(k), qv, gc, gs);
+                    record_accum<L, NS, NQA, jq0>(rec(k), mono, gc, gs, re, im);
                 }
             }
         });
@@ -112,15 +136,15 @@ __device__ __forceinline__ void run_class(Pipe& pp, const char* __restrict__ seg
 template <int NS>
 __global__ void __launch_bounds__(kThreads, 2) ff_v1_kernel(const V1Args a)
 {
-    __shared__ __align__(128) unsigned char stage_buf[kStages * kStageBytes];
+    __shared__ __align__(128) unsigned char smem[kStages * kStageBytes];
     __shared__ __align__(8) uint64_t full_bar[kStages];
-    const int tile = (int)(blockIdx.x % (unsigned)a.n_tiles), chunk = (int)(blockIdx.x / (unsigned)a.n_tiles);
+    const int tile = (int)blockIdx.x, chunk = (int)blockIdx.y;
     if (threadIdx.x == 0) {
         for (int s = 0; s < kStages; ++s) mbar_init(&full_bar[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    Pipe pp = {stage_buf, full_bar, 0u};
+    Pipe pp = {smem, full_bar, 0u};
 
     double qv[kNQ][4];
     long long iq[kNQ];
@@ -139,10 +163,11 @@ __global__ void __launch_bounds__(kThreads, 2) ff_v1_kernel(const V1Args a)
 #pragma unroll
         for (int s = 0; s < NS; ++s) re[j][s] = im[j][s] = 0.0;
 
-    const V1Chunk& ck = a.chunks[chunk];
+    const StreamDesc& d = *a.desc;
+    const V1Chunk& ck = d.chunks[chunk];
 #define SCARF_V1_CLASS(LV)                                                                                              \
-    if (ck.n[LV] > 0)                                                                                             \
-        run_class<LV, NS>(pp, a.base + a.cls_off[LV] + (size_t)ck.begin[LV] * (rec_doubles(LV, NS) * 8), ck.n[LV], qv, re, im);
+    if (ck.n[LV] > 0)                                                                                                   \
+        run_class<LV, NS>(pp, a.base + d.cls_off[LV] + (size_t)ck.begin[LV] * (rec_doubles(LV, NS) * 8), ck.n[LV], qv, re, im);
     SCARF_V1_CLASS(0)
     SCARF_V1_CLASS(1)
     SCARF_V1_CLASS(2)
@@ -152,28 +177,26 @@ __global__ void __launch_bounds__(kThreads, 2) ff_v1_kernel(const V1Args a)
     SCARF_V1_CLASS(6)
 #undef SCARF_V1_CLASS
 
-    double2* dst = reinterpret_cast<double2*>(a.dst) + (size_t)chunk * a.chunk_stride;
+    // ---- epilogue: store (one chunk) or add into `out` in chunk order (several) ------------------------------------------
+    double2* dst = reinterpret_cast<double2*>(a.dst);
+    const bool first = chunk == 0;
+    if (a.n_chunks > 1) ticket_wait(a.tickets + tile, chunk);
 #pragma unroll
     for (int j = 0; j < kNQ; ++j)
         if (iq[j] < a.n_q)
 #pragma unroll
             for (int s = 0; s < NS; ++s)
-                if (s < a.ns_real) dst[(size_t)s * a.n_q + iq[j]] = make_double2(re[j][s], im[j][s]);
-}
-
-// out[s][iq] = sum_k partial[k][s][iq], k ascending.
-__global__ void __launch_bounds__(256) reduce_partials_kernel(const double2* __restrict__ part, double2* __restrict__ out,
-                                                              long long n_elem, long long chunk_stride, int n_chunks)
-{
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n_elem) return;
-    double2 acc = part[i];
-    for (int k = 1; k < n_chunks; ++k) {
-        const double2 v = part[(size_t)k * chunk_stride + i];
-        acc.x += v.x;
-        acc.y += v.y;
-    }
-    out[i] = acc;
+                if (s < a.ns_real) {
+                    double2* o = dst + (size_t)s * a.n_q + iq[j];
+                    double2 v = make_double2(re[j][s], im[j][s]);
+                    if (!first) {
+                        const double2 p = __ldcg(o);      // written by another SM: read through L2
+                        v.x += p.x;
+                        v.y += p.y;
+                    }
+                    *o = v;
+                }
+    if (a.n_chunks > 1) ticket_pass(a.tickets + tile, chunk + 1 == a.n_chunks ? 0 : chunk + 1);
 }
 
 }  // namespace
@@ -183,26 +206,16 @@ int v1_tile_q() { return kTile; }
 cudaError_t launch_ff_v1(int NS, const V1Args& a, cudaStream_t st)
 {
     if (a.n_q <= 0 || a.n_chunks <= 0) return cudaSuccess;
-    const unsigned blocks = (unsigned)a.n_tiles * (unsigned)a.n_chunks;
+    const dim3 grid((unsigned)a.n_tiles, (unsigned)a.n_chunks, 1);    // dispatched x fastest: chunk-major
     switch (NS) {
-    case 1: ff_v1_kernel<1><<<blocks, kThreads, 0, st>>>(a); break;
-    case 2: ff_v1_kernel<2><<<blocks, kThreads, 0, st>>>(a); break;
-    case 4: ff_v1_kernel<4><<<blocks, kThreads, 0, st>>>(a); break;
-    case 6: ff_v1_kernel<6><<<blocks, kThreads, 0, st>>>(a); break;
-    case 8: ff_v1_kernel<8><<<blocks, kThreads, 0, st>>>(a); break;
-    case 12: ff_v1_kernel<12><<<blocks, kThreads, 0, st>>>(a); break;
+    case 1: ff_v1_kernel<1><<<grid, kThreads, 0, st>>>(a); break;
+    case 2: ff_v1_kernel<2><<<grid, kThreads, 0, st>>>(a); break;
+    case 4: ff_v1_kernel<4><<<grid, kThreads, 0, st>>>(a); break;
+    case 6: ff_v1_kernel<6><<<grid, kThreads, 0, st>>>(a); break;
+    case 8: ff_v1_kernel<8><<<grid, kThreads, 0, st>>>(a); break;
+    case 12: ff_v1_kernel<12><<<grid, kThreads, 0, st>>>(a); break;
     default: return cudaErrorInvalidValue;
     }
-    return cudaGetLastError();
-}
-
-cudaError_t launch_reduce_partials(const double* part, double* out, long long n_elem, long long chunk_stride, int n_chunks,
-                                   cudaStream_t st)
-{
-    if (n_elem <= 0) return cudaSuccess;
-    const unsigned blocks = (unsigned)((n_elem + 255) / 256);
-    reduce_partials_kernel<<<blocks, 256, 0, st>>>(reinterpret_cast<const double2*>(part), reinterpret_cast<double2*>(out),
-                                                   n_elem, chunk_stride, n_chunks);
     return cudaGetLastError();
 }
 

@@ -230,6 +230,39 @@ __global__ void __launch_bounds__(256) fft_post_kernel(const double2* __restrict
     out[i] = make_double2(vpix * (f.x * cs - f.y * sn), vpix * (f.x * sn + f.y * cs));
 }
 
+// ---- Parseval check, Eq. (75) PAPER.md:557-562 ---------------------------------------------------------------------------
+// sum_i |a_i|^2 per state of a complex array [ns][P]: kSumBlocks blocks per state over contiguous slices, fixed-order tree
+// inside a block, then one thread per state adds the block sums in block order (deterministic).
+constexpr int kSumBlocks = 256;
+__global__ void __launch_bounds__(256) sumsq_kernel(const double2* __restrict__ a, long long P, double* __restrict__ part)
+{
+    __shared__ double sh[8];
+    const int s = blockIdx.y;
+    const long long per = (P + kSumBlocks - 1) / kSumBlocks, i0 = (long long)blockIdx.x * per, i1 = min(P, i0 + per);
+    double acc = 0.0;
+    for (long long i = i0 + threadIdx.x; i < i1; i += 256) {
+        const double2 v = a[(size_t)s * P + i];
+        acc = fma(v.x, v.x, fma(v.y, v.y, acc));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += sh[w];
+        part[(size_t)s * kSumBlocks + blockIdx.x] = t;
+    }
+}
+__global__ void sumsq_final_kernel(const double* __restrict__ part, int ns, double scale, double* __restrict__ out, int stride, int col)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= ns) return;
+    double t = 0.0;
+    for (int b = 0; b < kSumBlocks; ++b) t += part[(size_t)s * kSumBlocks + b];
+    out[(size_t)s * stride + col] = t * scale;
+}
+
 // ---- cuFFT through dlopen (library step; keeps libscarf.so free of a link-time cuFFT dependency) -------------------
 // The function table is immutable once loaded (std::call_once); plans are owned by the calling context (CufftPlan).
 typedef int (*PlanFn)(int*, int, int, int, int);
@@ -305,6 +338,16 @@ cudaError_t launch_fft_post(const double* F, const FftGrid& g, int ns, double* o
     const long long n = g.P * ns;
     if (n <= 0) return cudaSuccess;
     fft_post_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const double2*>(F), g, ns, reinterpret_cast<double2*>(out));
+    return cudaGetLastError();
+}
+
+// out[s * stride + col] = scale * sum_i |a[s][i]|^2, s < ns; scratch: ns * 256 doubles.
+cudaError_t launch_sumsq(const double* a_complex, long long P, int ns, double scale, double* scratch, double* out, int stride, int col,
+                         cudaStream_t st)
+{
+    if (ns <= 0 || P <= 0) return cudaSuccess;
+    sumsq_kernel<<<dim3(kSumBlocks, (unsigned)ns), 256, 0, st>>>(reinterpret_cast<const double2*>(a_complex), P, scratch);
+    sumsq_final_kernel<<<(unsigned)((ns + 63) / 64), 64, 0, st>>>(scratch, ns, scale, out, stride, col);
     return cudaGetLastError();
 }
 

@@ -1,6 +1,8 @@
 // fold.cu — S3 of SURVEY.md §8(a): fold the transition matrices T^s into per-primitive-pair Hermite
 // coefficients (the paper's T M D product, Eq. (48)-(49) PAPER.md:326-334), compute the screening bound,
 // and pack the kept records.  Also the FP64 peak micro-benchmark.
+#include <algorithm>
+
 #include "kernels.cuh"
 
 namespace scarf {
@@ -97,14 +99,19 @@ __global__ void __launch_bounds__(128) fold_kernel(const FoldArgs a)
             }
     }
     double b = 0.0;
+    bool bad = false;                                     // fmax drops NaN: keep a non-finite bound (non-finite T) sticky
 #pragma unroll
     for (int s = 0; s < kMaxStateTile; ++s) {
         double x = bsum[s];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+        bad = bad || !(x <= 1.7976931348623157e308);
         b = fmax(b, x);
     }
-    if (lane == 0) a.bound[warp] = a.first_tile ? b : fmax(a.bound[warp], b);
+    if (lane == 0) {
+        const double prev = a.first_tile ? 0.0 : a.bound[warp];
+        a.bound[warp] = (bad || !(prev <= 1.7976931348623157e308)) ? __longlong_as_double(0x7ff8000000000000LL) : fmax(prev, b);
+    }
 }
 
 cudaError_t launch_fold(const FoldArgs& a, cudaStream_t st)
@@ -116,28 +123,210 @@ cudaError_t launch_fold(const FoldArgs& a, cudaStream_t st)
     return cudaGetLastError();
 }
 
-// One warp per kept record: copy it from the staging layout to its packed position (16-byte chunks).
-__global__ void __launch_bounds__(128) pack_kernel(const char* __restrict__ staging, char* __restrict__ packed,
-                                                   const unsigned long long* __restrict__ src_off,
-                                                   const unsigned long long* __restrict__ dst_off,
-                                                   const int* __restrict__ nbytes, long long n)
+// ---- screening on the device -----------------------------------------------------------------------------------------
+// One CTA.  Pass 1: sum, max and finiteness of the bounds (fixed-order tree: deterministic).  Threshold (DESIGN.md
+// reading #12):  thr = max(screen_tol * mean(B), threshold_eps * max(B));  a pair is kept iff B > 0 and B >= thr.
+// Pass 2: stable compaction of the kept indices (block scan over consecutive 1024-element windows, so the stream keeps
+// the host's class-sorted (i, j) order), kept counts per class, sum of the dropped bounds.
+constexpr int kScreenThreads = 1024;
+
+__device__ __forceinline__ double block_reduce(double v, double* sh, bool take_max)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double w = __shfl_xor_sync(0xffffffffu, v, o);
+        v = take_max ? fmax(v, w) : v + w;
+    }
+    __syncthreads();
+    if (lane == 0) sh[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        v = lane < kScreenThreads / 32 ? sh[lane] : (take_max ? 0.0 : 0.0);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double w = __shfl_xor_sync(0xffffffffu, v, o);
+            v = take_max ? fmax(v, w) : v + w;
+        }
+        if (lane == 0) sh[0] = v;
+    }
+    __syncthreads();
+    return sh[0];
+}
+
+__global__ void __launch_bounds__(kScreenThreads) screen_kernel(const ScreenArgs a)
+{
+    __shared__ double sh[kScreenThreads / 32];
+    __shared__ int sh_scan[kScreenThreads / 32];
+    __shared__ int sh_bad;
+    __shared__ int sh_cls[kNClasses];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) sh_bad = 0;
+    if (tid < kNClasses) sh_cls[tid] = 0;
+    double sum = 0.0, mx = 0.0;
+    bool bad = false;
+    for (long long i = tid; i < a.n_pairs; i += kScreenThreads) {
+        const double b = a.bound[i];
+        bad = bad || !isfinite(b);
+        sum += b;
+        mx = fmax(mx, b);
+    }
+    __syncthreads();
+    if (bad) sh_bad = 1;
+    const double sumB = block_reduce(sum, sh, false);
+    const double maxB = block_reduce(mx, sh, true);
+    const bool any_bad = sh_bad != 0;
+    // a non-finite bound means a non-finite T: keep everything so that the NaN reaches the output instead of silent zeros
+    const double thr = any_bad ? 0.0 : fmax(a.n_pairs > 0 ? a.screen_tol * sumB / (double)a.n_pairs : 0.0, a.threshold_eps * maxB);
+    double dropped = 0.0;
+    long long base = 0;
+    for (long long w0 = 0; w0 < a.n_pairs; w0 += kScreenThreads) {
+        const long long i = w0 + tid;
+        bool keep = false;
+        if (i < a.n_pairs) {
+            const double b = a.bound[i];
+            keep = any_bad || (b > 0.0 && b >= thr);
+            if (!keep) dropped += b;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, keep);
+        const int in_warp = __popc(m & ((1u << lane) - 1u));
+        if (lane == 0) sh_scan[warp] = __popc(m);
+        __syncthreads();
+        int before = 0, total = 0;
+#pragma unroll 1
+        for (int k = 0; k < kScreenThreads / 32; ++k) {
+            const int c = sh_scan[k];
+            if (k < warp) before += c;
+            total += c;
+        }
+        int c = -1;
+        if (keep) {
+            a.keep_idx[base + before + in_warp] = (int)i;
+            c = 0;
+#pragma unroll
+            for (int k = 1; k < kNClasses; ++k)
+                if (i >= a.class_first[k]) c = k;
+        }
+        // kept counts per class: warp-aggregated (a window usually lies in ONE class: per-thread atomics on one shared
+        // word serialise 1024 ways — 0.33 ms measured); integer counts, so the order of the adds does not matter
+#pragma unroll
+        for (int k = 0; k < kNClasses; ++k) {
+            const int n = __popc(__ballot_sync(0xffffffffu, c == k));
+            if (lane == 0 && n > 0) atomicAdd(&sh_cls[k], n);
+        }
+        base += total;
+        __syncthreads();
+    }
+    const double droppedB = block_reduce(dropped, sh, false);
+    if (tid == 0) {
+        ScreenResult r = {};
+        r.n_kept = base;
+        for (int c = 0; c < kNClasses; ++c) r.kept_per_class[c] = sh_cls[c];
+        r.sum_bound = sumB; r.max_bound = maxB; r.dropped_bound = any_bad ? 0.0 : droppedB;
+        r.bad = any_bad ? 1 : 0;
+        *a.result = r;
+    }
+}
+
+cudaError_t launch_screen(const ScreenArgs& a, cudaStream_t st)
+{
+    screen_kernel<<<1, kScreenThreads, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+// One warp per kept record: copy it from the staging layout to its packed position (16-byte pieces).  Every warp derives
+// the packed layout from the screening result (13-term prefix sums); block 0 also writes the tile's StreamDesc.
+__global__ void __launch_bounds__(128) pack_kernel(const PackArgs a)
 {
     const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
-    if (warp >= n) return;
-    const uint4* s = reinterpret_cast<const uint4*>(staging + src_off[warp]);
-    uint4* d = reinterpret_cast<uint4*>(packed + dst_off[warp]);
-    const int chunks = nbytes[warp] >> 4;
-    for (int i = lane; i < chunks; i += 32) d[i] = s[i];
+    const ScreenResult& r = *a.result;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        StreamDesc& d = *a.desc;
+        long long first = 0;
+        unsigned long long off = 0;
+        for (int c = 0; c < kNClasses; ++c) {
+            d.cls_n[c] = r.kept_per_class[c];
+            d.cls_first[c] = first;
+            d.cls_off[c] = off;
+            d.rec_bytes[c] = a.rec_bytes[c];
+            first += r.kept_per_class[c];
+            off += (unsigned long long)r.kept_per_class[c] * a.rec_bytes[c];
+        }
+        d.cls_first[kNClasses] = first;
+        d.n_kept = r.n_kept;
+        d.n_chunks = 0;
+    }
+    if (warp >= r.n_kept) return;
+    const long long i = a.keep_idx[warp];
+    int c = 0;
+#pragma unroll
+    for (int k = 1; k < kNClasses; ++k)
+        if (i >= a.class_first[k]) c = k;
+    long long kfirst = 0;
+    unsigned long long doff = 0;
+    for (int k = 0; k < c; ++k) {
+        kfirst += r.kept_per_class[k];
+        doff += (unsigned long long)r.kept_per_class[k] * a.rec_bytes[k];
+    }
+    const uint4* s = reinterpret_cast<const uint4*>(a.staging + a.cls_off[c] + (unsigned long long)(i - a.class_first[c]) * a.rec_bytes[c]);
+    uint4* d = reinterpret_cast<uint4*>(a.packed + doff + (unsigned long long)(warp - kfirst) * a.rec_bytes[c]);
+    const int pieces = a.rec_bytes[c] >> 4;
+    for (int k = lane; k < pieces; k += 32) d[k] = s[k];
 }
 
-cudaError_t launch_pack(const char* staging, char* packed, const unsigned long long* src_off,
-                        const unsigned long long* dst_off, const int* nbytes, long long n, cudaStream_t st)
+cudaError_t launch_pack(const PackArgs& a, cudaStream_t st)
 {
-    if (n <= 0) return cudaSuccess;
     const int threads = 128;
-    const long long blocks = (n * 32 + threads - 1) / threads;
-    pack_kernel<<<(unsigned)blocks, threads, 0, st>>>(staging, packed, src_off, dst_off, nbytes, n);
+    const long long blocks = std::max<long long>(1, (a.n_pairs * 32 + threads - 1) / threads);   // sized for "everything kept"
+    pack_kernel<<<(unsigned)blocks, threads, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+// ---- chunk planning on the device ------------------------------------------------------------------------------------
+// Split the fast classes of the class-sorted stream into exactly K chunks of (nearly) equal modelled cost
+// (w(c) = ns_real W(c) + ctr FP64 issue slots per record and q-point); a chunk may span classes; trailing chunks may be
+// empty when there are fewer records than chunks.  One thread: <= K + 7 loop trips.
+__global__ void plan_chunks_kernel(StreamDesc* d, int K, int ns_real, double ctr)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const double kW[kFastMaxClass + 1] = {2, 7, 13, 23, 38, 59, 87};
+    double w[kFastMaxClass + 1], total = 0.0;
+    for (int c = 0; c <= kFastMaxClass; ++c) {
+        w[c] = (double)ns_real * kW[c] + ctr;
+        total += (double)d->cls_n[c] * w[c];
+    }
+    for (int k = 0; k < kMaxChunks; ++k)
+        for (int c = 0; c < kNClasses; ++c) d->chunks[k].begin[c] = d->chunks[k].n[c] = 0;
+    d->n_chunks = K;
+    int k = 0;
+    double acc = 0.0;
+    bool cur_empty = true;
+    for (int c = 0; c <= kFastMaxClass; ++c) {
+        long long rem = d->cls_n[c], pos = 0;
+        while (rem > 0) {
+            long long take = rem;
+            if (k < K - 1) {
+                const double need = total * (double)(k + 1) / (double)K - acc;
+                take = min(rem, (long long)llrint(need / w[c]));
+                if (take <= 0) {
+                    if (cur_empty) take = 1;
+                    else { ++k; cur_empty = true; continue; }
+                }
+            }
+            d->chunks[k].begin[c] = (int)pos;
+            d->chunks[k].n[c] = (int)take;
+            cur_empty = false;
+            acc += (double)take * w[c];
+            pos += take; rem -= take;
+            if (k < K - 1 && acc >= total * (double)(k + 1) / (double)K - 0.5 * w[c]) { ++k; cur_empty = true; }
+        }
+    }
+}
+
+cudaError_t launch_plan_chunks(StreamDesc* desc, int K, int ns_real, double ctr, cudaStream_t st)
+{
+    plan_chunks_kernel<<<1, 32, 0, st>>>(desc, K, ns_real, ctr);
     return cudaGetLastError();
 }
 

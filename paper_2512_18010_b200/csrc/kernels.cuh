@@ -27,19 +27,39 @@ __host__ __device__ inline constexpr int rec_doubles(int L, int NS)
     return 4 + ((NS * nherm(L) + 1) & ~1);
 }
 
-struct ClassStream {
-    long long n;               // records in this class
-    unsigned long long off;    // byte offset of the class's first record from the tile base
-    int rec_bytes;
-    int pad;
+// ---- device-resident description of one state tile's packed pair stream ---------------------------------------------
+// Written on the device by the screening / pack / chunk-planning kernels of fold.cu, read by every S4 kernel, so that
+// scarf_set_transitions needs no device->host round trip (the host never learns the kept counts unless asked:
+// scarf_get_stats).  A chunk is a cost-balanced contiguous slice of the class-sorted stream; per class c it covers
+// records [begin[c], begin[c] + n[c]) of that class.
+constexpr int kMaxChunks = 32;
+struct V1Chunk {
+    int begin[kNClasses];
+    int n[kNClasses];
+};
+struct StreamDesc {
+    long long n_kept;                       // records in the packed stream
+    long long cls_n[kNClasses];             // kept records per class
+    long long cls_first[kNClasses + 1];     // stream-order index of each class's first record
+    unsigned long long cls_off[kNClasses];  // byte offset of each class's first record from the stream base
+    int rec_bytes[kNClasses];
+    int n_chunks;                           // chunks planned by the last plan_chunks launch (some may be empty)
+    V1Chunk chunks[kMaxChunks];
+};
+struct ScreenResult {                       // device -> pinned host, read lazily (scarf_get_stats)
+    long long n_kept;
+    long long kept_per_class[kNClasses];
+    double sum_bound, max_bound, dropped_bound;
+    int bad, pad;                           // bad != 0: a bound was NaN/Inf (non-finite T): nothing is dropped, the output carries the NaN
 };
 
-struct TileStream {            // one state tile of the pair stream
+struct TileStream {            // one state tile of the pair stream (host bookkeeping; the counts live in `desc`)
     int s0, ns_real, NS;       // first state, real states, padded/templated state count
     int pad;
-    char* base;                // device pointer
-    unsigned long long bytes;
-    ClassStream cls[kNClasses];
+    char* staging;             // device: records of ALL prescreened pairs, class-sorted (written by the fold)
+    char* base;                // device: packed stream of the kept pairs
+    StreamDesc* desc;          // device
+    unsigned long long staging_bytes;
 };
 
 struct FoldArgs {
@@ -57,32 +77,49 @@ struct FoldArgs {
     int rec_bytes[kNClasses];
 };
 
-cudaError_t launch_fold(const FoldArgs& a, cudaStream_t st);
-cudaError_t launch_pack(const char* staging, char* packed, const unsigned long long* src_off,
-                        const unsigned long long* dst_off, const int* nbytes, long long n, cudaStream_t st);
-
-// v1 (ff_v1.cu): the tuned kernel.  A chunk is a cost-balanced slice of the class-sorted stream; per class c it
-// covers records [begin[c], begin[c] + n[c]) of that class.
-constexpr int kMaxChunks = 32;
-struct V1Chunk {
-    int begin[kNClasses];
-    int n[kNClasses];
+struct ScreenArgs {
+    const double* bound;       // [n_pairs]
+    long long n_pairs;
+    long long class_first[kNClasses + 1];   // prescreened pairs per class (host knows these)
+    double screen_tol, threshold_eps;
+    int* keep_idx;             // [n_pairs] out: source index of the k-th kept record (stable order)
+    ScreenResult* result;      // device
 };
+
+struct PackArgs {
+    const char* staging;
+    char* packed;
+    const int* keep_idx;
+    const ScreenResult* result;
+    StreamDesc* desc;          // written by block 0
+    long long n_pairs;
+    long long class_first[kNClasses + 1];
+    unsigned long long cls_off[kNClasses];  // of the staging layout
+    int rec_bytes[kNClasses];
+};
+
+cudaError_t launch_fold(const FoldArgs& a, cudaStream_t st);
+cudaError_t launch_screen(const ScreenArgs& a, cudaStream_t st);
+cudaError_t launch_pack(const PackArgs& a, cudaStream_t st);
+// cost-balanced split of the FAST classes (0..kFastMaxClass) of the stream into exactly K chunks (K <= kMaxChunks);
+// w(c) = ns_real * W(c) + ctr.  One thread; ~2 us.
+cudaError_t launch_plan_chunks(StreamDesc* desc, int K, int ns_real, double ctr, cudaStream_t st);
+
+// v1 (ff_v1.cu): the general-q kernel.  Grid = (n_tiles, n_chunks), dispatched chunk-major; the chunks of one q tile add
+// their partial sums into `out` in chunk order through a per-tile ticket (no partial buffer in HBM, no second kernel).
+constexpr int kFastMaxClass = 6;            // classes 0..6 (shells up to f with f) run in the unrolled kernels
 struct V1Args {
     const char* base;                       // tile stream base
-    unsigned long long cls_off[kNClasses];  // byte offset of each class's first record
+    const StreamDesc* desc;                 // device: class offsets, chunk table
     const double* q;                        // [n_q][3]
     long long n_q;
-    int n_tiles, n_chunks;                  // grid = n_tiles * n_chunks CTAs, chunk-major
+    int n_tiles, n_chunks;                  // grid = (n_tiles, n_chunks)
     int ns_real, pad;
-    double* dst;                            // n_chunks == 1: out + s0*n_q*2; else the partial buffer
-    long long chunk_stride;                 // double2 elements between the partials of consecutive chunks
-    V1Chunk chunks[kMaxChunks];
+    double* dst;                            // out + s0*n_q*2
+    int* tickets;                           // [n_tiles], all zero at launch and again at exit (n_chunks > 1 only)
 };
 int v1_tile_q();                            // q-points per CTA
 cudaError_t launch_ff_v1(int NS, const V1Args& a, cudaStream_t st);
-cudaError_t launch_reduce_partials(const double* part, double* out, long long n_elem, long long chunk_stride,
-                                   int n_chunks, cudaStream_t st);
 
 // grid (ff_grid.cu): Cartesian product grid q = (qx[ix], qy[iy], qz[iz]), index (ix*ny + iy)*nz + iz.  The
 // Gaussian/phase factor separates, e^{-q^2/4p} e^{iq.P} = X_P(ix) Y_P(iy) Z_P(iz) (the V-tensor idea of Eq. (45)-(46)
@@ -90,26 +127,33 @@ cudaError_t launch_reduce_partials(const double* part, double* out, long long n_
 // (q, pair) instead of an exp and a sincos.  A CTA owns a kGridBX x kGridBY x kGridBZ box of the grid.
 constexpr int kGridBX = 4, kGridBY = 8, kGridBZ = 8;
 struct GridArgs {
-    V1Args v;                               // stream, chunks, dst as for v1; v.q unused; v.n_q = nx*ny*nz
+    V1Args v;                               // stream, desc, dst as for v1; v.q unused; v.n_q = nx*ny*nz
     const double *qx, *qy, *qz;             // axes (device)
     int nx, ny, nz;
-    int nbx, nby, nbz;                      // boxes per axis; v.n_tiles = nbx*nby*nbz
-    const double2 *tx, *ty, *tz;            // tables [box][record][kGridB*] of (re, im); zero beyond the axis end
-    long long n_rec;                        // records of the tile stream = rows of each table
-    long long class_first[kNClasses];       // stream-order index of each class's first record
-    int rec_bytes[kNClasses];               // record size of each class for this state tile
-    int pad;
+    int nbx, nby, nbz;                      // boxes per axis; v.n_tiles = nbx*nby*nbz.  With `sym` the boxes cover ix < nx_eval only
+    int sym, nx_eval;                       // sym != 0: the grid is inversion-symmetric (every axis ax[i] == -ax[n-1-i] bit for bit):
+                                            // only ix < nx_eval = ceil(nx/2) is evaluated and f(-q) = conj f(q) is stored for the mirror point
+    const double2 *tx, *ty, *tz;            // tables [box][row][kGridB*] of (re, im); zero beyond the axis end
+    long long n_rows;                       // row stride of the tables (>= kept records; the prescreened count, known to the host)
 };
 cudaError_t launch_grid_tables(const GridArgs& a, double2* tx, double2* ty, double2* tz, cudaStream_t st);
 cudaError_t launch_ff_grid(int NS, const GridArgs& a, cudaStream_t st);
 cudaError_t ff_grid_init_device();           // per-device function attributes (dynamic shared memory); idempotent
-cudaError_t launch_separable(const GridArgs& a, int NS, const double* wx, const double* wy, const double* wz, double* mom, double* part,
-                             int per_block, cudaStream_t st);
+cudaError_t launch_separable(const GridArgs& a, const double* wx, const double* wy, const double* wz, double* mom, double* part,
+                             int per_block, cudaStream_t st);   // grids sized for a.n_rows records; part[block][16] complex
 
 // angular moments (angular.cu, NEXT-3)
 void angular_host_tables(int l_max, int n_theta, const double* cos_theta, const double* w_theta, int n_phi,
                          std::vector<double>& Yw, std::vector<double>& tw);
 cudaError_t angular_init_device();           // per-device function attributes; idempotent
+constexpr int kAngularMaxSmem = 200 * 1024;  // dynamic shared memory the fused kernel may use (B fragments + F rows)
+void angular_fragment_table(int l_max, int n_phi, std::vector<double>& Bf, int& n_nt, int& n_ks);
+void angular_transpose_table(int l_max, int n_theta, const std::vector<double>& Yw, std::vector<double>& YwT);
+size_t angular_fused_smem(int n_theta, int l_max, int n_nt, int n_ks, bool fused);
+// F_glob == nullptr: fused (R, f2 written); else F [n_sr][n_theta][2 l_max + 1] complex and row2 [n_sr][n_theta] are written instead
+cudaError_t launch_angular_fused(const double* f, const double* Bf, const double* YwT, const double* w_theta, long long n_sr, int n_theta,
+                                 int n_phi, int l_max, int n_nt, int n_ks, double* R, double* f2, double* F_glob, double* row2_glob,
+                                 cudaStream_t st);
 cudaError_t launch_phi_dft(const double* f, const double* tw, long long n_rows, int n_phi, int l_max, double* F, double* rowsum2,
                            cudaStream_t st);
 cudaError_t launch_legendre(const double* F, const double* rowsum2, const double* Yw, const double* w_theta, long long n_sr,
@@ -135,6 +179,9 @@ cudaError_t launch_density(const double* V, const double* T, int nbf, long long 
                            cudaStream_t st);
 cudaError_t launch_density_mma(const double* V, const double* T, double* Csym, int nbf, int nbf_pad, long long P, int s0, int ns,
                                double g, double* out_complex, cudaStream_t st);
+// Parseval sums (Eq. 75): out[s * stride + col] = scale * sum_i |a[s][i]|^2; scratch holds ns * 256 doubles
+cudaError_t launch_sumsq(const double* a_complex, long long P, int ns, double scale, double* scratch, double* out, int stride, int col,
+                         cudaStream_t st);
 cudaError_t launch_fft_post(const double* F, const FftGrid& g, int ns, double* out, cudaStream_t st);
 struct CufftPlan { int handle = -1, nx = 0, ny = 0, nz = 0; };   // owned by a context, tied to its device
 int cufft_inverse_batch(CufftPlan& pl, double* data, int nx, int ny, int nz, int ns, cudaStream_t st);

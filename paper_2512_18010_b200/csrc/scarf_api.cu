@@ -40,6 +40,12 @@ const double kCtrGrid = 6.0, kCtrTable = 39.0;
 
 }  // namespace
 
+struct AngularCache {             // host tables of scarf_angular_moments and the arguments they were built for
+    bool valid = false;
+    int n_phi = 0, l_max = 0, n_nt = 0, n_ks = 0;
+    std::vector<double> ct, wt, Yw, YwT, tw, Bf;
+};
+
 struct scarf_ctx {
     int device = -1;
     bool host_only = true;
@@ -47,7 +53,13 @@ struct scarf_ctx {
     double prefactor = 2.0, screen_tol = 1e-16, threshold_eps = 0.0;
     bool timing = false;
     int n_chunks_opt = 0;     // 0 auto, else the number of stream chunks of the S4 kernels
+    int grid_symmetry = 1;    // 1: use f(-q) = conj f(q) on inversion-symmetric product grids; 0: never
     int fft_density_variant = 1;  // 1: DMMA kernel, 0: SIMT kernel (fft_method.cu)
+    int check_parseval = 0;       // 1: scarf_fft_form_factors also evaluates both sides of Eq. (75)
+    int parseval_states = 0;      // states whose sums the last scarf_fft_form_factors call left in d_parseval
+    DevBuf d_parseval;
+    int angular_variant = 1;      // 1: fused DMMA kernel, 0: SIMT phi kernel + Legendre kernel (angular.cu)
+    AngularCache ang;
     std::string err;
     HostSetup hs;
     bool have_basis = false, have_T = false;
@@ -57,12 +69,18 @@ struct scarf_ctx {
     std::vector<double> pure_ucoef;
     int n_states = 0;
     int sm_count = 148;
-    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_src, d_dst, d_nb, d_partial, d_axes, d_tab, d_ang_in, d_ang_F, d_ang_tab, d_ang_out, d_pure_map, d_Tcart, d_prim, d_V, d_fft, d_Csym;
+    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_keep, d_desc, d_screen, d_tickets, d_axes, d_tab, d_ang_in, d_ang_F, d_ang_tab, d_ang_out, d_pure_map, d_Tcart, d_prim, d_V, d_fft, d_Csym;
     const double* Tc_dev = nullptr;        // context-owned Cartesian T of the last set_transitions (FFT method)
     std::vector<DevBuf> staging, packed;
     std::vector<TileStream> tiles;
     scarf_stats st = {};
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev_slice = nullptr;
+    // screening result of the last set_transitions: written on the device, copied to pinned host memory asynchronously and
+    // harvested when somebody needs it (scarf_get_stats) or when it is already there (cudaEventQuery)
+    ScreenResult* h_screen = nullptr;      // pinned
+    cudaEvent_t ev_screen = nullptr;
+    bool screen_pending = false, T_bad = false;
+    double grid_eval_points = 0.0, grid_table_cols = 0.0;   // geometry of the last product-grid call (for its work model)
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev_m0 = nullptr, ev_m1 = nullptr, ev_slice = nullptr;
     cudaStream_t copy_stream = nullptr;    // device->host copies of form_factors' output slices
     CufftPlan fft_plan;                    // cuFFT plan of the last scarf_fft_form_factors grid (this context's device)
 };
@@ -119,56 +137,56 @@ int tile_size_for(int ns)  // smallest instantiated state tile >= ns (ns <= 12)
     return kMaxStateTile;
 }
 
-// Split the tile's class-sorted stream into <= K chunks of (nearly) equal modelled cost; a chunk may span classes.
-// Returns the number of non-empty chunks written to `out`.
-int build_chunks(const TileStream& t, int K, V1Chunk* out, double ctr = kCtr)
+// Number of stream chunks for a launch over n_tiles q tiles: enough equal-cost CTAs for ~24 waves (2 resident CTAs per SM),
+// so that the ragged last wave costs a few per cent; 1 when the tiles alone give that many.
+int choose_chunks(int sm_count, long long n_tiles, int forced)
 {
-    double w[kNClasses], total = 0.0;
-    long long nrec = 0;
-    for (int c = 0; c < kNClasses; ++c) {
-        w[c] = (double)t.ns_real * kW[c] + ctr;
-        total += (double)t.cls[c].n * w[c];
-        nrec += t.cls[c].n;
-    }
-    if (nrec == 0) return 0;
-    K = (int)std::max<long long>(1, std::min<long long>(K, nrec));
-    int k = 0;
-    double acc = 0.0;
-    std::memset(out, 0, sizeof(V1Chunk) * (size_t)K);
-    bool cur_empty = true;
-    for (int c = 0; c < kNClasses; ++c) {
-        long long rem = t.cls[c].n, pos = 0;
-        while (rem > 0) {
-            long long take = rem;
-            if (k < K - 1) {
-                const double need = total * (double)(k + 1) / (double)K - acc;
-                take = std::min<long long>(rem, (long long)std::llround(need / w[c]));
-                if (take <= 0) {
-                    if (cur_empty) take = 1;
-                    else { ++k; cur_empty = true; continue; }
-                }
-            }
-            out[k].begin[c] = (int)pos;
-            out[k].n[c] = (int)take;
-            cur_empty = false;
-            acc += (double)take * w[c];
-            pos += take; rem -= take;
-            if (k < K - 1 && acc >= total * (double)(k + 1) / (double)K - 0.5 * w[c]) { ++k; cur_empty = true; }
-        }
-    }
-    int n = 0;                                     // compact away chunks that stayed empty
-    for (int i = 0; i < K; ++i) {
-        bool any = false;
-        for (int c = 0; c < kNClasses; ++c) any = any || out[i].n[c] > 0;
-        if (any) { if (n != i) out[n] = out[i]; ++n; }
-    }
-    return n;
+    long long K = forced > 0 ? forced : (24LL * 2 * sm_count + n_tiles / 2) / std::max<long long>(1, n_tiles);
+    return (int)std::max<long long>(1, std::min<long long>(K, kMaxChunks));
 }
+
+// per-tile tickets of the ordered fix-up (ff_common.cuh): zeroed before every multi-chunk launch
+int prepare_tickets(scarf_ctx* ctx, long long n_tiles, int n_chunks, cudaStream_t st, int** out)
+{
+    *out = nullptr;
+    if (n_chunks <= 1) return SCARF_OK;
+    CU(ctx->d_tickets.ensure((size_t)n_tiles * sizeof(int)), "alloc tickets");
+    CU(cudaMemsetAsync(ctx->d_tickets.p, 0, (size_t)n_tiles * sizeof(int), st), "clear tickets");
+    *out = static_cast<int*>(ctx->d_tickets.p);
+    return SCARF_OK;
+}
+
+// Screening result of the last set_transitions -> stats.  wait: block until it has arrived; else only take it if it is there.
+int harvest_screen(scarf_ctx* c, bool wait)
+{
+    if (!c->screen_pending) return SCARF_OK;
+    cudaError_t e = wait ? cudaEventSynchronize(c->ev_screen) : cudaEventQuery(c->ev_screen);
+    if (e == cudaErrorNotReady) { cudaGetLastError(); return SCARF_OK; }
+    if (e != cudaSuccess) return cuda_fail(c, e, "screening result");
+    c->screen_pending = false;
+    const ScreenResult& r = *c->h_screen;
+    scarf_stats& s = c->st;
+    s.n_pairs_kept = r.n_kept;
+    s.dropped_bound = r.dropped_bound;
+    s.n_herm_kept = 0; s.slots_per_q = 0.0; s.stream_bytes = 0.0;
+    for (int k = 0; k < kNClasses; ++k) {
+        s.pairs_kept_per_class[k] = r.kept_per_class[k];
+        s.n_herm_kept += r.kept_per_class[k] * nherm(k);
+        s.slots_per_q += (double)r.kept_per_class[k] * ((double)c->n_states * kW[k] + kCtr * (double)c->tiles.size());
+        for (const auto& t : c->tiles) s.stream_bytes += (double)r.kept_per_class[k] * (double)(rec_doubles(k, t.NS) * 8);
+    }
+    s.evals_per_q = (double)r.n_kept * (double)c->n_states;
+    c->T_bad = r.bad != 0;
+    return SCARF_OK;
+}
+
+const char* kBadT = "the transition matrices passed to set_transitions contain NaN/Inf (detected on the device); results are NaN";
+
 
 void free_device(scarf_ctx* c)
 {
     c->d_pairs.release(); c->d_E.release(); c->d_bound.release(); c->d_T.release(); c->d_q.release();
-    c->d_out.release(); c->d_src.release(); c->d_dst.release(); c->d_nb.release(); c->d_partial.release();
+    c->d_out.release(); c->d_keep.release(); c->d_desc.release(); c->d_screen.release(); c->d_tickets.release(); c->d_parseval.release(); c->parseval_states = 0;
     c->d_axes.release(); c->d_tab.release();
     c->d_ang_in.release(); c->d_ang_F.release(); c->d_ang_tab.release(); c->d_ang_out.release();
     c->d_pure_map.release(); c->d_Tcart.release();
@@ -203,9 +221,13 @@ int scarf_create(scarf_ctx** out, int device)
         // per-device function attributes (idempotent; set for every context so that no process-wide flag is needed)
         if (e == cudaSuccess) e = ff_grid_init_device();
         if (e == cudaSuccess) e = angular_init_device();
+        if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->h_screen), sizeof(ScreenResult));
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_screen, cudaEventDisableTiming);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device);
         if (e == cudaSuccess) e = cudaEventCreate(&ctx->ev0);
         if (e == cudaSuccess) e = cudaEventCreate(&ctx->ev1);
+        if (e == cudaSuccess) e = cudaEventCreate(&ctx->ev_m0);
+        if (e == cudaSuccess) e = cudaEventCreate(&ctx->ev_m1);
         if (e != cudaSuccess) {
             cudaGetLastError();
             delete ctx;
@@ -228,7 +250,11 @@ void scarf_destroy(scarf_ctx* ctx)
         cufft_plan_release(ctx->fft_plan);
         if (ctx->ev0) cudaEventDestroy(ctx->ev0);
         if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+        if (ctx->ev_m0) cudaEventDestroy(ctx->ev_m0);
+        if (ctx->ev_m1) cudaEventDestroy(ctx->ev_m1);
         if (ctx->ev_slice) cudaEventDestroy(ctx->ev_slice);
+        if (ctx->ev_screen) cudaEventDestroy(ctx->ev_screen);
+        if (ctx->h_screen) cudaFreeHost(ctx->h_screen);
         if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     }
     delete ctx;
@@ -252,9 +278,17 @@ int scarf_set_option(scarf_ctx* ctx, const char* key, double value)
         ctx->screen_tol = value;
     } else if (k == "timing") ctx->timing = value != 0.0;
     else if (k == "threshold_eps") { if (!(value >= 0.0)) return fail(ctx, SCARF_EINVAL, "set_option: threshold_eps < 0"); ctx->threshold_eps = value; }
-    else if (k == "n_chunks") {
+    else if (k == "grid_symmetry") {
+        if (value != 0.0 && value != 1.0) return fail(ctx, SCARF_EINVAL, "set_option: grid_symmetry must be 0 or 1");
+        ctx->grid_symmetry = (int)value;
+    } else if (k == "n_chunks") {
         if (value < 0 || value > kMaxChunks) return fail(ctx, SCARF_EINVAL, "set_option: n_chunks outside 0..32");
         ctx->n_chunks_opt = (int)value;
+    } else if (k == "check_parseval") {
+        ctx->check_parseval = value != 0.0;
+    } else if (k == "angular_variant") {
+        if (value != 0.0 && value != 1.0) return fail(ctx, SCARF_EINVAL, "set_option: angular_variant must be 0 or 1");
+        ctx->angular_variant = (int)value;
     } else if (k == "fft_density_variant") {
         if (value != 0.0 && value != 1.0) return fail(ctx, SCARF_EINVAL, "set_option: fft_density_variant must be 0 or 1");
         ctx->fft_density_variant = (int)value;
@@ -402,8 +436,11 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T)
         if (ctx->staging.size() < tiles.size()) ctx->staging.resize(tiles.size());
         if (ctx->packed.size() < tiles.size()) ctx->packed.resize(tiles.size());
         CU(ctx->d_bound.ensure(std::max<size_t>(64, (size_t)np * sizeof(double))), "set_transitions: alloc bound");
+        CU(ctx->d_keep.ensure(std::max<size_t>(64, (size_t)np * sizeof(int))), "set_transitions: alloc index");
+        CU(ctx->d_desc.ensure(tiles.size() * sizeof(StreamDesc)), "set_transitions: alloc descriptors");
+        CU(ctx->d_screen.ensure(sizeof(ScreenResult)), "set_transitions: alloc screening result");
         if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "set_transitions: event");
-        // fold every tile into a staging stream that holds ALL prescreened pairs
+        // S3: fold every tile into a staging stream that holds ALL prescreened pairs (class-sorted) and the bounds B_P
         for (size_t it = 0; it < tiles.size(); ++it) {
             TileStream& t = tiles[it];
             FoldArgs a = {};
@@ -424,81 +461,54 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T)
             }
             a.class_first[kNClasses] = hs.class_first[kNClasses];
             CU(ctx->staging[it].ensure(std::max<unsigned long long>(64, off)), "set_transitions: alloc staging");
+            CU(ctx->packed[it].ensure(std::max<unsigned long long>(64, off)), "set_transitions: alloc packed");
             a.staging = static_cast<char*>(ctx->staging[it].p);
             CU(launch_fold(a, st), "set_transitions: fold kernel");
-            t.base = a.staging;
-            t.bytes = off;
+            t.staging = a.staging;
+            t.staging_bytes = off;
+            t.base = static_cast<char*>(ctx->packed[it].p);
+            t.desc = static_cast<StreamDesc*>(ctx->d_desc.p) + it;
+        }
+        // screening on the device (reading #12): B_P < max(screen_tol * mean(B), threshold_eps * max(B)) is dropped; stable
+        // compaction; then every tile's kept records are packed and its descriptor written.  No device->host round trip.
+        ScreenArgs sa = {};
+        sa.bound = static_cast<const double*>(ctx->d_bound.p);
+        sa.n_pairs = np;
+        for (int c = 0; c <= kNClasses; ++c) sa.class_first[c] = hs.class_first[c];
+        sa.screen_tol = ctx->screen_tol;
+        sa.threshold_eps = ctx->threshold_eps;
+        sa.keep_idx = static_cast<int*>(ctx->d_keep.p);
+        sa.result = static_cast<ScreenResult*>(ctx->d_screen.p);
+        CU(launch_screen(sa, st), "set_transitions: screen kernel");
+        for (size_t it = 0; it < tiles.size(); ++it) {
+            const TileStream& t = tiles[it];
+            PackArgs pa = {};
+            pa.staging = t.staging;
+            pa.packed = t.base;
+            pa.keep_idx = sa.keep_idx;
+            pa.result = sa.result;
+            pa.desc = t.desc;
+            pa.n_pairs = np;
+            unsigned long long off = 0;
             for (int c = 0; c < kNClasses; ++c) {
-                t.cls[c].n = hs.class_count[c];
-                t.cls[c].off = a.cls_off[c];
-                t.cls[c].rec_bytes = a.rec_bytes[c];
+                pa.class_first[c] = hs.class_first[c];
+                pa.cls_off[c] = off;
+                pa.rec_bytes[c] = rec_doubles(c, t.NS) * 8;
+                off += (unsigned long long)hs.class_count[c] * pa.rec_bytes[c];
             }
+            pa.class_first[kNClasses] = hs.class_first[kNClasses];
+            CU(launch_pack(pa, st), "set_transitions: pack kernel");
         }
-        // screening: B_P < screen_tol * mean(B) is dropped (rigorous: total dropped <= screen_tol * sum B)
-        std::vector<double> bound((size_t)np);
-        CU(cudaMemcpyAsync(bound.data(), ctx->d_bound.p, (size_t)np * sizeof(double), cudaMemcpyDeviceToHost, st), "set_transitions: read bounds");
-        CU(cudaStreamSynchronize(st), "set_transitions: sync");
-        double sumB = 0.0;
-        for (double b : bound) {
-            if (!std::isfinite(b)) return fail(ctx, SCARF_EINVAL, "set_transitions: NaN/Inf produced by T (device input not finite?)");
-            sumB += b;
-        }
-        double maxB = 0.0;
-        for (double b : bound) maxB = std::max(maxB, b);
-        // default: B_P < screen_tol * mean(B); NEXT-2 option (paper-style): B_P < threshold_eps * max(B)
-        const double thr = std::max(np > 0 ? ctx->screen_tol * sumB / (double)np : 0.0, ctx->threshold_eps * maxB);
-        double dropped_bound = 0.0;
-        for (double b : bound)
-            if (!(b > 0.0 && b >= thr)) dropped_bound += b;
-        std::vector<unsigned long long> src, dst;
-        std::vector<int> nb;
-        long long kept_per_class[kNClasses] = {};
-        std::vector<long long> kept_idx;
-        kept_idx.reserve((size_t)np);
-        for (int c = 0; c < kNClasses; ++c)
-            for (long long i = hs.class_first[c]; i < hs.class_first[c + 1]; ++i)
-                if (bound[(size_t)i] > 0.0 && bound[(size_t)i] >= thr) {
-                    kept_idx.push_back(i);
-                    ++kept_per_class[c];
-                }
-        const long long n_kept = (long long)kept_idx.size();
-        if (n_kept < np) {
-            src.resize((size_t)n_kept); dst.resize((size_t)n_kept); nb.resize((size_t)n_kept);
-            CU(ctx->d_src.ensure(std::max<size_t>(64, (size_t)n_kept * 8)), "set_transitions: alloc");
-            CU(ctx->d_dst.ensure(std::max<size_t>(64, (size_t)n_kept * 8)), "set_transitions: alloc");
-            CU(ctx->d_nb.ensure(std::max<size_t>(64, (size_t)n_kept * 4)), "set_transitions: alloc");
-            for (size_t it = 0; it < tiles.size(); ++it) {
-                TileStream& t = tiles[it];
-                unsigned long long off = 0, new_off[kNClasses];
-                for (int c = 0; c < kNClasses; ++c) {
-                    new_off[c] = off;
-                    off += (unsigned long long)kept_per_class[c] * t.cls[c].rec_bytes;
-                }
-                size_t k = 0;
-                for (int c = 0; c < kNClasses; ++c) {
-                    long long j = 0;
-                    for (; k < kept_idx.size() && kept_idx[k] < hs.class_first[c + 1]; ++k, ++j) {
-                        src[k] = t.cls[c].off + (unsigned long long)(kept_idx[k] - hs.class_first[c]) * t.cls[c].rec_bytes;
-                        dst[k] = new_off[c] + (unsigned long long)j * t.cls[c].rec_bytes;
-                        nb[k] = t.cls[c].rec_bytes;
-                    }
-                }
-                CU(ctx->packed[it].ensure(std::max<unsigned long long>(64, off)), "set_transitions: alloc packed");
-                CU(cudaMemcpyAsync(ctx->d_src.p, src.data(), (size_t)n_kept * 8, cudaMemcpyHostToDevice, st), "set_transitions: upload");
-                CU(cudaMemcpyAsync(ctx->d_dst.p, dst.data(), (size_t)n_kept * 8, cudaMemcpyHostToDevice, st), "set_transitions: upload");
-                CU(cudaMemcpyAsync(ctx->d_nb.p, nb.data(), (size_t)n_kept * 4, cudaMemcpyHostToDevice, st), "set_transitions: upload");
-                CU(launch_pack(static_cast<const char*>(ctx->staging[it].p), static_cast<char*>(ctx->packed[it].p),
-                               static_cast<const unsigned long long*>(ctx->d_src.p), static_cast<const unsigned long long*>(ctx->d_dst.p),
-                               static_cast<const int*>(ctx->d_nb.p), n_kept, st), "set_transitions: pack kernel");
-                CU(cudaStreamSynchronize(st), "set_transitions: sync");  // src/dst/nb host vectors are reused per tile
-                t.base = static_cast<char*>(ctx->packed[it].p);
-                t.bytes = off;
-                for (int c = 0; c < kNClasses; ++c) {
-                    t.cls[c].n = kept_per_class[c];
-                    t.cls[c].off = new_off[c];
-                }
-            }
-        }
+        CU(cudaMemcpyAsync(ctx->h_screen, ctx->d_screen.p, sizeof(ScreenResult), cudaMemcpyDeviceToHost, st), "set_transitions: result copy");
+        CU(cudaEventRecord(ctx->ev_screen, st), "set_transitions: event");
+        ctx->screen_pending = true;
+        ctx->T_bad = false;
+        ctx->tiles = tiles;
+        ctx->n_states = n_states;
+        scarf_stats& s = ctx->st;
+        s.n_states = n_states;
+        s.n_pairs_kept = -1;      // unknown until harvested (scarf_get_stats waits for it)
+        s.last_fold_launches = (int32_t)(2 * tiles.size() + 1 + (ctx->any_pure ? 1 : 0));
         if (ctx->timing) {
             CU(cudaEventRecord(ctx->ev1, st), "set_transitions: event");
             CU(cudaEventSynchronize(ctx->ev1), "set_transitions: event sync");
@@ -506,21 +516,6 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T)
             cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
             ctx->st.last_fold_ms = ms;
         }
-        ctx->tiles = tiles;
-        ctx->n_states = n_states;
-        scarf_stats& s = ctx->st;
-        s.n_states = n_states;
-        s.n_pairs_kept = n_kept;
-        s.dropped_bound = dropped_bound;
-        s.n_herm_kept = 0; s.slots_per_q = 0.0; s.stream_bytes = 0.0;
-        for (int c = 0; c < kNClasses; ++c) {
-            s.pairs_kept_per_class[c] = kept_per_class[c];
-            s.n_herm_kept += kept_per_class[c] * nherm(c);
-            s.slots_per_q += (double)kept_per_class[c] * ((double)n_states * kW[c] + kCtr * (double)tiles.size());
-        }
-        for (const auto& t : tiles) s.stream_bytes += (double)t.bytes;
-        s.evals_per_q = (double)n_kept * (double)n_states;
-        s.last_fold_launches = (int32_t)(tiles.size() * (n_kept < np ? 2 : 1));
         ctx->have_T = true;
         return SCARF_OK;
     } catch (const std::bad_alloc&) {
@@ -541,6 +536,8 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
     try {
         CU(cudaSetDevice(ctx->device), "form_factors");
         cudaStream_t st = ctx->stream;
+        if (harvest_screen(ctx, false) != SCARF_OK) return SCARF_ECUDA;
+        if (ctx->T_bad) return fail(ctx, SCARF_EINVAL, std::string("form_factors: ") + kBadT);
         const size_t qbytes = (size_t)n_q * 3 * sizeof(double);
         const size_t obytes = (size_t)ctx->n_states * (size_t)n_q * 2 * sizeof(double);
         const double* dq = q;
@@ -558,44 +555,34 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
         }
         if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "form_factors: event");
         int launches = 0;
+        double main_ms = 0.0;
         // all state tiles for the q range [dq, dq + 3 n_q) into dout [n_states][n_q]
         auto run_range = [&](const double* dq, long long n_q, double* dout) -> int {
         for (const TileStream& t : ctx->tiles) {
-            long long nrec = 0;
-            for (int L = 0; L < kNClasses; ++L) nrec += t.cls[L].n;
-            double* tile_out = dout + (size_t)t.s0 * n_q * 2;
-            if (nrec == 0) {  // no pair survived (T == 0): the answer is exactly zero
-                CU(cudaMemsetAsync(tile_out, 0, (size_t)t.ns_real * n_q * 2 * sizeof(double), st), "form_factors: memset");
-                continue;
-            }
             V1Args a = {};
             a.base = t.base;
-            for (int L = 0; L < kNClasses; ++L) a.cls_off[L] = t.cls[L].off;
+            a.desc = t.desc;
             a.q = dq;
             a.n_q = n_q;
             const long long n_tiles = (n_q + v1_tile_q() - 1) / v1_tile_q();
-            if (n_tiles > 0x7fffffffLL / kMaxChunks) return fail(ctx, SCARF_EINVAL, "form_factors: n_q too large for one call");
+            if (n_tiles > 0x7fffffffLL) return fail(ctx, SCARF_EINVAL, "form_factors: n_q too large for one call");
             a.n_tiles = (int)n_tiles;
-            // ~24 waves of CTAs (2 resident per SM) so that the ragged last wave costs a few per cent
-            long long K = ctx->n_chunks_opt > 0 ? ctx->n_chunks_opt : (24LL * 2 * ctx->sm_count + n_tiles / 2) / n_tiles;
-            K = std::max<long long>(1, std::min<long long>(K, kMaxChunks));
-            const size_t per_chunk = (size_t)t.ns_real * (size_t)n_q * 16;
-            while (K > 1 && (double)K * (double)per_chunk > 4e9) --K;  // partial buffer <= 4 GB
-            a.n_chunks = build_chunks(t, (int)K, a.chunks);
+            a.n_chunks = choose_chunks(ctx->sm_count, n_tiles, ctx->n_chunks_opt);
             a.ns_real = t.ns_real;
-            if (a.n_chunks == 1) {
-                a.dst = tile_out;
-                a.chunk_stride = 0;
-                CU(launch_ff_v1(t.NS, a, st), "form_factors: kernel");
-                ++launches;
-            } else {
-                CU(ctx->d_partial.ensure((size_t)a.n_chunks * per_chunk), "form_factors: alloc partials");
-                a.dst = static_cast<double*>(ctx->d_partial.p);
-                a.chunk_stride = (long long)t.ns_real * n_q;
-                CU(launch_ff_v1(t.NS, a, st), "form_factors: kernel");
-                CU(launch_reduce_partials(a.dst, tile_out, a.chunk_stride, a.chunk_stride, a.n_chunks, st), "form_factors: reduce kernel");
-                launches += 2;
+            a.dst = dout + (size_t)t.s0 * n_q * 2;
+            if (int rc = prepare_tickets(ctx, n_tiles, a.n_chunks, st, &a.tickets)) return rc;
+            CU(launch_plan_chunks(t.desc, a.n_chunks, t.ns_real, kCtr, st), "form_factors: chunk planning kernel");
+            if (ctx->timing) CU(cudaEventRecord(ctx->ev_m0, st), "form_factors: event");
+            CU(launch_ff_v1(t.NS, a, st), "form_factors: kernel");
+            if (ctx->timing) {
+                CU(cudaEventRecord(ctx->ev_m1, st), "form_factors: event");
+                CU(cudaEventSynchronize(ctx->ev_m1), "form_factors: event sync");
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, ctx->ev_m0, ctx->ev_m1);
+                main_ms += ms;
             }
+            ctx->st.last_n_chunks = a.n_chunks;
+            launches += 2;
         }
         return SCARF_OK;
         };
@@ -633,6 +620,7 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
             float ms = 0.f;
             cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
             ctx->st.last_kernel_ms = ms;
+            ctx->st.last_main_kernel_ms = main_ms;
         }
         if (out_host && n_slices > 1) {
             CU(cudaStreamSynchronize(ctx->copy_stream), "form_factors: sync copies");
@@ -642,6 +630,10 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
             CU(cudaStreamSynchronize(st), "form_factors: sync");
         } else if (q_host) {
             CU(cudaStreamSynchronize(st), "form_factors: sync");  // pageable q must not be reused before the copy ends
+        }
+        if (out_host || q_host) {                                   // the stream has drained: the screening result is there
+            if (harvest_screen(ctx, true) != SCARF_OK) return SCARF_ECUDA;
+            if (ctx->T_bad) return fail(ctx, SCARF_EINVAL, std::string("form_factors: ") + kBadT);
         }
         return SCARF_OK;
     } catch (const std::bad_alloc&) {
@@ -664,25 +656,43 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
     try {
         CU(cudaSetDevice(ctx->device), "form_factors_grid");
         cudaStream_t st = ctx->stream;
-        const int nbx = (nx + kGridBX - 1) / kGridBX, nby = (ny + kGridBY - 1) / kGridBY, nbz = (nz + kGridBZ - 1) / kGridBZ;
-        const long long n_tiles = (long long)nbx * nby * nbz;
-        if (n_tiles > 0x7fffffffLL / kMaxChunks) return fail(ctx, SCARF_EINVAL, "form_factors_grid: grid too large for one call");
-        // axes -> one device buffer [nx | ny | nz]
+        if (harvest_screen(ctx, false) != SCARF_OK) return SCARF_ECUDA;
+        if (ctx->T_bad) return fail(ctx, SCARF_EINVAL, std::string("form_factors_grid: ") + kBadT);
+        // axes -> one device buffer [nx | ny | nz]; a host copy of every axis decides whether the grid is inversion-symmetric
         const double* ax_in[3] = {qx, qy, qz};
         const int ax_n[3] = {nx, ny, nz};
         CU(ctx->d_axes.ensure(((size_t)nx + ny + nz) * sizeof(double)), "form_factors_grid: alloc axes");
         double* dax[3];
+        std::vector<double> hax[3];
         size_t off = 0;
-        bool any_host_axis = false;
+        bool need_sync = false;
         for (int k = 0; k < 3; ++k) {
             dax[k] = static_cast<double*>(ctx->d_axes.p) + off;
             off += (size_t)ax_n[k];
             const bool host = !is_device_ptr(ax_in[k]);
             if (host && !all_finite(ax_in[k], (size_t)ax_n[k])) return fail(ctx, SCARF_EINVAL, "form_factors_grid: NaN/Inf in an axis");
-            any_host_axis = any_host_axis || host;
+            // pageable host -> device copies of this size are staged by the runtime before the call returns: no sync needed
             CU(cudaMemcpyAsync(dax[k], ax_in[k], (size_t)ax_n[k] * sizeof(double), host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, st),
                "form_factors_grid: copy axis");
+            if (ctx->grid_symmetry) {
+                hax[k].resize((size_t)ax_n[k]);
+                if (host) std::memcpy(hax[k].data(), ax_in[k], (size_t)ax_n[k] * sizeof(double));
+                else {
+                    CU(cudaMemcpyAsync(hax[k].data(), ax_in[k], (size_t)ax_n[k] * sizeof(double), cudaMemcpyDeviceToHost, st),
+                       "form_factors_grid: read axis");
+                    need_sync = true;
+                }
+            }
         }
+        if (need_sync) CU(cudaStreamSynchronize(st), "form_factors_grid: sync");   // device axes: documented in scarf.h
+        // inversion symmetry: every axis antisymmetric, bit for bit (then q -> -q maps grid point i to n_q - 1 - i)
+        bool sym = ctx->grid_symmetry != 0 && nx >= 2;
+        for (int k = 0; k < 3 && sym; ++k)
+            for (int i = 0; i < ax_n[k] && sym; ++i) sym = hax[k][(size_t)i] == -hax[k][(size_t)(ax_n[k] - 1 - i)];
+        const int nx_eval = sym ? (nx + 1) / 2 : nx;
+        const int nbx = (nx_eval + kGridBX - 1) / kGridBX, nby = (ny + kGridBY - 1) / kGridBY, nbz = (nz + kGridBZ - 1) / kGridBZ;
+        const long long n_tiles = (long long)nbx * nby * nbz;
+        if (n_tiles > 0x7fffffffLL) return fail(ctx, SCARF_EINVAL, "form_factors_grid: grid too large for one call");
         const size_t obytes = (size_t)ctx->n_states * (size_t)n_q * 2 * sizeof(double);
         double* dout = out;
         const bool out_host = !is_device_ptr(out);
@@ -692,74 +702,64 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         }
         if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "form_factors_grid: event");
         int launches = 0;
-        double slots = 0.0;
+        double main_ms = 0.0;
         const long long ncol = (long long)nbx * kGridBX + (long long)nby * kGridBY + (long long)nbz * kGridBZ;
+        const long long n_rows = (long long)ctx->hs.pairs.size();    // prescreened pairs: an upper bound of the kept count
         for (const TileStream& t : ctx->tiles) {
             GridArgs a = {};
-            long long nrec = 0;
-            for (int L = 0; L < kNClasses; ++L) {
-                a.class_first[L] = nrec;
-                a.rec_bytes[L] = t.cls[L].rec_bytes;
-                a.v.cls_off[L] = t.cls[L].off;
-                nrec += t.cls[L].n;
-                slots += (double)t.cls[L].n * ((double)n_q * ((double)t.ns_real * kW[L] + kCtrGrid) + (double)(nx + ny + nz) * kCtrTable);
-            }
-            double* tile_out = dout + (size_t)t.s0 * n_q * 2;
-            if (nrec == 0) {
-                CU(cudaMemsetAsync(tile_out, 0, (size_t)t.ns_real * n_q * 2 * sizeof(double), st), "form_factors_grid: memset");
-                continue;
-            }
-            const size_t tab_elems = (size_t)nrec * (size_t)ncol;
+            const size_t tab_elems = (size_t)std::max<long long>(1, n_rows) * (size_t)ncol;
             if (tab_elems * 16 > (size_t)32e9) return fail(ctx, SCARF_ENOMEM, "form_factors_grid: factor tables would exceed 32 GB");
             CU(ctx->d_tab.ensure(tab_elems * 16), "form_factors_grid: alloc tables");
             double2* tx = static_cast<double2*>(ctx->d_tab.p);
-            double2* ty = tx + (size_t)nrec * nbx * kGridBX;
-            double2* tz = ty + (size_t)nrec * nby * kGridBY;
+            double2* ty = tx + (size_t)n_rows * nbx * kGridBX;
+            double2* tz = ty + (size_t)n_rows * nby * kGridBY;
             a.v.base = t.base;
+            a.v.desc = t.desc;
             a.v.n_q = n_q;
             a.v.n_tiles = (int)n_tiles;
             a.v.ns_real = t.ns_real;
+            a.v.dst = dout + (size_t)t.s0 * n_q * 2;
             a.qx = dax[0]; a.qy = dax[1]; a.qz = dax[2];
             a.nx = nx; a.ny = ny; a.nz = nz;
             a.nbx = nbx; a.nby = nby; a.nbz = nbz;
+            a.sym = sym ? 1 : 0;
+            a.nx_eval = nx_eval;
             a.tx = tx; a.ty = ty; a.tz = tz;
-            a.n_rec = nrec;
+            a.n_rows = n_rows;
+            a.v.n_chunks = choose_chunks(ctx->sm_count, n_tiles, ctx->n_chunks_opt);
+            if (int rc = prepare_tickets(ctx, n_tiles, a.v.n_chunks, st, &a.v.tickets)) return rc;
             CU(launch_grid_tables(a, tx, ty, tz, st), "form_factors_grid: table kernel");
-            ++launches;
-            long long K = ctx->n_chunks_opt > 0 ? ctx->n_chunks_opt : (24LL * 2 * ctx->sm_count + n_tiles / 2) / n_tiles;
-            K = std::max<long long>(1, std::min<long long>(K, kMaxChunks));
-            const size_t per_chunk = (size_t)t.ns_real * (size_t)n_q * 16;
-            while (K > 1 && (double)K * (double)per_chunk > 4e9) --K;
-            a.v.n_chunks = build_chunks(t, (int)K, a.v.chunks, kCtrGrid);
-            if (a.v.n_chunks == 1) {
-                a.v.dst = tile_out;
-                a.v.chunk_stride = 0;
-                CU(launch_ff_grid(t.NS, a, st), "form_factors_grid: kernel");
-                ++launches;
-            } else {
-                CU(ctx->d_partial.ensure((size_t)a.v.n_chunks * per_chunk), "form_factors_grid: alloc partials");
-                a.v.dst = static_cast<double*>(ctx->d_partial.p);
-                a.v.chunk_stride = (long long)t.ns_real * n_q;
-                CU(launch_ff_grid(t.NS, a, st), "form_factors_grid: kernel");
-                CU(launch_reduce_partials(a.v.dst, tile_out, a.v.chunk_stride, a.v.chunk_stride, a.v.n_chunks, st),
-                   "form_factors_grid: reduce kernel");
-                launches += 2;
+            CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, kCtrGrid, st), "form_factors_grid: chunk planning kernel");
+            if (ctx->timing) CU(cudaEventRecord(ctx->ev_m0, st), "form_factors_grid: event");
+            CU(launch_ff_grid(t.NS, a, st), "form_factors_grid: kernel");
+            if (ctx->timing) {
+                CU(cudaEventRecord(ctx->ev_m1, st), "form_factors_grid: event");
+                CU(cudaEventSynchronize(ctx->ev_m1), "form_factors_grid: event sync");
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, ctx->ev_m0, ctx->ev_m1);
+                main_ms += ms;
             }
+            ctx->st.last_n_chunks = a.v.n_chunks;
+            launches += 3;
         }
         ctx->st.last_kernel_launches = launches;
-        ctx->st.last_grid_slots = slots;
+        ctx->grid_eval_points = (double)nx_eval * ny * nz;
+        ctx->grid_table_cols = (double)(nx_eval + ny + nz);
+        ctx->st.last_grid_symmetric = sym ? 1 : 0;
+        ctx->st.last_grid_slots = -1.0;            // filled by scarf_get_stats from the kept counts
         if (ctx->timing) {
             CU(cudaEventRecord(ctx->ev1, st), "form_factors_grid: event");
             CU(cudaEventSynchronize(ctx->ev1), "form_factors_grid: event sync");
             float ms = 0.f;
             cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
             ctx->st.last_kernel_ms = ms;
+            ctx->st.last_main_kernel_ms = main_ms;
         }
         if (out_host) {
             CU(cudaMemcpyAsync(out, dout, obytes, cudaMemcpyDeviceToHost, st), "form_factors_grid: download out");
             CU(cudaStreamSynchronize(st), "form_factors_grid: sync");
-        } else if (any_host_axis) {
-            CU(cudaStreamSynchronize(st), "form_factors_grid: sync");  // pageable axes must not be reused before the copy ends
+            if (harvest_screen(ctx, true) != SCARF_OK) return SCARF_ECUDA;
+            if (ctx->T_bad) return fail(ctx, SCARF_EINVAL, std::string("form_factors_grid: ") + kBadT);
         }
         return SCARF_OK;
     } catch (const std::bad_alloc&) {
@@ -794,28 +794,23 @@ int scarf_separable_integral(scarf_ctx* ctx, int32_t nx, const double* qx, const
         }
         const int per_block = 64;
         int launches = 0;
+        const long long n_rows = (long long)ctx->hs.pairs.size();   // upper bound of the kept count (the kernels read the real one)
         for (const TileStream& t : ctx->tiles) {
-            GridArgs a = {};
-            long long nrec = 0;
-            for (int L = 0; L < kNClasses; ++L) {
-                a.class_first[L] = nrec;
-                a.rec_bytes[L] = t.cls[L].rec_bytes;
-                a.v.cls_off[L] = t.cls[L].off;
-                nrec += t.cls[L].n;
-            }
             for (int k = 0; k < t.ns_real; ++k) out[2 * (t.s0 + k)] = out[2 * (t.s0 + k) + 1] = 0.0;
-            if (nrec == 0) continue;
+            if (n_rows == 0) continue;
+            GridArgs a = {};
             a.v.base = t.base;
+            a.v.desc = t.desc;
             a.v.ns_real = t.ns_real;
             a.qx = d[0]; a.qy = d[1]; a.qz = d[2];
             a.nx = nx; a.ny = ny; a.nz = nz;
-            a.n_rec = nrec;
-            const size_t n_blocks = (size_t)((nrec + per_block - 1) / per_block);
-            const size_t mom_bytes = (size_t)nrec * 3 * kNClasses * 16, part_bytes = n_blocks * 16 * 16;
+            a.n_rows = n_rows;
+            const size_t n_blocks = (size_t)((n_rows + per_block - 1) / per_block);
+            const size_t mom_bytes = (size_t)n_rows * 3 * kNClasses * 16, part_bytes = n_blocks * 16 * 16;
             CU(ctx->d_tab.ensure(mom_bytes + part_bytes), "separable_integral: alloc scratch");
             double* mom = static_cast<double*>(ctx->d_tab.p);
             double* part = mom + mom_bytes / 8;
-            CU(launch_separable(a, t.NS, d[3], d[4], d[5], mom, part, per_block, st), "separable_integral: kernels");
+            CU(launch_separable(a, d[3], d[4], d[5], mom, part, per_block, st), "separable_integral: kernels");
             launches += 2;
             std::vector<double> hp(n_blocks * 32);
             CU(cudaMemcpyAsync(hp.data(), part, part_bytes, cudaMemcpyDeviceToHost, st), "separable_integral: download");
@@ -857,29 +852,48 @@ int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t
         CU(cudaSetDevice(ctx->device), "angular_moments");
         cudaStream_t st = ctx->stream;
         const long long n_rows = n_sr * n_theta;
-        const int n_m = 2 * l_max + 1, nlm = (l_max + 1) * (l_max + 1), nhalf = (l_max + 1) * (l_max + 2) / 2;
-        std::vector<double> Yw, tw;
-        angular_host_tables(l_max, n_theta, cos_theta, w_theta, n_phi, Yw, tw);
-        // tables: [tw (read as double2: first, 16-byte aligned) | Yw | w_theta]
-        const size_t tab_doubles = Yw.size() + tw.size() + (size_t)n_theta;
-        CU(ctx->d_ang_tab.ensure(tab_doubles * sizeof(double)), "angular_moments: alloc tables");
+        const int n_m = 2 * l_max + 1, nlm = (l_max + 1) * (l_max + 1);
+        // host tables, cached in the context: rebuilt and uploaded only when the nodes, weights, n_phi or l_max change
+        AngularCache& ac = ctx->ang;
+        const bool same = ac.valid && ac.n_phi == n_phi && ac.l_max == l_max && (int)ac.ct.size() == n_theta &&
+                          std::memcmp(ac.ct.data(), cos_theta, sizeof(double) * (size_t)n_theta) == 0 &&
+                          std::memcmp(ac.wt.data(), w_theta, sizeof(double) * (size_t)n_theta) == 0;
+        if (!same) {
+            ac.valid = false;
+            ac.ct.assign(cos_theta, cos_theta + n_theta);
+            ac.wt.assign(w_theta, w_theta + n_theta);
+            ac.n_phi = n_phi; ac.l_max = l_max;
+            angular_host_tables(l_max, n_theta, cos_theta, w_theta, n_phi, ac.Yw, ac.tw);
+            angular_fragment_table(l_max, n_phi, ac.Bf, ac.n_nt, ac.n_ks);
+            angular_transpose_table(l_max, n_theta, ac.Yw, ac.YwT);
+            // device layout (tw, Bf, YwT have even lengths: every block stays 16-byte aligned): [tw | Bf | YwT | Yw | w_theta]
+            const size_t tab_doubles = ac.tw.size() + ac.Bf.size() + ac.YwT.size() + ac.Yw.size() + (size_t)n_theta;
+            CU(ctx->d_ang_tab.ensure(tab_doubles * sizeof(double)), "angular_moments: alloc tables");
+            double* base = static_cast<double*>(ctx->d_ang_tab.p);
+            // pageable sources are staged by the runtime before each call returns; the cached vectors outlive the copies anyway
+            CU(cudaMemcpyAsync(base, ac.tw.data(), ac.tw.size() * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
+            CU(cudaMemcpyAsync(base + ac.tw.size(), ac.Bf.data(), ac.Bf.size() * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
+            double* p = base + ac.tw.size() + ac.Bf.size();
+            CU(cudaMemcpyAsync(p, ac.YwT.data(), ac.YwT.size() * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
+            p += ac.YwT.size();
+            CU(cudaMemcpyAsync(p, ac.Yw.data(), ac.Yw.size() * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
+            p += ac.Yw.size();
+            CU(cudaMemcpyAsync(p, w_theta, (size_t)n_theta * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
+            ac.valid = true;
+        }
         double* dtw = static_cast<double*>(ctx->d_ang_tab.p);
-        double* dYw = dtw + tw.size();
-        double* dw = dYw + Yw.size();
-        CU(cudaMemcpyAsync(dYw, Yw.data(), Yw.size() * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
-        CU(cudaMemcpyAsync(dtw, tw.data(), tw.size() * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
-        CU(cudaMemcpyAsync(dw, w_theta, (size_t)n_theta * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
+        double* dBf = dtw + ac.tw.size();
+        double* dYwT = dBf + ac.Bf.size();
+        double* dYw = dYwT + ac.YwT.size();
+        double* dw = dYw + ac.Yw.size();
         const size_t fbytes = (size_t)n_rows * n_phi * 2 * sizeof(double);
         const double* df = f;
-        if (!is_device_ptr(f)) {
+        const bool f_host = !is_device_ptr(f);
+        if (f_host) {
             CU(ctx->d_ang_in.ensure(fbytes), "angular_moments: alloc f");
             CU(cudaMemcpyAsync(ctx->d_ang_in.p, f, fbytes, cudaMemcpyHostToDevice, st), "angular_moments: upload f");
             df = static_cast<const double*>(ctx->d_ang_in.p);
         }
-        // scratch: F [n_rows][n_m] complex, rowsum2 [n_rows]
-        CU(ctx->d_ang_F.ensure(((size_t)n_rows * n_m * 2 + (size_t)n_rows) * sizeof(double)), "angular_moments: alloc scratch");
-        double* dF = static_cast<double*>(ctx->d_ang_F.p);
-        double* drow2 = dF + (size_t)n_rows * n_m * 2;
         const size_t rbytes = (size_t)n_sr * nlm * 2 * sizeof(double), f2bytes = (size_t)n_sr * sizeof(double);
         const bool R_host = !is_device_ptr(R_out), f2_host = f2_out && !is_device_ptr(f2_out);
         double *dR = R_out, *df2 = f2_out;
@@ -888,11 +902,28 @@ int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t
             if (R_host) dR = static_cast<double*>(ctx->d_ang_out.p);
             if (f2_host) df2 = static_cast<double*>(ctx->d_ang_out.p) + (size_t)n_sr * nlm * 2;
         }
-        (void)nhalf;
         if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "angular_moments: event");
-        CU(launch_phi_dft(df, dtw, n_rows, n_phi, l_max, dF, drow2, st), "angular_moments: phi kernel");
-        CU(launch_legendre(dF, drow2, dYw, dw, n_sr, n_theta, l_max, dR, df2, st), "angular_moments: legendre kernel");
-        ctx->st.last_kernel_launches = 2;
+        // route: fused tensor-core kernel (F rows of one (state, r) in shared memory); for shapes whose F does not fit, the
+        // same kernel writes F to global memory and legendre_kernel finishes; if even the cos/sin fragments do not fit, SIMT
+        const size_t smem_fused = angular_fused_smem(n_theta, l_max, ac.n_nt, ac.n_ks, true);
+        const size_t smem_unfused = angular_fused_smem(n_theta, l_max, ac.n_nt, ac.n_ks, false);
+        if (ctx->angular_variant == 1 && smem_fused <= (size_t)kAngularMaxSmem) {
+            CU(launch_angular_fused(df, dBf, dYwT, dw, n_sr, n_theta, n_phi, l_max, ac.n_nt, ac.n_ks, dR, df2, nullptr, nullptr, st),
+               "angular_moments: fused kernel");
+            ctx->st.last_kernel_launches = 1;
+        } else {
+            // scratch: F [n_rows][n_m] complex, rowsum2 [n_rows]
+            CU(ctx->d_ang_F.ensure(((size_t)n_rows * n_m * 2 + (size_t)n_rows) * sizeof(double)), "angular_moments: alloc scratch");
+            double* dF = static_cast<double*>(ctx->d_ang_F.p);
+            double* drow2 = dF + (size_t)n_rows * n_m * 2;
+            if (ctx->angular_variant == 1 && smem_unfused <= (size_t)kAngularMaxSmem)
+                CU(launch_angular_fused(df, dBf, dYwT, dw, n_sr, n_theta, n_phi, l_max, ac.n_nt, ac.n_ks, nullptr, nullptr, dF, drow2, st),
+                   "angular_moments: phi kernel (DMMA)");
+            else
+                CU(launch_phi_dft(df, dtw, n_rows, n_phi, l_max, dF, drow2, st), "angular_moments: phi kernel");
+            CU(launch_legendre(dF, drow2, dYw, dw, n_sr, n_theta, l_max, dR, df2, st), "angular_moments: legendre kernel");
+            ctx->st.last_kernel_launches = 2;
+        }
         if (ctx->timing) {
             CU(cudaEventRecord(ctx->ev1, st), "angular_moments: event");
             CU(cudaEventSynchronize(ctx->ev1), "angular_moments: event sync");
@@ -902,14 +933,57 @@ int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t
         }
         if (R_host) CU(cudaMemcpyAsync(R_out, dR, rbytes, cudaMemcpyDeviceToHost, st), "angular_moments: download R");
         if (f2_host) CU(cudaMemcpyAsync(f2_out, df2, f2bytes, cudaMemcpyDeviceToHost, st), "angular_moments: download f2");
-        // the host tables (Yw, tw) are pageable and go out of scope: the copies must have finished
-        CU(cudaStreamSynchronize(st), "angular_moments: sync");
+        // host buffers: the copies must have finished before the caller reads / reuses them; all-device calls stay asynchronous
+        if (R_host || f2_host || f_host) CU(cudaStreamSynchronize(st), "angular_moments: sync");
         return SCARF_OK;
     } catch (const std::bad_alloc&) {
         return fail(ctx, SCARF_ENOMEM, "angular_moments: out of host memory");
     } catch (...) {
         return fail(ctx, SCARF_EINVAL, "angular_moments: unexpected exception");
     }
+}
+
+/* Eq. (81)-(82) PAPER.md:591-596: least-squares fit  <|f_s|^2>_Omega(q) ~ A + B q^2 + C q^4  over the points with
+ * |q| <= q_max (all points if q_max <= 0).  HOST arrays.  Normal equations in the scaled variable x = (q / q_ref)^2,
+ * q_ref = the largest |q| used, solved by Gaussian elimination with partial pivoting. */
+int scarf_oscillator_fit(int32_t n_states, int32_t n_r, const double* q_abs, const double* f2, double q_max, double* coef_out)
+{
+    if (n_states < 0 || n_r < 1 || !q_abs || !f2 || !coef_out) return SCARF_EINVAL;
+    if (!all_finite(q_abs, (size_t)n_r) || !all_finite(f2, (size_t)n_states * n_r) || !std::isfinite(q_max)) return SCARF_EINVAL;
+    std::vector<int> use;
+    double q_ref = 0.0;
+    for (int i = 0; i < n_r; ++i)
+        if (q_max <= 0.0 || std::fabs(q_abs[i]) <= q_max) {
+            use.push_back(i);
+            q_ref = std::max(q_ref, std::fabs(q_abs[i]));
+        }
+    if (use.size() < 3 || !(q_ref > 0.0)) return SCARF_EINVAL;    // three unknowns
+    for (int s = 0; s < n_states; ++s) {
+        double N[3][4] = {};
+        for (int i : use) {
+            const double x = (q_abs[i] / q_ref) * (q_abs[i] / q_ref), b[3] = {1.0, x, x * x}, y = f2[(size_t)s * n_r + i];
+            for (int r = 0; r < 3; ++r) {
+                for (int c = 0; c < 3; ++c) N[r][c] += b[r] * b[c];
+                N[r][3] += b[r] * y;
+            }
+        }
+        for (int c = 0; c < 3; ++c) {
+            int piv = c;
+            for (int r = c + 1; r < 3; ++r)
+                if (std::fabs(N[r][c]) > std::fabs(N[piv][c])) piv = r;
+            if (!(std::fabs(N[piv][c]) > 0.0)) return SCARF_EINVAL;    // fewer than three distinct |q|
+            for (int k = 0; k < 4; ++k) std::swap(N[c][k], N[piv][k]);
+            for (int r = 0; r < 3; ++r)
+                if (r != c) {
+                    const double m = N[r][c] / N[c][c];
+                    for (int k = c; k < 4; ++k) N[r][k] -= m * N[c][k];
+                }
+        }
+        coef_out[3 * s + 0] = N[0][3] / N[0][0];
+        coef_out[3 * s + 1] = N[1][3] / N[1][1] / (q_ref * q_ref);
+        coef_out[3 * s + 2] = N[2][3] / N[2][2] / (q_ref * q_ref * q_ref * q_ref);
+    }
+    return SCARF_OK;
 }
 
 int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, const double* x_min, const double* box_len,
@@ -972,10 +1046,24 @@ int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, c
             }
         }
         CU(cudaStreamSynchronize(st), "fft_form_factors: sync");   // `first` (pageable) goes out of scope; cuFFT plans below
+        // Parseval check (Eq. 75), option "check_parseval": V_pix sum_abc |Phi|^2 now, (1 / V_box) sum_q |f|^2 after the transform
+        double* dpar = nullptr;
+        const double vbox = box_len[0] * box_len[1] * box_len[2];
+        if (ctx->check_parseval) {
+            CU(ctx->d_parseval.ensure(((size_t)ctx->n_states * 2 + (size_t)ctx->n_states * 256) * sizeof(double)), "fft_form_factors: alloc sums");
+            dpar = static_cast<double*>(ctx->d_parseval.p);
+            CU(launch_sumsq(dF, g.P, ctx->n_states, vbox / (double)g.P, dpar + 2 * ctx->n_states, dpar, 2, 0, st), "fft_form_factors: Parseval sum");
+        }
         const int frc = cufft_inverse_batch(ctx->fft_plan, dF, nx, ny, nz, ctx->n_states, st);
         if (frc < 0) return fail(ctx, SCARF_ECUDA, "fft_form_factors: the cuFFT library (libcufft.so.11) could not be loaded");
         if (frc > 0) return fail(ctx, frc == 2 ? SCARF_ENOMEM : SCARF_ECUDA, "fft_form_factors: cuFFT error " + std::to_string(frc));
         CU(launch_fft_post(dF, g, ctx->n_states, dout, st), "fft_form_factors: post kernel");
+        if (dpar) {
+            CU(launch_sumsq(dout, g.P, ctx->n_states, 1.0 / vbox, dpar + 2 * ctx->n_states, dpar, 2, 1, st), "fft_form_factors: Parseval sum");
+            ctx->parseval_states = ctx->n_states;
+            launches += 4;
+        } else
+            ctx->parseval_states = 0;
         ctx->st.last_kernel_launches = launches + 1;
         if (ctx->timing) {
             CU(cudaEventRecord(ctx->ev1, st), "fft_form_factors: event");
@@ -996,10 +1084,38 @@ int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, c
     }
 }
 
+int scarf_fft_parseval(scarf_ctx* ctx, double* out_host)
+{
+    if (!ctx || !out_host) return SCARF_EINVAL;
+    if (ctx->host_only) return fail(ctx, SCARF_ENODEVICE, "fft_parseval: host-only context");
+    if (ctx->parseval_states <= 0) return fail(ctx, SCARF_ESTATE, "fft_parseval: set option check_parseval = 1 and call scarf_fft_form_factors first");
+    CU(cudaSetDevice(ctx->device), "fft_parseval");
+    CU(cudaMemcpyAsync(out_host, ctx->d_parseval.p, (size_t)ctx->parseval_states * 2 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream),
+       "fft_parseval: download");
+    CU(cudaStreamSynchronize(ctx->stream), "fft_parseval: sync");
+    return SCARF_OK;
+}
+
 int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out)
 {
     if (!ctx || !out) return SCARF_EINVAL;
+    if (!ctx->host_only && ctx->screen_pending) {         // the kept counts come back lazily: wait for them here
+        cudaSetDevice(ctx->device);
+        const int rc = harvest_screen(ctx, true);
+        if (rc != SCARF_OK) return rc;
+    }
+    if (ctx->st.last_grid_slots < 0.0 && !ctx->screen_pending) {
+        double slots = 0.0, tab = 0.0;
+        const double nt = (double)ctx->tiles.size();
+        for (int c = 0; c < kNClasses; ++c) {
+            slots += (double)ctx->st.pairs_kept_per_class[c] * ctx->grid_eval_points * ((double)ctx->n_states * kW[c] + nt * kCtrGrid);
+            tab += (double)ctx->st.pairs_kept_per_class[c] * nt * ctx->grid_table_cols * kCtrTable;
+        }
+        ctx->st.last_grid_slots = slots + tab;
+        ctx->st.last_grid_kernel_slots = slots;
+    }
     *out = ctx->st;
+    if (ctx->T_bad) return fail(ctx, SCARF_EINVAL, std::string("get_stats: ") + kBadT);
     return SCARF_OK;
 }
 

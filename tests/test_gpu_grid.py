@@ -175,3 +175,75 @@ def test_separable_integral_full_size_config3(oracle_mod, Scarf, torch_cuda):
         scale = (f.abs() * W3.abs()).sum(dim=(1, 2, 3)).cpu().numpy()
         got = sc.separable_integral(ax, fx, ax, gy, ax, hz)
     assert np.all(np.abs(got - ref) <= 1e-11 * scale), np.max(np.abs(got - ref) / scale)
+
+
+def _all_class_basis():
+    return W.Basis(np.array([[0.1, 0.2, -0.9], [0.3, -0.4, 1.0]]), np.array([0, 0, 0, 0, 1, 1, 1, 1], np.int32),
+                   np.array([0, 1, 2, 3, 0, 1, 2, 3], np.int32), np.array([2, 1, 1, 1, 2, 1, 1, 1], np.int32),
+                   np.array([2.1, 0.4, 1.3, 0.9, 0.7, 1.9, 0.5, 1.1, 0.8, 0.6]),
+                   np.array([0.5, 0.6, 1.0, 1.0, 1.0, 0.7, 0.4, 1.0, 1.0, 1.0]))
+
+
+@pytest.mark.parametrize("shape", [(8, 8, 8), (9, 7, 11), (2, 2, 2), (3, 1, 1), (10, 16, 9), (13, 5, 6)])
+@pytest.mark.parametrize("device_axes", [True, False])
+def test_grid_inversion_symmetry_matches_oracle_on_both_halves(oracle_mod, Scarf, torch_cuda, shape, device_axes):
+    """f_s(-q) = conj f_s(q) (reading #6, Eq. (19)): on an exactly inversion-symmetric product grid only the
+    half ix < ceil(nx/2) is evaluated and the mirror point gets the conjugate.  Even, odd (centre plane its own mirror) and
+    ragged sizes, all classes L = 0..6, 12 states; every point of BOTH halves against the oracle."""
+    torch = torch_cuda
+    b = _all_class_basis()
+    rng = np.random.default_rng(sum(shape))
+    T = rng.normal(size=(12, b.nbf, b.nbf))
+    axes = [W.cartesian_axis(n, 3.0 + k) if n > 1 else np.zeros(1) for k, n in enumerate(shape)]
+    f_ref = oracle_mod.form_factors(b, T, expand(*axes))
+    f, st = grid_ff(Scarf, torch, b, T, *axes, device_axes=device_axes)
+    assert st["last_grid_symmetric"] == 1
+    assert_parity(f, f_ref)
+    assert np.array_equal(f[:, ::-1], np.conj(f))                       # exact mirror relation of the stored values
+    with Scarf(0) as sc:                                                # the plain path gives the same values to round-off
+        sc.set_basis(b)
+        sc.set_transitions(T)
+        sc.set_option("grid_symmetry", 0)
+        f0 = sc.form_factors_grid(*axes)
+        assert sc.stats()["last_grid_symmetric"] == 0
+    assert np.max(np.abs(f0 - f)) <= 1e-13 * np.max(np.abs(f_ref))
+    assert_parity(f0, f_ref)
+
+
+def test_grid_not_symmetric_falls_back(oracle_mod, Scarf, torch_cuda):
+    """One axis off by one ulp, one axis shifted, numpy's plain linspace (not bitwise antisymmetric): the plain path runs."""
+    b = _all_class_basis()
+    rng = np.random.default_rng(5)
+    T = rng.normal(size=(3, b.nbf, b.nbf))
+    sym = W.cartesian_axis(8, 4.0)
+    ulp = sym.copy()
+    ulp[1] = np.nextafter(ulp[1], 10.0)
+    for axes in ((sym, sym, ulp), (sym + 0.25, sym, sym), (sym, np.linspace(-10, 10, 64)[:8], sym)):
+        f, st = grid_ff(Scarf, torch_cuda, b, T, *axes)
+        assert st["last_grid_symmetric"] == 0
+        assert_parity(f, oracle_mod.form_factors(b, T, expand(*axes)))
+
+
+@pytest.mark.parametrize("K", [1, 2, 3, 7, 32])
+def test_chunk_counts_general_and_grid(oracle_mod, Scarf, torch_cuda, K):
+    """Option n_chunks: the pair stream cut into K cost-balanced slices whose partial sums are added by the thread-block
+    cluster in chunk order; every class, more chunks than some classes have records, both S4 kernels, against the oracle."""
+    torch = torch_cuda
+    b = _all_class_basis()
+    rng = np.random.default_rng(40 + K)
+    T = rng.normal(size=(5, b.nbf, b.nbf))
+    q = rng.uniform(-5, 5, size=(700, 3))
+    axes = [np.linspace(-4, 4, 9), np.linspace(-3, 5, 10), np.linspace(-5, 3, 7)]
+    f_ref = oracle_mod.form_factors(b, T, q)
+    g_ref = oracle_mod.form_factors(b, T, expand(*axes))
+    with Scarf(0) as sc:
+        sc.set_basis(b)
+        sc.set_option("n_chunks", K)
+        sc.set_transitions(torch.as_tensor(T, device="cuda"))
+        f = sc.form_factors(torch.as_tensor(q, device="cuda"))
+        g = sc.form_factors_grid(*[torch.as_tensor(a, device="cuda") for a in axes])
+        torch.cuda.synchronize()
+        assert_parity(f.cpu().numpy(), f_ref)
+        assert_parity(g.cpu().numpy(), g_ref)
+        sc.set_transitions(np.zeros_like(T))                            # no record survives: zeros through the same launches
+        assert np.all(sc.form_factors(q) == 0) and np.all(sc.form_factors_grid(*axes) == 0)

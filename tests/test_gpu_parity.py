@@ -274,3 +274,38 @@ def test_host_output_sliced_download_matches_device_output(oracle_mod, Scarf, to
     assert np.max(np.abs(f_host - f_dev) / scale) <= 1e-13
     idx = W.sample_q_indices(q.shape[0], 300, seed=3)
     assert_parity(f_host[:, idx], oracle_mod.form_factors(w.basis, T, q[idx]))
+
+
+def test_device_side_screening_matches_round1_counts(oracle_mod, Scarf, torch_cuda):
+    """set_transitions screens and packs on the device (no host round trip); the kept counts per class of config 3 are the
+    ones the host-side screening of round 1 produced (BENCH_r01.json), and they arrive lazily through scarf_get_stats."""
+    torch = torch_cuda
+    w = W.make_workload(3, oracle_mod.overlap, with_q=False)
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(torch.as_tensor(w.T, device="cuda"))
+        st = sc.stats()
+    assert st["pairs_kept_per_class"][:7] == [3301, 3444, 1877, 464, 55, 0, 0]
+    assert st["n_pairs_kept"] == 9141 and st["n_pairs_all"] == 12880
+    assert st["slots_per_q"] == 1180116.0
+
+
+def test_non_finite_device_T_is_reported(oracle_mod, Scarf, torch_cuda):
+    """Device T is validated on the device: the NaN reaches the output (no silent zeros) and the first call that can see the
+    screening result without stalling the stream reports SCARF_EINVAL."""
+    torch = torch_cuda
+    from paper_2512_18010_b200.binding import ScarfError, SCARF_EINVAL
+    w = W.make_workload(1, oracle_mod.overlap)
+    bad = w.T.copy()
+    bad[0, 1, 2] = np.nan
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(torch.as_tensor(bad, device="cuda"))       # asynchronous: cannot fail here
+        with pytest.raises(ScarfError) as e:
+            sc.stats()
+        assert e.value.code == SCARF_EINVAL
+        with pytest.raises(ScarfError) as e:
+            sc.form_factors(w.q[:8])
+        assert e.value.code == SCARF_EINVAL
+        sc.set_transitions(torch.as_tensor(w.T, device="cuda"))       # a good T clears the condition
+        assert_parity(sc.form_factors(w.q[:64]), oracle_mod.form_factors(w.basis, w.T, w.q[:64]))

@@ -109,3 +109,23 @@ def test_bad_arguments_are_rejected_on_the_host(binding):
                 sc.set_basis(**bad)
         with pytest.raises(binding.ScarfError):
             sc.set_option("no_such_option", 1.0)
+
+
+def test_oscillator_fit_host():
+    """scarf_oscillator_fit (Eq. 81-82): exact recovery of A + B q^2 + C q^4, the q_max cut, more than one
+    state, and the error paths (fewer than three usable radii)."""
+    from paper_2512_18010_b200 import binding
+    q = np.geomspace(0.01, 0.5, 17)
+    coefs = np.array([[1e-9, 0.37, -0.05], [0.0, 2.5, 0.4]])
+    f2 = coefs[:, :1] + coefs[:, 1:2] * q ** 2 + coefs[:, 2:3] * q ** 4
+    out = binding.oscillator_fit(q, f2)
+    np.testing.assert_allclose(out[:, 1:], coefs[:, 1:], rtol=1e-9)
+    np.testing.assert_allclose(out[:, 0], coefs[:, 0], atol=1e-12)
+    f2c = f2 + 3.0 * q ** 6                                  # a q^6 tail: the fit restricted to small q is closer to B
+    full, cut = binding.oscillator_fit(q, f2c)[0], binding.oscillator_fit(q, f2c, q_max=0.05)[0]
+    assert abs(cut[1] - coefs[0, 1]) < abs(full[1] - coefs[0, 1])
+    assert abs(cut[1] - coefs[0, 1]) <= 1e-4 * coefs[0, 1]
+    with pytest.raises(binding.ScarfError):
+        binding.oscillator_fit(q, f2, q_max=0.011)           # two radii left
+    with pytest.raises(binding.ScarfError):
+        binding.oscillator_fit(np.full(5, 0.1), f2[:, :5])   # one distinct |q|
