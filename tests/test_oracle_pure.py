@@ -13,7 +13,7 @@ def opure(oracle_mod):
     return pure
 
 
-@pytest.mark.parametrize("l", [2, 3])
+@pytest.mark.parametrize("l", [2, 3, 4, 5, 6])
 def test_pure_functions_orthonormal_also_when_contracted(oracle_mod, opure, l):
     """2l+1 functions, orthonormal within the shell, for one primitive and for a contracted shell (the matrix is
     built from one primitive: pins the claim that it does not depend on the radial part)."""
@@ -32,7 +32,8 @@ def test_pure_functions_orthonormal_also_when_contracted(oracle_mod, opure, l):
     assert np.max(np.abs(C.T @ S[:nc, nc:])) <= 1e-13
 
 
-@pytest.mark.parametrize("l,m", [(2, -2), (2, 0), (2, 2), (3, -3), (3, -1), (3, 0), (3, 2)])
+@pytest.mark.parametrize("l,m", [(2, -2), (2, 0), (2, 2), (3, -3), (3, -1), (3, 0), (3, 2), (4, -3), (4, 0), (4, 4), (5, -5), (5, 2),
+                                 (6, -6), (6, -1), (6, 0), (6, 5)])
 def test_pure_pair_integral_against_3d_quadrature(oracle_mod, opure, l, m):
     """phi_lm defined DIRECTLY (N r^l Y^real_lm(rhat) e^{-a r^2}, scipy's Y) times an s Gaussian on another centre:
     Int phi_lm phi_s e^{iq.r} d^3r by 3-D trapezoid quadrature against the oracle route (C T C^T through the pinned
