@@ -66,7 +66,7 @@ extern "C" {
 #define SCARF_ECUDA (-4)     /* CUDA runtime error; text in scarf_last_error                                       */
 #define SCARF_ENODEVICE (-5) /* the context was created host-only (device < 0) or no device is usable              */
 
-#define SCARF_MAX_L 3        /* highest shell angular momentum (f); pair classes L = l_a + l_b <= 6                */
+#define SCARF_MAX_L 6        /* highest shell angular momentum (i); pair classes L = l_a + l_b <= 12  */
 #define SCARF_N_CLASSES (2 * SCARF_MAX_L + 1)
 
 typedef struct scarf_ctx scarf_ctx; /* opaque; owns every device buffer it allocates */

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libscarf.so")
 
 SCARF_OK, SCARF_EINVAL, SCARF_ESTATE, SCARF_ENOMEM, SCARF_ECUDA, SCARF_ENODEVICE = 0, -1, -2, -3, -4, -5
-SCARF_MAX_L = 3
+SCARF_MAX_L = 6
 SCARF_N_CLASSES = 2 * SCARF_MAX_L + 1
 _CODES = {-1: "EINVAL", -2: "ESTATE", -3: "ENOMEM", -4: "ECUDA", -5: "ENODEVICE"}
 

@@ -10,14 +10,14 @@
 
 namespace scarf {
 
-constexpr int kMaxL = 3;                    // highest shell angular momentum (f)
+constexpr int kMaxL = 6;                    // highest shell angular momentum (i; "up to i orbitals")
 constexpr int kMaxClass = 2 * kMaxL;        // highest pair class L = la + lb
 constexpr int kNClasses = kMaxClass + 1;
 
 inline constexpr int ncart(int l) { return (l + 1) * (l + 2) / 2; }
 inline constexpr int nherm(int L) { return (L + 1) * (L + 2) * (L + 3) / 6; }
-constexpr int kMaxCart = ncart(kMaxL);      // 10
-constexpr int kMaxHerm = nherm(kMaxClass);  // 84
+constexpr int kMaxCart = ncart(kMaxL);      // 28
+constexpr int kMaxHerm = nherm(kMaxClass);  // 455
 
 struct PrimShell {
     int32_t shell, atom, l, bf0;  // contracted shell it belongs to, centre, angular momentum, first basis function

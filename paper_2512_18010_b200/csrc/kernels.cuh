@@ -121,6 +121,19 @@ struct V1Args {
 int v1_tile_q();                            // q-points per CTA
 cudaError_t launch_ff_v1(int NS, const V1Args& a, cudaStream_t st);
 
+// high classes (ff_highl.cu): pairs with g, h, i shells (L = 7..12); runs after the unrolled kernel and ADDS to out.
+struct HighLArgs {
+    const char* base;                       // tile stream base
+    const StreamDesc* desc;
+    const double* q;                        // list mode: [n_points][3]; nullptr: product-grid mode
+    const double *qx, *qy, *qz;             // grid mode: axes; points = (ix < nx_eval, iy, iz)
+    int nx, ny, nz, nx_eval, sym, ns_real;
+    long long n_points;                     // points evaluated (n_q, or nx_eval*ny*nz)
+    long long n_q;                          // points per state in out
+    double* dst;                            // out + s0*n_q*2
+};
+cudaError_t launch_ff_highl(const HighLArgs& a, cudaStream_t st);
+
 // grid (ff_grid.cu): Cartesian product grid q = (qx[ix], qy[iy], qz[iz]), index (ix*ny + iy)*nz + iz.  The
 // Gaussian/phase factor separates, e^{-q^2/4p} e^{iq.P} = X_P(ix) Y_P(iy) Z_P(iz) (the V-tensor idea of Eq. (45)-(46)
 // PAPER.md:309-316), so it is tabulated once per (pair, axis point) and S4 needs two complex multiplies per

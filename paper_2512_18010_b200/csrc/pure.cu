@@ -1,4 +1,4 @@
-// pure.cu — pure (real solid-harmonic) d and f shells (the paper builds such orbitals as
+// pure.cu — pure (real solid-harmonic) d, f, g, h and i shells (the paper builds such orbitals as
 // several Cartesian terms with prefactors, Eq. (A2), e.g. 3d_{x^2-y^2}).
 //
 // The kernels work in the Cartesian basis.  A pure shell of angular momentum l has 2l+1 functions
@@ -22,34 +22,49 @@ namespace scarf {
 
 namespace {
 
-struct Term { int a, b, c; double w; };
-
-// S_lm as a list of monomial terms (any overall scale: the column is normalised afterwards)
-int solid_harmonic_terms(int l, int m, Term* t)
+// Coefficients w[c] of the Cartesian monomials x^a y^b z^c (component order of the library) in the real solid harmonic
+// S_lm, any overall scale (the column is normalised afterwards), from the closed form
+//   S_{l, m>=0} = Pi_l^m(z, r^2) A_m(x, y),   S_{l, m<0} = Pi_l^{|m|}(z, r^2) B_{|m|}(x, y),
+//   A_m + i B_m = (x + i y)^m,
+//   Pi_l^m = sum_{k=0}^{floor((l-m)/2)} (-1)^k C(l,k) C(2l-2k, l) (l-2k)!/(l-2k-m)! r^{2k} z^{l-2k-m},   r^2 = x^2 + y^2 + z^2,
+// which reproduces the tabulated d and f functions of the header comment (signs included) and extends them to g, h, i.
+// l = 1 keeps the Cartesian order x, y, z (index m + 1 = 0, 1, 2).
+double binom(int n, int k)
 {
-    int n = 0;
-    auto add = [&](int a, int b, int c, double w) { t[n++] = Term{a, b, c, w}; };
-    if (l == 0) { add(0, 0, 0, 1); }
-    else if (l == 1) {                      // kept in the Cartesian order x, y, z (index m + 1 = 0, 1, 2)
-        if (m == -1) add(1, 0, 0, 1);
-        if (m == 0) add(0, 1, 0, 1);
-        if (m == 1) add(0, 0, 1, 1);
-    } else if (l == 2) {
-        if (m == -2) add(1, 1, 0, 1);
-        if (m == -1) add(0, 1, 1, 1);
-        if (m == 0) { add(0, 0, 2, 2); add(2, 0, 0, -1); add(0, 2, 0, -1); }
-        if (m == 1) add(1, 0, 1, 1);
-        if (m == 2) { add(2, 0, 0, 1); add(0, 2, 0, -1); }
-    } else if (l == 3) {
-        if (m == -3) { add(2, 1, 0, 3); add(0, 3, 0, -1); }
-        if (m == -2) add(1, 1, 1, 1);
-        if (m == -1) { add(0, 1, 2, 4); add(2, 1, 0, -1); add(0, 3, 0, -1); }
-        if (m == 0) { add(0, 0, 3, 2); add(2, 0, 1, -3); add(0, 2, 1, -3); }
-        if (m == 1) { add(1, 0, 2, 4); add(3, 0, 0, -1); add(1, 2, 0, -1); }
-        if (m == 2) { add(2, 0, 1, 1); add(0, 2, 1, -1); }
-        if (m == 3) { add(3, 0, 0, 1); add(1, 2, 0, -3); }
+    double r = 1.0;
+    for (int i = 1; i <= k; ++i) r = r * (double)(n - k + i) / (double)i;
+    return r;
+}
+
+void solid_harmonic_coeffs(int l, int m, double* w)   // w[ncart(l)]
+{
+    const int nc = ncart(l);
+    for (int c = 0; c < nc; ++c) w[c] = 0.0;
+    if (l == 0) { w[0] = 1.0; return; }
+    if (l == 1) { w[m + 1] = 1.0; return; }
+    auto comp_index = [&](int a, int b) {              // a descending, then b descending
+        int idx = 0;
+        for (int aa = l; aa > a; --aa) idx += l - aa + 1;
+        return idx + (l - a - b);
+    };
+    const int ma = m < 0 ? -m : m;
+    for (int k = 0; 2 * k <= l - ma; ++k) {
+        double ck = ((k & 1) ? -1.0 : 1.0) * binom(l, k) * binom(2 * l - 2 * k, l);
+        for (int i = 0; i < ma; ++i) ck *= (double)(l - 2 * k - i);      // (l-2k)!/(l-2k-m)!
+        // (x + i y)^ma: term x^p y^(ma-p) carries i^(ma-p); A takes the real part, B the imaginary part
+        for (int p = 0; p <= ma; ++p) {
+            const int e = ma - p;
+            double cp = 0.0;
+            if (m >= 0 && (e & 1) == 0) cp = ((e / 2) & 1) ? -1.0 : 1.0;
+            if (m < 0 && (e & 1) == 1) cp = (((e - 1) / 2) & 1) ? -1.0 : 1.0;
+            if (cp == 0.0) continue;
+            cp *= binom(ma, p);
+            // r^{2k} = sum_{i+j+n=k} k!/(i! j! n!) x^{2i} y^{2j} z^{2n}
+            for (int i = 0; i <= k; ++i)
+                for (int j = 0; i + j <= k; ++j)       // the z power follows: l - a - b
+                    w[comp_index(p + 2 * i, e + 2 * j)] += ck * cp * binom(k, i) * binom(k - i, j);
+        }
     }
-    return n;
 }
 
 double dfact_odd(int n)   // n!! for odd n >= -1
@@ -92,12 +107,9 @@ void pure_matrix(int l, double* C)
         cf[c] = component_factor(l, c);
     }
     for (int m = -l; m <= l; ++m) {
-        Term t[4];
-        const int nt = solid_harmonic_terms(l, m, t);
-        double v[kMaxCart] = {};
-        for (int k = 0; k < nt; ++k)
-            for (int c = 0; c < nc; ++c)
-                if (pw[c][0] == t[k].a && pw[c][1] == t[k].b && pw[c][2] == t[k].c) v[c] += t[k].w / cf[c];
+        double w[kMaxCart], v[kMaxCart] = {};
+        solid_harmonic_coeffs(l, m, w);
+        for (int c = 0; c < nc; ++c) v[c] = w[c] / cf[c];
         double nrm = 0.0;
         for (int c = 0; c < nc; ++c)
             for (int d = 0; d < nc; ++d) {

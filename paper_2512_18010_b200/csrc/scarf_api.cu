@@ -33,7 +33,7 @@ struct DevBuf {
 };
 
 // FP64 issue-slot model: per (q, pair, state) W(L), per (q, pair) C_tr.
-const double kW[kNClasses] = {2, 7, 13, 23, 38, 59, 87};
+const double kW[kNClasses] = {2, 7, 13, 23, 38, 59, 87, 123, 168, 223, 289, 367, 458};   // n_herm(L) + 3 (2 for L = 0)
 const double kCtr = 40.0;
 // product-grid kernel: YZ = Y Z, g0 = X0 YZ, g1 = X1 YZ: 12 slots per 2 q-points; tables: 39 per (pair, axis point)
 const double kCtrGrid = 6.0, kCtrTable = 39.0;
@@ -143,6 +143,13 @@ int choose_chunks(int sm_count, long long n_tiles, int forced)
 {
     long long K = forced > 0 ? forced : (24LL * 2 * sm_count + n_tiles / 2) / std::max<long long>(1, n_tiles);
     return (int)std::max<long long>(1, std::min<long long>(K, kMaxChunks));
+}
+
+bool has_high_classes(const HostSetup& hs)   // any prescreened pair of class > kFastMaxClass (needs ff_highl.cu)
+{
+    for (int c = kFastMaxClass + 1; c < kNClasses; ++c)
+        if (hs.class_count[c] > 0) return true;
+    return false;
 }
 
 // per-tile tickets of the ordered fix-up (ff_common.cuh): zeroed before every multi-chunk launch
@@ -583,6 +590,13 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
             }
             ctx->st.last_n_chunks = a.n_chunks;
             launches += 2;
+            if (has_high_classes(ctx->hs)) {            // pairs with g, h, i shells: separate kernel, adds to out
+                HighLArgs h = {};
+                h.base = t.base; h.desc = t.desc; h.q = dq;
+                h.ns_real = t.ns_real; h.n_points = n_q; h.n_q = n_q; h.dst = a.dst;
+                CU(launch_ff_highl(h, st), "form_factors: high-class kernel");
+                ++launches;
+            }
         }
         return SCARF_OK;
         };
@@ -741,6 +755,15 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
             }
             ctx->st.last_n_chunks = a.v.n_chunks;
             launches += 3;
+            if (has_high_classes(ctx->hs)) {
+                HighLArgs h = {};
+                h.base = t.base; h.desc = t.desc; h.q = nullptr;
+                h.qx = dax[0]; h.qy = dax[1]; h.qz = dax[2];
+                h.nx = nx; h.ny = ny; h.nz = nz; h.nx_eval = nx_eval; h.sym = sym ? 1 : 0;
+                h.ns_real = t.ns_real; h.n_points = (long long)nx_eval * ny * nz; h.n_q = n_q; h.dst = a.v.dst;
+                CU(launch_ff_highl(h, st), "form_factors_grid: high-class kernel");
+                ++launches;
+            }
         }
         ctx->st.last_kernel_launches = launches;
         ctx->grid_eval_points = (double)nx_eval * ny * nz;

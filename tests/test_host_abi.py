@@ -66,20 +66,20 @@ def test_hermite_E_against_quadrature(binding):
     Int ... e^{iqx} dx = sqrt(pi/p) e^{-q^2/4p} e^{iqP} sum_t E_t^{ij} (iq)^t; left side by trapezoid quadrature."""
     a, b, A, B = 0.9, 1.7, -0.4, 0.55
     p, P = a + b, (a * A + b * B) / (a + b)
-    E = binding.host_hermite_E(3, 3, a, b, A, B)
+    E = binding.host_hermite_E(6, 6, a, b, A, B)                      # up to i shells on both sides
     for q in (0.0, 0.8, -2.3):
-        for i in range(4):
-            for j in range(4):
+        for i in range(7):
+            for j in range(7):
                 lhs = BF._int1d(i, A, a, j, B, b, q)
                 rhs = np.sqrt(np.pi / p) * np.exp(-q * q / (4 * p)) * np.exp(1j * q * P) * sum(
                     E[i, j, t] * (1j * q) ** t for t in range(i + j + 1))
-                assert abs(lhs - rhs) <= 1e-12 * max(1.0, abs(lhs)), (q, i, j)
+                assert abs(lhs - rhs) <= 1e-12 * max(1.0, abs(BF._int1d(i, A, a, j, B, b, 0.0)), abs(lhs)), (q, i, j)
 
 
 def test_shell_norms_against_oracle(binding, oracle_mod):
     """Effective coefficients N_mu d_k xi_k of a contracted shell: every component has unit self-overlap."""
     e, d = np.array([2.3, 0.7, 0.25]), np.array([0.4, 0.9, 0.6])
-    for l in range(4):
+    for l in range(7):
         c = binding.host_shell_norms(l, e, d)
         b = W.Basis(np.zeros((1, 3)), np.array([0], np.int32), np.array([l], np.int32), np.array([3], np.int32), e, d)
         xi, N = oracle_mod.norms(b)
@@ -103,7 +103,7 @@ def test_bad_arguments_are_rejected_on_the_host(binding):
     with binding.Scarf(None) as sc:
         good = dict(atom_xyz=np.zeros((1, 3)), shell_atom=[0], shell_l=[0], shell_nprim=[1], exponents=[1.0], coeffs=[1.0])
         sc.set_basis(**good)
-        for bad in (dict(good, shell_l=[4]), dict(good, exponents=[-1.0]), dict(good, shell_atom=[3]),
+        for bad in (dict(good, shell_l=[7]), dict(good, exponents=[-1.0]), dict(good, shell_atom=[3]),
                     dict(good, exponents=[np.nan])):
             with pytest.raises(binding.ScarfError):
                 sc.set_basis(**bad)
@@ -129,3 +129,36 @@ def test_oscillator_fit_host():
         binding.oscillator_fit(q, f2, q_max=0.011)           # two radii left
     with pytest.raises(binding.ScarfError):
         binding.oscillator_fit(np.full(5, 0.1), f2[:, :5])   # one distinct |q|
+
+
+def test_host_overlap_g_h_i_shells(binding, oracle_mod):
+    """Shells up to i (l = 6): S0-S2 on the host against the oracle (itself pinned by quadrature in
+    tests/test_oracle_pins_high_l.py); SCARF_EINVAL beyond l = 6."""
+    from tests.test_oracle_pins_high_l import _ghi_basis
+    b = _ghi_basis()
+    with binding.Scarf(None) as sc:
+        sc.set_basis(b)
+        S = sc.overlap()
+        st = sc.stats()
+    assert st["l_max"] == 6 and st["nbf"] == b.nbf
+    assert np.max(np.abs(S - oracle_mod.overlap(b))) <= 1e-12
+    with binding.Scarf(None) as sc:
+        with pytest.raises(binding.ScarfError) as e:
+            sc.set_basis(atom_xyz=np.zeros((1, 3)), shell_atom=[0], shell_l=[7], shell_nprim=[1], exponents=[1.0], coeffs=[1.0])
+        assert e.value.code == binding.SCARF_EINVAL
+
+
+def test_host_pure_overlap_g_h_i(binding, oracle_mod):
+    """Pure (solid-harmonic) g, h, i shells: 2l+1 functions from the closed-form S_lm (csrc/pure.cu) against the oracle's
+    route (scipy's Y_lm fitted onto the Cartesian components, oracle/pure.py)."""
+    from oracle import pure as opure
+    from tests.test_oracle_pins_high_l import _ghi_basis
+    b = _ghi_basis()
+    flags = np.array([1, 1, 1, 0], np.int32)
+    with binding.Scarf(None) as sc:
+        sc.set_basis(b, shell_pure=flags)
+        assert sc.nbf == 9 + 11 + 13 + 3
+        S = sc.overlap()
+    S_ref = opure.overlap(b, flags)
+    assert np.max(np.abs(S - S_ref)) <= 1e-12
+    assert np.allclose(np.diag(S), 1.0, atol=1e-12)
