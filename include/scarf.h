@@ -94,6 +94,8 @@ typedef struct scarf_stats {
     int32_t last_n_chunks;                     /* stream chunks (= cluster size) of the last S4 launch                */
     double last_main_kernel_ms;                /* "timing": device time of the S4 kernel(s) alone (no tables/planning)*/
     double last_grid_kernel_slots;             /* FP64 issue-slot model of the product-grid S4 kernel alone (no tables)*/
+    double adaptive_bound;                     /* option adaptive_tol: |f_s(q) - exact| <= this for every q, s (0 when off) */
+    double last_adaptive_work_fraction;        /* modelled work of the last S4 call / work without the cut-off (1 when off) */
 } scarf_stats;
 
 /* device >= 0: CUDA ordinal.  device < 0: host-only context (set_basis, overlap, stats work; the rest ENODEVICE). */
@@ -113,6 +115,14 @@ int scarf_set_stream(scarf_ctx* ctx, void* cuda_stream);
  *                         a primitive shell pair is also dropped when B_P < threshold_eps * max_P B_P (B_P already is
  *                         the max over the states, so a pair survives if any transition needs it).  An APPROXIMATION
  *                         whose error is bounded: scarf_stats.dropped_bound.  Takes effect at set_transitions.
+ *           "adaptive_tol": default 0 (off).  q-adaptive evaluation: with tau = adaptive_tol *
+ *                         mean(B), a kept pair P is skipped for the q tiles that lie entirely beyond q_cut(P), the radius
+ *                         past which its rigorous envelope sum_n c_n sup_{q' >= q} q'^n e^{-q'^2/4p} stays below tau
+ *                         (e^{-q^2/4p} kills diffuse pairs at large |q|).  An APPROXIMATION with a reported bound:
+ *                         |f_s(q) - exact| <= scarf_stats.adaptive_bound = n_kept * tau <= adaptive_tol * sum(B) for every
+ *                         q and s; scarf_stats.last_adaptive_work_fraction says how much work was left.  Records are
+ *                         re-ordered by q_cut inside their class (results differ from the default path by round-off
+ *                         even where nothing is skipped).  Takes effect at set_transitions; at most 96 states.
  *           "timing": 1 records CUDA-event times of S3/S4 into the stats (adds a stream sync per call).
  *           "n_chunks": default 0 (automatic).  1..32 forces the number of cost-balanced slices the pair stream is cut
  *                         into (the S4 grid is q-tiles x chunks; the chunks of one q tile add their partial sums into
@@ -199,6 +209,11 @@ int scarf_separable_integral(scarf_ctx* ctx, int32_t nx, const double* qx, const
 int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t n_theta, const double* cos_theta,
                           const double* w_theta, int32_t n_phi, int32_t l_max, const double* f, double* R_out,
                           double* f2_out);
+
+/* S5, the optional output of the hot path: out[i] = |f[i]|^2 for n complex values (what Fig. 6 plots), e.g.
+ * n = n_states * n_q of a form-factor array.  f [n][2], out [n]: host or device pointers, independently; asynchronous on
+ * the context stream when both are device pointers. */
+int scarf_abs2(scarf_ctx* ctx, int64_t n, const double* f, double* out);
 
 /* Oscillator-strength fit, Eq. (81)-(82) PAPER.md:591-596: least squares of  <|f_s|^2>_Omega(q) ~ A + B q^2 + C q^4  over the
  * radial points with |q_abs[i]| <= q_max (q_max <= 0: all of them; at least three distinct |q| are needed).  f2 is the

@@ -19,7 +19,7 @@ SCARF_N_CLASSES = 2 * SCARF_MAX_L + 1
 _CODES = {-1: "EINVAL", -2: "ESTATE", -3: "ENOMEM", -4: "ECUDA", -5: "ENODEVICE"}
 
 EXPORTS = ["scarf_create", "scarf_destroy", "scarf_set_stream", "scarf_set_option", "scarf_set_basis", "scarf_set_basis_pure", "scarf_nbf",
-           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_separable_integral", "scarf_angular_moments", "scarf_oscillator_fit", "scarf_fft_form_factors", "scarf_fft_parseval", "scarf_get_stats", "scarf_last_error",
+           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_separable_integral", "scarf_angular_moments", "scarf_oscillator_fit", "scarf_abs2", "scarf_fft_form_factors", "scarf_fft_parseval", "scarf_get_stats", "scarf_last_error",
            "scarf_version", "scarf_fp64_peak", "scarf_host_hermite_E", "scarf_host_shell_norms", "scarf_host_ylm_table"]
 
 
@@ -34,7 +34,8 @@ class ScarfStats(C.Structure):
                 ("last_kernel_launches", C.c_int32), ("last_fold_launches", C.c_int32),
                 ("last_grid_slots", C.c_double), ("dropped_bound", C.c_double),
                 ("last_grid_symmetric", C.c_int32), ("last_n_chunks", C.c_int32),
-                ("last_main_kernel_ms", C.c_double), ("last_grid_kernel_slots", C.c_double)]
+                ("last_main_kernel_ms", C.c_double), ("last_grid_kernel_slots", C.c_double),
+                ("adaptive_bound", C.c_double), ("last_adaptive_work_fraction", C.c_double)]
 
     def as_dict(self):
         d = {}
@@ -70,6 +71,7 @@ def _load():
     L.scarf_form_factors_grid.argtypes = [vp, C.c_int32, vp, C.c_int32, vp, C.c_int32, vp, vp]
     L.scarf_separable_integral.argtypes = [vp, C.c_int32, dp, dp, C.c_int32, dp, dp, C.c_int32, dp, dp, dp]
     L.scarf_angular_moments.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, C.c_int32, C.c_int32, vp, vp, vp]
+    L.scarf_abs2.argtypes = [vp, C.c_int64, vp, vp]
     L.scarf_oscillator_fit.argtypes = [C.c_int32, C.c_int32, dp, dp, C.c_double, dp]
     L.scarf_host_ylm_table.argtypes = [C.c_int, C.c_int, dp, dp, dp]
     L.scarf_fft_form_factors.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, vp]
@@ -337,6 +339,19 @@ class Scarf:
             import torch
             return torch.view_as_complex(out.view(self.n_states, n_q, 2))
         return out.reshape(self.n_states, n_q, 2).view(np.complex128)[..., 0]
+
+    def abs2(self, f):
+        """|f|^2 elementwise (S5): f complex128 torch (cuda or host) or numpy; returns float64 of the same shape and kind."""
+        if _is_torch(f):
+            import torch
+            fr = torch.view_as_real(f.contiguous())
+            out = torch.empty(f.shape, dtype=torch.float64, device=f.device)
+            self._check(_lib.scarf_abs2(self._h, f.numel(), C.c_void_p(fr.data_ptr()), C.c_void_p(out.data_ptr())))
+            return out
+        fa = np.ascontiguousarray(f, dtype=np.complex128)
+        out = np.empty(fa.shape)
+        self._check(_lib.scarf_abs2(self._h, fa.size, C.c_void_p(fa.ctypes.data), C.c_void_p(out.ctypes.data)))
+        return out
 
     def fft_parseval(self) -> np.ndarray:
         """[n_states][2]: (V_pix sum |Phi|^2, sum |f|^2 / V_box) of the last fft_form_factors call (option check_parseval = 1)."""

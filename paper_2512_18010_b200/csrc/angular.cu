@@ -394,4 +394,20 @@ cudaError_t launch_angular_fused(const double* f, const double* Bf, const double
     return cudaGetLastError();
 }
 
+// S5 (optional output of SURVEY.md §8(a)): |f|^2 of a complex array, what Fig. 6 of the paper plots.
+__global__ void __launch_bounds__(256) abs2_kernel(const double2* __restrict__ f, long long n, double* __restrict__ out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double2 v = f[i];
+    out[i] = fma(v.x, v.x, v.y * v.y);
+}
+
+cudaError_t launch_abs2(const double* f_complex, long long n, double* out, cudaStream_t st)
+{
+    if (n <= 0) return cudaSuccess;
+    abs2_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const double2*>(f_complex), n, out);
+    return cudaGetLastError();
+}
+
 }  // namespace scarf

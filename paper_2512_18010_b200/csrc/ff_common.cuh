@@ -100,6 +100,30 @@ __device__ __forceinline__ void ticket_pass(int* ticket, int next)
     if (threadIdx.x == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(ticket), "r"(next) : "memory");
 }
 
+// ---- q-adaptive cut-off helpers (fold.cu: qcut_kernel) -------------------------------------------------------------------
+// smallest value of x over the CTA's threads (whole-CTA call; `sh` holds one double per warp)
+__device__ __forceinline__ double block_min(double x, double* sh)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x = fmin(x, __shfl_xor_sync(0xffffffffu, x, o));
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = x;
+    __syncthreads();
+    double m = sh[0];
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) m = fmin(m, sh[w]);
+    return m;
+}
+// number of leading entries of the DESCENDING array qc[0..n) that exceed q: the records a tile with smallest |q| = q keeps
+__device__ __forceinline__ int active_prefix(const double* __restrict__ qc, long long n, double q)
+{
+    long long lo = 0, hi = n;                             // invariant: qc[i] > q for i < lo, qc[i] <= q for i >= hi
+    while (lo < hi) {
+        const long long mid = (lo + hi) >> 1;
+        if (qc[mid] > q) lo = mid + 1; else hi = mid;
+    }
+    return (int)lo;
+}
+
 // ---- one record = transcendental part (record_trans) + the (state, h) loop (record_accum) -------------------
 // The two are separate so that run_class can software-pipeline them: the exp/sincos chains of record k+1 (low
 // ILP: two dependent Horner chains per q-point) are issued in the same basic block as the 4 NS n_herm independent

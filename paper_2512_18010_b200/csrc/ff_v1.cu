@@ -165,9 +165,25 @@ __global__ void __launch_bounds__(kThreads, 2) ff_v1_kernel(const V1Args a)
 
     const StreamDesc& d = *a.desc;
     const V1Chunk& ck = d.chunks[chunk];
+    // q-adaptive cut-off: this tile keeps, of every class, the records whose q_cut exceeds its smallest |q|
+    double q_min = 0.0;
+    if (a.qcut != nullptr) {
+        __shared__ double sh_min[kThreads / 32];
+        double m2 = 1e300;
+#pragma unroll
+        for (int j = 0; j < kNQ; ++j)
+            if (iq[j] < a.n_q) m2 = fmin(m2, qv[j][3]);
+        q_min = sqrt(block_min(m2, sh_min));
+    }
+    auto class_records = [&](int L) {
+        int n = ck.n[L];
+        if (a.qcut != nullptr && n > 0) n = max(0, min(n, active_prefix(a.qcut + d.cls_first[L], d.cls_n[L], q_min) - ck.begin[L]));
+        if (a.work != nullptr && threadIdx.x == 0 && n > 0) atomicAdd(a.work + L, (unsigned long long)n);
+        return n;
+    };
 #define SCARF_V1_CLASS(LV)                                                                                              \
-    if (ck.n[LV] > 0)                                                                                                   \
-        run_class<LV, NS>(pp, a.base + d.cls_off[LV] + (size_t)ck.begin[LV] * (rec_doubles(LV, NS) * 8), ck.n[LV], qv, re, im);
+    if (const int n_rec = class_records(LV); n_rec > 0)                                                                 \
+        run_class<LV, NS>(pp, a.base + d.cls_off[LV] + (size_t)ck.begin[LV] * (rec_doubles(LV, NS) * 8), n_rec, qv, re, im);
     SCARF_V1_CLASS(0)
     SCARF_V1_CLASS(1)
     SCARF_V1_CLASS(2)

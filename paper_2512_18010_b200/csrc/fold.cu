@@ -283,6 +283,95 @@ cudaError_t launch_pack(const PackArgs& a, cudaStream_t st)
     return cudaGetLastError();
 }
 
+// ---- q-adaptive cut-off (NEXT-2, second half; PAPER.md:499 thresholding made q-dependent) ----------------------------------
+// A kept pair contributes  |term_P(q)| <= e^{-q^2/4p} sum_n c_n |q|^n,  c_n = sum_{deg h = n} max_s |D^s_h|.  The envelope
+//   U_P(q) = sum_n c_n sup_{q' >= q} q'^n e^{-q'^2/4p}      (each term: its value at q beyond its peak sqrt(2 p n), else the peak)
+// is non-increasing, so q_cut(P) = inf{q : U_P(q) < tau} is well defined and the pair can be skipped for every q-point with
+// |q| >= q_cut at a cost of < tau each.  Records are then sorted by q_cut (descending, stable) inside their class, so that a
+// q tile whose smallest |q| is q_min evaluates a PREFIX of every class: records with q_cut > q_min.  Error per (q, state):
+// < (number of skipped records) * tau <= n_kept * tau, reported as scarf_stats.adaptive_bound.
+__device__ double envelope(const double* c, int L, double p, double q)
+{
+    double u = c[0] * exp(-q * q / (4.0 * p));
+    for (int n = 1; n <= L; ++n) {
+        const double qs = sqrt(2.0 * p * n), qq = q > qs ? q : qs;       // beyond the peak: the value; before it: the peak
+        u += c[n] * pow(qq, (double)n) * exp(-qq * qq / (4.0 * p));
+    }
+    return u;
+}
+
+// one thread per kept record
+__global__ void __launch_bounds__(128) qcut_kernel(const AdaptArgs a)
+{
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const ScreenResult& r = *a.result;
+    if (k >= r.n_kept) return;
+    const long long i = a.keep_idx[k];
+    int c = 0;
+#pragma unroll
+    for (int j = 1; j < kNClasses; ++j)
+        if (i >= a.class_first[j]) c = j;
+    if (c > kFastMaxClass || r.bad) { a.key[k] = 1e300; return; }        // high classes are never cut
+    double cn[kFastMaxClass + 1];
+#pragma unroll
+    for (int n = 0; n <= kFastMaxClass; ++n) cn[n] = 0.0;
+    const int nh = nherm(c);
+    double p = 1.0;
+    for (int h = 0; h < nh; ++h) {
+        double m = 0.0;
+        for (int t = 0; t < a.n_tiles; ++t) {
+            const double* rec = reinterpret_cast<const double*>(a.staging[t] + a.cls_off[t][c] + (unsigned long long)(i - a.class_first[c]) * a.rec_bytes[t][c]);
+            if (h == 0 && t == 0) p = 0.25 / rec[3];
+            for (int s = 0; s < a.NS[t]; ++s) m = fmax(m, fabs(rec[4 + s * nh + h]));
+        }
+        const int n = c_tab.herm[h][3];
+#pragma unroll
+        for (int j = 0; j <= kFastMaxClass; ++j)
+            if (j == n) cn[j] += m;
+    }
+    const double tau = a.adaptive_tol * r.sum_bound / (double)(a.n_pairs > 0 ? a.n_pairs : 1);
+    double lo = 0.0, hi = 1e4;
+    if (!(envelope(cn, c, p, lo) >= tau)) { a.key[k] = 0.0; return; }    // below tau everywhere
+    if (envelope(cn, c, p, hi) >= tau) { a.key[k] = 1e300; return; }     // never below tau in any sane range
+    for (int it = 0; it < 64; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (envelope(cn, c, p, mid) >= tau) lo = mid; else hi = mid;
+    }
+    a.key[k] = hi;                                                       // U(q) < tau for every q >= hi
+}
+
+// stable rank sort inside each class: position = first kept index of the class + #{j : key_j > key_k or (== and j < k)}
+__global__ void __launch_bounds__(128) qcut_rank_kernel(const AdaptArgs a)
+{
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const ScreenResult& r = *a.result;
+    if (k >= r.n_kept) return;
+    long long first = 0;
+    int c = 0;
+    for (; c < kNClasses; ++c) {
+        if (k < first + r.kept_per_class[c]) break;
+        first += r.kept_per_class[c];
+    }
+    const long long last = first + r.kept_per_class[c];
+    const double key = a.key[k];
+    long long rank = 0;
+    for (long long j = first; j < last; ++j) {
+        const double kj = a.key[j];
+        rank += (kj > key || (kj == key && j < k)) ? 1 : 0;
+    }
+    a.keep_sorted[first + rank] = a.keep_idx[k];
+    a.qcut_sorted[first + rank] = key;
+}
+
+cudaError_t launch_adaptive_sort(const AdaptArgs& a, cudaStream_t st)
+{
+    if (a.n_pairs <= 0) return cudaSuccess;
+    const unsigned blocks = (unsigned)((a.n_pairs + 127) / 128);
+    qcut_kernel<<<blocks, 128, 0, st>>>(a);
+    qcut_rank_kernel<<<blocks, 128, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
 // ---- chunk planning on the device ------------------------------------------------------------------------------------
 // Split the fast classes of the class-sorted stream into exactly K chunks of (nearly) equal modelled cost
 // (w(c) = ns_real W(c) + ctr FP64 issue slots per record and q-point); a chunk may span classes; trailing chunks may be

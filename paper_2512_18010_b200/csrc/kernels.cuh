@@ -98,6 +98,24 @@ struct PackArgs {
     int rec_bytes[kNClasses];
 };
 
+constexpr int kMaxAdaptTiles = 8;           // state tiles the q-adaptive cut-off supports (96 states)
+struct AdaptArgs {
+    const int* keep_idx;                    // stable, class-sorted kept indices (screen_kernel)
+    const ScreenResult* result;
+    long long class_first[kNClasses + 1];   // of the prescreened (staging) order
+    int n_tiles;
+    const char* staging[kMaxAdaptTiles];    // every state tile's staging stream
+    unsigned long long cls_off[kMaxAdaptTiles][kNClasses];
+    int rec_bytes[kMaxAdaptTiles][kNClasses];
+    int NS[kMaxAdaptTiles];
+    double adaptive_tol;                    // tau = adaptive_tol * mean bound
+    long long n_pairs;
+    double* key;                            // [n_pairs] out: q_cut of the k-th kept record (screen order)
+    int* keep_sorted;                       // [n_pairs] out: kept indices, q_cut-descending inside each class
+    double* qcut_sorted;                    // [n_pairs] out: q_cut in that order (what the S4 kernels search)
+};
+
+cudaError_t launch_adaptive_sort(const AdaptArgs& a, cudaStream_t st);
 cudaError_t launch_fold(const FoldArgs& a, cudaStream_t st);
 cudaError_t launch_screen(const ScreenArgs& a, cudaStream_t st);
 cudaError_t launch_pack(const PackArgs& a, cudaStream_t st);
@@ -117,6 +135,8 @@ struct V1Args {
     int ns_real, pad;
     double* dst;                            // out + s0*n_q*2
     int* tickets;                           // [n_tiles], all zero at launch and again at exit (n_chunks > 1 only)
+    const double* qcut;                     // q-adaptive cut-off: q_cut per record in stream order (descending inside a class); nullptr: off
+    unsigned long long* work;               // [kNClasses] += records evaluated per CTA and class (q-adaptive statistics); nullptr: off
 };
 int v1_tile_q();                            // q-points per CTA
 cudaError_t launch_ff_v1(int NS, const V1Args& a, cudaStream_t st);
@@ -171,6 +191,8 @@ cudaError_t launch_phi_dft(const double* f, const double* tw, long long n_rows, 
                            cudaStream_t st);
 cudaError_t launch_legendre(const double* F, const double* rowsum2, const double* Yw, const double* w_theta, long long n_sr,
                             int n_theta, int l_max, double* R, double* f2, cudaStream_t st);
+
+cudaError_t launch_abs2(const double* f_complex, long long n, double* out, cudaStream_t st);   // S5: |f|^2
 
 // pure (solid-harmonic) shells (pure.cu, NEXT-5): T_cart = C T_user C^T
 constexpr int kPureMaxNnz = 4;              // user functions one Cartesian component contributes to, at most

@@ -53,6 +53,10 @@ struct scarf_ctx {
     double prefactor = 2.0, screen_tol = 1e-16, threshold_eps = 0.0;
     bool timing = false;
     int n_chunks_opt = 0;     // 0 auto, else the number of stream chunks of the S4 kernels
+    double adaptive_tol = 0.0;  // > 0: q-adaptive cut-off (tau = adaptive_tol * mean bound); takes effect at set_transitions
+    const double* qcut_dev = nullptr;   // q_cut per record of the current stream (sorted order), or nullptr
+    double last_q_tiles = 0.0;          // q tiles of the last S4 call (for the skipped-work statistics)
+    double last_ctr = 40.0;
     int grid_symmetry = 1;    // 1: use f(-q) = conj f(q) on inversion-symmetric product grids; 0: never
     int fft_density_variant = 1;  // 1: DMMA kernel, 0: SIMT kernel (fft_method.cu)
     int check_parseval = 0;       // 1: scarf_fft_form_factors also evaluates both sides of Eq. (75)
@@ -69,7 +73,7 @@ struct scarf_ctx {
     std::vector<double> pure_ucoef;
     int n_states = 0;
     int sm_count = 148;
-    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_keep, d_desc, d_screen, d_tickets, d_axes, d_tab, d_ang_in, d_ang_F, d_ang_tab, d_ang_out, d_pure_map, d_Tcart, d_prim, d_V, d_fft, d_Csym;
+    DevBuf d_pairs, d_E, d_bound, d_T, d_q, d_out, d_keep, d_desc, d_screen, d_tickets, d_key, d_keep2, d_qcut, d_work, d_axes, d_tab, d_ang_in, d_ang_F, d_ang_tab, d_ang_out, d_pure_map, d_Tcart, d_prim, d_V, d_fft, d_Csym;
     const double* Tc_dev = nullptr;        // context-owned Cartesian T of the last set_transitions (FFT method)
     std::vector<DevBuf> staging, packed;
     std::vector<TileStream> tiles;
@@ -78,7 +82,7 @@ struct scarf_ctx {
     // harvested when somebody needs it (scarf_get_stats) or when it is already there (cudaEventQuery)
     ScreenResult* h_screen = nullptr;      // pinned
     cudaEvent_t ev_screen = nullptr;
-    bool screen_pending = false, T_bad = false;
+    bool screen_pending = false, T_bad = false, work_pending = false;
     double grid_eval_points = 0.0, grid_table_cols = 0.0;   // geometry of the last product-grid call (for its work model)
     cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev_m0 = nullptr, ev_m1 = nullptr, ev_slice = nullptr;
     cudaStream_t copy_stream = nullptr;    // device->host copies of form_factors' output slices
@@ -193,7 +197,7 @@ const char* kBadT = "the transition matrices passed to set_transitions contain N
 void free_device(scarf_ctx* c)
 {
     c->d_pairs.release(); c->d_E.release(); c->d_bound.release(); c->d_T.release(); c->d_q.release();
-    c->d_out.release(); c->d_keep.release(); c->d_desc.release(); c->d_screen.release(); c->d_tickets.release(); c->d_parseval.release(); c->parseval_states = 0;
+    c->d_out.release(); c->d_keep.release(); c->d_desc.release(); c->d_screen.release(); c->d_tickets.release(); c->d_key.release(); c->d_keep2.release(); c->d_qcut.release(); c->d_work.release(); c->qcut_dev = nullptr; c->d_parseval.release(); c->parseval_states = 0;
     c->d_axes.release(); c->d_tab.release();
     c->d_ang_in.release(); c->d_ang_F.release(); c->d_ang_tab.release(); c->d_ang_out.release();
     c->d_pure_map.release(); c->d_Tcart.release();
@@ -285,7 +289,10 @@ int scarf_set_option(scarf_ctx* ctx, const char* key, double value)
         ctx->screen_tol = value;
     } else if (k == "timing") ctx->timing = value != 0.0;
     else if (k == "threshold_eps") { if (!(value >= 0.0)) return fail(ctx, SCARF_EINVAL, "set_option: threshold_eps < 0"); ctx->threshold_eps = value; }
-    else if (k == "grid_symmetry") {
+    else if (k == "adaptive_tol") {
+        if (value < 0) return fail(ctx, SCARF_EINVAL, "set_option: adaptive_tol must be >= 0");
+        ctx->adaptive_tol = value;
+    } else if (k == "grid_symmetry") {
         if (value != 0.0 && value != 1.0) return fail(ctx, SCARF_EINVAL, "set_option: grid_symmetry must be 0 or 1");
         ctx->grid_symmetry = (int)value;
     } else if (k == "n_chunks") {
@@ -487,12 +494,45 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T)
         sa.keep_idx = static_cast<int*>(ctx->d_keep.p);
         sa.result = static_cast<ScreenResult*>(ctx->d_screen.p);
         CU(launch_screen(sa, st), "set_transitions: screen kernel");
+        // q-adaptive cut-off (option adaptive_tol): q_cut per kept record, records re-ordered by it inside each class
+        const int* keep_for_pack = sa.keep_idx;
+        ctx->qcut_dev = nullptr;
+        if (ctx->adaptive_tol > 0.0) {
+            if ((int)tiles.size() > kMaxAdaptTiles) return fail(ctx, SCARF_EINVAL, "set_transitions: adaptive_tol supports at most 96 states");
+            CU(ctx->d_key.ensure(std::max<size_t>(64, (size_t)np * sizeof(double))), "set_transitions: alloc keys");
+            CU(ctx->d_qcut.ensure(std::max<size_t>(64, (size_t)np * sizeof(double))), "set_transitions: alloc q_cut");
+            CU(ctx->d_keep2.ensure(std::max<size_t>(64, (size_t)np * sizeof(int))), "set_transitions: alloc index");
+            CU(ctx->d_work.ensure(kNClasses * sizeof(unsigned long long)), "set_transitions: alloc counters");
+            AdaptArgs aa = {};
+            aa.keep_idx = sa.keep_idx;
+            aa.result = sa.result;
+            for (int c = 0; c <= kNClasses; ++c) aa.class_first[c] = hs.class_first[c];
+            aa.n_tiles = (int)tiles.size();
+            for (size_t it = 0; it < tiles.size(); ++it) {
+                aa.staging[it] = tiles[it].staging;
+                aa.NS[it] = tiles[it].NS;
+                unsigned long long off = 0;
+                for (int c = 0; c < kNClasses; ++c) {
+                    aa.cls_off[it][c] = off;
+                    aa.rec_bytes[it][c] = rec_doubles(c, tiles[it].NS) * 8;
+                    off += (unsigned long long)hs.class_count[c] * aa.rec_bytes[it][c];
+                }
+            }
+            aa.adaptive_tol = ctx->adaptive_tol;
+            aa.n_pairs = np;
+            aa.key = static_cast<double*>(ctx->d_key.p);
+            aa.keep_sorted = static_cast<int*>(ctx->d_keep2.p);
+            aa.qcut_sorted = static_cast<double*>(ctx->d_qcut.p);
+            CU(launch_adaptive_sort(aa, st), "set_transitions: q-adaptive kernels");
+            keep_for_pack = aa.keep_sorted;
+            ctx->qcut_dev = aa.qcut_sorted;
+        }
         for (size_t it = 0; it < tiles.size(); ++it) {
             const TileStream& t = tiles[it];
             PackArgs pa = {};
             pa.staging = t.staging;
             pa.packed = t.base;
-            pa.keep_idx = sa.keep_idx;
+            pa.keep_idx = keep_for_pack;
             pa.result = sa.result;
             pa.desc = t.desc;
             pa.n_pairs = np;
@@ -515,7 +555,8 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T)
         scarf_stats& s = ctx->st;
         s.n_states = n_states;
         s.n_pairs_kept = -1;      // unknown until harvested (scarf_get_stats waits for it)
-        s.last_fold_launches = (int32_t)(2 * tiles.size() + 1 + (ctx->any_pure ? 1 : 0));
+        s.last_fold_launches = (int32_t)(2 * tiles.size() + 1 + (ctx->any_pure ? 1 : 0) + (ctx->qcut_dev ? 2 : 0));
+        s.adaptive_bound = 0.0; s.last_adaptive_work_fraction = 1.0;
         if (ctx->timing) {
             CU(cudaEventRecord(ctx->ev1, st), "set_transitions: event");
             CU(cudaEventSynchronize(ctx->ev1), "set_transitions: event sync");
@@ -563,6 +604,10 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
         if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "form_factors: event");
         int launches = 0;
         double main_ms = 0.0;
+        if (ctx->qcut_dev) {
+            CU(cudaMemsetAsync(ctx->d_work.p, 0, kNClasses * sizeof(unsigned long long), st), "form_factors: clear counters");
+            ctx->last_q_tiles = 0.0; ctx->last_ctr = kCtr; ctx->work_pending = true;
+        }
         // all state tiles for the q range [dq, dq + 3 n_q) into dout [n_states][n_q]
         auto run_range = [&](const double* dq, long long n_q, double* dout) -> int {
         for (const TileStream& t : ctx->tiles) {
@@ -578,6 +623,9 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
             a.ns_real = t.ns_real;
             a.dst = dout + (size_t)t.s0 * n_q * 2;
             if (int rc = prepare_tickets(ctx, n_tiles, a.n_chunks, st, &a.tickets)) return rc;
+            a.qcut = ctx->qcut_dev;
+            a.work = ctx->qcut_dev ? static_cast<unsigned long long*>(ctx->d_work.p) : nullptr;
+            if (&t == &ctx->tiles.front()) ctx->last_q_tiles += (double)n_tiles;
             CU(launch_plan_chunks(t.desc, a.n_chunks, t.ns_real, kCtr, st), "form_factors: chunk planning kernel");
             if (ctx->timing) CU(cudaEventRecord(ctx->ev_m0, st), "form_factors: event");
             CU(launch_ff_v1(t.NS, a, st), "form_factors: kernel");
@@ -717,6 +765,10 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "form_factors_grid: event");
         int launches = 0;
         double main_ms = 0.0;
+        if (ctx->qcut_dev) {
+            CU(cudaMemsetAsync(ctx->d_work.p, 0, kNClasses * sizeof(unsigned long long), st), "form_factors_grid: clear counters");
+            ctx->last_q_tiles = (double)n_tiles; ctx->last_ctr = kCtrGrid; ctx->work_pending = true;
+        }
         const long long ncol = (long long)nbx * kGridBX + (long long)nby * kGridBY + (long long)nbz * kGridBZ;
         const long long n_rows = (long long)ctx->hs.pairs.size();    // prescreened pairs: an upper bound of the kept count
         for (const TileStream& t : ctx->tiles) {
@@ -742,6 +794,8 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
             a.n_rows = n_rows;
             a.v.n_chunks = choose_chunks(ctx->sm_count, n_tiles, ctx->n_chunks_opt);
             if (int rc = prepare_tickets(ctx, n_tiles, a.v.n_chunks, st, &a.v.tickets)) return rc;
+            a.v.qcut = ctx->qcut_dev;
+            a.v.work = ctx->qcut_dev ? static_cast<unsigned long long*>(ctx->d_work.p) : nullptr;
             CU(launch_grid_tables(a, tx, ty, tz, st), "form_factors_grid: table kernel");
             CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, kCtrGrid, st), "form_factors_grid: chunk planning kernel");
             if (ctx->timing) CU(cudaEventRecord(ctx->ev_m0, st), "form_factors_grid: event");
@@ -966,6 +1020,33 @@ int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t
     }
 }
 
+int scarf_abs2(scarf_ctx* ctx, int64_t n, const double* f, double* out)
+{
+    if (!ctx) return SCARF_EINVAL;
+    if (ctx->host_only) return fail(ctx, SCARF_ENODEVICE, "abs2: host-only context; there is no CPU fallback");
+    if (n < 0) return fail(ctx, SCARF_EINVAL, "abs2: n < 0");
+    if (n == 0) return SCARF_OK;
+    if (!f || !out) return fail(ctx, SCARF_EINVAL, "abs2: null pointer");
+    CU(cudaSetDevice(ctx->device), "abs2");
+    cudaStream_t st = ctx->stream;
+    const bool f_host = !is_device_ptr(f), o_host = !is_device_ptr(out);
+    const double* df = f;
+    double* dout = out;
+    if (f_host) {
+        CU(ctx->d_ang_in.ensure((size_t)n * 16), "abs2: alloc");
+        CU(cudaMemcpyAsync(ctx->d_ang_in.p, f, (size_t)n * 16, cudaMemcpyHostToDevice, st), "abs2: upload");
+        df = static_cast<const double*>(ctx->d_ang_in.p);
+    }
+    if (o_host) {
+        CU(ctx->d_ang_out.ensure((size_t)n * 8), "abs2: alloc");
+        dout = static_cast<double*>(ctx->d_ang_out.p);
+    }
+    CU(launch_abs2(df, n, dout, st), "abs2: kernel");
+    if (o_host) CU(cudaMemcpyAsync(out, dout, (size_t)n * 8, cudaMemcpyDeviceToHost, st), "abs2: download");
+    if (o_host || f_host) CU(cudaStreamSynchronize(st), "abs2: sync");
+    return SCARF_OK;
+}
+
 /* Eq. (81)-(82) PAPER.md:591-596: least-squares fit  <|f_s|^2>_Omega(q) ~ A + B q^2 + C q^4  over the points with
  * |q| <= q_max (all points if q_max <= 0).  HOST arrays.  Normal equations in the scaled variable x = (q / q_ref)^2,
  * q_ref = the largest |q| used, solved by Gaussian elimination with partial pivoting. */
@@ -1136,6 +1217,27 @@ int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out)
         }
         ctx->st.last_grid_slots = slots + tab;
         ctx->st.last_grid_kernel_slots = slots;
+    }
+    if (!ctx->host_only && ctx->qcut_dev && !ctx->screen_pending) {
+        const double np_all = (double)std::max<size_t>(1, ctx->hs.pairs.size());
+        ctx->st.adaptive_bound = (double)ctx->st.n_pairs_kept * ctx->adaptive_tol * ctx->h_screen->sum_bound / np_all;
+        if (ctx->work_pending) {                                  // records evaluated per class by the last S4 call
+            unsigned long long wk[kNClasses] = {};
+            cudaSetDevice(ctx->device);
+            if (cudaMemcpyAsync(wk, ctx->d_work.p, sizeof wk, cudaMemcpyDeviceToHost, ctx->stream) == cudaSuccess &&
+                cudaStreamSynchronize(ctx->stream) == cudaSuccess) {
+                const double nt = (double)std::max<size_t>(1, ctx->tiles.size());
+                double done = 0.0, full = 0.0;
+                for (int c = 0; c <= kFastMaxClass; ++c) {
+                    const double w = (double)ctx->n_states / nt * kW[c] + ctx->last_ctr;
+                    done += (double)wk[c] * w;
+                    full += (double)ctx->st.pairs_kept_per_class[c] * ctx->last_q_tiles * nt * w;
+                }
+                ctx->st.last_adaptive_work_fraction = full > 0.0 ? done / full : 1.0;
+                ctx->work_pending = false;
+            } else
+                cudaGetLastError();
+        }
     }
     *out = ctx->st;
     if (ctx->T_bad) return fail(ctx, SCARF_EINVAL, std::string("get_stats: ") + kBadT);

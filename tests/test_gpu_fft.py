@@ -144,3 +144,31 @@ def test_fft_density_padded_fragments(oracle_mod, Scarf, torch_cuda, n_s):
         for variant in (1, 0):
             sc.set_option("fft_density_variant", variant)
             assert_parity(sc.fft_form_factors(n, x_min, L, device_out=False), f_ref)
+
+
+def test_parseval_check_eq75(oracle_mod, Scarf, torch_cuda):
+    """Option check_parseval (the paper's check_parseval flag, Eq. (75)): both sides as the library reports
+    them against the oracle's arrays, ragged grid, 13 states (two tiles); ESTATE without a checked call."""
+    from oracle import fft_method as offt
+    from paper_2512_18010_b200.binding import ScarfError, SCARF_ESTATE
+    from tests.test_oracle_fft import soft_basis
+    b = soft_basis()
+    rng = np.random.default_rng(15)
+    T = rng.normal(size=(13, b.nbf, b.nbf))
+    n, x_min, L = (14, 9, 11), np.array([-4.0, -3.5, -4.5]), np.array([8.0, 7.5, 9.0])
+    phi = offt.density_grid(b, T, n, x_min, L)
+    f_ref = offt.transform(phi, x_min, L)
+    vpix, vbox = np.prod(L) / np.prod(n), np.prod(L)
+    with Scarf(0) as sc:
+        sc.set_basis(b)
+        sc.set_transitions(T)
+        sc.fft_form_factors(n, x_min, L)
+        with pytest.raises(ScarfError) as e:
+            sc.fft_parseval()
+        assert e.value.code == SCARF_ESTATE
+        sc.set_option("check_parseval", 1)
+        sc.fft_form_factors(n, x_min, L)
+        P = sc.fft_parseval()
+    np.testing.assert_allclose(P[:, 0], vpix * np.sum(phi ** 2, axis=(1, 2, 3)), rtol=1e-12)
+    np.testing.assert_allclose(P[:, 1], np.sum(np.abs(f_ref) ** 2, axis=1) / vbox, rtol=1e-12)
+    np.testing.assert_allclose(P[:, 0], P[:, 1], rtol=1e-12)

@@ -309,3 +309,53 @@ def test_non_finite_device_T_is_reported(oracle_mod, Scarf, torch_cuda):
         assert e.value.code == SCARF_EINVAL
         sc.set_transitions(torch.as_tensor(w.T, device="cuda"))       # a good T clears the condition
         assert_parity(sc.form_factors(w.q[:64]), oracle_mod.form_factors(w.basis, w.T, w.q[:64]))
+
+
+@pytest.mark.parametrize("tol", [1e-16, 1e-9, 1e-4])
+def test_q_adaptive_cutoff_error_within_reported_bound(oracle_mod, Scarf, torch_cuda, tol):
+    """NEXT-2, second half (PAPER.md:499 made q-dependent): option adaptive_tol skips a pair for the q tiles beyond the radius
+    where its rigorous envelope falls below tau.  Config 2 at full size, point list sorted by |q| (so that tiles have large
+    smallest |q|) and the product grid: the error against the EXACT path on every point, and against the oracle on a sample,
+    stays below the bound the library reports; the work fraction drops as the tolerance grows."""
+    torch = torch_cuda
+    w = W.make_workload(2, oracle_mod.overlap)
+    order = np.argsort(np.linalg.norm(w.q, axis=1), kind="stable")
+    q = np.ascontiguousarray(w.q[order])
+    ax = W.cartesian_axis(w.grid["n_per_axis"], w.grid["qmax"])
+    idx = W.sample_q_indices(w.n_q, 200, seed=11)
+    f_ref = oracle_mod.form_factors(w.basis, w.T, q[idx])
+    Td, qd = torch.as_tensor(w.T, device="cuda"), torch.as_tensor(q, device="cuda")
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(Td)
+        f0 = sc.form_factors(qd).cpu().numpy()
+        g0 = sc.form_factors_grid(ax, ax, ax)
+        sc.set_option("adaptive_tol", tol)
+        sc.set_transitions(Td)
+        f1 = sc.form_factors(qd).cpu().numpy()
+        st_list = sc.stats()
+        g1 = sc.form_factors_grid(ax, ax, ax)
+        st_grid = sc.stats()
+    scale = np.max(np.abs(f0))
+    bound = st_list["adaptive_bound"]
+    assert bound > 0.0
+    assert np.max(np.abs(f1 - f0)) <= bound + 1e-12 * scale
+    assert np.max(np.abs(g1 - g0)) <= bound + 1e-12 * scale
+    assert np.max(np.abs(f1[:, idx] - f_ref)) <= bound + TOL * np.max(np.abs(f_ref))
+    for st in (st_list, st_grid):
+        assert 0.0 < st["last_adaptive_work_fraction"] <= 1.0
+    if tol >= 1e-9:
+        assert st_list["last_adaptive_work_fraction"] < 0.999
+    print(f"adaptive_tol={tol:g}: bound {bound:.3e} (scale {scale:.3e}), measured {np.max(np.abs(f1 - f0)):.3e}, "
+          f"work list {st_list['last_adaptive_work_fraction']:.4f} grid {st_grid['last_adaptive_work_fraction']:.4f}")
+
+
+def test_abs2_output(oracle_mod, Scarf, torch_cuda):
+    """S5, the optional |f_s|^2 output (Fig. 6): elementwise on device and host buffers, ragged size."""
+    torch = torch_cuda
+    rng = np.random.default_rng(2)
+    f = rng.normal(size=(3, 1001)) + 1j * rng.normal(size=(3, 1001))
+    ref = f.real ** 2 + f.imag ** 2
+    with Scarf(0) as sc:
+        np.testing.assert_allclose(sc.abs2(f), ref, rtol=5e-16, atol=0)   # one FMA vs two roundings: <= 2 ulp
+        np.testing.assert_allclose(sc.abs2(torch.as_tensor(f, device="cuda")).cpu().numpy(), ref, rtol=5e-16, atol=0)   # one FMA vs two roundings: <= 2 ulp

@@ -64,3 +64,25 @@ def test_density_is_the_orbital_product(oracle_mod, offt):
     assert abs(phi.sum() * vpix - 2.0 * oracle_mod.overlap(b)[p, q_]) <= 1e-9
     # every orbital is normalised on the grid too (Appendix A)
     assert np.allclose(np.sum(V * V, axis=1) * vpix, 1.0, rtol=1e-9)
+
+
+def test_parseval_eq75(oracle_mod, offt):
+    """Eq. (75): Int d^3r |Phi|^2 = Int d^3q/(2 pi)^3 |f|^2.  On the method's grids the relation is exact
+    (discrete Parseval): V_pix sum |Phi_abc|^2 == (1 / V_box) sum_q |f_q|^2 — a pin of the transform's normalisation (V_pix,
+    unnormalised DFT, unit-modulus phase) that is independent of the triple-sum pin; and on a soft basis in a large box both
+    equal the analytic continuum value Int d^3q/(2 pi)^3 |f|^2 by quadrature of the ANALYTIC oracle on the same q grid."""
+    b = soft_basis()
+    rng = np.random.default_rng(6)
+    T = rng.normal(size=(2, b.nbf, b.nbf))
+    for n, x_min, L in (((12, 9, 10), np.array([-3.0, -2.5, -3.5]), np.array([6.0, 5.5, 7.0])),
+                        ((40, 40, 40), np.array([-8.0] * 3), np.array([16.0] * 3))):
+        phi = offt.density_grid(b, T, n, x_min, L)
+        f = offt.transform(phi, x_min, L)
+        vpix, vbox = np.prod(L) / np.prod(n), np.prod(L)
+        lhs = vpix * np.sum(phi ** 2, axis=(1, 2, 3))
+        rhs = np.sum(np.abs(f) ** 2, axis=1) / vbox
+        np.testing.assert_allclose(lhs, rhs, rtol=1e-13)
+    # continuum check on the large box: the analytic form factor on the same q lattice gives the same q-space integral
+    q = offt.q_points(n, L)
+    f_ana = oracle_mod.form_factors(b, T, q)
+    np.testing.assert_allclose(np.sum(np.abs(f_ana) ** 2, axis=1) / vbox, lhs, rtol=1e-6)
