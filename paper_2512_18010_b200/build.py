@@ -36,8 +36,10 @@ def _stale() -> bool:
     return any(os.path.exists(d) and os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False, ptxas_verbose: bool = False) -> str:
-    if not force and not _stale():
+def build(force: bool = False, verbose: bool = False, ptxas_verbose: bool = False, debug_checks: bool = False) -> str:
+    """debug_checks: compile the device-side invariant checks (SCARF_CHECK, ff_common.cuh) in; the library is written to
+    libscarf.so all the same (rebuild without the flag afterwards)."""
+    if not force and not debug_checks and not _stale():
         return LIB
     objs = []
     build_dir = os.path.join(HERE, "build")
@@ -48,7 +50,8 @@ def build(force: bool = False, verbose: bool = False, ptxas_verbose: bool = Fals
         if not os.path.exists(src):
             continue
         obj = os.path.join(build_dir, os.path.splitext(s)[0] + ".o")
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if ptxas_verbose else []) + ["-c", src, "-o", obj]
+        cmd = ([_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if ptxas_verbose else []) + (["-DSCARF_DEBUG_CHECKS"] if debug_checks else [])
+               + ["-c", src, "-o", obj])
         if verbose:
             print(" ".join(cmd), file=sys.stderr)
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
@@ -72,4 +75,4 @@ def build(force: bool = False, verbose: bool = False, ptxas_verbose: bool = Fals
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv or "-v" in sys.argv,
-                ptxas_verbose="--ptxas" in sys.argv))
+                ptxas_verbose="--ptxas" in sys.argv, debug_checks="--debug-checks" in sys.argv))

@@ -242,38 +242,51 @@ __global__ void __launch_bounds__(kFusedWarps * 32) angular_fused_kernel(const d
     }
     if (F_glob) return;
     __syncthreads();
-    // step 2: R[l(l+1) +- m] = (-1)^{m for -m} sum_j Yw[j][l(l+1)/2 + m] F[j][+-m + l_max].  One work item = (l, m >= 0): the
-    // weight serves +m and -m; YwT is the transposed table [l(l+1)/2 + m][n_theta_pad], so a thread streams its row with
-    // 16-byte loads, 8 in flight (the j loop was one dependent 8-byte L2 load per FMA pair before: 20 us per CTA).
-    const int nlm = (l_max + 1) * (l_max + 1), nhalf = (l_max + 1) * (l_max + 2) / 2, ntp = (n_theta + 1) & ~1;
-    for (int o = threadIdx.x; o < nhalf; o += blockDim.x) {
-        int l = (int)((sqrt(8.0 * o + 1.0) - 1.0) * 0.5);
-        while (l * (l + 1) / 2 > o) --l;
-        while ((l + 1) * (l + 2) / 2 <= o) ++l;
-        const int m = o - l * (l + 1) / 2;
-        const double2* yrow = reinterpret_cast<const double2*>(YwT + (size_t)o * ntp);
-        double pr = 0.0, pi = 0.0, nr = 0.0, ni = 0.0;
-        constexpr int kYB = 16;                             // 16-byte loads issued back to back before their values are used
-        for (int jb = 0; jb < ntp / 2; jb += kYB) {
-            double2 y[kYB];
+    // step 2: R[l(l+1) +- m] = (-1)^{m for -m} sum_j Yw[j][l(l+1)/2 + m] F[j][+-m + l_max].  One work item = (m >= 0, group g):
+    // the thread reads F[j][+-m] ONCE per j from shared memory and uses it for its up to kLG degrees l = m + g + k G (the
+    // per-(l, m) mapping read it once per l: the shared-memory wavefronts of step 2 cost as much as the tensor-core step);
+    // YwT is the transposed weight table [l(l+1)/2 + m][n_theta_pad], streamed with 16-byte loads (kLG independent loads in flight).
+    constexpr int kLG = 8;
+    const int nlm = (l_max + 1) * (l_max + 1), ntp = (n_theta + 1) & ~1, G = (l_max + kLG) / kLG;
+    for (int item = threadIdx.x; item < (l_max + 1) * G; item += blockDim.x) {
+        const int m = item / G, g = item % G;
+        const double2* yrow[kLG];
+        int nk = 0;
 #pragma unroll
-            for (int u = 0; u < kYB; ++u) y[u] = jb + u < ntp / 2 ? __ldg(yrow + jb + u) : make_double2(0.0, 0.0);
+        for (int k = 0; k < kLG; ++k) {
+            const int l = m + g + k * G;
+            yrow[k] = reinterpret_cast<const double2*>(YwT + (size_t)(l <= l_max ? l * (l + 1) / 2 + m : 0) * ntp);
+            if (l <= l_max) nk = k + 1;
+        }
+        double pr[kLG], pi[kLG], nr[kLG], ni[kLG];
 #pragma unroll
-            for (int u = 0; u < kYB; ++u) {
-                const int j = 2 * (jb + u);
-                if (j < n_theta) {
-                    const double2 p0 = s_F[(size_t)j * n_m + (l_max + m)], q0 = s_F[(size_t)j * n_m + (l_max - m)];
-                    pr = fma(y[u].x, p0.x, pr); pi = fma(y[u].x, p0.y, pi); nr = fma(y[u].x, q0.x, nr); ni = fma(y[u].x, q0.y, ni);
-                }
-                if (j + 1 < n_theta) {
-                    const double2 p1 = s_F[(size_t)(j + 1) * n_m + (l_max + m)], q1 = s_F[(size_t)(j + 1) * n_m + (l_max - m)];
-                    pr = fma(y[u].y, p1.x, pr); pi = fma(y[u].y, p1.y, pi); nr = fma(y[u].y, q1.x, nr); ni = fma(y[u].y, q1.y, ni);
-                }
+        for (int k = 0; k < kLG; ++k) pr[k] = pi[k] = nr[k] = ni[k] = 0.0;
+        for (int j2 = 0; j2 < ntp / 2; ++j2) {
+            const int j = 2 * j2;
+            double2 y[kLG];
+#pragma unroll
+            for (int k = 0; k < kLG; ++k) y[k] = k < nk ? __ldg(yrow[k] + j2) : make_double2(0.0, 0.0);
+            const double2 p0 = s_F[(size_t)j * n_m + (l_max + m)], q0 = s_F[(size_t)j * n_m + (l_max - m)];
+            const bool two = j + 1 < n_theta;
+            const double2 p1 = two ? s_F[(size_t)(j + 1) * n_m + (l_max + m)] : make_double2(0.0, 0.0);
+            const double2 q1 = two ? s_F[(size_t)(j + 1) * n_m + (l_max - m)] : make_double2(0.0, 0.0);
+#pragma unroll
+            for (int k = 0; k < kLG; ++k) {
+                pr[k] = fma(y[k].x, p0.x, pr[k]); pi[k] = fma(y[k].x, p0.y, pi[k]);
+                nr[k] = fma(y[k].x, q0.x, nr[k]); ni[k] = fma(y[k].x, q0.y, ni[k]);
+                pr[k] = fma(y[k].y, p1.x, pr[k]); pi[k] = fma(y[k].y, p1.y, pi[k]);
+                nr[k] = fma(y[k].y, q1.x, nr[k]); ni[k] = fma(y[k].y, q1.y, ni[k]);
             }
         }
         const double sgn = (m & 1) ? -1.0 : 1.0;
-        R[(size_t)sr * nlm + l * (l + 1) + m] = make_double2(pr, pi);
-        if (m > 0) R[(size_t)sr * nlm + l * (l + 1) - m] = make_double2(sgn * nr, sgn * ni);
+#pragma unroll
+        for (int k = 0; k < kLG; ++k) {
+            const int l = m + g + k * G;
+            if (k < nk) {
+                R[(size_t)sr * nlm + l * (l + 1) + m] = make_double2(pr[k], pi[k]);
+                if (m > 0) R[(size_t)sr * nlm + l * (l + 1) - m] = make_double2(sgn * nr[k], sgn * ni[k]);
+            }
+        }
     }
     if (f2 != nullptr && threadIdx.x == 0) {
         double acc = 0.0;

@@ -50,6 +50,18 @@ __host__ __device__ constexpr int hindex(int t, int u, int v)
     return 0;
 }
 
+// ---- optional device-side invariant checks (build with -DSCARF_DEBUG_CHECKS: python -m paper_2512_18010_b200.build --debug-checks).
+// compute-sanitizer is not available on the measurement pool, so the hand-rolled pipelines carry their own bounds / protocol
+// assertions; a violated one traps (the launch fails with cudaErrorLaunchFailure and every later call reports it).
+#ifdef SCARF_DEBUG_CHECKS
+#define SCARF_CHECK(cond)        \
+    do {                         \
+        if (!(cond)) __trap();   \
+    } while (0)
+#else
+#define SCARF_CHECK(cond) ((void)0)
+#endif
+
 // ---- mbarrier / bulk-copy wrappers (PTX ISA: mbarrier, cp.async.bulk) -------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -89,6 +101,7 @@ __device__ __forceinline__ void ticket_wait(int* ticket, int turn)
         int v;
         do {
             asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(ticket) : "memory");
+            SCARF_CHECK(v >= 0 && v <= turn);             // tickets only move forward, one chunk at a time
         } while (v != turn);
     }
     __syncthreads();

@@ -101,6 +101,7 @@ __device__ __forceinline__ void run_class_grid(GPipe& pp, const GridArgs& a, con
         const int first = j * SREC, cnt = min(SREC, n_rec - first);
         unsigned char* sb = pp.buf + slot * kSlotBytes;
         const long long r = r0 + first;
+        SCARF_CHECK(cnt >= 1 && cnt <= kMaxRec && cnt * REC <= kStageBytes && r >= 0 && r + cnt <= a.n_rows && slot >= 0 && slot < kStages);
         mbar_expect_tx(&pp.full[slot], (uint32_t)cnt * (REC + kXB + kYB + kZB));
         bulk_g2s(sb, seg + (size_t)first * REC, (uint32_t)cnt * REC, &pp.full[slot]);
         bulk_g2s(sb + kStageBytes, a.tx + ((size_t)bx * a.n_rows + r) * kGridBX, (uint32_t)cnt * kXB, &pp.full[slot]);
@@ -211,6 +212,7 @@ __global__ void __launch_bounds__(kThreads, 2) ff_grid_kernel(const GridArgs a)
     }
     auto class_records = [&](int L) {
         int n = ck.n[L];
+        SCARF_CHECK(n >= 0 && ck.begin[L] >= 0 && (long long)ck.begin[L] + n <= d.cls_n[L]);
         if (a.v.qcut != nullptr && n > 0) n = max(0, min(n, active_prefix(a.v.qcut + d.cls_first[L], d.cls_n[L], q_min) - ck.begin[L]));
         if (a.v.work != nullptr && threadIdx.x == 0 && n > 0) atomicAdd(a.v.work + L, (unsigned long long)n);
         return n;
@@ -239,6 +241,7 @@ __global__ void __launch_bounds__(kThreads, 2) ff_grid_kernel(const GridArgs a)
         if (ix < a.nx_eval && iy < a.ny && iz < a.nz) {
             const long long i = ((long long)ix * a.ny + iy) * a.nz + iz;
             const bool mirror = last && a.sym && 2 * ix < a.nx - 1;
+            SCARF_CHECK(i >= 0 && i < a.v.n_q);
 #pragma unroll
             for (int s = 0; s < NS; ++s)
                 if (s < a.v.ns_real) {

@@ -60,6 +60,7 @@ __device__ __forceinline__ void run_class(Pipe& pp, const char* __restrict__ seg
         const int slot = (int)((pp.it + (uint32_t)j) % kStages);
         const int first = j * SREC, cnt = min(SREC, n_rec - first);
         const uint32_t bytes = (uint32_t)cnt * REC;
+        SCARF_CHECK(cnt >= 1 && bytes <= (uint32_t)kStageBytes && (bytes & 15u) == 0 && slot >= 0 && slot < kStages);
         mbar_expect_tx(&pp.full[slot], bytes);
         bulk_g2s(pp.buf + slot * kStageBytes, seg + (size_t)first * REC, bytes, &pp.full[slot]);
     };
@@ -177,6 +178,7 @@ __global__ void __launch_bounds__(kThreads, 2) ff_v1_kernel(const V1Args a)
     }
     auto class_records = [&](int L) {
         int n = ck.n[L];
+        SCARF_CHECK(n >= 0 && ck.begin[L] >= 0 && (long long)ck.begin[L] + n <= d.cls_n[L]);
         if (a.qcut != nullptr && n > 0) n = max(0, min(n, active_prefix(a.qcut + d.cls_first[L], d.cls_n[L], q_min) - ck.begin[L]));
         if (a.work != nullptr && threadIdx.x == 0 && n > 0) atomicAdd(a.work + L, (unsigned long long)n);
         return n;

@@ -5,6 +5,12 @@
 
 #include "kernels.cuh"
 
+#ifdef SCARF_DEBUG_CHECKS
+#define SCARF_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define SCARF_CHECK(cond) ((void)0)
+#endif
+
 namespace scarf {
 
 // Index tables in the constant bank, initialised at compile time (no per-process upload step, no mutable global state):
@@ -269,6 +275,7 @@ __global__ void __launch_bounds__(128) pack_kernel(const PackArgs a)
         kfirst += r.kept_per_class[k];
         doff += (unsigned long long)r.kept_per_class[k] * a.rec_bytes[k];
     }
+    SCARF_CHECK(i >= a.class_first[c] && i < a.class_first[c + 1] && warp >= kfirst && warp < kfirst + r.kept_per_class[c]);
     const uint4* s = reinterpret_cast<const uint4*>(a.staging + a.cls_off[c] + (unsigned long long)(i - a.class_first[c]) * a.rec_bytes[c]);
     uint4* d = reinterpret_cast<uint4*>(a.packed + doff + (unsigned long long)(warp - kfirst) * a.rec_bytes[c]);
     const int pieces = a.rec_bytes[c] >> 4;
@@ -393,6 +400,7 @@ __global__ void plan_chunks_kernel(StreamDesc* d, int K, int ns_real, double ctr
     bool cur_empty = true;
     for (int c = 0; c <= kFastMaxClass; ++c) {
         long long rem = d->cls_n[c], pos = 0;
+        SCARF_CHECK(rem >= 0 && rem < 0x7fffffffLL);
         while (rem > 0) {
             long long take = rem;
             if (k < K - 1) {
@@ -411,6 +419,14 @@ __global__ void plan_chunks_kernel(StreamDesc* d, int K, int ns_real, double ctr
             if (k < K - 1 && acc >= total * (double)(k + 1) / (double)K - 0.5 * w[c]) { ++k; cur_empty = true; }
         }
     }
+#ifdef SCARF_DEBUG_CHECKS
+    for (int c = 0; c <= kFastMaxClass; ++c) {            // the chunks tile every class exactly once, in order
+        long long pos = 0;
+        for (int kk = 0; kk < K; ++kk)
+            if (d->chunks[kk].n[c] > 0) { SCARF_CHECK(d->chunks[kk].begin[c] == pos); pos += d->chunks[kk].n[c]; }
+        SCARF_CHECK(pos == d->cls_n[c]);
+    }
+#endif
 }
 
 cudaError_t launch_plan_chunks(StreamDesc* desc, int K, int ns_real, double ctr, cudaStream_t st)

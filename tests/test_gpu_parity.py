@@ -359,3 +359,28 @@ def test_abs2_output(oracle_mod, Scarf, torch_cuda):
     with Scarf(0) as sc:
         np.testing.assert_allclose(sc.abs2(f), ref, rtol=5e-16, atol=0)   # one FMA vs two roundings: <= 2 ulp
         np.testing.assert_allclose(sc.abs2(torch.as_tensor(f, device="cuda")).cpu().numpy(), ref, rtol=5e-16, atol=0)   # one FMA vs two roundings: <= 2 ulp
+
+
+def test_repeated_runs_are_bitwise_identical(oracle_mod, Scarf, torch_cuda):
+    """No race detector is available on the measurement pool (profiles/r02_sanitizers.md); a race in the shared-memory stage
+    ring, the mbarrier protocol or the ordered ticket fix-up would show up as run-to-run differences.  Config 2 at full size,
+    both S4 kernels, several chunk counts, device-side screening included: every repetition must be bit-for-bit the same."""
+    torch = torch_cuda
+    w = W.make_workload(2, oracle_mod.overlap)
+    ax = W.cartesian_axis(w.grid["n_per_axis"], w.grid["qmax"])
+    Td, qd = torch.as_tensor(w.T, device="cuda"), torch.as_tensor(w.q, device="cuda")
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        for K in (0, 5):
+            sc.set_option("n_chunks", K)
+            ref_l = ref_g = None
+            for rep in range(6):
+                sc.set_transitions(Td)
+                fl = sc.form_factors(qd).clone()
+                fg = sc.form_factors_grid(ax, ax, ax).copy()
+                torch.cuda.synchronize()
+                if rep == 0:
+                    ref_l, ref_g = fl, fg
+                else:
+                    assert torch.equal(torch.view_as_real(fl), torch.view_as_real(ref_l)), (K, rep)
+                    assert np.array_equal(fg.view(np.float64), ref_g.view(np.float64)), (K, rep)
