@@ -197,30 +197,40 @@ __global__ void __launch_bounds__(kThreads, 2) ff_grid_kernel(const GridArgs a)
 #pragma unroll
         for (int s = 0; s < NS; ++s) re[j][s] = im[j][s] = 0.0;
 
-    const StreamDesc& d = *a.v.desc;
-    const V1Chunk& ck = d.chunks[chunk];
-    // q-adaptive cut-off: this box keeps, of every class, the records whose q_cut exceeds its smallest |q|
-    double q_min = 0.0;
-    if (a.v.qcut != nullptr) {
-        __shared__ double sh_min[kThreads / 32];
-        double m2 = 1e300;
+    // Per class: the records this CTA evaluates, where they start in the stream and in the tables — worked out once by
+    // threads 0..6 and parked in shared memory (nothing of it stays live in registers across the class loops).
+    // q-adaptive cut-off (option): of every class the box keeps the records whose q_cut exceeds its smallest |q|.
+    __shared__ int s_nrec[kFastMaxClass + 1];
+    __shared__ unsigned long long s_off[kFastMaxClass + 1];
+    __shared__ long long s_row[kFastMaxClass + 1];
+    {
+        double q_min = 0.0;
+        if (a.v.qcut != nullptr) {
+            __shared__ double sh_min[kThreads / 32];
+            double m2 = 1e300;
 #pragma unroll
-        for (int j = 0; j < kNQ; ++j)
-            if (bx * kGridBX + ixl + 2 * j < a.nx_eval && iy < a.ny && iz < a.nz)
-                m2 = fmin(m2, qv[j][0] * qv[j][0] + qv[j][1] * qv[j][1] + qv[j][2] * qv[j][2]);
-        q_min = sqrt(block_min(m2, sh_min));
+            for (int j = 0; j < kNQ; ++j)
+                if (bx * kGridBX + ixl + 2 * j < a.nx_eval && iy < a.ny && iz < a.nz)
+                    m2 = fmin(m2, qv[j][0] * qv[j][0] + qv[j][1] * qv[j][1] + qv[j][2] * qv[j][2]);
+            q_min = sqrt(block_min(m2, sh_min));
+        }
+        if (threadIdx.x <= kFastMaxClass) {
+            const int L = threadIdx.x;
+            const StreamDesc& d = *a.v.desc;
+            const V1Chunk& ck = d.chunks[chunk];
+            int n = ck.n[L];
+            SCARF_CHECK(n >= 0 && ck.begin[L] >= 0 && (long long)ck.begin[L] + n <= d.cls_n[L]);
+            if (a.v.qcut != nullptr && n > 0) n = max(0, min(n, active_prefix(a.v.qcut + d.cls_first[L], d.cls_n[L], q_min) - ck.begin[L]));
+            if (a.v.work != nullptr && n > 0) atomicAdd(a.v.work + L, (unsigned long long)n);
+            s_nrec[L] = n;
+            s_off[L] = d.cls_off[L] + (unsigned long long)ck.begin[L] * (unsigned long long)(rec_doubles(L, NS) * 8);
+            s_row[L] = d.cls_first[L] + ck.begin[L];
+        }
+        __syncthreads();
     }
-    auto class_records = [&](int L) {
-        int n = ck.n[L];
-        SCARF_CHECK(n >= 0 && ck.begin[L] >= 0 && (long long)ck.begin[L] + n <= d.cls_n[L]);
-        if (a.v.qcut != nullptr && n > 0) n = max(0, min(n, active_prefix(a.v.qcut + d.cls_first[L], d.cls_n[L], q_min) - ck.begin[L]));
-        if (a.v.work != nullptr && threadIdx.x == 0 && n > 0) atomicAdd(a.v.work + L, (unsigned long long)n);
-        return n;
-    };
-#define SCARF_GRID_CLASS(LV)                                                                                          \
-    if (const int n_rec = class_records(LV); n_rec > 0)                                                               \
-        run_class_grid<LV, NS>(pp, a, a.v.base + d.cls_off[LV] + (size_t)ck.begin[LV] * (rec_doubles(LV, NS) * 8), \
-                               d.cls_first[LV] + ck.begin[LV], n_rec, bx, by, bz, ixl, iyl, izl, qv, re, im);
+#define SCARF_GRID_CLASS(LV)                                                                                        \
+    if (s_nrec[LV] > 0)                                                                                             \
+        run_class_grid<LV, NS>(pp, a, a.v.base + s_off[LV], s_row[LV], s_nrec[LV], bx, by, bz, ixl, iyl, izl, qv, re, im);
     SCARF_GRID_CLASS(0)
     SCARF_GRID_CLASS(1)
     SCARF_GRID_CLASS(2)

@@ -164,28 +164,36 @@ __global__ void __launch_bounds__(kThreads, 2) ff_v1_kernel(const V1Args a)
 #pragma unroll
         for (int s = 0; s < NS; ++s) re[j][s] = im[j][s] = 0.0;
 
-    const StreamDesc& d = *a.desc;
-    const V1Chunk& ck = d.chunks[chunk];
-    // q-adaptive cut-off: this tile keeps, of every class, the records whose q_cut exceeds its smallest |q|
-    double q_min = 0.0;
-    if (a.qcut != nullptr) {
-        __shared__ double sh_min[kThreads / 32];
-        double m2 = 1e300;
+    // Per class: the records this CTA evaluates and where they start — worked out once by threads 0..6 and parked in shared
+    // memory, so that nothing of it stays live in registers across the class loops (the kernel sits at the 255-register limit).
+    // q-adaptive cut-off (option): of every class the tile keeps the records whose q_cut exceeds its smallest |q|.
+    __shared__ int s_nrec[kFastMaxClass + 1];
+    __shared__ unsigned long long s_off[kFastMaxClass + 1];
+    {
+        double q_min = 0.0;
+        if (a.qcut != nullptr) {
+            __shared__ double sh_min[kThreads / 32];
+            double m2 = 1e300;
 #pragma unroll
-        for (int j = 0; j < kNQ; ++j)
-            if (iq[j] < a.n_q) m2 = fmin(m2, qv[j][3]);
-        q_min = sqrt(block_min(m2, sh_min));
+            for (int j = 0; j < kNQ; ++j)
+                if (iq[j] < a.n_q) m2 = fmin(m2, qv[j][3]);
+            q_min = sqrt(block_min(m2, sh_min));
+        }
+        if (threadIdx.x <= kFastMaxClass) {
+            const int L = threadIdx.x;
+            const StreamDesc& d = *a.desc;
+            const V1Chunk& ck = d.chunks[chunk];
+            int n = ck.n[L];
+            SCARF_CHECK(n >= 0 && ck.begin[L] >= 0 && (long long)ck.begin[L] + n <= d.cls_n[L]);
+            if (a.qcut != nullptr && n > 0) n = max(0, min(n, active_prefix(a.qcut + d.cls_first[L], d.cls_n[L], q_min) - ck.begin[L]));
+            if (a.work != nullptr && n > 0) atomicAdd(a.work + L, (unsigned long long)n);
+            s_nrec[L] = n;
+            s_off[L] = d.cls_off[L] + (unsigned long long)ck.begin[L] * (unsigned long long)(rec_doubles(L, NS) * 8);
+        }
+        __syncthreads();
     }
-    auto class_records = [&](int L) {
-        int n = ck.n[L];
-        SCARF_CHECK(n >= 0 && ck.begin[L] >= 0 && (long long)ck.begin[L] + n <= d.cls_n[L]);
-        if (a.qcut != nullptr && n > 0) n = max(0, min(n, active_prefix(a.qcut + d.cls_first[L], d.cls_n[L], q_min) - ck.begin[L]));
-        if (a.work != nullptr && threadIdx.x == 0 && n > 0) atomicAdd(a.work + L, (unsigned long long)n);
-        return n;
-    };
-#define SCARF_V1_CLASS(LV)                                                                                              \
-    if (const int n_rec = class_records(LV); n_rec > 0)                                                                 \
-        run_class<LV, NS>(pp, a.base + d.cls_off[LV] + (size_t)ck.begin[LV] * (rec_doubles(LV, NS) * 8), n_rec, qv, re, im);
+#define SCARF_V1_CLASS(LV) \
+    if (s_nrec[LV] > 0) run_class<LV, NS>(pp, a.base + s_off[LV], s_nrec[LV], qv, re, im);
     SCARF_V1_CLASS(0)
     SCARF_V1_CLASS(1)
     SCARF_V1_CLASS(2)
