@@ -142,10 +142,18 @@ int tile_size_for(int ns)  // smallest instantiated state tile >= ns (ns <= 12)
 }
 
 // Number of stream chunks for a launch over n_tiles q tiles: enough equal-cost CTAs for ~24 waves (2 resident CTAs per SM),
-// so that the ragged last wave costs a few per cent; 1 when the tiles alone give that many.
-int choose_chunks(int sm_count, long long n_tiles, int forced)
+// so that the ragged last wave costs a few per cent; 1 when the tiles alone give that many.  The chunks of a tile add into
+// `out` one after the other (ordered tickets, ~2 us per step), so K is also kept below sqrt(T1 / 2 us), T1 = the modelled time
+// of one tile's whole stream on one CTA slot (from the prescreened pair counts, which the host knows): tiny jobs (config 1:
+// T1 ~ 30 us) would otherwise spend longer passing tickets than computing.
+int choose_chunks(const scarf_ctx* ctx, long long n_tiles, double ctr, int ns_real, int forced)
 {
-    long long K = forced > 0 ? forced : (24LL * 2 * sm_count + n_tiles / 2) / std::max<long long>(1, n_tiles);
+    if (forced > 0) return std::min(forced, kMaxChunks);
+    long long K = (24LL * 2 * ctx->sm_count + n_tiles / 2) / std::max<long long>(1, n_tiles);
+    double slots = 0.0;
+    for (int c = 0; c <= kFastMaxClass; ++c) slots += (double)ctx->hs.class_count[c] * ((double)ns_real * kW[c] + ctr);
+    const double t1_us = slots * 256.0 / (64.0 * 1.9e9 / 2.0) * 1e6;
+    K = std::min<long long>(K, (long long)std::llround(std::sqrt(t1_us / 2.0)));
     return (int)std::max<long long>(1, std::min<long long>(K, kMaxChunks));
 }
 
@@ -619,7 +627,7 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
             const long long n_tiles = (n_q + v1_tile_q() - 1) / v1_tile_q();
             if (n_tiles > 0x7fffffffLL) return fail(ctx, SCARF_EINVAL, "form_factors: n_q too large for one call");
             a.n_tiles = (int)n_tiles;
-            a.n_chunks = choose_chunks(ctx->sm_count, n_tiles, ctx->n_chunks_opt);
+            a.n_chunks = choose_chunks(ctx, n_tiles, kCtr, t.ns_real, ctx->n_chunks_opt);
             a.ns_real = t.ns_real;
             a.dst = dout + (size_t)t.s0 * n_q * 2;
             if (int rc = prepare_tickets(ctx, n_tiles, a.n_chunks, st, &a.tickets)) return rc;
@@ -727,15 +735,26 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         double* dax[3];
         std::vector<double> hax[3];
         size_t off = 0;
-        bool need_sync = false;
+        bool need_sync = false, all_host = true;
         for (int k = 0; k < 3; ++k) {
             dax[k] = static_cast<double*>(ctx->d_axes.p) + off;
             off += (size_t)ax_n[k];
             const bool host = !is_device_ptr(ax_in[k]);
+            all_host = all_host && host;
             if (host && !all_finite(ax_in[k], (size_t)ax_n[k])) return fail(ctx, SCARF_EINVAL, "form_factors_grid: NaN/Inf in an axis");
-            // pageable host -> device copies of this size are staged by the runtime before the call returns: no sync needed
-            CU(cudaMemcpyAsync(dax[k], ax_in[k], (size_t)ax_n[k] * sizeof(double), host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, st),
-               "form_factors_grid: copy axis");
+        }
+        if (all_host) {      // one staged upload instead of three (pageable host -> device copies of this size are staged by
+                             // the runtime before the call returns: no sync needed, the vector may die at once)
+            std::vector<double> cat;
+            cat.reserve(off);
+            for (int k = 0; k < 3; ++k) cat.insert(cat.end(), ax_in[k], ax_in[k] + ax_n[k]);
+            CU(cudaMemcpyAsync(ctx->d_axes.p, cat.data(), off * sizeof(double), cudaMemcpyHostToDevice, st), "form_factors_grid: copy axes");
+        }
+        for (int k = 0; k < 3; ++k) {
+            const bool host = !is_device_ptr(ax_in[k]);
+            if (!all_host)
+                CU(cudaMemcpyAsync(dax[k], ax_in[k], (size_t)ax_n[k] * sizeof(double), host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, st),
+                   "form_factors_grid: copy axis");
             if (ctx->grid_symmetry) {
                 hax[k].resize((size_t)ax_n[k]);
                 if (host) std::memcpy(hax[k].data(), ax_in[k], (size_t)ax_n[k] * sizeof(double));
@@ -792,7 +811,7 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
             a.nx_eval = nx_eval;
             a.tx = tx; a.ty = ty; a.tz = tz;
             a.n_rows = n_rows;
-            a.v.n_chunks = choose_chunks(ctx->sm_count, n_tiles, ctx->n_chunks_opt);
+            a.v.n_chunks = choose_chunks(ctx, n_tiles, kCtrGrid, t.ns_real, ctx->n_chunks_opt);
             if (int rc = prepare_tickets(ctx, n_tiles, a.v.n_chunks, st, &a.v.tickets)) return rc;
             a.v.qcut = ctx->qcut_dev;
             a.v.work = ctx->qcut_dev ? static_cast<unsigned long long*>(ctx->d_work.p) : nullptr;
