@@ -130,8 +130,11 @@ int scarf_set_stream(scarf_ctx* ctx, void* cuda_stream);
  *           "grid_symmetry": default 1.  scarf_form_factors_grid evaluates only one half of a product grid whose three
  *                         axes are antisymmetric bit for bit (ax[i] == -ax[n-1-i]) and stores conj f for the mirror
  *                         points (f(-q) = conj f(q), exact for real T); 0 always evaluates every point.
- *           "fft_density_variant": default 1 = FP64 tensor-core (DMMA) density kernel of scarf_fft_form_factors,
- *                         0 = SIMT kernel (same result to round-off; slower).
+ *           "fft_density_variant": default 1 = FP64 tensor-core (DMMA) density kernel of scarf_fft_form_factors with the
+ *                         orbital values evaluated per point tile in shared memory (falls back to 2 when the tile of a
+ *                         very large basis does not fit), 2 = DMMA kernel reading orbital values tabulated in device
+ *                         memory (nbf * nx*ny*nz doubles of scratch), 0 = SIMT kernel on the same table (same results to
+ *                         round-off; slower).
  *           "check_parseval": default 0.  1: scarf_fft_form_factors also evaluates both sides of Parseval's relation
  *                         (Eq. 75, the paper's check_parseval flag); read them with scarf_fft_parseval.
  *           "angular_variant": default 1 = fused FP64 tensor-core kernel of scarf_angular_moments, 0 = SIMT kernels
@@ -228,7 +231,8 @@ int scarf_oscillator_fit(int32_t n_states, int32_t n_r, const double* q_abs, con
  *     out[s][(ia*ny + ib)*nz + ic] = V_pix sum_abc Phi_abc exp(+i q.x_abc),  q = 2 pi ((ia - nx/2)/box_len[0], ...)
  * (Eq. 27, 30-33; integer division; "most negative frequencies first").  Accuracy is set by the box (truncation) and
  * the spacing (aliasing beyond pi/h), not by this library.  x_min, box_len: HOST double[3].  out [n_states][nx*ny*nz][2],
- * host or device.  Scratch: nbf*nx*ny*nz doubles + 2 complex arrays of the output size (SCARF_ENOMEM above 64 GB). */
+ * host or device.  Scratch: 2 complex arrays of the output size (+ nbf*nx*ny*nz doubles with fft_density_variant 0 or 2;
+ * SCARF_ENOMEM above 64 GB). */
 int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, const double* x_min, const double* box_len,
                            double* out);
 

@@ -211,6 +211,183 @@ __global__ void __launch_bounds__(kMmaWarps * 32) density_mma_kernel(const doubl
         }
 }
 
+// ---- fused route: orbital values evaluated per point tile straight into shared memory ---------------------------------------
+// The kernel above reads V from HBM (nbf x P x 8 B: 3.2 GB at 190 bf / 128^3, 10 GB at 600 bf) and every warp streams the whole
+// fragment table of C for its 16 points.  Here a CTA owns PT = 8 MT points: phase A evaluates every contracted orbital at those
+// points into a shared-memory tile Vs[nu][point] (row stride PT + 4 doubles: the 4 nu x 8 points of an A fragment then fall on 16
+// distinct 8-byte banks per half-warp); phase B runs the same DMMA contraction with A fragments from that tile.  The 8 warps
+// split the work as (state group of kFusedNSW states) x (parity of the mu chunk), so every B fragment of C is read ONCE per CTA
+// and feeds MT point tiles (4 or 8 instead of 2): the L2 traffic of the fragments drops by MT / 2 and the V buffer disappears.
+// NPAR = 2: 8 warps, one CTA per SM (large tiles); NPAR = 1: 4 warps (one per state group) and two CTAs per SM, so that one CTA's
+// orbital phase overlaps the other's tensor-core phase (small bases).
+constexpr int kFusedNSW = 3;                 // states per warp; 12 / 3 = 4 state groups x 2 mu parities = 8 warps
+constexpr int kFusedKPF = 4;                 // k-steps whose B fragments are in flight ahead of the DMMAs
+static_assert(kMaxStateTile == 4 * kFusedNSW, "state groups");
+
+// 1 / sqrt((2a-1)!!(2b-1)!!(2c-1)!!) at compile time (Newton iterations on small integers converge to the correctly rounded
+// double well within the parity tolerance; the tabulating kernel above calls rsqrt at run time)
+constexpr double cx_sqrt(double x)
+{
+    double y = x > 1.0 ? x : 1.0;
+    for (int i = 0; i < 64; ++i) y = 0.5 * (y + x / y);
+    return y;
+}
+constexpr double cx_dfo(int n)
+{
+    double r = 1.0;
+    for (int k = 2 * n - 1; k > 1; k -= 2) r *= k;
+    return r;
+}
+constexpr double comp_factor(int a, int b, int c) { return 1.0 / cx_sqrt(cx_dfo(a) * cx_dfo(b) * cx_dfo(c)); }
+
+// all components of one shell of angular momentum LL at one point: dst[c * stride] (component order a desc, b desc), everything
+// compile-time indexed (no local memory)
+template <int LL>
+__device__ __forceinline__ void shell_components(double rad, double dx, double dy, double dz, double* __restrict__ dst, int stride)
+{
+    double px[LL + 1], py[LL + 1], pz[LL + 1];
+    px[0] = py[0] = pz[0] = 1.0;
+#pragma unroll
+    for (int i = 1; i <= LL; ++i) { px[i] = px[i - 1] * dx; py[i] = py[i - 1] * dy; pz[i] = pz[i - 1] * dz; }
+    int c = 0;
+#pragma unroll
+    for (int a = LL; a >= 0; --a)
+#pragma unroll
+        for (int b = LL - a; b >= 0; --b) {
+            dst[(size_t)c * stride] = (rad * comp_factor(a, b, LL - a - b)) * ((px[a] * py[b]) * pz[LL - a - b]);
+            ++c;
+        }
+}
+
+__device__ __forceinline__ void orbital_values_at(const PrimShell* __restrict__ prim, int k0, int k1, double x, double y, double z,
+                                                  double* __restrict__ dst, int stride)   // dst[c * stride], c = component
+{
+    const double Ax = __ldg(&prim[k0].A[0]), Ay = __ldg(&prim[k0].A[1]), Az = __ldg(&prim[k0].A[2]);
+    const int l = __ldg(&prim[k0].l);
+    const double dx = x - Ax, dy = y - Ay, dz = z - Az;
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    double rad = 0.0;
+    for (int k = k0; k < k1; ++k) rad = fma(__ldg(&prim[k].cprim), exp(-__ldg(&prim[k].alpha) * r2), rad);
+    switch (l) {
+    case 0: shell_components<0>(rad, dx, dy, dz, dst, stride); break;
+    case 1: shell_components<1>(rad, dx, dy, dz, dst, stride); break;
+    case 2: shell_components<2>(rad, dx, dy, dz, dst, stride); break;
+    case 3: shell_components<3>(rad, dx, dy, dz, dst, stride); break;
+    case 4: shell_components<4>(rad, dx, dy, dz, dst, stride); break;
+    case 5: shell_components<5>(rad, dx, dy, dz, dst, stride); break;
+    default: shell_components<6>(rad, dx, dy, dz, dst, stride); break;
+    }
+}
+
+template <int MT, int NPAR>
+__global__ void __launch_bounds__(4 * NPAR * 32) density_fused_kernel(const PrimShell* __restrict__ prim, const int* __restrict__ shell_first,
+                                                                          int n_shells, FftGrid g, const double* __restrict__ C, int nbf,
+                                                                          int nbf_pad, int s0, int ns, double gfac, double2* __restrict__ out)
+{
+    constexpr int PT = 8 * MT, S = PT + 4;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double* Vs = reinterpret_cast<double*>(smem_raw);                 // [nbf_pad][S]
+    double* phis = Vs + (size_t)nbf_pad * S;                          // [kMaxStateTile][PT]
+    const long long p0 = (long long)blockIdx.x * PT;
+    // ---- phase A: orbital values of this CTA's points
+    for (int i = threadIdx.x; i < (nbf_pad - nbf) * S; i += blockDim.x) Vs[(size_t)nbf * S + i] = 0.0;   // zero padding rows
+    // a work item = (shell, point); consecutive threads take consecutive points of one shell, so a warp's loads of the shell data
+    // are broadcasts and its switch on l is uniform
+    for (int idx = threadIdx.x; idx < n_shells * PT; idx += blockDim.x) {
+        const int sh = idx / PT, pt = idx % PT;
+        const long long p = p0 + pt;
+        const int k0 = __ldg(shell_first + sh), k1 = __ldg(shell_first + sh + 1);
+        double* dst = Vs + (size_t)__ldg(&prim[k0].bf0) * S + pt;
+        // points past the end of the grid are evaluated at the grid origin (finite values, never stored)
+        const long long pe = p < g.P ? p : 0;
+        const int ic = (int)(pe % g.nz), ib = (int)((pe / g.nz) % g.ny), ia = (int)(pe / ((long long)g.nz * g.ny));
+        orbital_values_at(prim, k0, k1, g.xmin[0] + g.len[0] * ((double)ia / g.nx), g.xmin[1] + g.len[1] * ((double)ib / g.ny),
+                          g.xmin[2] + g.len[2] * ((double)ic / g.nz), dst, S);
+    }
+    __syncthreads();
+    // ---- phase B: W[p][mu] = sum_{nu >= mu} C_s[mu][nu] v_nu(p) on the tensor cores, phi_s(p) += sum_mu W[p][mu] v_mu(p)
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gid = lane >> 2, tig = lane & 3;
+    const int sg = warp & 3, par = warp >> 2, s_off = sg * kFusedNSW;
+    const size_t per = (size_t)nbf_pad * nbf_pad;
+    const int n_kc = nbf_pad / 4;
+    double phi[MT][kFusedNSW];
+#pragma unroll
+    for (int t = 0; t < MT; ++t)
+#pragma unroll
+        for (int s = 0; s < kFusedNSW; ++s) phi[t][s] = 0.0;
+    if (s_off < ns) {
+        for (int mc = par; mc < nbf_pad / 8; mc += NPAR) {
+            double D[MT][kFusedNSW][2];
+#pragma unroll
+            for (int t = 0; t < MT; ++t)
+#pragma unroll
+                for (int s = 0; s < kFusedNSW; ++s) D[t][s][0] = D[t][s][1] = 0.0;
+            const double* Cb = C + (size_t)s_off * per + (size_t)mc * n_kc * 32 + lane;   // + s * per + kc * 32
+            const int kc0 = 2 * mc;                                    // nu0 = mu0: first k-chunk of the upper triangle
+            auto load_b = [&](int kc, double (&b)[kFusedKPF][kFusedNSW]) {
+#pragma unroll
+                for (int u = 0; u < kFusedKPF; ++u)
+#pragma unroll
+                    for (int s = 0; s < kFusedNSW; ++s) b[u][s] = kc + u < n_kc ? __ldg(Cb + (size_t)s * per + (size_t)(kc + u) * 32) : 0.0;
+            };
+            double bc[kFusedKPF][kFusedNSW], bn[kFusedKPF][kFusedNSW];
+            load_b(kc0, bc);
+#pragma unroll 1
+            for (int kc = kc0; kc < n_kc; kc += kFusedKPF) {
+                if (kc + kFusedKPF < n_kc) load_b(kc + kFusedKPF, bn);
+#pragma unroll
+                for (int u = 0; u < kFusedKPF; ++u)
+                    if (kc + u < n_kc) {
+                        const double* vrow = Vs + (size_t)(4 * (kc + u) + tig) * S + gid;   // A[row = gid][k = tig] = v_nu(point)
+#pragma unroll
+                        for (int t = 0; t < MT; ++t) {
+                            const double av = vrow[8 * t];
+#pragma unroll
+                            for (int s = 0; s < kFusedNSW; ++s) dmma884(D[t][s], av, bc[u][s]);
+                        }
+                    }
+#pragma unroll
+                for (int u = 0; u < kFusedKPF; ++u)
+#pragma unroll
+                    for (int s = 0; s < kFusedNSW; ++s) bc[u][s] = bn[u][s];
+            }
+            // D[row = gid][col = 2 tig + i] = W[point][8 mc + 2 tig + i]
+            const double* v0 = Vs + (size_t)(8 * mc + 2 * tig) * S + gid;
+#pragma unroll
+            for (int t = 0; t < MT; ++t) {
+                const double a0 = v0[8 * t], a1 = v0[S + 8 * t];
+#pragma unroll
+                for (int s = 0; s < kFusedNSW; ++s) phi[t][s] = fma(D[t][s][0], a0, fma(D[t][s][1], a1, phi[t][s]));
+            }
+        }
+    }
+    // ---- reduce over the 4 column lanes, then over the two mu parities (fixed order), store
+#pragma unroll
+    for (int t = 0; t < MT; ++t)
+#pragma unroll
+        for (int s = 0; s < kFusedNSW; ++s) {
+            double x = phi[t][s];
+            x += __shfl_xor_sync(0xffffffffu, x, 1);
+            x += __shfl_xor_sync(0xffffffffu, x, 2);
+            phi[t][s] = x;
+        }
+    if (NPAR == 2 && par == 0 && tig == 0)
+#pragma unroll
+        for (int t = 0; t < MT; ++t)
+#pragma unroll
+            for (int s = 0; s < kFusedNSW; ++s) phis[(s_off + s) * PT + 8 * t + gid] = phi[t][s];
+    if (NPAR == 2) __syncthreads();
+    if (par == NPAR - 1 && tig == 0)
+#pragma unroll
+        for (int t = 0; t < MT; ++t)
+#pragma unroll
+            for (int s = 0; s < kFusedNSW; ++s) {
+                const long long p = p0 + 8 * t + gid;
+                if (s_off + s < ns && p < g.P)
+                    out[(size_t)(s0 + s_off + s) * g.P + p] = make_double2(gfac * ((NPAR == 2 ? phis[(s_off + s) * PT + 8 * t + gid] : 0.0) + phi[t][s]), 0.0);
+            }
+}
+
 // out[s][(ia, ib, ic)] = V_pix e^{i q.x_min} F[s][(alpha mod N, ...)],  alpha = ia - floor(N/2)
 __global__ void __launch_bounds__(256) fft_post_kernel(const double2* __restrict__ F, FftGrid g, int ns, double2* __restrict__ out)
 {
@@ -330,6 +507,45 @@ cudaError_t launch_density_mma(const double* V, const double* T, double* Csym, i
     for (int s_off = 0; s_off < ns; s_off += kMmaNSP)
         density_mma_kernel<<<(unsigned)((P + per_cta - 1) / per_cta), kMmaWarps * 32, 0, st>>>(V, Csym, nbf, nbf_pad, P, s0, ns, s_off, g,
                                                                                            reinterpret_cast<double2*>(out_complex));
+    return cudaGetLastError();
+}
+
+// Shared memory of the fused density kernel for MT point tiles per CTA; 0 if it does not fit.
+static size_t fused_smem(int nbf_pad, int MT) { return ((size_t)nbf_pad * (8 * MT + 4) + (size_t)kMaxStateTile * 8 * MT) * sizeof(double); }
+
+cudaError_t density_fused_init_device()
+{
+    cudaError_t e = cudaFuncSetAttribute(density_fused_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDensityFusedMaxSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(density_fused_kernel<8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDensityFusedMaxSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(density_fused_kernel<4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDensityFusedMaxSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(density_fused_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDensityFusedMaxSmem);
+    return e;
+}
+
+bool density_fused_fits(int nbf_pad) { return fused_smem(nbf_pad, 2) <= (size_t)kDensityFusedMaxSmem; }
+
+// Csym must have been filled by launch_symmetrize for this (s0, ns).
+cudaError_t launch_density_fused(const PrimShell* prim, const int* shell_first, int n_shells, const FftGrid& g, const double* Csym, int nbf,
+                                 int nbf_pad, int s0, int ns, double gfac, double* out_complex, cudaStream_t st)
+{
+    if (g.P <= 0 || ns <= 0) return cudaSuccess;
+    double2* out = reinterpret_cast<double2*>(out_complex);
+    // 64 points per CTA: two 4-warp CTAs per SM while their tiles fit, else one 8-warp CTA; then 32 and 16 points
+#define SCARF_FUSED(MTV, NPARV, PTS)                                                                                             \
+    density_fused_kernel<MTV, NPARV><<<(unsigned)((g.P + PTS - 1) / PTS), 4 * NPARV * 32, fused_smem(nbf_pad, MTV), st>>>(          \
+        prim, shell_first, n_shells, g, Csym, nbf, nbf_pad, s0, ns, gfac, out)
+    if (fused_smem(nbf_pad, 8) <= (size_t)(110 * 1024)) SCARF_FUSED(8, 1, 64);
+    else if (fused_smem(nbf_pad, 8) <= (size_t)kDensityFusedMaxSmem) SCARF_FUSED(8, 2, 64);
+    else if (fused_smem(nbf_pad, 4) <= (size_t)kDensityFusedMaxSmem) SCARF_FUSED(4, 2, 32);
+    else SCARF_FUSED(2, 2, 16);
+#undef SCARF_FUSED
+    return cudaGetLastError();
+}
+
+cudaError_t launch_symmetrize(const double* T, double* Csym, int nbf, int nbf_pad, int s0, int ns, cudaStream_t st)
+{
+    const long long nsym = (long long)kMaxStateTile * nbf_pad * nbf_pad;
+    symmetrize_kernel<<<(unsigned)((nsym + 255) / 256), 256, 0, st>>>(T, nbf, nbf_pad, s0, ns, Csym);
     return cudaGetLastError();
 }
 

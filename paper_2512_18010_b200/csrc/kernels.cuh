@@ -214,6 +214,12 @@ cudaError_t launch_density(const double* V, const double* T, int nbf, long long 
                            cudaStream_t st);
 cudaError_t launch_density_mma(const double* V, const double* T, double* Csym, int nbf, int nbf_pad, long long P, int s0, int ns,
                                double g, double* out_complex, cudaStream_t st);
+constexpr int kDensityFusedMaxSmem = 225 * 1024;
+cudaError_t density_fused_init_device();
+bool density_fused_fits(int nbf_pad);        // the orbital tile of 16 points fits in shared memory
+cudaError_t launch_symmetrize(const double* T, double* Csym, int nbf, int nbf_pad, int s0, int ns, cudaStream_t st);
+cudaError_t launch_density_fused(const PrimShell* prim, const int* shell_first, int n_shells, const FftGrid& g, const double* Csym, int nbf,
+                                 int nbf_pad, int s0, int ns, double gfac, double* out_complex, cudaStream_t st);
 // Parseval sums (Eq. 75): out[s * stride + col] = scale * sum_i |a[s][i]|^2; scratch holds ns * 256 doubles
 cudaError_t launch_sumsq(const double* a_complex, long long P, int ns, double scale, double* scratch, double* out, int stride, int col,
                          cudaStream_t st);

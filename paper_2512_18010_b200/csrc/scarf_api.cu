@@ -240,6 +240,7 @@ int scarf_create(scarf_ctx** out, int device)
         // per-device function attributes (idempotent; set for every context so that no process-wide flag is needed)
         if (e == cudaSuccess) e = ff_grid_init_device();
         if (e == cudaSuccess) e = angular_init_device();
+        if (e == cudaSuccess) e = density_fused_init_device();
         if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->h_screen), sizeof(ScreenResult));
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_screen, cudaEventDisableTiming);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device);
@@ -312,7 +313,7 @@ int scarf_set_option(scarf_ctx* ctx, const char* key, double value)
         if (value != 0.0 && value != 1.0) return fail(ctx, SCARF_EINVAL, "set_option: angular_variant must be 0 or 1");
         ctx->angular_variant = (int)value;
     } else if (k == "fft_density_variant") {
-        if (value != 0.0 && value != 1.0) return fail(ctx, SCARF_EINVAL, "set_option: fft_density_variant must be 0 or 1");
+        if (value != 0.0 && value != 1.0 && value != 2.0) return fail(ctx, SCARF_EINVAL, "set_option: fft_density_variant must be 0, 1 or 2");
         ctx->fft_density_variant = (int)value;
     }
     else return fail(ctx, SCARF_EINVAL, "set_option: unknown key '" + k + "'");
@@ -1127,7 +1128,11 @@ int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, c
         g.nx = nx; g.ny = ny; g.nz = nz;
         g.P = (long long)nx * ny * nz;
         for (int k = 0; k < 3; ++k) { g.xmin[k] = x_min[k]; g.len[k] = box_len[k]; }
-        const size_t vbytes = (size_t)hs.nbf * (size_t)((g.P + 7) / 8 * 8) * sizeof(double);
+        const int nbf_pad = (hs.nbf + 7) & ~7;
+        // default route: orbital values evaluated per point tile inside the density kernel (no V buffer); the V-buffer routes
+        // remain for bases whose tile does not fit in shared memory and as second implementations (variants 2 and 0)
+        const bool fused = ctx->fft_density_variant == 1 && density_fused_fits(nbf_pad);
+        const size_t vbytes = fused ? 0 : (size_t)hs.nbf * (size_t)((g.P + 7) / 8 * 8) * sizeof(double);
         const size_t fbytes = (size_t)ctx->n_states * (size_t)g.P * 2 * sizeof(double);
         if ((double)vbytes + 2.0 * (double)fbytes > 64e9) return fail(ctx, SCARF_ENOMEM, "fft_form_factors: grid needs more than 64 GB of scratch");
         // primitive shells and the first primitive of every contracted shell
@@ -1141,7 +1146,7 @@ int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, c
         char* pb = static_cast<char*>(ctx->d_prim.p);
         CU(cudaMemcpyAsync(pb, hs.prim.data(), pbytes, cudaMemcpyHostToDevice, st), "fft_form_factors: upload basis");
         CU(cudaMemcpyAsync(pb + pbytes, first.data(), first.size() * sizeof(int), cudaMemcpyHostToDevice, st), "fft_form_factors: upload basis");
-        CU(ctx->d_V.ensure(vbytes), "fft_form_factors: alloc orbital values");
+        if (!fused) CU(ctx->d_V.ensure(vbytes), "fft_form_factors: alloc orbital values");
         CU(ctx->d_fft.ensure(fbytes), "fft_form_factors: alloc transform buffer");
         const bool out_host = !is_device_ptr(out);
         double* dout = out;
@@ -1150,21 +1155,30 @@ int scarf_fft_form_factors(scarf_ctx* ctx, int32_t nx, int32_t ny, int32_t nz, c
             dout = static_cast<double*>(ctx->d_out.p);
         }
         if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "fft_form_factors: event");
-        double* dV = static_cast<double*>(ctx->d_V.p);
+        double* dV = fused ? nullptr : static_cast<double*>(ctx->d_V.p);
         double* dF = static_cast<double*>(ctx->d_fft.p);
-        CU(launch_orbitals(reinterpret_cast<const PrimShell*>(pb), reinterpret_cast<const int*>(pb + pbytes), n_sh, hs.nbf, g, dV, st),
-           "fft_form_factors: orbital kernel");
-        int launches = 1;
+        const PrimShell* dprim = reinterpret_cast<const PrimShell*>(pb);
+        const int* dfirst = reinterpret_cast<const int*>(pb + pbytes);
+        int launches = 0;
+        if (!fused) {
+            CU(launch_orbitals(dprim, dfirst, n_sh, hs.nbf, g, dV, st), "fft_form_factors: orbital kernel");
+            ++launches;
+        }
         for (int s0 = 0; s0 < ctx->n_states; s0 += kMaxStateTile) {
             const int ns_t = std::min(kMaxStateTile, ctx->n_states - s0);
             if (ctx->fft_density_variant == 0) {
                 CU(launch_density(dV, ctx->Tc_dev, hs.nbf, g.P, s0, ns_t, ctx->prefactor, dF, st), "fft_form_factors: density kernel");
                 ++launches;
             } else {
-                const int nbf_pad = (hs.nbf + 7) & ~7;
                 CU(ctx->d_Csym.ensure((size_t)kMaxStateTile * nbf_pad * nbf_pad * sizeof(double)), "fft_form_factors: alloc C");
-                CU(launch_density_mma(dV, ctx->Tc_dev, static_cast<double*>(ctx->d_Csym.p), hs.nbf, nbf_pad, g.P, s0, ns_t,
-                                      ctx->prefactor, dF, st), "fft_form_factors: density kernel (DMMA)");
+                double* dC = static_cast<double*>(ctx->d_Csym.p);
+                if (fused) {
+                    CU(launch_symmetrize(ctx->Tc_dev, dC, hs.nbf, nbf_pad, s0, ns_t, st), "fft_form_factors: symmetrize kernel");
+                    CU(launch_density_fused(dprim, dfirst, n_sh, g, dC, hs.nbf, nbf_pad, s0, ns_t, ctx->prefactor, dF, st),
+                       "fft_form_factors: fused density kernel (DMMA)");
+                } else
+                    CU(launch_density_mma(dV, ctx->Tc_dev, dC, hs.nbf, nbf_pad, g.P, s0, ns_t, ctx->prefactor, dF, st),
+                       "fft_form_factors: density kernel (DMMA)");
                 launches += 2;
             }
         }

@@ -59,7 +59,7 @@ def main():
             w = [rng.uniform(0.1, 1, a.size) for a in ax]
             total += float(np.abs(sc.separable_integral(ax[0], w[0], ax[1], w[1], ax[2], w[2])).sum())
             sc.set_option("check_parseval", 1)
-            for variant in (1, 0):
+            for variant in (1, 2, 0):
                 sc.set_option("fft_density_variant", variant)
                 total += float(np.abs(sc.fft_form_factors((8, 6, 10), np.array([-6.0, -6.0, -6.5]), np.array([12.0, 12.5, 13.0]),
                                                           device_out=False)).sum())
@@ -74,7 +74,7 @@ def main():
         for shape, l_max in (((2, 3, 10, 18), 6), ((1, 1, 150, 64), 31), ((1, 2, 5, 2048), 3)):
             f = rng.normal(size=shape) + 1j * rng.normal(size=shape)
             ct, wt = np.polynomial.legendre.leggauss(shape[2])
-            for variant in (1, 0):
+            for variant in (1, 2, 0):
                 sc.set_option("angular_variant", variant)
                 R, f2 = sc.angular_moments(torch.as_tensor(f, device="cuda"), ct, wt, shape[3], l_max, n_r=shape[1])
                 total += float(R.abs().sum().item()) + float(f2.sum().item())

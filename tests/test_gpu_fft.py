@@ -113,7 +113,7 @@ def test_fft_density_at_config_basis_sizes(oracle_mod, Scarf, torch_cuda, config
     with Scarf(0) as sc:
         sc.set_basis(w.basis)
         sc.set_transitions(torch.as_tensor(T, device="cuda"))
-        for variant in (1, 0):
+        for variant in (1, 2, 0):
             sc.set_option("fft_density_variant", variant)
             f = sc.fft_form_factors(n, lo, L)
             torch.cuda.synchronize()
@@ -141,7 +141,7 @@ def test_fft_density_padded_fragments(oracle_mod, Scarf, torch_cuda, n_s):
     with Scarf(0) as sc:
         sc.set_basis(b)
         sc.set_transitions(T)
-        for variant in (1, 0):
+        for variant in (1, 2, 0):
             sc.set_option("fft_density_variant", variant)
             assert_parity(sc.fft_form_factors(n, x_min, L, device_out=False), f_ref)
 
