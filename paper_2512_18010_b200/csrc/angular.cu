@@ -22,6 +22,7 @@
 #include <cmath>
 #include <vector>
 
+#include "ff_common.cuh"   // mbarrier / cp.async.bulk wrappers
 #include "kernels.cuh"
 
 namespace scarf {
@@ -127,6 +128,7 @@ __global__ void __launch_bounds__(kThreads) legendre_kernel(const double2* __res
 // Rows = theta nodes of this (state, r); k = phi index; columns 2m (cos) and 2m+1 (sin), m = 4 nt + tig for n-tile nt.
 constexpr int kFusedWarps = 4;
 constexpr int kFusedMT = 2;            // 8-row tiles per warp and sweep (they share every B fragment)
+constexpr int kYJ = 8;                 // theta nodes per staged chunk of the weight table (Legendre step)
 constexpr int kFusedKG = 4;            // k-steps per software-pipeline group (loads of the next group overlap this group's DMMAs)
 constexpr int kFusedNT = 7;            // n-tiles per pass: m = 0..27 in one pass (l_max <= 27); more passes beyond
 
@@ -141,8 +143,10 @@ __global__ void __launch_bounds__(kFusedWarps * 32) angular_fused_kernel(const d
                                                                         const double* __restrict__ YwT, const double* __restrict__ w_theta,
                                                                         int n_theta, int n_phi, int l_max, int n_nt, int n_ks,
                                                                         double2* __restrict__ R, double* __restrict__ f2,
-                                                                        double2* __restrict__ F_glob, double* __restrict__ row2_glob)
+                                                                        double2* __restrict__ F_glob, double* __restrict__ row2_glob,
+                                                                        const double* __restrict__ YwC, int ycb)
 {
+    __shared__ __align__(8) uint64_t ybar[2];
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const long long sr = blockIdx.x;
     const int n_m = 2 * l_max + 1;
@@ -248,6 +252,70 @@ __global__ void __launch_bounds__(kFusedWarps * 32) angular_fused_kernel(const d
     // YwT is the transposed weight table [l(l+1)/2 + m][n_theta_pad], streamed with 16-byte loads (kLG independent loads in flight).
     constexpr int kLG = 8;
     const int nlm = (l_max + 1) * (l_max + 1), ntp = (n_theta + 1) & ~1, G = (l_max + kLG) / kLG;
+    if (ycb > 0) {
+        // Staged route: the weight table arrives in chunks of kYJ theta nodes, YwC[chunk][(l,m)][kYJ + 1] (one pad double per
+        // row: the rows of a warp's lanes then fall on distinct banks), by cp.async.bulk into the two halves of the fragment
+        // area, which step 1 no longer needs — the loads of chunk c + 1 run while chunk c is being used, instead of every
+        // thread waiting on L2 for the weights of each theta pair.  One item per thread ((l_max + 1) G <= blockDim).
+        unsigned char* ybuf = smem_raw;
+        const int n_chunks = (n_theta + kYJ - 1) / kYJ;
+        if (threadIdx.x == 0) {
+            mbar_init(&ybar[0], 1);
+            mbar_init(&ybar[1], 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            for (int c = 0; c < min(2, n_chunks); ++c) {
+                mbar_expect_tx(&ybar[c], (uint32_t)ycb);
+                bulk_g2s(ybuf + (size_t)c * ycb, reinterpret_cast<const unsigned char*>(YwC) + (size_t)c * ycb, (uint32_t)ycb, &ybar[c]);
+            }
+        }
+        __syncthreads();
+        const int item = threadIdx.x;
+        const bool active = item < (l_max + 1) * G;
+        const int m = active ? item / G : 0, g = active ? item % G : 0;
+        int row[kLG], nk = 0;
+#pragma unroll
+        for (int k = 0; k < kLG; ++k) {
+            const int l = m + g + k * G;
+            row[k] = (l <= l_max ? l * (l + 1) / 2 + m : 0) * (kYJ + 1);
+            if (active && l <= l_max) nk = k + 1;
+        }
+        double pr[kLG], pi[kLG], nr[kLG], ni[kLG];
+#pragma unroll
+        for (int k = 0; k < kLG; ++k) pr[k] = pi[k] = nr[k] = ni[k] = 0.0;
+        for (int c = 0; c < n_chunks; ++c) {
+            mbar_wait(&ybar[c & 1], (uint32_t)((c >> 1) & 1));
+            const double* yb = reinterpret_cast<const double*>(ybuf + (size_t)(c & 1) * ycb);
+#pragma unroll
+            for (int jj = 0; jj < kYJ; ++jj) {
+                const int j = c * kYJ + jj;
+                if (j < n_theta) {
+                    const double2 p0 = s_F[(size_t)j * n_m + (l_max + m)], q0 = s_F[(size_t)j * n_m + (l_max - m)];
+#pragma unroll
+                    for (int k = 0; k < kLG; ++k)
+                        if (k < nk) {
+                            const double y = yb[row[k] + jj];
+                            pr[k] = fma(y, p0.x, pr[k]); pi[k] = fma(y, p0.y, pi[k]);
+                            nr[k] = fma(y, q0.x, nr[k]); ni[k] = fma(y, q0.y, ni[k]);
+                        }
+                }
+            }
+            __syncthreads();                              // everybody has left this half: refill it with chunk c + 2
+            if (threadIdx.x == 0 && c + 2 < n_chunks) {
+                mbar_expect_tx(&ybar[c & 1], (uint32_t)ycb);
+                bulk_g2s(ybuf + (size_t)(c & 1) * ycb, reinterpret_cast<const unsigned char*>(YwC) + (size_t)(c + 2) * ycb, (uint32_t)ycb,
+                         &ybar[c & 1]);
+            }
+        }
+        const double sgn = (m & 1) ? -1.0 : 1.0;
+#pragma unroll
+        for (int k = 0; k < kLG; ++k) {
+            const int l = m + g + k * G;
+            if (k < nk) {
+                R[(size_t)sr * nlm + l * (l + 1) + m] = make_double2(pr[k], pi[k]);
+                if (m > 0) R[(size_t)sr * nlm + l * (l + 1) - m] = make_double2(sgn * nr[k], sgn * ni[k]);
+            }
+        }
+    } else
     for (int item = threadIdx.x; item < (l_max + 1) * G; item += blockDim.x) {
         const int m = item / G, g = item % G;
         const double2* yrow[kLG];
@@ -390,6 +458,18 @@ void angular_transpose_table(int l_max, int n_theta, const std::vector<double>& 
         for (int p = 0; p < nhalf; ++p) YwT[(size_t)p * ntp + j] = Yw[(size_t)j * nhalf + p];
 }
 
+// Chunked weight table of the staged Legendre step: YwC[c][l(l+1)/2 + m][kYJ + 1], theta nodes c kYJ .. c kYJ + kYJ - 1 (zeros past
+// n_theta and in the pad column), every chunk padded to a multiple of 16 bytes.  Returns the chunk size in bytes.  HOST.
+int angular_chunk_table(int l_max, int n_theta, const std::vector<double>& Yw, std::vector<double>& YwC)
+{
+    const int nhalf = (l_max + 1) * (l_max + 2) / 2, nc = (n_theta + kYJ - 1) / kYJ;
+    const int chunk_doubles = (nhalf * (kYJ + 1) + 1) & ~1;
+    YwC.assign((size_t)nc * chunk_doubles, 0.0);
+    for (int j = 0; j < n_theta; ++j)
+        for (int p = 0; p < nhalf; ++p) YwC[(size_t)(j / kYJ) * chunk_doubles + (size_t)p * (kYJ + 1) + (j % kYJ)] = Yw[(size_t)j * nhalf + p];
+    return chunk_doubles * 8;
+}
+
 size_t angular_fused_smem(int n_theta, int l_max, int n_nt, int n_ks, bool fused)
 {
     return (size_t)n_nt * n_ks * 32 * 8 + (fused ? (size_t)n_theta * (2 * l_max + 1) * 16 : 0) + (size_t)n_theta * 8;
@@ -397,13 +477,16 @@ size_t angular_fused_smem(int n_theta, int l_max, int n_nt, int n_ks, bool fused
 
 cudaError_t launch_angular_fused(const double* f, const double* Bf, const double* YwT, const double* w_theta, long long n_sr, int n_theta,
                                  int n_phi, int l_max, int n_nt, int n_ks, double* R, double* f2, double* F_glob, double* row2_glob,
-                                 cudaStream_t st)
+                                 const double* YwC, int chunk_bytes, cudaStream_t st)
 {
     if (n_sr <= 0) return cudaSuccess;
     const size_t smem = angular_fused_smem(n_theta, l_max, n_nt, n_ks, F_glob == nullptr);
+    // the staged Legendre step needs two chunks inside the fragment area and one work item per thread
+    const bool staged = F_glob == nullptr && YwC != nullptr && 2 * (size_t)chunk_bytes <= (size_t)n_nt * n_ks * 32 * 8 &&
+                        (l_max + 1) * ((l_max + 8) / 8) <= kFusedWarps * 32;
     angular_fused_kernel<<<(unsigned)n_sr, kFusedWarps * 32, smem, st>>>(reinterpret_cast<const double2*>(f), Bf, YwT, w_theta, n_theta, n_phi,
                                                                         l_max, n_nt, n_ks, reinterpret_cast<double2*>(R), f2,
-                                                                        reinterpret_cast<double2*>(F_glob), row2_glob);
+                                                                        reinterpret_cast<double2*>(F_glob), row2_glob, YwC, staged ? chunk_bytes : 0);
     return cudaGetLastError();
 }
 

@@ -32,6 +32,8 @@ namespace {
 constexpr int kThreads = 128;
 constexpr int kStages = 3;
 constexpr int kStageBytes = 8192;             // records of one stage (>= the largest record, L = 6, NS = 12)
+constexpr int kGridSwpMaxL = 2;                // classes whose record loop is software-pipelined
+__host__ __device__ constexpr int grid_swp_records(int L) { return L <= 1 ? 2 : 1; }
 constexpr int kMaxRec = 32;                   // records per stage at most (bounds the table slices)
 constexpr int kXB = kGridBX * 16, kYB = kGridBY * 16, kZB = kGridBZ * 16;   // table bytes per record and box
 constexpr int kSlotBytes = kStageBytes + kMaxRec * (kXB + kYB + kZB);
@@ -146,17 +148,50 @@ __device__ __forceinline__ void run_class_grid(GPipe& pp, const GridArgs& a, con
             constexpr int jq0 = decltype(jc)::value * NQA;
             double mono[NQA][nherm(L)];
             make_monomials<L, NQA, jq0>(qv, mono);
-#pragma unroll 1
-            for (int k = 0; k < cnt; ++k) {
+            auto rec = [&](int k) { return reinterpret_cast<const double2*>(sp + k * REC); };
+            auto factors = [&](int k, double (&gc)[NQA], double (&gs)[NQA]) {      // g = X Y Z for this thread's points
                 const double2 yz = cmul(Ys[k * kGridBY + iyl], Zs[k * kGridBZ + izl]);
-                double gc[NQA], gs[NQA];
 #pragma unroll
                 for (int jj = 0; jj < NQA; ++jj) {
                     const double2 gq = cmul(Xs[k * kGridBX + ixl + 2 * (jq0 + jj)], yz);
                     gc[jj] = gq.x;
                     gs[jj] = gq.y;
                 }
-                record_accum<L, NS, NQA, jq0>(reinterpret_cast<const double2*>(sp + k * REC), mono, gc, gs, re, im);
+            };
+            if constexpr (L <= kGridSwpMaxL) {          // software-pipelined by groups of U records: the per-lane table loads and
+                constexpr int U = grid_swp_records(L);  // complex products of group k+1 are issued alongside the accumulate of group k
+                const int n_full = cnt / U * U;
+                double gc[U][NQA], gs[U][NQA];
+                if (n_full > 0) {
+#pragma unroll
+                    for (int u = 0; u < U; ++u) factors(u, gc[u], gs[u]);
+#pragma unroll 1
+                    for (int k = 0; k + U < n_full; k += U) {
+                        double gcn[U][NQA], gsn[U][NQA];
+#pragma unroll
+                        for (int u = 0; u < U; ++u) factors(k + U + u, gcn[u], gsn[u]);
+#pragma unroll
+                        for (int u = 0; u < U; ++u) record_accum<L, NS, NQA, jq0>(rec(k + u), mono, gc[u], gs[u], re, im);
+#pragma unroll
+                        for (int u = 0; u < U; ++u)
+#pragma unroll
+                            for (int jj = 0; jj < NQA; ++jj) { gc[u][jj] = gcn[u][jj]; gs[u][jj] = gsn[u][jj]; }
+                    }
+#pragma unroll
+                    for (int u = 0; u < U; ++u) record_accum<L, NS, NQA, jq0>(rec(n_full - U + u), mono, gc[u], gs[u], re, im);
+                }
+#pragma unroll 1
+                for (int k = n_full; k < cnt; ++k) {
+                    factors(k, gc[0], gs[0]);
+                    record_accum<L, NS, NQA, jq0>(rec(k), mono, gc[0], gs[0], re, im);
+                }
+            } else {
+#pragma unroll 1
+                for (int k = 0; k < cnt; ++k) {
+                    double gc[NQA], gs[NQA];
+                    factors(k, gc, gs);
+                    record_accum<L, NS, NQA, jq0>(rec(k), mono, gc, gs, re, im);
+                }
             }
         });
         __syncthreads();                                 // the slot is free again

@@ -182,11 +182,12 @@ cudaError_t angular_init_device();           // per-device function attributes; 
 constexpr int kAngularMaxSmem = 200 * 1024;  // dynamic shared memory the fused kernel may use (B fragments + F rows)
 void angular_fragment_table(int l_max, int n_phi, std::vector<double>& Bf, int& n_nt, int& n_ks);
 void angular_transpose_table(int l_max, int n_theta, const std::vector<double>& Yw, std::vector<double>& YwT);
+int angular_chunk_table(int l_max, int n_theta, const std::vector<double>& Yw, std::vector<double>& YwC);   // returns the chunk size in bytes
 size_t angular_fused_smem(int n_theta, int l_max, int n_nt, int n_ks, bool fused);
 // F_glob == nullptr: fused (R, f2 written); else F [n_sr][n_theta][2 l_max + 1] complex and row2 [n_sr][n_theta] are written instead
 cudaError_t launch_angular_fused(const double* f, const double* Bf, const double* YwT, const double* w_theta, long long n_sr, int n_theta,
                                  int n_phi, int l_max, int n_nt, int n_ks, double* R, double* f2, double* F_glob, double* row2_glob,
-                                 cudaStream_t st);
+                                 const double* YwC, int chunk_bytes, cudaStream_t st);   // YwC: chunked weight table (staged Legendre step) or nullptr
 cudaError_t launch_phi_dft(const double* f, const double* tw, long long n_rows, int n_phi, int l_max, double* F, double* rowsum2,
                            cudaStream_t st);
 cudaError_t launch_legendre(const double* F, const double* rowsum2, const double* Yw, const double* w_theta, long long n_sr,

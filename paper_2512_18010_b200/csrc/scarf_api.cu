@@ -43,7 +43,8 @@ const double kCtrGrid = 6.0, kCtrTable = 39.0;
 struct AngularCache {             // host tables of scarf_angular_moments and the arguments they were built for
     bool valid = false;
     int n_phi = 0, l_max = 0, n_nt = 0, n_ks = 0;
-    std::vector<double> ct, wt, Yw, YwT, tw, Bf;
+    std::vector<double> ct, wt, Yw, YwT, YwC, tw, Bf;
+    int chunk_bytes = 0;
 };
 
 struct scarf_ctx {
@@ -963,8 +964,9 @@ int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t
             angular_host_tables(l_max, n_theta, cos_theta, w_theta, n_phi, ac.Yw, ac.tw);
             angular_fragment_table(l_max, n_phi, ac.Bf, ac.n_nt, ac.n_ks);
             angular_transpose_table(l_max, n_theta, ac.Yw, ac.YwT);
-            // device layout (tw, Bf, YwT have even lengths: every block stays 16-byte aligned): [tw | Bf | YwT | Yw | w_theta]
-            const size_t tab_doubles = ac.tw.size() + ac.Bf.size() + ac.YwT.size() + ac.Yw.size() + (size_t)n_theta;
+            ac.chunk_bytes = angular_chunk_table(l_max, n_theta, ac.Yw, ac.YwC);
+            // device layout (tw, Bf, YwT, YwC have even lengths: every block stays 16-byte aligned): [tw | Bf | YwT | YwC | Yw | w_theta]
+            const size_t tab_doubles = ac.tw.size() + ac.Bf.size() + ac.YwT.size() + ac.YwC.size() + ac.Yw.size() + (size_t)n_theta;
             CU(ctx->d_ang_tab.ensure(tab_doubles * sizeof(double)), "angular_moments: alloc tables");
             double* base = static_cast<double*>(ctx->d_ang_tab.p);
             // pageable sources are staged by the runtime before each call returns; the cached vectors outlive the copies anyway
@@ -973,6 +975,8 @@ int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t
             double* p = base + ac.tw.size() + ac.Bf.size();
             CU(cudaMemcpyAsync(p, ac.YwT.data(), ac.YwT.size() * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
             p += ac.YwT.size();
+            CU(cudaMemcpyAsync(p, ac.YwC.data(), ac.YwC.size() * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
+            p += ac.YwC.size();
             CU(cudaMemcpyAsync(p, ac.Yw.data(), ac.Yw.size() * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
             p += ac.Yw.size();
             CU(cudaMemcpyAsync(p, w_theta, (size_t)n_theta * sizeof(double), cudaMemcpyHostToDevice, st), "angular_moments: upload");
@@ -981,7 +985,8 @@ int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t
         double* dtw = static_cast<double*>(ctx->d_ang_tab.p);
         double* dBf = dtw + ac.tw.size();
         double* dYwT = dBf + ac.Bf.size();
-        double* dYw = dYwT + ac.YwT.size();
+        double* dYwC = dYwT + ac.YwT.size();
+        double* dYw = dYwC + ac.YwC.size();
         double* dw = dYw + ac.Yw.size();
         const size_t fbytes = (size_t)n_rows * n_phi * 2 * sizeof(double);
         const double* df = f;
@@ -1005,7 +1010,7 @@ int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t
         const size_t smem_fused = angular_fused_smem(n_theta, l_max, ac.n_nt, ac.n_ks, true);
         const size_t smem_unfused = angular_fused_smem(n_theta, l_max, ac.n_nt, ac.n_ks, false);
         if (ctx->angular_variant == 1 && smem_fused <= (size_t)kAngularMaxSmem) {
-            CU(launch_angular_fused(df, dBf, dYwT, dw, n_sr, n_theta, n_phi, l_max, ac.n_nt, ac.n_ks, dR, df2, nullptr, nullptr, st),
+            CU(launch_angular_fused(df, dBf, dYwT, dw, n_sr, n_theta, n_phi, l_max, ac.n_nt, ac.n_ks, dR, df2, nullptr, nullptr, dYwC, ac.chunk_bytes, st),
                "angular_moments: fused kernel");
             ctx->st.last_kernel_launches = 1;
         } else {
@@ -1014,7 +1019,7 @@ int scarf_angular_moments(scarf_ctx* ctx, int32_t n_states, int32_t n_r, int32_t
             double* dF = static_cast<double*>(ctx->d_ang_F.p);
             double* drow2 = dF + (size_t)n_rows * n_m * 2;
             if (ctx->angular_variant == 1 && smem_unfused <= (size_t)kAngularMaxSmem)
-                CU(launch_angular_fused(df, dBf, dYwT, dw, n_sr, n_theta, n_phi, l_max, ac.n_nt, ac.n_ks, nullptr, nullptr, dF, drow2, st),
+                CU(launch_angular_fused(df, dBf, dYwT, dw, n_sr, n_theta, n_phi, l_max, ac.n_nt, ac.n_ks, nullptr, nullptr, dF, drow2, nullptr, 0, st),
                    "angular_moments: phi kernel (DMMA)");
             else
                 CU(launch_phi_dft(df, dtw, n_rows, n_phi, l_max, dF, drow2, st), "angular_moments: phi kernel");
