@@ -163,7 +163,8 @@ struct GridArgs {
     V1Args v;                               // stream, desc, dst as for v1; v.q unused; v.n_q = nx*ny*nz
     const double *qx, *qy, *qz;             // axes (device)
     int nx, ny, nz;
-    int nbx, nby, nbz;                      // boxes per axis; v.n_tiles = nbx*nby*nbz.  With `sym` the boxes cover ix < nx_eval only
+    int nbx, nby, nbz;                      // boxes per axis.  With `sym` the boxes cover ix < nx_eval only
+    int bx0, pad0;                          // this launch covers x boxes bx0 .. bx0 + v.n_tiles/(nby*nbz) - 1 (host output is computed in x slabs)
     int sym, nx_eval;                       // sym != 0: the grid is inversion-symmetric (every axis ax[i] == -ax[n-1-i] bit for bit):
                                             // only ix < nx_eval = ceil(nx/2) is evaluated and f(-q) = conj f(q) is stored for the mirror point
     const double2 *tx, *ty, *tz;            // tables [box][row][kGridB*] of (re, im); zero beyond the axis end

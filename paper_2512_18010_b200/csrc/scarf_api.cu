@@ -792,6 +792,13 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         }
         const long long ncol = (long long)nbx * kGridBX + (long long)nby * kGridBY + (long long)nbz * kGridBZ;
         const long long n_rows = (long long)ctx->hs.pairs.size();    // prescreened pairs: an upper bound of the kept count
+        const int n_slabs = (out_host && nbx >= 4 && n_q >= 4 * 16384 && !has_high_classes(ctx->hs)) ? 4 : 1;
+        if (n_slabs > 1) {
+            if (!ctx->copy_stream) CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking), "form_factors_grid: copy stream");
+            if (!ctx->ev_slice) CU(cudaEventCreateWithFlags(&ctx->ev_slice, cudaEventDisableTiming), "form_factors_grid: event");
+        }
+        // on any failure the copies already queued into the caller's `out` must have landed before we return
+        auto drain = [&](int rc) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamSynchronize(st); return rc; };
         for (const TileStream& t : ctx->tiles) {
             GridArgs a = {};
             const size_t tab_elems = (size_t)std::max<long long>(1, n_rows) * (size_t)ncol;
@@ -813,23 +820,48 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
             a.nx_eval = nx_eval;
             a.tx = tx; a.ty = ty; a.tz = tz;
             a.n_rows = n_rows;
-            a.v.n_chunks = choose_chunks(ctx, n_tiles, kCtrGrid, t.ns_real, ctx->n_chunks_opt);
-            if (int rc = prepare_tickets(ctx, n_tiles, a.v.n_chunks, st, &a.v.tickets)) return rc;
             a.v.qcut = ctx->qcut_dev;
             a.v.work = ctx->qcut_dev ? static_cast<unsigned long long*>(ctx->d_work.p) : nullptr;
             CU(launch_grid_tables(a, tx, ty, tz, st), "form_factors_grid: table kernel");
-            CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, kCtrGrid, st), "form_factors_grid: chunk planning kernel");
-            if (ctx->timing) CU(cudaEventRecord(ctx->ev_m0, st), "form_factors_grid: event");
-            CU(launch_ff_grid(t.NS, a, st), "form_factors_grid: kernel");
-            if (ctx->timing) {
-                CU(cudaEventRecord(ctx->ev_m1, st), "form_factors_grid: event");
-                CU(cudaEventSynchronize(ctx->ev_m1), "form_factors_grid: event sync");
-                float ms = 0.f;
-                cudaEventElapsedTime(&ms, ctx->ev_m0, ctx->ev_m1);
-                main_ms += ms;
+            ++launches;
+            // Host output: the x boxes are cut into slabs; the device->host copies of a finished slab (and of its mirror slab on
+            // a symmetric grid) run on a second stream while the next slab is being computed.
+            for (int sl = 0; sl < n_slabs; ++sl) {
+                const int b0 = (int)((long long)nbx * sl / n_slabs), b1 = (int)((long long)nbx * (sl + 1) / n_slabs);
+                if (b1 <= b0) continue;
+                const long long tiles_s = (long long)(b1 - b0) * nby * nbz;
+                a.bx0 = b0;
+                a.v.n_tiles = (int)tiles_s;
+                a.v.n_chunks = choose_chunks(ctx, tiles_s, kCtrGrid, t.ns_real, ctx->n_chunks_opt);
+                if (int rc = prepare_tickets(ctx, tiles_s, a.v.n_chunks, st, &a.v.tickets)) return n_slabs > 1 ? drain(rc) : rc;
+                CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, kCtrGrid, st), "form_factors_grid: chunk planning kernel");
+                if (ctx->timing) CU(cudaEventRecord(ctx->ev_m0, st), "form_factors_grid: event");
+                CU(launch_ff_grid(t.NS, a, st), "form_factors_grid: kernel");
+                if (ctx->timing) {
+                    CU(cudaEventRecord(ctx->ev_m1, st), "form_factors_grid: event");
+                    CU(cudaEventSynchronize(ctx->ev_m1), "form_factors_grid: event sync");
+                    float ms = 0.f;
+                    cudaEventElapsedTime(&ms, ctx->ev_m0, ctx->ev_m1);
+                    main_ms += ms;
+                }
+                ctx->st.last_n_chunks = a.v.n_chunks;
+                launches += 2;
+                if (n_slabs > 1) {
+                    const long long plane = (long long)ny * nz;
+                    const long long ix0 = (long long)b0 * kGridBX, ix1 = std::min<long long>((long long)b1 * kGridBX, nx_eval);
+                    cudaError_t e = cudaEventRecord(ctx->ev_slice, st);
+                    if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_slice, 0);
+                    for (int s = 0; s < t.ns_real && e == cudaSuccess; ++s) {
+                        const size_t so = (size_t)(t.s0 + s) * (size_t)n_q;
+                        e = cudaMemcpyAsync(out + (so + (size_t)(ix0 * plane)) * 2, dout + (so + (size_t)(ix0 * plane)) * 2,
+                                            (size_t)((ix1 - ix0) * plane) * 16, cudaMemcpyDeviceToHost, ctx->copy_stream);
+                        if (e == cudaSuccess && sym)       // the mirror slab: ix in [nx - ix1, nx - ix0)
+                            e = cudaMemcpyAsync(out + (so + (size_t)((nx - ix1) * plane)) * 2, dout + (so + (size_t)((nx - ix1) * plane)) * 2,
+                                                (size_t)((ix1 - ix0) * plane) * 16, cudaMemcpyDeviceToHost, ctx->copy_stream);
+                    }
+                    if (e != cudaSuccess) return drain(cuda_fail(ctx, e, "form_factors_grid: download slab"));
+                }
             }
-            ctx->st.last_n_chunks = a.v.n_chunks;
-            launches += 3;
             if (has_high_classes(ctx->hs)) {
                 HighLArgs h = {};
                 h.base = t.base; h.desc = t.desc; h.q = nullptr;
@@ -854,7 +886,8 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
             ctx->st.last_main_kernel_ms = main_ms;
         }
         if (out_host) {
-            CU(cudaMemcpyAsync(out, dout, obytes, cudaMemcpyDeviceToHost, st), "form_factors_grid: download out");
+            if (n_slabs > 1) CU(cudaStreamSynchronize(ctx->copy_stream), "form_factors_grid: sync copies");
+            else CU(cudaMemcpyAsync(out, dout, obytes, cudaMemcpyDeviceToHost, st), "form_factors_grid: download out");
             CU(cudaStreamSynchronize(st), "form_factors_grid: sync");
             if (harvest_screen(ctx, true) != SCARF_OK) return SCARF_ECUDA;
             if (ctx->T_bad) return fail(ctx, SCARF_EINVAL, std::string("form_factors_grid: ") + kBadT);

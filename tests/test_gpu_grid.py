@@ -247,3 +247,28 @@ def test_chunk_counts_general_and_grid(oracle_mod, Scarf, torch_cuda, K):
         assert_parity(g.cpu().numpy(), g_ref)
         sc.set_transitions(np.zeros_like(T))                            # no record survives: zeros through the same launches
         assert np.all(sc.form_factors(q) == 0) and np.all(sc.form_factors_grid(*axes) == 0)
+
+
+@pytest.mark.parametrize("shape,symmetric", [((40, 41, 40), True), ((41, 40, 40), True), ((43, 39, 40), False)])
+def test_grid_host_output_in_slabs_matches_device_output(oracle_mod, Scarf, torch_cuda, shape, symmetric):
+    """Host `out` with >= 65 536 points is computed in four x slabs whose downloads (the slab and, on a symmetric grid, its
+    mirror slab) overlap the next slab's kernel: bit-identical to the device-output call (same chunking per box is not
+    guaranteed, so: equal to round-off), every point; oracle on a sample; even and odd nx, plain grid."""
+    torch = torch_cuda
+    w = W.make_workload(1, oracle_mod.overlap)
+    rng = np.random.default_rng(sum(shape))
+    T = rng.normal(size=(3, w.basis.nbf, w.basis.nbf))
+    axes = [W.cartesian_axis(n, 3.0 + 0.5 * k) for k, n in enumerate(shape)]
+    if not symmetric:
+        axes[0] = axes[0] + 0.125
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(T)
+        f_host = sc.form_factors_grid(*axes)                                        # numpy in -> host out, slabs
+        assert sc.stats()["last_grid_symmetric"] == int(symmetric)
+        f_dev = sc.form_factors_grid(*[torch.as_tensor(a, device="cuda") for a in axes]).cpu().numpy()
+    scale = np.max(np.abs(f_dev), axis=1, keepdims=True)
+    assert np.max(np.abs(f_host - f_dev) / scale) <= 1e-13
+    q = expand(*axes)
+    idx = W.sample_q_indices(q.shape[0], 200, seed=5)
+    assert_parity(f_host[:, idx], oracle_mod.form_factors(w.basis, T, q[idx]))
