@@ -384,3 +384,20 @@ def test_repeated_runs_are_bitwise_identical(oracle_mod, Scarf, torch_cuda):
                 else:
                     assert torch.equal(torch.view_as_real(fl), torch.view_as_real(ref_l)), (K, rep)
                     assert np.array_equal(fg.view(np.float64), ref_g.view(np.float64)), (K, rep)
+
+
+def test_huge_q_underflows_cleanly(oracle_mod, Scarf, torch_cuda):
+    """|q| ~ 1e4..1e6 against a diffuse pair: q^2/4p is far beyond the exponent range of e^{-x}; the argument is clamped before
+    the exponent arithmetic (the 32-bit n used to wrap), so the result is an honest 0, never Inf/NaN/garbage."""
+    w = W.make_workload(1, oracle_mod.overlap)
+    q = np.array([[2.4e4, 0.0, 0.0], [0.0, -1.0e5, 3.0e4], [1.0e6, 1.0e6, -1.0e6], [3.0e3, 0.1, 0.2], [0.3, 0.2, 0.1]])
+    f_ref = oracle_mod.form_factors(w.basis, w.T, q)
+    with Scarf(0) as sc:
+        sc.set_basis(w.basis)
+        sc.set_transitions(w.T)
+        f = sc.form_factors(q)
+        g = sc.form_factors_grid(np.array([2.4e4, -1.0e6, 0.3]), np.array([0.0, 0.2]), np.array([0.0, 0.1]))
+    assert np.all(np.isfinite(f.view(np.float64))) and np.all(np.isfinite(g.view(np.float64)))
+    # the library flushes e^{-x} to ~1e-301 (times O(1e10) polynomial values at these |q|) instead of 0: nothing, either way
+    assert np.max(np.abs(f[:, :4])) <= 1e-250 and np.max(np.abs(f_ref[:, :4])) <= 1e-250
+    assert_parity(f[:, 4:], f_ref[:, 4:])
