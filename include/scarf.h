@@ -38,7 +38,8 @@
  *     compile-time initialised, kernel attributes are set per context at scarf_create, the cuFFT plan belongs to
  *     the context (the only process-wide object is the immutable cuFFT function table, loaded once under
  *     std::call_once).  A context is not thread-safe; distinct contexts are independent and may be driven from
- *     different threads and on different devices.
+ *     different threads and on different devices.  ONE exception, by design: scarf_form_factors_noalloc keeps its scratch
+ *     in a static device array shared by all contexts on a device (see there); no other call touches it.
  *   - Argument range: |q . P| <= 2^30 for every Gaussian-product centre P (i.e. |q| * molecular extent < 1e9);
  *     full accuracy of the phase needs |q . P| <~ 1e5.  e^{-q^2/4p} underflows to (effectively) 0 for large |q|, any
  *     finite q is safe there.  Host q arrays are checked for NaN/Inf; device arrays are not.
@@ -174,6 +175,24 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T);
 /* q [n_q][3] FP64; out [n_states][n_q][2] FP64 (re, im interleaved).  Host or device pointers, independently.
  * Any point set (no grid structure is assumed).  May be called repeatedly. */
 int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out);
+
+/* The same call for callers that must not allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): Eq. (48) PAPER.md:326-330 with the same kernels and the same chunking as scarf_form_factors, so the result is
+ * bit-identical to it.  This entry point calls no cudaMalloc/cudaFree and no allocating library routine, and never
+ * synchronises: it only enqueues work on the context stream.
+ *   q [n_q][3], out [n_states][n_q][2]: DEVICE pointers, both owned by the caller (host pointers: SCARF_EINVAL — staging
+ *   them would need an allocation).
+ *   Scratch: the per-tile tickets of the ordered chunk fix-up (one int per tile of 256 q-points) live in a static device
+ *   array of SCARF_NOALLOC_MAX_TILES entries (256 KB, held by every GPU that loads the library until the process exits)
+ *   instead of a context buffer.  n_q > 256 * SCARF_NOALLOC_MAX_TILES = 16 777 216 is rejected with SCARF_EINVAL and a
+ *   message naming the limit; cut larger point sets into several calls.
+ *   The array is shared by ALL contexts of the process on that device and keeps the last call's contents; every call clears
+ *   the entries it uses (on the context stream) before its kernel.  Calls that overlap on the GPU — two contexts on
+ *   different streams — race on it: serialise such calls (one stream, or events).  Calls on one stream are ordered.
+ *   Needs a context that has seen set_basis and set_transitions (those allocate; call them before the capture / the loop).
+ *   The option "timing" is ignored here (its event synchronisation would block); stats carry launches and chunk count. */
+#define SCARF_NOALLOC_MAX_TILES 65536
+int scarf_form_factors_noalloc(scarf_ctx* ctx, int64_t n_q, const double* q_dev, double* out_dev);
 
 /* The same f_s(q) on a Cartesian PRODUCT grid q = (qx[ix], qy[iy], qz[iz]), out index (ix*ny + iy)*nz + iz:
  * out [n_states][nx*ny*nz][2].  On such a grid the pair factor separates per axis (the V-tensor idea of Eq. (45)-(46)

@@ -18,8 +18,11 @@ SCARF_MAX_L = 6
 SCARF_N_CLASSES = 2 * SCARF_MAX_L + 1
 _CODES = {-1: "EINVAL", -2: "ESTATE", -3: "ENOMEM", -4: "ECUDA", -5: "ENODEVICE"}
 
+NOALLOC_MAX_TILES = 65536                  # SCARF_NOALLOC_MAX_TILES (include/scarf.h)
+NOALLOC_MAX_Q = NOALLOC_MAX_TILES * 256     # q-points per scarf_form_factors_noalloc call
+
 EXPORTS = ["scarf_create", "scarf_destroy", "scarf_set_stream", "scarf_set_option", "scarf_set_basis", "scarf_set_basis_pure", "scarf_nbf",
-           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_grid", "scarf_separable_integral", "scarf_angular_moments", "scarf_oscillator_fit", "scarf_abs2", "scarf_fft_form_factors", "scarf_fft_parseval", "scarf_get_stats", "scarf_last_error",
+           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_noalloc", "scarf_form_factors_grid", "scarf_separable_integral", "scarf_angular_moments", "scarf_oscillator_fit", "scarf_abs2", "scarf_fft_form_factors", "scarf_fft_parseval", "scarf_get_stats", "scarf_last_error",
            "scarf_version", "scarf_fp64_peak", "scarf_host_hermite_E", "scarf_host_shell_norms", "scarf_host_ylm_table"]
 
 
@@ -68,6 +71,7 @@ def _load():
     L.scarf_overlap.argtypes = [vp, dp]
     L.scarf_set_transitions.argtypes = [vp, C.c_int, vp]
     L.scarf_form_factors.argtypes = [vp, C.c_int64, vp, vp]
+    L.scarf_form_factors_noalloc.argtypes = [vp, C.c_int64, vp, vp]
     L.scarf_form_factors_grid.argtypes = [vp, C.c_int32, vp, C.c_int32, vp, C.c_int32, vp, vp]
     L.scarf_separable_integral.argtypes = [vp, C.c_int32, dp, dp, C.c_int32, dp, dp, C.c_int32, dp, dp, dp]
     L.scarf_angular_moments.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, C.c_int32, C.c_int32, vp, vp, vp]
@@ -257,6 +261,21 @@ class Scarf:
             import torch
             return torch.view_as_complex(out.view(self.n_states, n_q, 2))
         return out.reshape(self.n_states, n_q, 2).view(np.complex128)[..., 0]
+
+    def form_factors_noalloc(self, q, out):
+        """scarf_form_factors_noalloc: the same result as form_factors without any device allocation or synchronisation
+        inside the library (tickets in a static device array; at most NOALLOC_MAX_Q q-points per call).  q [n_q][3] and
+        out [n_states][n_q][2]: float64 CUDA tensors, both supplied by the caller.  Returns a complex view of `out`."""
+        import torch
+        if not (_is_torch(q) and _is_torch(out) and q.is_cuda and out.is_cuda):
+            raise ValueError("form_factors_noalloc: q and out must be CUDA tensors")
+        n_q = int(q.shape[0])
+        if tuple(q.shape) != (n_q, 3):
+            raise ValueError("form_factors_noalloc: q must be [n_q][3]")
+        qp, qkeep = _ptr(q, "q", 3 * n_q)
+        op, okeep = _ptr(out, "out", self.n_states * n_q * 2)
+        self._check(_lib.scarf_form_factors_noalloc(self._h, n_q, qp, op))
+        return torch.view_as_complex(out.view(self.n_states, n_q, 2))
 
     def form_factors_grid(self, qx, qy, qz, out=None):
         """Product grid q = (qx[ix], qy[iy], qz[iz]), point index (ix*ny + iy)*nz + iz.  qx, qy, qz: 1-D float64

@@ -25,6 +25,14 @@
 // (q, pair, state) n_herm + 3 (2 for L = 0) — the work model of DESIGN.md.
 #include "ff_common.cuh"
 
+#include <mutex>
+
+// Scratch of the allocation-free entry point (scarf_form_factors_noalloc, include/scarf.h): the per-tile tickets of the
+// ordered fix-up, one int per q tile.  256 KB on every device that loads the library, until the process exits.  In HOST code
+// this name is only a stand-in for the symbol: the device address comes from cudaGetSymbolAddress (static_tickets() below).
+constexpr int kStaticTickets = 65536;        // == SCARF_NOALLOC_MAX_TILES (checked in scarf_api.cu)
+static __device__ __align__(256) int scarf_static_tickets[kStaticTickets];
+
 namespace scarf {
 
 namespace {
@@ -268,6 +276,54 @@ cudaError_t launch_ff_v1(int NS, const V1Args& a, cudaStream_t st)
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
+}
+
+// ---- allocation-free variant: tickets in the static device array ---------------------------------------------------------
+int v1_static_tiles() { return kStaticTickets; }
+
+// Device address of scarf_static_tickets on the CURRENT device; resolved once per device (the address of a __device__ symbol
+// differs from device to device, and the host-side name is not a device pointer).
+static cudaError_t static_tickets(int** out)
+{
+    constexpr int kMaxDevices = 64;
+    static std::mutex mu;
+    static int* addr[kMaxDevices] = {};
+    *out = nullptr;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (addr[dev] == nullptr) {
+        int* p = nullptr;
+        e = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), scarf_static_tickets);
+        if (e != cudaSuccess) return e;
+        if (p == nullptr) return cudaErrorInvalidSymbol;
+        addr[dev] = p;
+    }
+    *out = addr[dev];
+    return cudaSuccess;
+}
+
+cudaError_t ff_v1_static_setup() { int* p; return static_tickets(&p); }
+
+// Same kernel, same launch geometry as launch_ff_v1; a.tickets is ignored and replaced by the static array, whose first
+// n_tiles entries are cleared on `st` first.  No allocation.  n_tiles beyond the array: cudaErrorInvalidValue (the C-ABI
+// entry point checks the size before it gets here and reports the limit).
+cudaError_t launch_ff_v1_static(int NS, V1Args a, cudaStream_t st)
+{
+    if (a.n_q <= 0 || a.n_chunks <= 0) return cudaSuccess;
+    if (a.n_tiles > kStaticTickets) return cudaErrorInvalidValue;
+    a.tickets = nullptr;
+    if (a.n_chunks > 1) {
+        int* t = nullptr;
+        cudaError_t e = static_tickets(&t);
+        if (e != cudaSuccess) return e;
+        e = cudaMemsetAsync(t, 0, (size_t)a.n_tiles * sizeof(int), st);
+        if (e != cudaSuccess) return e;
+        a.tickets = t;
+    }
+    return launch_ff_v1(NS, a, st);
 }
 
 }  // namespace scarf

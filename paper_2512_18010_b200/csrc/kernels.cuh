@@ -140,6 +140,10 @@ struct V1Args {
 };
 int v1_tile_q();                            // q-points per CTA
 cudaError_t launch_ff_v1(int NS, const V1Args& a, cudaStream_t st);
+// allocation-free variant (scarf_form_factors_noalloc): tickets in a static device array of v1_static_tiles() entries
+int v1_static_tiles();
+cudaError_t ff_v1_static_setup();            // resolves the array's address on the current device (once per device)
+cudaError_t launch_ff_v1_static(int NS, V1Args a, cudaStream_t st);
 
 // high classes (ff_highl.cu): pairs with g, h, i shells (L = 7..12); runs after the unrolled kernel and ADDS to out.
 struct HighLArgs {

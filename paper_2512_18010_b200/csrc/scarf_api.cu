@@ -715,6 +715,71 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
     }
 }
 
+// Allocation-free S4 (include/scarf.h): the launches of scarf_form_factors for device q / device out, with the tickets of the
+// ordered fix-up in ff_v1.cu's static device array.  Nothing here allocates device memory or synchronises.
+int scarf_form_factors_noalloc(scarf_ctx* ctx, int64_t n_q, const double* q_dev, double* out_dev)
+{
+    static_assert(SCARF_NOALLOC_MAX_TILES == 65536, "keep in step with kStaticTickets (ff_v1.cu)");
+    if (!ctx) return SCARF_EINVAL;
+    if (ctx->host_only) return fail(ctx, SCARF_ENODEVICE, "form_factors_noalloc: host-only context; there is no CPU fallback");
+    if (!ctx->have_T) return fail(ctx, SCARF_ESTATE, "form_factors_noalloc: set_basis and set_transitions first");
+    if (n_q < 0) return fail(ctx, SCARF_EINVAL, "form_factors_noalloc: n_q < 0");
+    if (n_q == 0) return SCARF_OK;
+    const long long n_tiles = (n_q + v1_tile_q() - 1) / v1_tile_q();
+    if (v1_static_tiles() != SCARF_NOALLOC_MAX_TILES) return fail(ctx, SCARF_EINVAL, "form_factors_noalloc: library built inconsistently");
+    if (n_tiles > SCARF_NOALLOC_MAX_TILES)
+        return fail(ctx, SCARF_EINVAL, "form_factors_noalloc: n_q = " + std::to_string((long long)n_q) + " exceeds the static scratch (" +
+                                           std::to_string(SCARF_NOALLOC_MAX_TILES) + " tiles of " + std::to_string(v1_tile_q()) + " q-points = " +
+                                           std::to_string((long long)SCARF_NOALLOC_MAX_TILES * v1_tile_q()) +
+                                           " q-points per call); split the point set or use scarf_form_factors");
+    if (!q_dev || !out_dev) return fail(ctx, SCARF_EINVAL, "form_factors_noalloc: null q or out");
+    try {
+        CU(cudaSetDevice(ctx->device), "form_factors_noalloc");
+        if (!is_device_ptr(q_dev) || !is_device_ptr(out_dev))
+            return fail(ctx, SCARF_EINVAL, "form_factors_noalloc: q and out must be device pointers (staging host data would allocate)");
+        cudaStream_t st = ctx->stream;
+        if (harvest_screen(ctx, false) != SCARF_OK) return SCARF_ECUDA;          // non-blocking
+        if (ctx->T_bad) return fail(ctx, SCARF_EINVAL, std::string("form_factors_noalloc: ") + kBadT);
+        CU(ff_v1_static_setup(), "form_factors_noalloc: static scratch address");
+        int launches = 0;
+        if (ctx->qcut_dev) {                       // q-adaptive cut-off: counters were allocated by set_transitions
+            CU(cudaMemsetAsync(ctx->d_work.p, 0, kNClasses * sizeof(unsigned long long), st), "form_factors_noalloc: clear counters");
+            ctx->last_q_tiles = 0.0; ctx->last_ctr = kCtr; ctx->work_pending = true;
+        }
+        for (const TileStream& t : ctx->tiles) {
+            V1Args a = {};
+            a.base = t.base;
+            a.desc = t.desc;
+            a.q = q_dev;
+            a.n_q = n_q;
+            a.n_tiles = (int)n_tiles;
+            a.n_chunks = choose_chunks(ctx, n_tiles, kCtr, t.ns_real, ctx->n_chunks_opt);
+            a.ns_real = t.ns_real;
+            a.dst = out_dev + (size_t)t.s0 * n_q * 2;
+            a.qcut = ctx->qcut_dev;
+            a.work = ctx->qcut_dev ? static_cast<unsigned long long*>(ctx->d_work.p) : nullptr;
+            if (&t == &ctx->tiles.front()) ctx->last_q_tiles += (double)n_tiles;
+            CU(launch_plan_chunks(t.desc, a.n_chunks, t.ns_real, kCtr, st), "form_factors_noalloc: chunk planning kernel");
+            CU(launch_ff_v1_static(t.NS, a, st), "form_factors_noalloc: kernel");
+            ctx->st.last_n_chunks = a.n_chunks;
+            launches += 2;
+            if (has_high_classes(ctx->hs)) {            // pairs with g, h, i shells: separate kernel, adds to out
+                HighLArgs h = {};
+                h.base = t.base; h.desc = t.desc; h.q = q_dev;
+                h.ns_real = t.ns_real; h.n_points = n_q; h.n_q = n_q; h.dst = a.dst;
+                CU(launch_ff_highl(h, st), "form_factors_noalloc: high-class kernel");
+                ++launches;
+            }
+        }
+        ctx->st.last_kernel_launches = launches;
+        return SCARF_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(ctx, SCARF_ENOMEM, "form_factors_noalloc: out of host memory");
+    } catch (...) {
+        return fail(ctx, SCARF_EINVAL, "form_factors_noalloc: unexpected exception");
+    }
+}
+
 int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_t ny, const double* qy, int32_t nz,
                             const double* qz, double* out)
 {
