@@ -450,8 +450,15 @@ def run_ours(args):
     kW = [2, 7, 13, 23, 38, 59, 87] + [0] * 6
     poly_per_q = float(sum(n * w.n_states * kW[c] for c, n in enumerate(st["pairs_kept_per_class"])))
     if path == "grid":
-        slots = st["last_grid_kernel_slots"]
+        slots = st["last_grid_kernel_slots"]        # the kernel's own count: W_grid(L) = 2, 6, 10.5, 17, n_herm + 3 ... and 6 per (q, pair)
         roofline = alu_roofline(slots, head["main_kernel_ms"], "ff_grid_kernel<12>", poly_per_q * n_eval_q)
+        # the same time against the monomial-form model of the list kernel (n_herm + 3 per (q, pair, state)),
+        # i.e. the slots this launch would have cost without sharing the (q_y, q_z) part between a thread's two points
+        survey_slots = n_eval_q * (poly_per_q + 6.0 * st["n_pairs_kept"] * len(range(0, w.n_states, 12)))
+        roofline["frac_survey_model"] = survey_slots / (head["main_kernel_ms"] * 1e-3) / peak_meas
+        roofline["slots_model_note"] = ("frac: FP64 slots the kernel's algorithm needs (two points of a thread share the (q_y, q_z) part of "
+                                        "every polynomial: 6 / 10.5 / 17 slots per (q, pair, state) for L = 1 / 2 / 3); frac_survey_model: "
+                                        "the monomial-form count n_herm + 3 over the same time")
         alg_bytes = st["stream_bytes"] + 16.0 * w.n_states * w.n_q + 32.0 * st["n_pairs_kept"] * (n_eval_q ** (1 / 3))
     else:
         slots = st["slots_per_q"] * w.n_q

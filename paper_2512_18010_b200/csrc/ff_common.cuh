@@ -216,6 +216,102 @@ __device__ __forceinline__ void make_monomials(const double (&qv)[kNQ][4], doubl
     }
 }
 
+// ---- product grid: two points that differ in q_x only (ff_grid.cu; the thread's points (ixl, iy, iz), (ixl + 2, iy, iz)) ----
+// Eq. (48)'s polynomial, sorted by the power of q_x:  A + iB = sum_t q_x^t (Ce_t + i Co_t),
+//   Ce_t = sum_{(u,v): t+u+v even} D_tuv q_y^u q_z^v,   Co_t likewise for t+u+v odd
+// (i^n is folded into D).  The (q_y, q_z) sums are the same for both points: evaluated ONCE per (record, state), then
+// each point needs only the short polynomial in its own q_x.  FP64 slots per (q, pair, state), accumulate included:
+// L = 1: 5 + 2/2 = 6 (monomial form: 7), L = 2: 7 + 7/2 = 10.5 (13), L = 3: 9 + 16/2 = 17 (23).
+__host__ __device__ constexpr int yz_index(int u, int v) { return (u + v) * (u + v + 1) / 2 - 1 + v; }   // u + v >= 1
+__host__ __device__ constexpr int yz_count(int L) { return (L + 1) * (L + 2) / 2 - 1; }
+// is h the first Hermite index (in stream order) of its (parity of n, t) group?
+__host__ __device__ constexpr bool xgroup_first(int h)
+{
+    for (int g = 0; g < h; ++g)
+        if (((hdeg(g) ^ hdeg(h)) & 1) == 0 && hexp(g, 0) == hexp(h, 0)) return false;
+    return true;
+}
+__host__ __device__ constexpr bool xgroup_exists(int L, int par, int t)
+{
+    for (int h = 0; h < nherm(L); ++h)
+        if ((hdeg(h) & 1) == par && hexp(h, 0) == t) return true;
+    return false;
+}
+
+// yzm[yz_index(u, v)] = q_y^u q_z^v (1 <= u + v <= L); xp[j][t] = q_x(point j)^t
+template <int L>
+__device__ __forceinline__ void make_xpair_monomials(const double (&qv)[kNQ][4], double (&yzm)[yz_count(L) > 0 ? yz_count(L) : 1],
+                                                     double (&xp)[kNQ][L + 1])
+{
+    static_for<yz_count(L)>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        constexpr int d = i < 2 ? 1 : (i < 5 ? 2 : 3);
+        constexpr int v = i - (d * (d + 1) / 2 - 1), u = d - v;
+        if constexpr (d == 1) yzm[i] = v ? qv[0][2] : qv[0][1];
+        else if constexpr (u > 0) yzm[i] = yzm[yz_index(u - 1, v)] * qv[0][1];
+        else yzm[i] = yzm[yz_index(u, v - 1)] * qv[0][2];
+    });
+#pragma unroll
+    for (int j = 0; j < kNQ; ++j) {
+        xp[j][0] = 1.0;
+#pragma unroll
+        for (int t = 1; t <= L; ++t) xp[j][t] = t == 1 ? qv[j][0] : xp[j][t - 1] * qv[j][0];
+    }
+}
+
+template <int L, int NS>
+__device__ __forceinline__ void record_accum_xpair(const double2* __restrict__ r2, const double (&yzm)[yz_count(L) > 0 ? yz_count(L) : 1],
+                                                   const double (&xp)[kNQ][L + 1], const double (&gc)[kNQ], const double (&gs)[kNQ],
+                                                   double (&re)[kNQ][NS], double (&im)[kNQ][NS])
+{
+    static_assert(L <= 3, "degree blocks take over beyond L = 3");
+    constexpr int NH = nherm(L), N = NS * NH;
+    const double2* __restrict__ D2 = r2 + 2;
+    double G[2][L + 1];                                   // [parity of n][t]: the (q_y, q_z) sums of the current state
+    static_for<(N + 1) / 2>([&](auto i2c) {
+        constexpr int i2 = decltype(i2c)::value;
+        const double2 c = D2[i2];
+        static_for<2>([&](auto halfc) {
+            constexpr int half = decltype(halfc)::value;
+            constexpr int i = 2 * i2 + half;
+            if constexpr (i < N) {
+                constexpr int s = i / NH, h = i % NH;
+                constexpr int t = hexp(h, 0), u = hexp(h, 1), v = hexp(h, 2), par = hdeg(h) & 1;
+                const double cv = half ? c.y : c.x;
+                if constexpr (u + v == 0) G[par][t] = cv;            // lowest degree of its group: always its first term
+                else if constexpr (xgroup_first(h)) G[par][t] = cv * yzm[yz_index(u, v)];
+                else G[par][t] = fma(cv, yzm[yz_index(u, v)], G[par][t]);
+                if constexpr (h == NH - 1) {
+#pragma unroll
+                    for (int j = 0; j < kNQ; ++j) {
+                        double A = G[0][0], B = 0.0;
+                        static_for<L>([&](auto tc) {
+                            constexpr int tt = decltype(tc)::value + 1;
+                            if constexpr (xgroup_exists(L, 0, tt)) A = fma(G[0][tt], xp[j][tt], A);
+                        });
+                        if constexpr (L > 0) {
+                            if constexpr (xgroup_exists(L, 1, 0)) B = G[1][0];
+                            static_for<L>([&](auto tc) {
+                                constexpr int tt = decltype(tc)::value + 1;
+                                if constexpr (xgroup_exists(L, 1, tt)) {
+                                    if constexpr (tt == 1 && !xgroup_exists(L, 1, 0)) B = G[1][1] * xp[j][1];
+                                    else B = fma(G[1][tt], xp[j][tt], B);
+                                }
+                            });
+                        }
+                        re[j][s] = fma(gc[j], A, re[j][s]);
+                        im[j][s] = fma(gs[j], A, im[j][s]);
+                        if constexpr (L > 0) {
+                            re[j][s] = fma(-gs[j], B, re[j][s]);
+                            im[j][s] = fma(gc[j], B, im[j][s]);
+                        }
+                    }
+                }
+            }
+        });
+    });
+}
+
 
 // ---- high classes (L >= 4): degree-block evaluation ---------------------------------------------------------
 // Holding all n_herm(L) monomials of two q-points in registers is impossible beyond L = 3 (35..84 doubles per

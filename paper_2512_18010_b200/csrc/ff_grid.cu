@@ -144,10 +144,13 @@ __device__ __forceinline__ void run_class_grid(GPipe& pp, const GridArgs& a, con
                 accum_blocks<L, NS>(sp + k0 * REC, nb, qv, gcb, gsb, re, im);
             }
         } else
-        static_for<kNQ / NQA>([&](auto jc) {
-            constexpr int jq0 = decltype(jc)::value * NQA;
-            double mono[NQA][nherm(L)];
-            make_monomials<L, NQA, jq0>(qv, mono);
+        {
+            // L <= 3: the thread's two points share (q_y, q_z): the (y, z) part of every polynomial is evaluated once for both
+            // (ff_common.cuh: record_accum_xpair)
+            constexpr int jq0 = 0;
+            static_assert(NQA == kNQ, "both points together");
+            double yzm[yz_count(L) > 0 ? yz_count(L) : 1], xp[kNQ][L + 1];
+            make_xpair_monomials<L>(qv, yzm, xp);
             auto rec = [&](int k) { return reinterpret_cast<const double2*>(sp + k * REC); };
             auto factors = [&](int k, double (&gc)[NQA], double (&gs)[NQA]) {      // g = X Y Z for this thread's points
                 const double2 yz = cmul(Ys[k * kGridBY + iyl], Zs[k * kGridBZ + izl]);
@@ -171,29 +174,29 @@ __device__ __forceinline__ void run_class_grid(GPipe& pp, const GridArgs& a, con
 #pragma unroll
                         for (int u = 0; u < U; ++u) factors(k + U + u, gcn[u], gsn[u]);
 #pragma unroll
-                        for (int u = 0; u < U; ++u) record_accum<L, NS, NQA, jq0>(rec(k + u), mono, gc[u], gs[u], re, im);
+                        for (int u = 0; u < U; ++u) record_accum_xpair<L, NS>(rec(k + u), yzm, xp, gc[u], gs[u], re, im);
 #pragma unroll
                         for (int u = 0; u < U; ++u)
 #pragma unroll
                             for (int jj = 0; jj < NQA; ++jj) { gc[u][jj] = gcn[u][jj]; gs[u][jj] = gsn[u][jj]; }
                     }
 #pragma unroll
-                    for (int u = 0; u < U; ++u) record_accum<L, NS, NQA, jq0>(rec(n_full - U + u), mono, gc[u], gs[u], re, im);
+                    for (int u = 0; u < U; ++u) record_accum_xpair<L, NS>(rec(n_full - U + u), yzm, xp, gc[u], gs[u], re, im);
                 }
 #pragma unroll 1
                 for (int k = n_full; k < cnt; ++k) {
                     factors(k, gc[0], gs[0]);
-                    record_accum<L, NS, NQA, jq0>(rec(k), mono, gc[0], gs[0], re, im);
+                    record_accum_xpair<L, NS>(rec(k), yzm, xp, gc[0], gs[0], re, im);
                 }
             } else {
 #pragma unroll 1
                 for (int k = 0; k < cnt; ++k) {
                     double gc[NQA], gs[NQA];
                     factors(k, gc, gs);
-                    record_accum<L, NS, NQA, jq0>(rec(k), mono, gc, gs, re, im);
+                    record_accum_xpair<L, NS>(rec(k), yzm, xp, gc, gs, re, im);
                 }
             }
-        });
+        }
         __syncthreads();                                 // the slot is free again
         if (producer && j + kStages < n_st) issue(j + kStages);
     }

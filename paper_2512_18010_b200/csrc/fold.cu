@@ -383,10 +383,12 @@ cudaError_t launch_adaptive_sort(const AdaptArgs& a, cudaStream_t st)
 // Split the fast classes of the class-sorted stream into exactly K chunks of (nearly) equal modelled cost
 // (w(c) = ns_real W(c) + ctr FP64 issue slots per record and q-point); a chunk may span classes; trailing chunks may be
 // empty when there are fewer records than chunks.  One thread: <= K + 7 loop trips.
-__global__ void plan_chunks_kernel(StreamDesc* d, int K, int ns_real, double ctr)
+__global__ void plan_chunks_kernel(StreamDesc* d, int K, int ns_real, double ctr, bool grid_model)
 {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    const double kW[kFastMaxClass + 1] = {2, 7, 13, 23, 38, 59, 87};
+    // slots per (q, pair, state): n_herm + 3; the product-grid kernel shares the (q_y, q_z) part between its two points
+    const double kWl[kFastMaxClass + 1] = {2, 7, 13, 23, 38, 59, 87}, kWg[kFastMaxClass + 1] = {2, 6, 10.5, 17, 38, 59, 87};
+    const double* kW = grid_model ? kWg : kWl;
     double w[kFastMaxClass + 1], total = 0.0;
     for (int c = 0; c <= kFastMaxClass; ++c) {
         w[c] = (double)ns_real * kW[c] + ctr;
@@ -429,9 +431,9 @@ __global__ void plan_chunks_kernel(StreamDesc* d, int K, int ns_real, double ctr
 #endif
 }
 
-cudaError_t launch_plan_chunks(StreamDesc* desc, int K, int ns_real, double ctr, cudaStream_t st)
+cudaError_t launch_plan_chunks(StreamDesc* desc, int K, int ns_real, double ctr, cudaStream_t st, bool grid_model)
 {
-    plan_chunks_kernel<<<1, 32, 0, st>>>(desc, K, ns_real, ctr);
+    plan_chunks_kernel<<<1, 32, 0, st>>>(desc, K, ns_real, ctr, grid_model);
     return cudaGetLastError();
 }
 

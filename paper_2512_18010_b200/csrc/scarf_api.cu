@@ -37,6 +37,9 @@ const double kW[kNClasses] = {2, 7, 13, 23, 38, 59, 87, 123, 168, 223, 289, 367,
 const double kCtr = 40.0;
 // product-grid kernel: YZ = Y Z, g0 = X0 YZ, g1 = X1 YZ: 12 slots per 2 q-points; tables: 39 per (pair, axis point)
 const double kCtrGrid = 6.0, kCtrTable = 39.0;
+// ... and its polynomial: the two points of a thread share (q_y, q_z), whose part is evaluated once (ff_common.cuh:
+// record_accum_xpair): 6, 10.5, 17 slots for L = 1, 2, 3 instead of 7, 13, 23; the other classes as in the list kernel
+const double kWGrid[kNClasses] = {2, 6, 10.5, 17, 38, 59, 87, 123, 168, 223, 289, 367, 458};
 
 }  // namespace
 
@@ -899,7 +902,7 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
                 a.v.n_tiles = (int)tiles_s;
                 a.v.n_chunks = choose_chunks(ctx, tiles_s, kCtrGrid, t.ns_real, ctx->n_chunks_opt);
                 if (int rc = prepare_tickets(ctx, tiles_s, a.v.n_chunks, st, &a.v.tickets)) return n_slabs > 1 ? drain(rc) : rc;
-                CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, kCtrGrid, st), "form_factors_grid: chunk planning kernel");
+                CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, kCtrGrid, st, /*grid_model=*/true), "form_factors_grid: chunk planning kernel");
                 if (ctx->timing) CU(cudaEventRecord(ctx->ev_m0, st), "form_factors_grid: event");
                 CU(launch_ff_grid(t.NS, a, st), "form_factors_grid: kernel");
                 if (ctx->timing) {
@@ -1348,7 +1351,7 @@ int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out)
         double slots = 0.0, tab = 0.0;
         const double nt = (double)ctx->tiles.size();
         for (int c = 0; c < kNClasses; ++c) {
-            slots += (double)ctx->st.pairs_kept_per_class[c] * ctx->grid_eval_points * ((double)ctx->n_states * kW[c] + nt * kCtrGrid);
+            slots += (double)ctx->st.pairs_kept_per_class[c] * ctx->grid_eval_points * ((double)ctx->n_states * kWGrid[c] + nt * kCtrGrid);
             tab += (double)ctx->st.pairs_kept_per_class[c] * nt * ctx->grid_table_cols * kCtrTable;
         }
         ctx->st.last_grid_slots = slots + tab;
@@ -1365,7 +1368,7 @@ int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out)
                 const double nt = (double)std::max<size_t>(1, ctx->tiles.size());
                 double done = 0.0, full = 0.0;
                 for (int c = 0; c <= kFastMaxClass; ++c) {
-                    const double w = (double)ctx->n_states / nt * kW[c] + ctx->last_ctr;
+                    const double w = (double)ctx->n_states / nt * (ctx->last_ctr == kCtrGrid ? kWGrid[c] : kW[c]) + ctx->last_ctr;
                     done += (double)wk[c] * w;
                     full += (double)ctx->st.pairs_kept_per_class[c] * ctx->last_q_tiles * nt * w;
                 }
