@@ -268,6 +268,14 @@ def run_ours(args):
         step_grid()
         sc.set_option("grid_symmetry", 1)
 
+    def step_grid_box():                    # the box kernel (ff_grid.cu) where the row kernel (ff_row.cu) is the automatic choice
+        sc.set_option("grid_variant", 0)
+        step_grid()
+        sc.set_option("grid_variant", -1)
+
+    def grid_kernel_name(stats):
+        return "ff_row_kernel<12>" if stats.get("last_grid_variant", 0) == 1 else "ff_grid_kernel<12>"
+
     def run_timed(step, steps, warmup, sample_clocks=False):
         """W untimed steps, then `steps` steps timed with CUDA events on the library's stream (L2 flushed before each,
         outside the events), asynchronous (no per-call sync); then the same steps again with the library's per-kernel
@@ -324,9 +332,10 @@ def run_ours(args):
         return {"ms_per_step": ms, "job_seconds": ms * 1e-3, "kernel_ms": r["kernel_ms"], "main_kernel_ms": r["main_kernel_ms"],
                 "fold_ms": r["fold_ms"], "value": world * s2["evals_per_q"] * n_q_exec / (ms * 1e-3), "unit": UNIT,
                 "slots_main_kernel": slots, "n_chunks": s2["last_n_chunks"],
+                "kernel": grid_kernel_name(s2) if slots_key == "grid" else "ff_v1_kernel<12>",
                 "launches_per_step": int(s2["last_kernel_launches"] + s2["last_fold_launches"])}
 
-    list_path = grid_path = grid_plain = None
+    list_path = grid_path = grid_plain = grid_box = None
     if cartesian:
         if path == "grid":
             list_path = dict(side(step_list, w.n_q, "list"), api="scarf_form_factors")
@@ -334,6 +343,10 @@ def run_ours(args):
             n_ax = w.grid["n_per_axis"]
             grid_path = dict(side(step_grid, ((n_ax + 1) // 2) * n_ax * n_ax, "grid"), api="scarf_form_factors_grid", symmetric=True)
         grid_plain = dict(side(step_grid_plain, w.n_q, "grid"), api="scarf_form_factors_grid", symmetric=False)
+        if st.get("last_grid_variant", 0) == 1 or (grid_path is not None and grid_path["kernel"].startswith("ff_row")):
+            n_ax = w.grid["n_per_axis"]
+            grid_box = dict(side(step_grid_box, ((n_ax + 1) // 2) * n_ax * n_ax, "grid"), api="scarf_form_factors_grid", symmetric=True,
+                            option="grid_variant = 0")
         (step_grid if path == "grid" else step_list)()        # leave the headline path's result in out_dev for the parity sample
         torch.cuda.synchronize()
 
@@ -450,15 +463,21 @@ def run_ours(args):
     kW = [2, 7, 13, 23, 38, 59, 87] + [0] * 6
     poly_per_q = float(sum(n * w.n_states * kW[c] for c, n in enumerate(st["pairs_kept_per_class"])))
     if path == "grid":
-        slots = st["last_grid_kernel_slots"]        # the kernel's own count: W_grid(L) = 2, 6, 10.5, 17, n_herm + 3 ... and 6 per (q, pair)
-        roofline = alu_roofline(slots, head["main_kernel_ms"], "ff_grid_kernel<12>", poly_per_q * n_eval_q)
+        slots = st["last_grid_kernel_slots"]        # the kernel's own count: W(L) per (q, pair, state) (n_herm + 3 beyond L = 3) and 6 per (q, pair)
+        roofline = alu_roofline(slots, head["main_kernel_ms"], grid_kernel_name(st), poly_per_q * n_eval_q)
         # the same time against the monomial-form model of the list kernel (n_herm + 3 per (q, pair, state)),
         # i.e. the slots this launch would have cost without sharing the (q_y, q_z) part between a thread's two points
         survey_slots = n_eval_q * (poly_per_q + 6.0 * st["n_pairs_kept"] * len(range(0, w.n_states, 12)))
         roofline["frac_survey_model"] = survey_slots / (head["main_kernel_ms"] * 1e-3) / peak_meas
-        roofline["slots_model_note"] = ("frac: FP64 slots the kernel's algorithm needs (two points of a thread share the (q_y, q_z) part of "
-                                        "every polynomial: 6 / 10.5 / 17 slots per (q, pair, state) for L = 1 / 2 / 3); frac_survey_model: "
-                                        "the monomial-form count n_herm + 3 over the same time")
+        if st.get("last_grid_variant", 0) == 1:
+            roofline["slots_model_note"] = ("frac: FP64 slots the kernel's algorithm needs (the 64 points of a warp's row share the (q_x, q_y) "
+                                            "part of every polynomial: 5 / 7 / 9 slots per (q, pair, state) for L = 1 / 2 / 3 plus the "
+                                            "per-row part, 2 / 7 / 16 slots per (row, pair, state)); frac_survey_model: the monomial-form "
+                                            "count n_herm + 3 over the same time")
+        else:
+            roofline["slots_model_note"] = ("frac: FP64 slots the kernel's algorithm needs (two points of a thread share the (q_y, q_z) part "
+                                            "of every polynomial: 6 / 10.5 / 17 slots per (q, pair, state) for L = 1 / 2 / 3); "
+                                            "frac_survey_model: the monomial-form count n_herm + 3 over the same time")
         alg_bytes = st["stream_bytes"] + 16.0 * w.n_states * w.n_q + 32.0 * st["n_pairs_kept"] * (n_eval_q ** (1 / 3))
     else:
         slots = st["slots_per_q"] * w.n_q
@@ -493,10 +512,10 @@ def run_ours(args):
             "gpu_launches": int(steps * (st["last_kernel_launches"] + st["last_fold_launches"])),
             "clocks": clocks, "roofline": roofline}
 
-    for name, obj, kname, nq_exec in (("list_path", list_path, "ff_v1_kernel<12>", w.n_q), ("grid_path", grid_path, "ff_grid_kernel<12>", None),
-                                      ("grid_path_no_symmetry", grid_plain, "ff_grid_kernel<12>", w.n_q)):
+    for name, obj in (("list_path", list_path), ("grid_path", grid_path), ("grid_path_no_symmetry", grid_plain),
+                      ("grid_path_box_kernel", grid_box)):
         if obj is not None:
-            obj["roofline"] = alu_roofline(obj["slots_main_kernel"], obj["main_kernel_ms"], kname)
+            obj["roofline"] = alu_roofline(obj["slots_main_kernel"], obj["main_kernel_ms"], obj["kernel"])
             line[name] = obj
     if angular is not None:
         line["angular_moments"] = angular

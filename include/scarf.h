@@ -97,6 +97,8 @@ typedef struct scarf_stats {
     double last_grid_kernel_slots;             /* FP64 issue-slot model of the product-grid S4 kernel alone (no tables)*/
     double adaptive_bound;                     /* option adaptive_tol: |f_s(q) - exact| <= this for every q, s (0 when off) */
     double last_adaptive_work_fraction;        /* modelled work of the last S4 call / work without the cut-off (1 when off) */
+    int32_t last_grid_variant;                 /* kernel of the last scarf_form_factors_grid call: 0 box, 1 row (option grid_variant) */
+    int32_t reserved0;
 } scarf_stats;
 
 /* device >= 0: CUDA ordinal.  device < 0: host-only context (set_basis, overlap, stats work; the rest ENODEVICE). */
@@ -131,6 +133,11 @@ int scarf_set_stream(scarf_ctx* ctx, void* cuda_stream);
  *           "grid_symmetry": default 1.  scarf_form_factors_grid evaluates only one half of a product grid whose three
  *                         axes are antisymmetric bit for bit (ax[i] == -ax[n-1-i]) and stores conj f for the mirror
  *                         points (f(-q) = conj f(q), exact for real T); 0 always evaluates every point.
+ *           "grid_variant": default -1 (automatic).  Kernel of scarf_form_factors_grid: 0 = box kernel (a CTA owns a 4 x 8 x 8
+ *                         box of the grid; the two points of a thread share (q_y, q_z)), 1 = row kernel (a warp owns 64
+ *                         consecutive z-points of one (ix, iy) row, so the (q_x, q_y) part of every polynomial is evaluated
+ *                         once per warp: fewer FP64 operations per point, but lanes beyond the end of a row idle), -1 = the
+ *                         row kernel when its 4 (y) x 64 (z) boxes are at least 80 % full.  Same results to round-off.
  *           "fft_density_variant": default 1 = FP64 tensor-core (DMMA) density kernel of scarf_fft_form_factors with the
  *                         orbital values evaluated per point tile in shared memory (falls back to 2 when the tile of a
  *                         very large basis does not fit), 2 = DMMA kernel reading orbital values tabulated in device

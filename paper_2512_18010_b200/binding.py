@@ -38,7 +38,8 @@ class ScarfStats(C.Structure):
                 ("last_grid_slots", C.c_double), ("dropped_bound", C.c_double),
                 ("last_grid_symmetric", C.c_int32), ("last_n_chunks", C.c_int32),
                 ("last_main_kernel_ms", C.c_double), ("last_grid_kernel_slots", C.c_double),
-                ("adaptive_bound", C.c_double), ("last_adaptive_work_fraction", C.c_double)]
+                ("adaptive_bound", C.c_double), ("last_adaptive_work_fraction", C.c_double),
+                ("last_grid_variant", C.c_int32), ("reserved0", C.c_int32)]
 
     def as_dict(self):
         d = {}

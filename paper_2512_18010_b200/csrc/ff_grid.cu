@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(256) grid_table_kernel(const GridArgs a, doubl
                                                          double2* __restrict__ tz)
 {
     const StreamDesc& d = *a.v.desc;
-    const int NXp = a.nbx * kGridBX, NYp = a.nby * kGridBY, NZp = a.nbz * kGridBZ, ncol = NXp + NYp + NZp;
+    const int NXp = a.nbx * a.bxs, NYp = a.nby * a.bys, NZp = a.nbz * a.bzs, ncol = NXp + NYp + NZp;
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= d.n_kept * ncol) return;
     const long long r = idx / ncol;
@@ -64,11 +64,11 @@ __global__ void __launch_bounds__(256) grid_table_kernel(const GridArgs a, doubl
         if (r >= d.cls_first[k]) c = k;
     const double* hdr = reinterpret_cast<const double*>(a.v.base + d.cls_off[c] + (size_t)(r - d.cls_first[c]) * d.rec_bytes[c]);
     const double inv4p = hdr[3];
-    int axis = 0, n = a.nx_eval, B = kGridBX;
+    int axis = 0, n = a.nx_eval, B = a.bxs;
     const double* ax = a.qx;
     double2* tab = tx;
-    if (col >= NXp + NYp) { axis = 2; col -= NXp + NYp; n = a.nz; B = kGridBZ; ax = a.qz; tab = tz; }
-    else if (col >= NXp) { axis = 1; col -= NXp; n = a.ny; B = kGridBY; ax = a.qy; tab = ty; }
+    if (col >= NXp + NYp) { axis = 2; col -= NXp + NYp; n = a.nz; B = a.bzs; ax = a.qz; tab = tz; }
+    else if (col >= NXp) { axis = 1; col -= NXp; n = a.ny; B = a.bys; ax = a.qy; tab = ty; }
     double2 v = make_double2(0.0, 0.0);
     if (col < n) {
         const double q = ax[col];
@@ -337,7 +337,7 @@ __global__ void __launch_bounds__(kThreads, 2) ff_grid_kernel(const GridArgs a)
 
 cudaError_t launch_grid_tables(const GridArgs& a, double2* tx, double2* ty, double2* tz, cudaStream_t st)
 {
-    const long long ncol = (long long)a.nbx * kGridBX + (long long)a.nby * kGridBY + (long long)a.nbz * kGridBZ;
+    const long long ncol = (long long)a.nbx * a.bxs + (long long)a.nby * a.bys + (long long)a.nbz * a.bzs;
     const long long n = a.n_rows * ncol;
     if (n <= 0) return cudaSuccess;
     grid_table_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(a, tx, ty, tz);

@@ -383,12 +383,14 @@ cudaError_t launch_adaptive_sort(const AdaptArgs& a, cudaStream_t st)
 // Split the fast classes of the class-sorted stream into exactly K chunks of (nearly) equal modelled cost
 // (w(c) = ns_real W(c) + ctr FP64 issue slots per record and q-point); a chunk may span classes; trailing chunks may be
 // empty when there are fewer records than chunks.  One thread: <= K + 7 loop trips.
-__global__ void plan_chunks_kernel(StreamDesc* d, int K, int ns_real, double ctr, bool grid_model)
+__global__ void plan_chunks_kernel(StreamDesc* d, int K, int ns_real, double ctr, int model)
 {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     // slots per (q, pair, state): n_herm + 3; the product-grid kernel shares the (q_y, q_z) part between its two points
-    const double kWl[kFastMaxClass + 1] = {2, 7, 13, 23, 38, 59, 87}, kWg[kFastMaxClass + 1] = {2, 6, 10.5, 17, 38, 59, 87};
-    const double* kW = grid_model ? kWg : kWl;
+    // and the row kernel the (q_x, q_y) part between the 64 points of a warp
+    const double kWl[kFastMaxClass + 1] = {2, 7, 13, 23, 38, 59, 87}, kWg[kFastMaxClass + 1] = {2, 6, 10.5, 17, 38, 59, 87},
+                 kWr[kFastMaxClass + 1] = {2, 5.03, 7.11, 9.25, 38, 59, 87};
+    const double* kW = model == 2 ? kWr : (model == 1 ? kWg : kWl);
     double w[kFastMaxClass + 1], total = 0.0;
     for (int c = 0; c <= kFastMaxClass; ++c) {
         w[c] = (double)ns_real * kW[c] + ctr;
@@ -431,9 +433,9 @@ __global__ void plan_chunks_kernel(StreamDesc* d, int K, int ns_real, double ctr
 #endif
 }
 
-cudaError_t launch_plan_chunks(StreamDesc* desc, int K, int ns_real, double ctr, cudaStream_t st, bool grid_model)
+cudaError_t launch_plan_chunks(StreamDesc* desc, int K, int ns_real, double ctr, cudaStream_t st, int model)
 {
-    plan_chunks_kernel<<<1, 32, 0, st>>>(desc, K, ns_real, ctr, grid_model);
+    plan_chunks_kernel<<<1, 32, 0, st>>>(desc, K, ns_real, ctr, model);
     return cudaGetLastError();
 }
 

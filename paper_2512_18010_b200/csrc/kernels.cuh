@@ -121,7 +121,8 @@ cudaError_t launch_screen(const ScreenArgs& a, cudaStream_t st);
 cudaError_t launch_pack(const PackArgs& a, cudaStream_t st);
 // cost-balanced split of the FAST classes (0..kFastMaxClass) of the stream into exactly K chunks (K <= kMaxChunks);
 // w(c) = ns_real * W(c) + ctr.  One thread; ~2 us.
-cudaError_t launch_plan_chunks(StreamDesc* desc, int K, int ns_real, double ctr, cudaStream_t st, bool grid_model = false);
+// model: per-class slot counts of 0 the list kernel, 1 the box kernel (ff_grid.cu), 2 the row kernel (ff_row.cu)
+cudaError_t launch_plan_chunks(StreamDesc* desc, int K, int ns_real, double ctr, cudaStream_t st, int model = 0);
 
 // v1 (ff_v1.cu): the general-q kernel.  Grid = (n_tiles, n_chunks), dispatched chunk-major; the chunks of one q tile add
 // their partial sums into `out` in chunk order through a per-tile ticket (no partial buffer in HBM, no second kernel).
@@ -171,12 +172,19 @@ struct GridArgs {
     int bx0, pad0;                          // this launch covers x boxes bx0 .. bx0 + v.n_tiles/(nby*nbz) - 1 (host output is computed in x slabs)
     int sym, nx_eval;                       // sym != 0: the grid is inversion-symmetric (every axis ax[i] == -ax[n-1-i] bit for bit):
                                             // only ix < nx_eval = ceil(nx/2) is evaluated and f(-q) = conj f(q) is stored for the mirror point
-    const double2 *tx, *ty, *tz;            // tables [box][row][kGridB*] of (re, im); zero beyond the axis end
+    const double2 *tx, *ty, *tz;            // tables [box][row][box edge] of (re, im); zero beyond the axis end
     long long n_rows;                       // row stride of the tables (>= kept records; the prescreened count, known to the host)
+    int bxs, bys, bzs, pad1;                // box edges the tables are laid out for: kGridB* (ff_grid.cu) or kRowB* (ff_row.cu)
 };
 cudaError_t launch_grid_tables(const GridArgs& a, double2* tx, double2* ty, double2* tz, cudaStream_t st);
 cudaError_t launch_ff_grid(int NS, const GridArgs& a, cudaStream_t st);
 cudaError_t ff_grid_init_device();           // per-device function attributes (dynamic shared memory); idempotent
+// row decomposition (ff_row.cu): a warp owns one (ix, iy) row of 64 z-points, so the (q_x, q_y) part of every polynomial is
+// warp-uniform: it is evaluated once per (record, state, row) by the warp's lanes in parallel, and a point only needs the short
+// polynomial in its own q_z.  Same GridArgs, tables laid out for 1 x 4 x 64 boxes.
+constexpr int kRowBX = 1, kRowBY = 4, kRowBZ = 64;
+cudaError_t launch_ff_row(int NS, const GridArgs& a, cudaStream_t st);
+cudaError_t ff_row_init_device();
 cudaError_t launch_separable(const GridArgs& a, const double* wx, const double* wy, const double* wz, double* mom, double* part,
                              int per_block, cudaStream_t st);   // grids sized for a.n_rows records; part[block][16] complex
 

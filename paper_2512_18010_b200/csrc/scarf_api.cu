@@ -40,6 +40,9 @@ const double kCtrGrid = 6.0, kCtrTable = 39.0;
 // ... and its polynomial: the two points of a thread share (q_y, q_z), whose part is evaluated once (ff_common.cuh:
 // record_accum_xpair): 6, 10.5, 17 slots for L = 1, 2, 3 instead of 7, 13, 23; the other classes as in the list kernel
 const double kWGrid[kNClasses] = {2, 6, 10.5, 17, 38, 59, 87, 123, 168, 223, 289, 367, 458};
+// row kernel (ff_row.cu): a warp's 64 points share (q_x, q_y): 5, 7, 9 slots per point for L = 1, 2, 3 plus the pre-pass
+// (2, 7, 16 slots per (record, state)) spread over the 64 points of the row
+const double kWRow[kNClasses] = {2, 5 + 2 / 64.0, 7 + 7 / 64.0, 9 + 16 / 64.0, 38, 59, 87, 123, 168, 223, 289, 367, 458};
 
 }  // namespace
 
@@ -62,6 +65,8 @@ struct scarf_ctx {
     double last_q_tiles = 0.0;          // q tiles of the last S4 call (for the skipped-work statistics)
     double last_ctr = 40.0;
     int grid_symmetry = 1;    // 1: use f(-q) = conj f(q) on inversion-symmetric product grids; 0: never
+    int grid_variant = -1;    // product-grid kernel: 0 box kernel (ff_grid.cu), 1 row kernel (ff_row.cu), -1 by the grid's shape
+    const double* last_grid_w = nullptr;   // work model of the last product-grid call (kWGrid or kWRow)
     int fft_density_variant = 1;  // 1: DMMA kernel, 0: SIMT kernel (fft_method.cu)
     int check_parseval = 0;       // 1: scarf_fft_form_factors also evaluates both sides of Eq. (75)
     int parseval_states = 0;      // states whose sums the last scarf_fft_form_factors call left in d_parseval
@@ -243,6 +248,7 @@ int scarf_create(scarf_ctx** out, int device)
         e = cudaSetDevice(device);
         // per-device function attributes (idempotent; set for every context so that no process-wide flag is needed)
         if (e == cudaSuccess) e = ff_grid_init_device();
+        if (e == cudaSuccess) e = ff_row_init_device();
         if (e == cudaSuccess) e = angular_init_device();
         if (e == cudaSuccess) e = density_fused_init_device();
         if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->h_screen), sizeof(ScreenResult));
@@ -308,6 +314,9 @@ int scarf_set_option(scarf_ctx* ctx, const char* key, double value)
     } else if (k == "grid_symmetry") {
         if (value != 0.0 && value != 1.0) return fail(ctx, SCARF_EINVAL, "set_option: grid_symmetry must be 0 or 1");
         ctx->grid_symmetry = (int)value;
+    } else if (k == "grid_variant") {
+        if (value != 0.0 && value != 1.0 && value != -1.0) return fail(ctx, SCARF_EINVAL, "set_option: grid_variant must be -1, 0 or 1");
+        ctx->grid_variant = (int)value;
     } else if (k == "n_chunks") {
         if (value < 0 || value > kMaxChunks) return fail(ctx, SCARF_EINVAL, "set_option: n_chunks outside 0..32");
         ctx->n_chunks_opt = (int)value;
@@ -841,7 +850,13 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         for (int k = 0; k < 3 && sym; ++k)
             for (int i = 0; i < ax_n[k] && sym; ++i) sym = hax[k][(size_t)i] == -hax[k][(size_t)(ax_n[k] - 1 - i)];
         const int nx_eval = sym ? (nx + 1) / 2 : nx;
-        const int nbx = (nx_eval + kGridBX - 1) / kGridBX, nby = (ny + kGridBY - 1) / kGridBY, nbz = (nz + kGridBZ - 1) / kGridBZ;
+        // Kernel: the row kernel (a warp = 64 z-points of one (ix, iy) row, 4 rows per CTA) needs fewer FP64 slots per point but
+        // wastes the lanes beyond the end of a row; it is taken when the 4 x 64 boxes are at least 80 % full.
+        const double row_fill = ((double)ny * nz) / ((double)((ny + kRowBY - 1) / kRowBY * kRowBY) * (double)((nz + kRowBZ - 1) / kRowBZ * kRowBZ));
+        const bool row = ctx->grid_variant == 1 || (ctx->grid_variant < 0 && row_fill >= 0.8);
+        const int BXs = row ? kRowBX : kGridBX, BYs = row ? kRowBY : kGridBY, BZs = row ? kRowBZ : kGridBZ;
+        const double* kWg = row ? kWRow : kWGrid;
+        const int nbx = (nx_eval + BXs - 1) / BXs, nby = (ny + BYs - 1) / BYs, nbz = (nz + BZs - 1) / BZs;
         const long long n_tiles = (long long)nbx * nby * nbz;
         if (n_tiles > 0x7fffffffLL) return fail(ctx, SCARF_EINVAL, "form_factors_grid: grid too large for one call");
         const size_t obytes = (size_t)ctx->n_states * (size_t)n_q * 2 * sizeof(double);
@@ -858,7 +873,7 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
             CU(cudaMemsetAsync(ctx->d_work.p, 0, kNClasses * sizeof(unsigned long long), st), "form_factors_grid: clear counters");
             ctx->last_q_tiles = (double)n_tiles; ctx->last_ctr = kCtrGrid; ctx->work_pending = true;
         }
-        const long long ncol = (long long)nbx * kGridBX + (long long)nby * kGridBY + (long long)nbz * kGridBZ;
+        const long long ncol = (long long)nbx * BXs + (long long)nby * BYs + (long long)nbz * BZs;
         const long long n_rows = (long long)ctx->hs.pairs.size();    // prescreened pairs: an upper bound of the kept count
         const int n_slabs = (out_host && nbx >= 4 && n_q >= 4 * 16384 && !has_high_classes(ctx->hs)) ? 4 : 1;
         if (n_slabs > 1) {
@@ -873,8 +888,9 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
             if (tab_elems * 16 > (size_t)32e9) return fail(ctx, SCARF_ENOMEM, "form_factors_grid: factor tables would exceed 32 GB");
             CU(ctx->d_tab.ensure(tab_elems * 16), "form_factors_grid: alloc tables");
             double2* tx = static_cast<double2*>(ctx->d_tab.p);
-            double2* ty = tx + (size_t)n_rows * nbx * kGridBX;
-            double2* tz = ty + (size_t)n_rows * nby * kGridBY;
+            double2* ty = tx + (size_t)n_rows * nbx * BXs;
+            double2* tz = ty + (size_t)n_rows * nby * BYs;
+            a.bxs = BXs; a.bys = BYs; a.bzs = BZs;
             a.v.base = t.base;
             a.v.desc = t.desc;
             a.v.n_q = n_q;
@@ -902,9 +918,9 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
                 a.v.n_tiles = (int)tiles_s;
                 a.v.n_chunks = choose_chunks(ctx, tiles_s, kCtrGrid, t.ns_real, ctx->n_chunks_opt);
                 if (int rc = prepare_tickets(ctx, tiles_s, a.v.n_chunks, st, &a.v.tickets)) return n_slabs > 1 ? drain(rc) : rc;
-                CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, kCtrGrid, st, /*grid_model=*/true), "form_factors_grid: chunk planning kernel");
+                CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, kCtrGrid, st, /*model=*/row ? 2 : 1), "form_factors_grid: chunk planning kernel");
                 if (ctx->timing) CU(cudaEventRecord(ctx->ev_m0, st), "form_factors_grid: event");
-                CU(launch_ff_grid(t.NS, a, st), "form_factors_grid: kernel");
+                CU(row ? launch_ff_row(t.NS, a, st) : launch_ff_grid(t.NS, a, st), "form_factors_grid: kernel");
                 if (ctx->timing) {
                     CU(cudaEventRecord(ctx->ev_m1, st), "form_factors_grid: event");
                     CU(cudaEventSynchronize(ctx->ev_m1), "form_factors_grid: event sync");
@@ -916,7 +932,7 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
                 launches += 2;
                 if (n_slabs > 1) {
                     const long long plane = (long long)ny * nz;
-                    const long long ix0 = (long long)b0 * kGridBX, ix1 = std::min<long long>((long long)b1 * kGridBX, nx_eval);
+                    const long long ix0 = (long long)b0 * BXs, ix1 = std::min<long long>((long long)b1 * BXs, nx_eval);
                     cudaError_t e = cudaEventRecord(ctx->ev_slice, st);
                     if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_slice, 0);
                     for (int s = 0; s < t.ns_real && e == cudaSuccess; ++s) {
@@ -944,6 +960,8 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         ctx->grid_eval_points = (double)nx_eval * ny * nz;
         ctx->grid_table_cols = (double)(nx_eval + ny + nz);
         ctx->st.last_grid_symmetric = sym ? 1 : 0;
+        ctx->last_grid_w = kWg;
+        ctx->st.last_grid_variant = row ? 1 : 0;
         ctx->st.last_grid_slots = -1.0;            // filled by scarf_get_stats from the kept counts
         if (ctx->timing) {
             CU(cudaEventRecord(ctx->ev1, st), "form_factors_grid: event");
@@ -1351,7 +1369,7 @@ int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out)
         double slots = 0.0, tab = 0.0;
         const double nt = (double)ctx->tiles.size();
         for (int c = 0; c < kNClasses; ++c) {
-            slots += (double)ctx->st.pairs_kept_per_class[c] * ctx->grid_eval_points * ((double)ctx->n_states * kWGrid[c] + nt * kCtrGrid);
+            slots += (double)ctx->st.pairs_kept_per_class[c] * ctx->grid_eval_points * ((double)ctx->n_states * (ctx->last_grid_w ? ctx->last_grid_w : kWGrid)[c] + nt * kCtrGrid);
             tab += (double)ctx->st.pairs_kept_per_class[c] * nt * ctx->grid_table_cols * kCtrTable;
         }
         ctx->st.last_grid_slots = slots + tab;
@@ -1368,7 +1386,7 @@ int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out)
                 const double nt = (double)std::max<size_t>(1, ctx->tiles.size());
                 double done = 0.0, full = 0.0;
                 for (int c = 0; c <= kFastMaxClass; ++c) {
-                    const double w = (double)ctx->n_states / nt * (ctx->last_ctr == kCtrGrid ? kWGrid[c] : kW[c]) + ctx->last_ctr;
+                    const double w = (double)ctx->n_states / nt * (ctx->last_ctr == kCtrGrid ? (ctx->last_grid_w ? ctx->last_grid_w : kWGrid)[c] : kW[c]) + ctx->last_ctr;
                     done += (double)wk[c] * w;
                     full += (double)ctx->st.pairs_kept_per_class[c] * ctx->last_q_tiles * nt * w;
                 }
