@@ -9,12 +9,15 @@
 // ("pre-pass", into a warp-private shared-memory area), then every lane runs the short polynomial in its own q_z with the G as
 // broadcast coefficients.  FP64 slots per (q, pair, state), accumulate included: 2, 5, 7, 9 for L = 0..3 (ff_grid.cu: 2, 6, 10.5,
 // 17; monomial form: 2, 7, 13, 23) plus S(L)/64 for the pre-pass (S = 2, 7, 16).  Classes L >= 4 use the degree blocks of
-// ff_common.cuh as the other kernels do.
+// ff_common.cuh as the other kernels do.  The factor: X Y is the row's too (pre-pass, one lane per record), so a point needs
+// g = (X Y) Z only: 4 slots per (q, pair) instead of 6.
 //
-// A CTA = 4 warps = 4 consecutive iy at one ix: a 1 x 4 x 64 box.  Everything else — the pair stream through a 3-stage ring of 1-D
-// TMA bulk copies on one mbarrier per stage, per-axis factor tables [box][record][point in box], cost-balanced stream chunks that add
-// into `out` in chunk order through the box's ticket, the conjugate mirror store on inversion-symmetric grids, the q-adaptive
-// prefix — is the scheme of ff_grid.cu.
+// A CTA = 4 warps = 4 consecutive iy at one ix: a 1 x 4 x 64 box.  Everything else — the pair stream through a ring of 1-D TMA
+// bulk copies on one mbarrier per stage (two stages of up to 24 records here: a stage carries 1 KB of Z factors per record), per-axis
+// factor tables [box][record][point in box], cost-balanced stream chunks that add into `out` in chunk order through the box's
+// ticket, the conjugate mirror store on inversion-symmetric grids, the q-adaptive prefix — is the scheme of ff_grid.cu.
+// Measured on config 3 (64^3, symmetric half, B200): 6.41 ms against 7.52 ms for ff_grid.cu.  Not kept: three stages of 16 records
+// (6.51 ms), a last-arriver refill instead of the __syncthreads per stage (6.68 ms).
 #include "ff_common.cuh"
 
 namespace scarf {
@@ -23,12 +26,12 @@ namespace {
 
 constexpr int kThreads = 128;
 constexpr int kWarps = kThreads / 32;
-constexpr int kStages = 3;
-constexpr int kStageBytes = 8192;             // records of one stage (>= the largest record, L = 6, NS = 12)
-constexpr int kMaxRec = 16;                   // records per stage at most (bounds the table slices)
+constexpr int kStages = 2;
+constexpr int kStageBytes = 12288;            // records of one stage (>= the largest record, L = 6, NS = 12)
+constexpr int kMaxRec = 24;                   // records per stage at most (bounds the table slices)
 constexpr int kXB = kRowBX * 16, kYB = kRowBY * 16, kZB = kRowBZ * 16;   // table bytes per record and box
 constexpr int kSlotBytes = kStageBytes + kMaxRec * (kXB + kYB + kZB);
-static_assert(kRowBX == 1 && kRowBY == kWarps && kRowBZ == 32 * kNQ, "warp = one (ix, iy) row, two z-points per lane");
+static_assert(kMaxRec <= 32 && kRowBX == 1 && kRowBY == kWarps && kRowBZ == 32 * kNQ, "warp = one (ix, iy) row, two z-points per lane");
 
 // (parity of n, power of q_z) groups of class L, par 0 first, v ascending
 __host__ __device__ constexpr bool zgroup_exists(int L, int par, int v) { return ((v & 1) == par ? v : v + 1) <= L; }
@@ -56,6 +59,7 @@ __host__ __device__ constexpr int stage_records(int L, int NS)
     const int n = kStageBytes / (rec_doubles(L, NS) * 8);
     return n < kMaxRec ? n : kMaxRec;
 }
+// warp-private area: XY[kMaxRec] (the row's X_P(ix) Y_P(iy) of the stage's records, complex) followed by the G of the stage
 __host__ __device__ constexpr int g_warp_bytes(int NS)
 {
     int m = 16;
@@ -63,7 +67,7 @@ __host__ __device__ constexpr int g_warp_bytes(int NS)
         const int b = stage_records(L, NS) * g_stride(L, NS) * 8;
         if (b > m) m = b;
     }
-    return m;
+    return m + kMaxRec * 16;
 }
 template <int NS> constexpr int smem_bytes() { return kStages * kSlotBytes + kWarps * g_warp_bytes(NS) + 64; }
 
@@ -84,8 +88,15 @@ template <int L, int NS>
 __device__ __forceinline__ void row_prepass(const unsigned char* sp, int cnt, const double (&xym)[yz_count(L)], double* Gw, int lane)
 {
     constexpr int REC = rec_doubles(L, NS) * 8, NH = nherm(L), NG = zgroup_count(L), GS = g_stride(L, NS);
-#pragma unroll 1
-    for (int i = lane; i < cnt * NS; i += 32) {
+    // Unrolled over the at most TRIPS items of a lane (a rolled loop cost 1 % of the kernel more).  Measured alternatives: two or
+    // three items per branch-free group, so that their loads are in flight together, shorten the pre-pass (3.8 % -> 2.2 % of the
+    // samples for L = 1) but the kernel as a whole got 1.4 % slower (the main loops lost what the pre-pass gained).
+    constexpr int TRIPS = (stage_records(L, NS) * NS + 31) / 32;
+    const int n = cnt * NS;
+#pragma unroll 5
+    for (int tr = 0; tr < TRIPS; ++tr) {
+        const int i = lane + 32 * tr;
+        if (i >= n) break;
         const int k = i / NS, s = i - k * NS;
         const double* D = reinterpret_cast<const double*>(sp + k * REC) + 4 + s * NH;
         double G[NG];
@@ -143,7 +154,7 @@ __device__ __forceinline__ void record_accum_row(const double2* __restrict__ G2,
 // r0 = stream-order index of the segment's first record (row of the tables).  qv[j] = (q_x, q_y, q_z of point j, 0).
 template <int L, int NS>
 __device__ __forceinline__ void run_class_row(RPipe& pp, const GridArgs& a, const char* __restrict__ seg, long long r0, int n_rec,
-                                              int bx, int by, int bz, int warp, int lane, double* Gw,
+                                              int bx, int by, int bz, int warp, int lane, double* Ww,
                                               const double (&qv)[kNQ][4], double (&re)[kNQ][NS], double (&im)[kNQ][NS])
 {
     constexpr int REC = rec_doubles(L, NS) * 8;
@@ -185,8 +196,13 @@ __device__ __forceinline__ void run_class_row(RPipe& pp, const GridArgs& a, cons
         const double2* Xs = reinterpret_cast<const double2*>(sp + kStageBytes);
         const double2* Ys = reinterpret_cast<const double2*>(sp + kStageBytes + kMaxRec * kXB) + warp;
         const double2* Zs = reinterpret_cast<const double2*>(sp + kStageBytes + kMaxRec * (kXB + kYB)) + lane;
+        // pre-pass, part 1: X Y of the row, once per record (lane k: record k) instead of once per lane and record
+        double2* XYw = reinterpret_cast<double2*>(Ww);
+        double* Gw = Ww + 2 * kMaxRec;
+        if (lane < cnt) XYw[lane] = cmul(Xs[lane * kRowBX], Ys[lane * kRowBY]);
+        if constexpr (L == 0 || L >= 4) __syncwarp();
         auto factors = [&](int k, double (&gc)[kNQ], double (&gs)[kNQ]) {      // g = X Y Z for this lane's points
-            const double2 xy = cmul(Xs[k * kRowBX], Ys[k * kRowBY]);
+            const double2 xy = XYw[k];
 #pragma unroll
             for (int jj = 0; jj < kNQ; ++jj) {
                 const double2 gq = cmul(Zs[k * kRowBZ + 32 * jj], xy);
@@ -268,7 +284,7 @@ __global__ void __launch_bounds__(kThreads, 2) ff_row_kernel(const GridArgs a)
     __syncthreads();
     RPipe pp = {smem, full_bar, 0u};
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    double* Gw = reinterpret_cast<double*>(smem + kStages * kSlotBytes + 64 + warp * g_warp_bytes(NS));
+    double* Ww = reinterpret_cast<double*>(smem + kStages * kSlotBytes + 64 + warp * g_warp_bytes(NS));   // the warp's private area
 
     const int bz = tile % a.nbz, by = (tile / a.nbz) % a.nby, bx = a.bx0 + tile / (a.nbz * a.nby);
     const int ix = bx, iy = by * kRowBY + warp;
@@ -339,7 +355,7 @@ __global__ void __launch_bounds__(kThreads, 2) ff_row_kernel(const GridArgs a)
     }
 #define SCARF_ROW_CLASS(LV)                                                                                          \
     if (s_nrec[LV] > 0)                                                                                              \
-        run_class_row<LV, NS>(pp, a, a.v.base + s_off[LV], s_row[LV], s_nrec[LV], bx, by, bz, warp, lane, Gw, qv, re, im);
+        run_class_row<LV, NS>(pp, a, a.v.base + s_off[LV], s_row[LV], s_nrec[LV], bx, by, bz, warp, lane, Ww, qv, re, im);
     SCARF_ROW_CLASS(0)
     SCARF_ROW_CLASS(1)
     SCARF_ROW_CLASS(2)

@@ -185,6 +185,23 @@ cudaError_t ff_grid_init_device();           // per-device function attributes (
 constexpr int kRowBX = 1, kRowBY = 4, kRowBZ = 64;
 cudaError_t launch_ff_row(int NS, const GridArgs& a, cudaStream_t st);
 cudaError_t ff_row_init_device();
+// spherical product grid (ff_sph.cu): q = r_i n_d, n_d = (sin t_j cos phi_k, sin t_j sin phi_k, cos t_j), d = j n_phi + k; point index
+// i * n_theta * n_phi + d (the layout of scarf_angular_moments' input).  A warp owns one direction and 64 radii.
+constexpr int kSphBD = 4, kSphBR = 64;
+struct SphArgs {
+    V1Args v;                               // stream, desc, dst, tickets, qcut as for v1; v.q unused; v.n_q = n_r * n_theta * n_phi
+    const double* r;                        // [n_r] radii (device)
+    const double* dirs;                     // [n_theta * n_phi][3] unit vectors (device); with `sym` dirs[mirror(d)] == -dirs[d] exactly
+    int n_r, n_theta, n_phi;
+    int n_dir_eval;                         // directions evaluated: all, or the first half (in d order) of an inversion-symmetric grid
+    int n_rbox, n_dbox;                     // tiles = n_dbox * n_rbox (radius box fastest)
+    int sym, pad0;
+    const double* te;                       // table E[rbox][row][kSphBR] = exp(-r^2/4p); zero beyond the last radius
+    long long n_rows;                       // row stride of the table (the prescreened pair count)
+};
+cudaError_t launch_sph_table(const SphArgs& a, double* te, cudaStream_t st);
+cudaError_t launch_ff_sph(int NS, const SphArgs& a, cudaStream_t st);
+cudaError_t ff_sph_init_device();
 cudaError_t launch_separable(const GridArgs& a, const double* wx, const double* wy, const double* wz, double* mom, double* part,
                              int per_block, cudaStream_t st);   // grids sized for a.n_rows records; part[block][16] complex
 

@@ -42,6 +42,8 @@ const double kCtrGrid = 6.0, kCtrTable = 39.0;
 const double kWGrid[kNClasses] = {2, 6, 10.5, 17, 38, 59, 87, 123, 168, 223, 289, 367, 458};
 // row kernel (ff_row.cu): a warp's 64 points share (q_x, q_y): 5, 7, 9 slots per point for L = 1, 2, 3 plus the pre-pass
 // (2, 7, 16 slots per (record, state)) spread over the 64 points of the row
+// ... and 4 slots per point for g = (X Y) Z, X Y once per (row, pair): 4 more, spread over the row's 64 points
+const double kCtrRow = 4.0 + 4.0 / 64.0;
 const double kWRow[kNClasses] = {2, 5 + 2 / 64.0, 7 + 7 / 64.0, 9 + 16 / 64.0, 38, 59, 87, 123, 168, 223, 289, 367, 458};
 
 }  // namespace
@@ -67,6 +69,8 @@ struct scarf_ctx {
     int grid_symmetry = 1;    // 1: use f(-q) = conj f(q) on inversion-symmetric product grids; 0: never
     int grid_variant = -1;    // product-grid kernel: 0 box kernel (ff_grid.cu), 1 row kernel (ff_row.cu), -1 by the grid's shape
     const double* last_grid_w = nullptr;   // work model of the last product-grid call (kWGrid or kWRow)
+    double last_grid_ctr = 6.0;            // ... and its per-(q, pair) slots (kCtrGrid or kCtrRow)
+    bool last_was_grid = false;            // the last S4 call was scarf_form_factors_grid
     int fft_density_variant = 1;  // 1: DMMA kernel, 0: SIMT kernel (fft_method.cu)
     int check_parseval = 0;       // 1: scarf_fft_form_factors also evaluates both sides of Eq. (75)
     int parseval_states = 0;      // states whose sums the last scarf_fft_form_factors call left in d_parseval
@@ -628,7 +632,7 @@ int scarf_form_factors(scarf_ctx* ctx, int64_t n_q, const double* q, double* out
         double main_ms = 0.0;
         if (ctx->qcut_dev) {
             CU(cudaMemsetAsync(ctx->d_work.p, 0, kNClasses * sizeof(unsigned long long), st), "form_factors: clear counters");
-            ctx->last_q_tiles = 0.0; ctx->last_ctr = kCtr; ctx->work_pending = true;
+            ctx->last_q_tiles = 0.0; ctx->last_ctr = kCtr; ctx->last_was_grid = false; ctx->work_pending = true;
         }
         // all state tiles for the q range [dq, dq + 3 n_q) into dout [n_states][n_q]
         auto run_range = [&](const double* dq, long long n_q, double* dout) -> int {
@@ -756,7 +760,7 @@ int scarf_form_factors_noalloc(scarf_ctx* ctx, int64_t n_q, const double* q_dev,
         int launches = 0;
         if (ctx->qcut_dev) {                       // q-adaptive cut-off: counters were allocated by set_transitions
             CU(cudaMemsetAsync(ctx->d_work.p, 0, kNClasses * sizeof(unsigned long long), st), "form_factors_noalloc: clear counters");
-            ctx->last_q_tiles = 0.0; ctx->last_ctr = kCtr; ctx->work_pending = true;
+            ctx->last_q_tiles = 0.0; ctx->last_ctr = kCtr; ctx->last_was_grid = false; ctx->work_pending = true;
         }
         for (const TileStream& t : ctx->tiles) {
             V1Args a = {};
@@ -856,6 +860,7 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         const bool row = ctx->grid_variant == 1 || (ctx->grid_variant < 0 && row_fill >= 0.8);
         const int BXs = row ? kRowBX : kGridBX, BYs = row ? kRowBY : kGridBY, BZs = row ? kRowBZ : kGridBZ;
         const double* kWg = row ? kWRow : kWGrid;
+        const double ctr_g = row ? kCtrRow : kCtrGrid;
         const int nbx = (nx_eval + BXs - 1) / BXs, nby = (ny + BYs - 1) / BYs, nbz = (nz + BZs - 1) / BZs;
         const long long n_tiles = (long long)nbx * nby * nbz;
         if (n_tiles > 0x7fffffffLL) return fail(ctx, SCARF_EINVAL, "form_factors_grid: grid too large for one call");
@@ -871,7 +876,7 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         double main_ms = 0.0;
         if (ctx->qcut_dev) {
             CU(cudaMemsetAsync(ctx->d_work.p, 0, kNClasses * sizeof(unsigned long long), st), "form_factors_grid: clear counters");
-            ctx->last_q_tiles = (double)n_tiles; ctx->last_ctr = kCtrGrid; ctx->work_pending = true;
+            ctx->last_q_tiles = (double)n_tiles; ctx->last_ctr = ctr_g; ctx->last_was_grid = true; ctx->last_grid_w = kWg; ctx->work_pending = true;
         }
         const long long ncol = (long long)nbx * BXs + (long long)nby * BYs + (long long)nbz * BZs;
         const long long n_rows = (long long)ctx->hs.pairs.size();    // prescreened pairs: an upper bound of the kept count
@@ -916,9 +921,9 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
                 const long long tiles_s = (long long)(b1 - b0) * nby * nbz;
                 a.bx0 = b0;
                 a.v.n_tiles = (int)tiles_s;
-                a.v.n_chunks = choose_chunks(ctx, tiles_s, kCtrGrid, t.ns_real, ctx->n_chunks_opt);
+                a.v.n_chunks = choose_chunks(ctx, tiles_s, ctr_g, t.ns_real, ctx->n_chunks_opt);
                 if (int rc = prepare_tickets(ctx, tiles_s, a.v.n_chunks, st, &a.v.tickets)) return n_slabs > 1 ? drain(rc) : rc;
-                CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, kCtrGrid, st, /*model=*/row ? 2 : 1), "form_factors_grid: chunk planning kernel");
+                CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, ctr_g, st, /*model=*/row ? 2 : 1), "form_factors_grid: chunk planning kernel");
                 if (ctx->timing) CU(cudaEventRecord(ctx->ev_m0, st), "form_factors_grid: event");
                 CU(row ? launch_ff_row(t.NS, a, st) : launch_ff_grid(t.NS, a, st), "form_factors_grid: kernel");
                 if (ctx->timing) {
@@ -961,6 +966,7 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         ctx->grid_table_cols = (double)(nx_eval + ny + nz);
         ctx->st.last_grid_symmetric = sym ? 1 : 0;
         ctx->last_grid_w = kWg;
+        ctx->last_grid_ctr = ctr_g;
         ctx->st.last_grid_variant = row ? 1 : 0;
         ctx->st.last_grid_slots = -1.0;            // filled by scarf_get_stats from the kept counts
         if (ctx->timing) {
@@ -1369,7 +1375,7 @@ int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out)
         double slots = 0.0, tab = 0.0;
         const double nt = (double)ctx->tiles.size();
         for (int c = 0; c < kNClasses; ++c) {
-            slots += (double)ctx->st.pairs_kept_per_class[c] * ctx->grid_eval_points * ((double)ctx->n_states * (ctx->last_grid_w ? ctx->last_grid_w : kWGrid)[c] + nt * kCtrGrid);
+            slots += (double)ctx->st.pairs_kept_per_class[c] * ctx->grid_eval_points * ((double)ctx->n_states * (ctx->last_grid_w ? ctx->last_grid_w : kWGrid)[c] + nt * ctx->last_grid_ctr);
             tab += (double)ctx->st.pairs_kept_per_class[c] * nt * ctx->grid_table_cols * kCtrTable;
         }
         ctx->st.last_grid_slots = slots + tab;
@@ -1386,7 +1392,7 @@ int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out)
                 const double nt = (double)std::max<size_t>(1, ctx->tiles.size());
                 double done = 0.0, full = 0.0;
                 for (int c = 0; c <= kFastMaxClass; ++c) {
-                    const double w = (double)ctx->n_states / nt * (ctx->last_ctr == kCtrGrid ? (ctx->last_grid_w ? ctx->last_grid_w : kWGrid)[c] : kW[c]) + ctx->last_ctr;
+                    const double w = (double)ctx->n_states / nt * (ctx->last_was_grid ? (ctx->last_grid_w ? ctx->last_grid_w : kWGrid)[c] : kW[c]) + ctx->last_ctr;
                     done += (double)wk[c] * w;
                     full += (double)ctx->st.pairs_kept_per_class[c] * ctx->last_q_tiles * nt * w;
                 }
