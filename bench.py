@@ -92,8 +92,9 @@ def parse():
     ap.add_argument("--seed", type=int, default=None)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target wall time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--path", default="auto", choices=["auto", "grid", "list"],
-                    help="S4 entry point of the headline step: product-grid API or arbitrary point list (auto: grid on the Cartesian configs)")
+    ap.add_argument("--path", default="auto", choices=["auto", "grid", "list", "sph"],
+                    help="S4 entry point of the headline step: Cartesian product-grid API, spherical product-grid API or arbitrary point list "
+                         "(auto: grid on the Cartesian configs, sph on the spherical one)")
     ap.add_argument("--fft-grid", type=int, default=None, help="points per axis of the FFT-method grid (default: the config's q grid size)")
     return ap.parse_args()
 
@@ -241,9 +242,16 @@ def run_ours(args):
     w = W.make_workload(args.config, overlap, seed=args.seed)
     sc.set_basis(w.basis)
     cartesian = w.grid.get("kind") == "cartesian"
-    path = args.path if args.path != "auto" else ("grid" if cartesian else "list")
+    spherical = w.grid.get("kind") == "spherical"
+    path = args.path if args.path != "auto" else ("grid" if cartesian else ("sph" if spherical else "list"))
     if path == "grid" and not cartesian:
         raise SystemExit("--path grid needs a Cartesian product grid (configs 1-4)")
+    if path == "sph" and not spherical:
+        raise SystemExit("--path sph needs the spherical product grid (config 5)")
+    if spherical:
+        sph_r = np.geomspace(w.grid["qmin"], w.grid["qmax"], w.grid["n_r"])
+        sph_ct, _sph_w = np.polynomial.legendre.leggauss(w.grid["n_theta"])
+        sph_nphi = w.grid["n_phi"]
     T_dev = torch.as_tensor(w.T, device="cuda")
     q_dev = torch.as_tensor(w.q, device="cuda")
     out_dev = torch.empty((w.n_states, w.n_q, 2), dtype=torch.float64, device="cuda")
@@ -263,6 +271,15 @@ def run_ours(args):
         sc.set_transitions(T_dev)
         sc.form_factors_grid(ax_host, ax_host, ax_host, out=out_dev)
 
+    def step_sph():
+        sc.set_transitions(T_dev)
+        sc.form_factors_sph(sph_r, sph_ct, sph_nphi, out=out_dev)
+
+    def step_sph_plain():
+        sc.set_option("grid_symmetry", 0)
+        step_sph()
+        sc.set_option("grid_symmetry", 1)
+
     def step_grid_plain():
         sc.set_option("grid_symmetry", 0)
         step_grid()
@@ -274,7 +291,7 @@ def run_ours(args):
         sc.set_option("grid_variant", -1)
 
     def grid_kernel_name(stats):
-        return "ff_row_kernel<12>" if stats.get("last_grid_variant", 0) == 1 else "ff_grid_kernel<12>"
+        return {1: "ff_row_kernel<12>", 2: "ff_sph_kernel<12>"}.get(stats.get("last_grid_variant", 0), "ff_grid_kernel<12>")
 
     def run_timed(step, steps, warmup, sample_clocks=False):
         """W untimed steps, then `steps` steps timed with CUDA events on the library's stream (L2 flushed before each,
@@ -313,12 +330,19 @@ def run_ours(args):
                 "main_kernel_ms_mean": float(np.mean(main))}
 
     steps, warmup = args.steps, max(3, args.warmup)
-    head = run_timed(step_grid if path == "grid" else step_list, steps, warmup, sample_clocks=True)
+    step_head = {"grid": step_grid, "sph": step_sph, "list": step_list}[path]
+    head = run_timed(step_head, steps, warmup, sample_clocks=True)
     st = head["stats"]
     n_eval_q = w.n_q
     if path == "grid" and st["last_grid_symmetric"]:
         n_ax = w.grid["n_per_axis"]
         n_eval_q = ((n_ax + 1) // 2) * n_ax * n_ax
+
+    def sph_eval_points():
+        n_t, n_p = w.grid["n_theta"], w.grid["n_phi"]
+        return w.grid["n_r"] * ((n_t // 2) * n_p + (n_p // 2 if n_t % 2 else 0))
+    if path == "sph" and st["last_grid_symmetric"]:
+        n_eval_q = sph_eval_points()
     evals_per_step = st["evals_per_q"] * n_eval_q                      # executed (q, kept pair, state) triples
     value, ms_per_step = replicas.whole_job_value(evals_per_step, steps, head["sum_ms"], "cuda")
     clocks = head["clocks"]
@@ -335,7 +359,15 @@ def run_ours(args):
                 "kernel": grid_kernel_name(s2) if slots_key == "grid" else "ff_v1_kernel<12>",
                 "launches_per_step": int(s2["last_kernel_launches"] + s2["last_fold_launches"])}
 
-    list_path = grid_path = grid_plain = grid_box = None
+    list_path = grid_path = grid_plain = grid_box = sph_path = sph_plain = None
+    if spherical:
+        if path == "sph":
+            list_path = dict(side(step_list, w.n_q, "list"), api="scarf_form_factors")
+        else:
+            sph_path = dict(side(step_sph, sph_eval_points(), "grid"), api="scarf_form_factors_sph", symmetric=True)
+        sph_plain = dict(side(step_sph_plain, w.n_q, "grid"), api="scarf_form_factors_sph", symmetric=False)
+        step_head()                                            # leave the headline path's result in out_dev for the parity sample
+        torch.cuda.synchronize()
     if cartesian:
         if path == "grid":
             list_path = dict(side(step_list, w.n_q, "list"), api="scarf_form_factors")
@@ -420,6 +452,8 @@ def run_ours(args):
         sc.set_transitions(T_host)
         if path == "grid":
             sc.form_factors_grid(ax_host, ax_host, ax_host, out=out_host)
+        elif path == "sph":
+            sc.form_factors_sph(sph_r, sph_ct, sph_nphi, out=out_host)
         else:
             sc.form_factors(q_host, out=out_host)
 
@@ -435,7 +469,7 @@ def run_ours(args):
         e2e_s = (time.perf_counter() - t0) / e2e_steps
     e2e_s = replicas.max_over_ranks(e2e_s, "cuda")
     e2e_value = world * evals_per_step / e2e_s
-    h2d = T_host.numel() * 8 + (3 * ax_host.size * 8 if path == "grid" else q_host.numel() * 8)
+    h2d = T_host.numel() * 8 + (3 * ax_host.size * 8 if path == "grid" else ((sph_r.size + sph_ct.size) * 8 if path == "sph" else q_host.numel() * 8))
     d2h = out_host.numel() * 8
 
     if rank != 0:
@@ -479,6 +513,16 @@ def run_ours(args):
                                             "of every polynomial: 6 / 10.5 / 17 slots per (q, pair, state) for L = 1 / 2 / 3); "
                                             "frac_survey_model: the monomial-form count n_herm + 3 over the same time")
         alg_bytes = st["stream_bytes"] + 16.0 * w.n_states * w.n_q + 32.0 * st["n_pairs_kept"] * (n_eval_q ** (1 / 3))
+    elif path == "sph":
+        slots = st["last_grid_kernel_slots"]        # the kernel's own count: W(L) = 2, 5, 6, 7 (+ the per-direction sums / 64), n_herm + 3 beyond L = 3; 22 per (q, pair)
+        roofline = alu_roofline(slots, head["main_kernel_ms"], grid_kernel_name(st), poly_per_q * n_eval_q)
+        survey_slots = n_eval_q * st["slots_per_q"]
+        roofline["frac_survey_model"] = survey_slots / (head["main_kernel_ms"] * 1e-3) / peak_meas
+        roofline["slots_model_note"] = ("frac: FP64 slots the kernel's algorithm needs (the 64 radii of a warp's direction share the phase slope "
+                                        "n.P and the per-degree sums of the polynomial: 5 / 6 / 7 slots per (q, pair, state) for L = 1 / 2 / 3 and "
+                                        "22 per (q, pair)); frac_survey_model: the list kernel's count (n_herm + 3, and 40 per (q, pair)) over "
+                                        "the same time")
+        alg_bytes = st["stream_bytes"] + 16.0 * w.n_states * w.n_q + 8.0 * st["n_pairs_kept"] * w.grid["n_r"]
     else:
         slots = st["slots_per_q"] * w.n_q
         roofline = alu_roofline(slots, head["main_kernel_ms"], "ff_v1_kernel<12>", poly_per_q * w.n_q)
@@ -497,8 +541,8 @@ def run_ours(args):
             "config": {"workload": w.name, "config": args.config, "seed": w.seed, "n_q": w.n_q, "n_states": w.n_states,
                        "nbf": w.basis.nbf, "n_pairs_all": st["n_pairs_all"], "n_pairs_kept": st["n_pairs_kept"],
                        "pairs_kept_per_class": st["pairs_kept_per_class"], "cond_S": w.cond_S,
-                       "s4_api": "scarf_form_factors_grid" if path == "grid" else "scarf_form_factors",
-                       "inversion_symmetry_used": bool(path == "grid" and st["last_grid_symmetric"]),
+                       "s4_api": {"grid": "scarf_form_factors_grid", "sph": "scarf_form_factors_sph", "list": "scarf_form_factors"}[path],
+                       "inversion_symmetry_used": bool(path in ("grid", "sph") and st["last_grid_symmetric"]),
                        "q_points_evaluated": int(n_eval_q),
                        "l2": "flushed between timed steps (256 MB write, untimed)",
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
@@ -513,7 +557,7 @@ def run_ours(args):
             "clocks": clocks, "roofline": roofline}
 
     for name, obj in (("list_path", list_path), ("grid_path", grid_path), ("grid_path_no_symmetry", grid_plain),
-                      ("grid_path_box_kernel", grid_box)):
+                      ("grid_path_box_kernel", grid_box), ("sph_path", sph_path), ("sph_path_no_symmetry", sph_plain)):
         if obj is not None:
             obj["roofline"] = alu_roofline(obj["slots_main_kernel"], obj["main_kernel_ms"], obj["kernel"])
             line[name] = obj

@@ -97,7 +97,7 @@ typedef struct scarf_stats {
     double last_grid_kernel_slots;             /* FP64 issue-slot model of the product-grid S4 kernel alone (no tables)*/
     double adaptive_bound;                     /* option adaptive_tol: |f_s(q) - exact| <= this for every q, s (0 when off) */
     double last_adaptive_work_fraction;        /* modelled work of the last S4 call / work without the cut-off (1 when off) */
-    int32_t last_grid_variant;                 /* kernel of the last scarf_form_factors_grid call: 0 box, 1 row (option grid_variant) */
+    int32_t last_grid_variant;                 /* kernel of the last product-grid call: 0 box, 1 row (option grid_variant), 2 scarf_form_factors_sph */
     int32_t reserved0;
 } scarf_stats;
 
@@ -213,6 +213,22 @@ int scarf_form_factors_noalloc(scarf_ctx* ctx, int64_t n_q, const double* q_dev,
  * host memory when the call must stay asynchronous.  scarf_stats.last_grid_symmetric says which path ran. */
 int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_t ny, const double* qy, int32_t nz,
                             const double* qz, double* out);
+
+/* The same f_s(q) on a SPHERICAL product grid — the grid of scarf_angular_moments (Eq. (57)-(60) PAPER.md:380-398):
+ *     q = r[i] (sin t_j cos phi_k, sin t_j sin phi_k, cos t_j),  cos t_j = cos_theta[j],  phi_k = 2 pi k / n_phi,
+ * out [n_states][n_r][n_theta][n_phi][2], point index (i*n_theta + j)*n_phi + k — exactly the input layout of
+ * scarf_angular_moments.  Along one direction n the polynomial of Eq. (48) PAPER.md:326-330 is a polynomial in r whose
+ * coefficients (the sums of D over each total degree, weighted with the monomials of n) and the phase slope n.P are the same for
+ * every radius: they are evaluated once per (direction, pair, state), the Gaussian e^{-r^2/4p} comes from a table per (pair, radius).
+ * Inversion symmetry (option "grid_symmetry", default on): when cos_theta[j] == -cos_theta[n_theta-1-j] bit for bit (Gauss-Legendre
+ * nodes) and n_phi is even, -q of a grid point is a grid point; half of the directions are evaluated and the mirror points get
+ * conj f (f(-q) = conj f(q), exact for real T).  The library builds the direction table itself (mirror directions are the exact
+ * negatives): its points agree with a caller's own list of the same grid to FP64 round-off of the trigonometric functions.
+ * r, cos_theta: HOST pointers (r finite, |cos_theta| <= 1).  out: host or device; with a device `out` the call is asynchronous
+ * on the context stream.  Results equal scarf_form_factors on the expanded point list up to FP64 round-off.  Bases with
+ * g, h, i shells run that list path internally.  scarf_stats: last_grid_symmetric, last_grid_variant = 2, last_grid_kernel_slots. */
+int scarf_form_factors_sph(scarf_ctx* ctx, int32_t n_r, const double* r, int32_t n_theta, const double* cos_theta, int32_t n_phi,
+                           double* out);
 
 /* Separable integrals (Eq. (64)-(65) PAPER.md:481-487): the weighted sum of f_s over a Cartesian product grid,
  *     out[s] = sum_{ix,iy,iz} fx[ix] gy[iy] hz[iz] f_s(qx[ix], qy[iy], qz[iz])        (fx = quadrature weight x f(qx), ...),

@@ -22,7 +22,7 @@ NOALLOC_MAX_TILES = 65536                  # SCARF_NOALLOC_MAX_TILES (include/sc
 NOALLOC_MAX_Q = NOALLOC_MAX_TILES * 256     # q-points per scarf_form_factors_noalloc call
 
 EXPORTS = ["scarf_create", "scarf_destroy", "scarf_set_stream", "scarf_set_option", "scarf_set_basis", "scarf_set_basis_pure", "scarf_nbf",
-           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_noalloc", "scarf_form_factors_grid", "scarf_separable_integral", "scarf_angular_moments", "scarf_oscillator_fit", "scarf_abs2", "scarf_fft_form_factors", "scarf_fft_parseval", "scarf_get_stats", "scarf_last_error",
+           "scarf_overlap", "scarf_set_transitions", "scarf_form_factors", "scarf_form_factors_noalloc", "scarf_form_factors_grid", "scarf_form_factors_sph", "scarf_separable_integral", "scarf_angular_moments", "scarf_oscillator_fit", "scarf_abs2", "scarf_fft_form_factors", "scarf_fft_parseval", "scarf_get_stats", "scarf_last_error",
            "scarf_version", "scarf_fp64_peak", "scarf_host_hermite_E", "scarf_host_shell_norms", "scarf_host_ylm_table"]
 
 
@@ -74,6 +74,7 @@ def _load():
     L.scarf_form_factors.argtypes = [vp, C.c_int64, vp, vp]
     L.scarf_form_factors_noalloc.argtypes = [vp, C.c_int64, vp, vp]
     L.scarf_form_factors_grid.argtypes = [vp, C.c_int32, vp, C.c_int32, vp, C.c_int32, vp, vp]
+    L.scarf_form_factors_sph.argtypes = [vp, C.c_int32, vp, C.c_int32, vp, C.c_int32, vp]
     L.scarf_separable_integral.argtypes = [vp, C.c_int32, dp, dp, C.c_int32, dp, dp, C.c_int32, dp, dp, dp]
     L.scarf_angular_moments.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, C.c_int32, C.c_int32, vp, vp, vp]
     L.scarf_abs2.argtypes = [vp, C.c_int64, vp, vp]
@@ -296,6 +297,31 @@ class Scarf:
         if not _is_torch(out) and okeep is not out:
             raise ValueError("form_factors_grid: out must be a C-contiguous float64 array")
         self._check(_lib.scarf_form_factors_grid(self._h, nx, xp, ny, yp, nz, zp, op))
+        if _is_torch(out):
+            import torch
+            return torch.view_as_complex(out.view(self.n_states, n_q, 2))
+        return out.reshape(self.n_states, n_q, 2).view(np.complex128)[..., 0]
+
+    def form_factors_sph(self, r, cos_theta, n_phi: int, out=None, device: bool = True):
+        """Spherical product grid q = r[i] (sin t_j cos phi_k, sin t_j sin phi_k, cos t_j), phi_k = 2 pi k / n_phi, point index
+        (i*n_theta + j)*n_phi + k (the input layout of angular_moments).  r, cos_theta: 1-D float64 host arrays.  `out`: torch
+        (host or cuda) or numpy [n_states][n_q][2]; if None a CUDA tensor (device=True) or a numpy array is allocated.
+        Returns complex128 [n_states][n_r*n_theta*n_phi] (a view of `out`)."""
+        rr = np.ascontiguousarray(r, dtype=np.float64)
+        ct = np.ascontiguousarray(cos_theta, dtype=np.float64)
+        n_r, n_theta = int(rr.shape[0]), int(ct.shape[0])
+        n_q = n_r * n_theta * int(n_phi)
+        if out is None:
+            if device:
+                import torch
+                out = torch.empty((self.n_states, n_q, 2), dtype=torch.float64, device="cuda")
+            else:
+                out = np.empty((self.n_states, n_q, 2))
+        op, okeep = _ptr(out, "out", self.n_states * n_q * 2)
+        if not _is_torch(out) and okeep is not out:
+            raise ValueError("form_factors_sph: out must be a C-contiguous float64 array")
+        self._check(_lib.scarf_form_factors_sph(self._h, n_r, rr.ctypes.data_as(C.c_void_p), n_theta, ct.ctypes.data_as(C.c_void_p),
+                                                int(n_phi), op))
         if _is_torch(out):
             import torch
             return torch.view_as_complex(out.view(self.n_states, n_q, 2))

@@ -121,7 +121,7 @@ cudaError_t launch_screen(const ScreenArgs& a, cudaStream_t st);
 cudaError_t launch_pack(const PackArgs& a, cudaStream_t st);
 // cost-balanced split of the FAST classes (0..kFastMaxClass) of the stream into exactly K chunks (K <= kMaxChunks);
 // w(c) = ns_real * W(c) + ctr.  One thread; ~2 us.
-// model: per-class slot counts of 0 the list kernel, 1 the box kernel (ff_grid.cu), 2 the row kernel (ff_row.cu)
+// model: per-class slot counts of 0 the list kernel, 1 the box kernel (ff_grid.cu), 2 the row kernel (ff_row.cu), 3 the spherical-grid kernel (ff_sph.cu)
 cudaError_t launch_plan_chunks(StreamDesc* desc, int K, int ns_real, double ctr, cudaStream_t st, int model = 0);
 
 // v1 (ff_v1.cu): the general-q kernel.  Grid = (n_tiles, n_chunks), dispatched chunk-major; the chunks of one q tile add

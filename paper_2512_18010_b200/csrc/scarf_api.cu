@@ -44,6 +44,11 @@ const double kWGrid[kNClasses] = {2, 6, 10.5, 17, 38, 59, 87, 123, 168, 223, 289
 // (2, 7, 16 slots per (record, state)) spread over the 64 points of the row
 // ... and 4 slots per point for g = (X Y) Z, X Y once per (row, pair): 4 more, spread over the row's 64 points
 const double kCtrRow = 4.0 + 4.0 / 64.0;
+// spherical-grid kernel (ff_sph.cu): a warp's 64 radii share the direction: per point r d_P, sincos, E cos, E sin = 22 slots, d_P = n.P
+// once per (direction, pair); the polynomial in r: 5, 6, 7 slots per point for L = 1, 2, 3 plus the per-direction sums G_n
+// (3, 9, 19 slots per (direction, pair, state)); the E table: one exp (16 slots) per (pair, radius)
+const double kCtrSph = 22.0 + 3.0 / 64.0, kCtrSphTable = 16.0;
+const double kWSph[kNClasses] = {2, 5 + 3 / 64.0, 6 + 9 / 64.0, 7 + 19 / 64.0, 38, 59, 87, 123, 168, 223, 289, 367, 458};
 const double kWRow[kNClasses] = {2, 5 + 2 / 64.0, 7 + 7 / 64.0, 9 + 16 / 64.0, 38, 59, 87, 123, 168, 223, 289, 367, 458};
 
 }  // namespace
@@ -70,6 +75,11 @@ struct scarf_ctx {
     int grid_variant = -1;    // product-grid kernel: 0 box kernel (ff_grid.cu), 1 row kernel (ff_row.cu), -1 by the grid's shape
     const double* last_grid_w = nullptr;   // work model of the last product-grid call (kWGrid or kWRow)
     double last_grid_ctr = 6.0;            // ... and its per-(q, pair) slots (kCtrGrid or kCtrRow)
+    double last_table_ctr = 39.0;          // ... and the slots per table entry (kCtrTable or kCtrSphTable)
+    // direction table of scarf_form_factors_sph and the arguments it was built for
+    std::vector<double> sph_ct;
+    int sph_n_phi = 0, sph_sym = -1;
+    DevBuf d_sph_dirs;
     bool last_was_grid = false;            // the last S4 call was scarf_form_factors_grid
     int fft_density_variant = 1;  // 1: DMMA kernel, 0: SIMT kernel (fft_method.cu)
     int check_parseval = 0;       // 1: scarf_fft_form_factors also evaluates both sides of Eq. (75)
@@ -219,7 +229,7 @@ void free_device(scarf_ctx* c)
 {
     c->d_pairs.release(); c->d_E.release(); c->d_bound.release(); c->d_T.release(); c->d_q.release();
     c->d_out.release(); c->d_keep.release(); c->d_desc.release(); c->d_screen.release(); c->d_tickets.release(); c->d_key.release(); c->d_keep2.release(); c->d_qcut.release(); c->d_work.release(); c->qcut_dev = nullptr; c->d_parseval.release(); c->parseval_states = 0;
-    c->d_axes.release(); c->d_tab.release();
+    c->d_axes.release(); c->d_tab.release(); c->d_sph_dirs.release();
     c->d_ang_in.release(); c->d_ang_F.release(); c->d_ang_tab.release(); c->d_ang_out.release();
     c->d_pure_map.release(); c->d_Tcart.release();
     c->d_prim.release(); c->d_V.release(); c->d_fft.release(); c->d_Csym.release();
@@ -253,6 +263,7 @@ int scarf_create(scarf_ctx** out, int device)
         // per-device function attributes (idempotent; set for every context so that no process-wide flag is needed)
         if (e == cudaSuccess) e = ff_grid_init_device();
         if (e == cudaSuccess) e = ff_row_init_device();
+        if (e == cudaSuccess) e = ff_sph_init_device();
         if (e == cudaSuccess) e = angular_init_device();
         if (e == cudaSuccess) e = density_fused_init_device();
         if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->h_screen), sizeof(ScreenResult));
@@ -967,6 +978,7 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         ctx->st.last_grid_symmetric = sym ? 1 : 0;
         ctx->last_grid_w = kWg;
         ctx->last_grid_ctr = ctr_g;
+        ctx->last_table_ctr = kCtrTable;
         ctx->st.last_grid_variant = row ? 1 : 0;
         ctx->st.last_grid_slots = -1.0;            // filled by scarf_get_stats from the kept counts
         if (ctx->timing) {
@@ -989,6 +1001,168 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         return fail(ctx, SCARF_ENOMEM, "form_factors_grid: out of host memory");
     } catch (...) {
         return fail(ctx, SCARF_EINVAL, "form_factors_grid: unexpected exception");
+    }
+}
+
+int scarf_form_factors_sph(scarf_ctx* ctx, int32_t n_r, const double* r, int32_t n_theta, const double* cos_theta, int32_t n_phi,
+                           double* out)
+{
+    if (!ctx) return SCARF_EINVAL;
+    if (ctx->host_only) return fail(ctx, SCARF_ENODEVICE, "form_factors_sph: host-only context; there is no CPU fallback");
+    if (!ctx->have_T) return fail(ctx, SCARF_ESTATE, "form_factors_sph: set_basis and set_transitions first");
+    if (n_r < 0 || n_theta < 0 || n_phi < 0) return fail(ctx, SCARF_EINVAL, "form_factors_sph: negative grid size");
+    const long long n_dir = (long long)n_theta * n_phi, n_q = n_dir * n_r;
+    if (n_q == 0) return SCARF_OK;
+    if (!r || !cos_theta || !out) return fail(ctx, SCARF_EINVAL, "form_factors_sph: null r, cos_theta or out");
+    if (is_device_ptr(r) || is_device_ptr(cos_theta)) return fail(ctx, SCARF_EINVAL, "form_factors_sph: r and cos_theta must be HOST pointers");
+    if (n_dir > 0x7fffffffLL / 4) return fail(ctx, SCARF_EINVAL, "form_factors_sph: too many directions for one call");
+    try {
+        if (!all_finite(r, (size_t)n_r) || !all_finite(cos_theta, (size_t)n_theta)) return fail(ctx, SCARF_EINVAL, "form_factors_sph: NaN/Inf in r or cos_theta");
+        for (int j = 0; j < n_theta; ++j)
+            if (std::fabs(cos_theta[j]) > 1.0) return fail(ctx, SCARF_EINVAL, "form_factors_sph: |cos_theta| > 1");
+        CU(cudaSetDevice(ctx->device), "form_factors_sph");
+        cudaStream_t st = ctx->stream;
+        if (harvest_screen(ctx, false) != SCARF_OK) return SCARF_ECUDA;
+        if (ctx->T_bad) return fail(ctx, SCARF_EINVAL, std::string("form_factors_sph: ") + kBadT);
+        // inversion symmetry: -q of (i, j, k) is the grid point (i, n_theta-1-j, k + n_phi/2) when the theta nodes are antisymmetric
+        // bit for bit and n_phi is even
+        bool sym = ctx->grid_symmetry != 0 && (n_phi % 2) == 0;
+        for (int j = 0; j < n_theta && sym; ++j) sym = cos_theta[j] == -cos_theta[n_theta - 1 - j];
+        const int mid = (n_theta % 2) ? n_theta / 2 : -1;
+        const int n_dir_eval = sym ? (n_theta / 2) * n_phi + (mid >= 0 ? n_phi / 2 : 0) : (int)n_dir;
+        // direction table (cached: rebuilt when the nodes, n_phi or the symmetry decision change); mirror directions are the exact
+        // negatives of the evaluated ones, so that the stored conjugate is what the kernel would compute at -q
+        const bool cached = ctx->sph_n_phi == n_phi && ctx->sph_sym == (sym ? 1 : 0) && ctx->sph_ct.size() == (size_t)n_theta &&
+                            std::memcmp(ctx->sph_ct.data(), cos_theta, (size_t)n_theta * sizeof(double)) == 0;
+        std::vector<double> dirs;
+        auto build_dirs = [&]() {
+            dirs.assign((size_t)n_dir * 3, 0.0);
+            const double two_pi = 6.283185307179586476925286766559;
+            auto direct = [&](int j, int k) {
+                const double c = cos_theta[j], s = std::sqrt(std::max(0.0, 1.0 - c * c)), ph = two_pi * (double)k / (double)n_phi;
+                double* o = &dirs[((size_t)j * n_phi + k) * 3];
+                o[0] = s * std::cos(ph); o[1] = s * std::sin(ph); o[2] = c;
+            };
+            for (int j = 0; j < n_theta; ++j)
+                for (int k = 0; k < n_phi; ++k) {
+                    const bool evaluated = !sym || j < n_theta / 2 || (j == mid && k < n_phi / 2);
+                    if (evaluated) direct(j, k);
+                }
+            if (sym)
+                for (int j = 0; j < n_theta; ++j)
+                    for (int k = 0; k < n_phi; ++k) {
+                        const bool evaluated = j < n_theta / 2 || (j == mid && k < n_phi / 2);
+                        if (evaluated) continue;
+                        const double* src = &dirs[((size_t)(n_theta - 1 - j) * n_phi + (k + n_phi / 2) % n_phi) * 3];
+                        double* o = &dirs[((size_t)j * n_phi + k) * 3];
+                        o[0] = -src[0]; o[1] = -src[1]; o[2] = -src[2];
+                    }
+        };
+        if (has_high_classes(ctx->hs)) {
+            // pairs with g, h, i shells: the same points as a list through scarf_form_factors (its high-class kernel)
+            build_dirs();
+            std::vector<double> q((size_t)n_q * 3);
+            for (int i = 0; i < n_r; ++i)
+                for (long long d = 0; d < n_dir; ++d)
+                    for (int c = 0; c < 3; ++c) q[((size_t)i * n_dir + d) * 3 + c] = r[i] * dirs[(size_t)d * 3 + c];
+            const int rc = scarf_form_factors(ctx, n_q, q.data(), out);
+            if (rc == SCARF_OK) CU(cudaStreamSynchronize(st), "form_factors_sph: sync");      // q dies with this frame
+            ctx->st.last_grid_symmetric = 0;
+            ctx->st.last_grid_variant = -1;
+            return rc;
+        }
+        CU(ctx->d_axes.ensure((size_t)n_r * sizeof(double)), "form_factors_sph: alloc radii");
+        CU(cudaMemcpyAsync(ctx->d_axes.p, r, (size_t)n_r * sizeof(double), cudaMemcpyHostToDevice, st), "form_factors_sph: copy radii");
+        if (!cached) {
+            build_dirs();
+            CU(ctx->d_sph_dirs.ensure(dirs.size() * sizeof(double)), "form_factors_sph: alloc directions");
+            CU(cudaMemcpyAsync(ctx->d_sph_dirs.p, dirs.data(), dirs.size() * sizeof(double), cudaMemcpyHostToDevice, st), "form_factors_sph: copy directions");
+            ctx->sph_ct.assign(cos_theta, cos_theta + n_theta);
+            ctx->sph_n_phi = n_phi;
+            ctx->sph_sym = sym ? 1 : 0;
+        }
+        const int n_rbox = (n_r + kSphBR - 1) / kSphBR, n_dbox = (n_dir_eval + kSphBD - 1) / kSphBD;
+        const long long n_tiles = (long long)n_rbox * n_dbox;
+        const size_t obytes = (size_t)ctx->n_states * (size_t)n_q * 2 * sizeof(double);
+        double* dout = out;
+        const bool out_host = !is_device_ptr(out);
+        if (out_host) {
+            CU(ctx->d_out.ensure(obytes), "form_factors_sph: alloc out");
+            dout = static_cast<double*>(ctx->d_out.p);
+        }
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "form_factors_sph: event");
+        int launches = 0;
+        double main_ms = 0.0;
+        if (ctx->qcut_dev) {
+            CU(cudaMemsetAsync(ctx->d_work.p, 0, kNClasses * sizeof(unsigned long long), st), "form_factors_sph: clear counters");
+            ctx->last_q_tiles = (double)n_tiles; ctx->last_ctr = kCtrSph; ctx->last_was_grid = true; ctx->last_grid_w = kWSph; ctx->work_pending = true;
+        }
+        const long long n_rows = (long long)ctx->hs.pairs.size();    // prescreened pairs: an upper bound of the kept count
+        for (const TileStream& t : ctx->tiles) {
+            SphArgs a = {};
+            const size_t tab_elems = (size_t)std::max<long long>(1, n_rows) * (size_t)n_rbox * kSphBR;
+            CU(ctx->d_tab.ensure(tab_elems * sizeof(double)), "form_factors_sph: alloc table");
+            double* te = static_cast<double*>(ctx->d_tab.p);
+            a.v.base = t.base;
+            a.v.desc = t.desc;
+            a.v.n_q = n_q;
+            a.v.n_tiles = (int)n_tiles;
+            a.v.ns_real = t.ns_real;
+            a.v.dst = dout + (size_t)t.s0 * n_q * 2;
+            a.v.qcut = ctx->qcut_dev;
+            a.v.work = ctx->qcut_dev ? static_cast<unsigned long long*>(ctx->d_work.p) : nullptr;
+            a.r = static_cast<const double*>(ctx->d_axes.p);
+            a.dirs = static_cast<const double*>(ctx->d_sph_dirs.p);
+            a.n_r = n_r; a.n_theta = n_theta; a.n_phi = n_phi;
+            a.n_dir_eval = n_dir_eval;
+            a.n_rbox = n_rbox; a.n_dbox = n_dbox;
+            a.sym = sym ? 1 : 0;
+            a.te = te;
+            a.n_rows = n_rows;
+            CU(launch_sph_table(a, te, st), "form_factors_sph: table kernel");
+            a.v.n_chunks = choose_chunks(ctx, n_tiles, kCtrSph, t.ns_real, ctx->n_chunks_opt);
+            if (int rc = prepare_tickets(ctx, n_tiles, a.v.n_chunks, st, &a.v.tickets)) return rc;
+            CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, kCtrSph, st, /*model=*/3), "form_factors_sph: chunk planning kernel");
+            if (ctx->timing) CU(cudaEventRecord(ctx->ev_m0, st), "form_factors_sph: event");
+            CU(launch_ff_sph(t.NS, a, st), "form_factors_sph: kernel");
+            if (ctx->timing) {
+                CU(cudaEventRecord(ctx->ev_m1, st), "form_factors_sph: event");
+                CU(cudaEventSynchronize(ctx->ev_m1), "form_factors_sph: event sync");
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, ctx->ev_m0, ctx->ev_m1);
+                main_ms += ms;
+            }
+            ctx->st.last_n_chunks = a.v.n_chunks;
+            launches += 3;
+        }
+        ctx->st.last_kernel_launches = launches;
+        ctx->grid_eval_points = (double)n_dir_eval * n_r;
+        ctx->grid_table_cols = (double)n_r;
+        ctx->st.last_grid_symmetric = sym ? 1 : 0;
+        ctx->st.last_grid_variant = 2;
+        ctx->last_grid_w = kWSph;
+        ctx->last_grid_ctr = kCtrSph;
+        ctx->last_table_ctr = kCtrSphTable;
+        ctx->st.last_grid_slots = -1.0;            // filled by scarf_get_stats from the kept counts
+        if (ctx->timing) {
+            CU(cudaEventRecord(ctx->ev1, st), "form_factors_sph: event");
+            CU(cudaEventSynchronize(ctx->ev1), "form_factors_sph: event sync");
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
+            ctx->st.last_kernel_ms = ms;
+            ctx->st.last_main_kernel_ms = main_ms;
+        }
+        if (out_host) {
+            CU(cudaMemcpyAsync(out, dout, obytes, cudaMemcpyDeviceToHost, st), "form_factors_sph: download out");
+            CU(cudaStreamSynchronize(st), "form_factors_sph: sync");
+            if (harvest_screen(ctx, true) != SCARF_OK) return SCARF_ECUDA;
+            if (ctx->T_bad) return fail(ctx, SCARF_EINVAL, std::string("form_factors_sph: ") + kBadT);
+        }
+        return SCARF_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(ctx, SCARF_ENOMEM, "form_factors_sph: out of host memory");
+    } catch (...) {
+        return fail(ctx, SCARF_EINVAL, "form_factors_sph: unexpected exception");
     }
 }
 
@@ -1376,7 +1550,7 @@ int scarf_get_stats(scarf_ctx* ctx, scarf_stats* out)
         const double nt = (double)ctx->tiles.size();
         for (int c = 0; c < kNClasses; ++c) {
             slots += (double)ctx->st.pairs_kept_per_class[c] * ctx->grid_eval_points * ((double)ctx->n_states * (ctx->last_grid_w ? ctx->last_grid_w : kWGrid)[c] + nt * ctx->last_grid_ctr);
-            tab += (double)ctx->st.pairs_kept_per_class[c] * nt * ctx->grid_table_cols * kCtrTable;
+            tab += (double)ctx->st.pairs_kept_per_class[c] * nt * ctx->grid_table_cols * ctx->last_table_ctr;
         }
         ctx->st.last_grid_slots = slots + tab;
         ctx->st.last_grid_kernel_slots = slots;
