@@ -552,7 +552,11 @@ def run_ours(args):
                            "term_pair_q_state_per_s": world * float(st["cart_term_pairs"]) * w.n_q * w.n_states / (ms_per_step * 1e-3),
                            "note": "ordered Cartesian-term pairs N_c^2 of Eq. (68) PAPER.md:505-508 x q-points x states delivered per second"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                    "job_seconds": e2e_s},
+                    "job_seconds": e2e_s,
+                    "note": ("host T (pinned) -> device copy and the pinned host `out` inside the timed region; on the product-grid paths the "
+                             "kernel's last chunks store the finished values straight into the pinned buffer (option host_zero_copy), so the "
+                             "d2h bytes cross PCIe while the kernel runs" if path in ("grid", "sph") else
+                             "host T, q (pinned) -> device copies and the sliced device -> host download of `out` inside the timed region")},
             "gpu_launches": int(steps * (st["last_kernel_launches"] + st["last_fold_launches"])),
             "clocks": clocks, "roofline": roofline}
 

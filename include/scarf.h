@@ -133,6 +133,13 @@ int scarf_set_stream(scarf_ctx* ctx, void* cuda_stream);
  *           "grid_symmetry": default 1.  scarf_form_factors_grid evaluates only one half of a product grid whose three
  *                         axes are antisymmetric bit for bit (ax[i] == -ax[n-1-i]) and stores conj f for the mirror
  *                         points (f(-q) = conj f(q), exact for real T); 0 always evaluates every point.
+ *           "host_zero_copy": default 1.  When `out` of scarf_form_factors_grid is PINNED host memory
+ *                         (cudaHostAlloc / cudaHostRegister; torch's pin_memory), the kernel stores the finished values straight
+ *                         into it through its mapped device alias — the output crosses PCIe while the kernel runs and no
+ *                         device->host copy follows; partial sums stay on the device.  0: always compute on the device and copy.
+ *                         Pageable host memory always takes the copy.  The call returns when `out` is complete either way.
+ *           "host_tile_group": default 0 (automatic).  Tiles per dispatch group of the product-grid kernels when they write a
+ *                         pinned host `out` (see host_zero_copy).  A tuning/testing knob; results do not depend on it.
  *           "grid_variant": default -1 (automatic).  Kernel of scarf_form_factors_grid: 0 = box kernel (a CTA owns a 4 x 8 x 8
  *                         box of the grid; the two points of a thread share (q_y, q_z)), 1 = row kernel (a warp owns 64
  *                         consecutive z-points of one (ix, iy) row, so the (q_x, q_y) part of every polynomial is evaluated

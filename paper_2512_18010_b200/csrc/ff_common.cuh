@@ -113,6 +113,23 @@ __device__ __forceinline__ void ticket_pass(int* ticket, int next)
     if (threadIdx.x == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(ticket), "r"(next) : "memory");
 }
 
+// ---- which (tile, chunk) a CTA of the (n_tiles, n_chunks) grid works on (V1Args::tile_group; CTAs are dispatched x fastest) ----
+__device__ __forceinline__ void cta_tile_chunk(const V1Args& v, int& tile, int& chunk)
+{
+    if (v.tile_group <= 0) {
+        tile = (int)blockIdx.x;
+        chunk = (int)blockIdx.y;
+        return;
+    }
+    const long long lin = (long long)blockIdx.x + (long long)gridDim.x * (long long)blockIdx.y;
+    const long long per = (long long)v.tile_group * v.n_chunks;
+    const int g = (int)(lin / per), rem = (int)(lin - (long long)g * per);
+    const int gs = min(v.tile_group, v.n_tiles - g * v.tile_group);       // the last group may be short
+    chunk = rem / gs;
+    tile = g * v.tile_group + rem % gs;
+    SCARF_CHECK(tile >= 0 && tile < v.n_tiles && chunk >= 0 && chunk < v.n_chunks);
+}
+
 // ---- q-adaptive cut-off helpers (fold.cu: qcut_kernel) -------------------------------------------------------------------
 // smallest value of x over the CTA's threads (whole-CTA call; `sh` holds one double per warp)
 __device__ __forceinline__ double block_min(double x, double* sh)

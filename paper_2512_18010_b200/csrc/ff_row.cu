@@ -276,7 +276,8 @@ __global__ void __launch_bounds__(kThreads, 2) ff_row_kernel(const GridArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + kStages * kSlotBytes);
-    const int tile = (int)blockIdx.x, chunk = (int)blockIdx.y;
+    int tile, chunk;
+    cta_tile_chunk(a.v, tile, chunk);
     if (threadIdx.x == 0) {
         for (int s = 0; s < kStages; ++s) mbar_init(&full_bar[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -368,6 +369,7 @@ __global__ void __launch_bounds__(kThreads, 2) ff_row_kernel(const GridArgs a)
     // ---- epilogue: store (one chunk) or add into `out` in chunk order (several); the LAST chunk holds the final value and
     // also stores its conjugate at the mirror point when the grid is inversion-symmetric
     double2* dst = reinterpret_cast<double2*>(a.v.dst);
+    double2* fin = a.v.dst_final != nullptr ? reinterpret_cast<double2*>(a.v.dst_final) : dst;    // finished values (last chunk)
     const int turn = s_turn;
     if (turn < 0) return;                                   // a chunk without work (uniform over the CTA)
     const bool first = turn == 0, last = s_next == 0;
@@ -389,8 +391,9 @@ __global__ void __launch_bounds__(kThreads, 2) ff_row_kernel(const GridArgs a)
                         v.x += p.x;
                         v.y += p.y;
                     }
-                    o[i] = v;
-                    if (mirror) o[a.v.n_q - 1 - i] = make_double2(v.x, -v.y);   // f(-q) = conj f(q)
+                    double2* w = (last ? fin : dst) + (size_t)s * a.v.n_q;
+                    w[i] = v;
+                    if (mirror) w[a.v.n_q - 1 - i] = make_double2(v.x, -v.y);   // f(-q) = conj f(q)
                 }
         }
     }

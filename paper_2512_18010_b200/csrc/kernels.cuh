@@ -133,8 +133,14 @@ struct V1Args {
     const double* q;                        // [n_q][3]
     long long n_q;
     int n_tiles, n_chunks;                  // grid = (n_tiles, n_chunks)
-    int ns_real, pad;
+    int ns_real;
+    int tile_group;                         // product-grid kernels: 0 = CTAs dispatched chunk-major over ALL tiles; G > 0 = chunk-major inside
+                                            // groups of G consecutive tiles, group after group (finished tiles leave the kernel all along
+                                            // its run instead of in its last 1/n_chunks: what a pinned host `out` needs, see dst_final)
     double* dst;                            // out + s0*n_q*2
+    double* dst_final;                      // product-grid kernels: where the LAST chunk of a tile stores the finished values (and the
+                                            // mirror points): nullptr = dst; else a device alias of the caller's pinned host `out`, so that
+                                            // the results cross PCIe as the kernel produces them (partial sums stay in dst, on the device)
     int* tickets;                           // [n_tiles], all zero at launch and again at exit (n_chunks > 1 only)
     const double* qcut;                     // q-adaptive cut-off: q_cut per record in stream order (descending inside a class); nullptr: off
     unsigned long long* work;               // [kNClasses] += records evaluated per CTA and class (q-adaptive statistics); nullptr: off

@@ -72,6 +72,8 @@ struct scarf_ctx {
     double last_q_tiles = 0.0;          // q tiles of the last S4 call (for the skipped-work statistics)
     double last_ctr = 40.0;
     int grid_symmetry = 1;    // 1: use f(-q) = conj f(q) on inversion-symmetric product grids; 0: never
+    int host_tile_group = 0;  // tiles per dispatch group when the kernel writes a pinned host `out` (0: automatic)
+    int host_zero_copy = 1;   // 1: a pinned host `out` of the product-grid calls is written by the kernel itself (no device->host copies)
     int grid_variant = -1;    // product-grid kernel: 0 box kernel (ff_grid.cu), 1 row kernel (ff_row.cu), -1 by the grid's shape
     const double* last_grid_w = nullptr;   // work model of the last product-grid call (kWGrid or kWRow)
     double last_grid_ctr = 6.0;            // ... and its per-(q, pair) slots (kCtrGrid or kCtrRow)
@@ -141,6 +143,17 @@ bool is_device_ptr(const void* p)
         return false;
     }
     return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// Device alias of a pinned (page-locked, mapped) host buffer, or nullptr for pageable host memory.
+double* mapped_host_alias(const void* p)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    return a.type == cudaMemoryTypeHost ? static_cast<double*>(a.devicePointer) : nullptr;
 }
 
 bool all_finite(const double* x, size_t n)
@@ -329,6 +342,12 @@ int scarf_set_option(scarf_ctx* ctx, const char* key, double value)
     } else if (k == "grid_symmetry") {
         if (value != 0.0 && value != 1.0) return fail(ctx, SCARF_EINVAL, "set_option: grid_symmetry must be 0 or 1");
         ctx->grid_symmetry = (int)value;
+    } else if (k == "host_tile_group") {
+        if (value < 0 || value > 1e6) return fail(ctx, SCARF_EINVAL, "set_option: host_tile_group outside 0..1e6");
+        ctx->host_tile_group = (int)value;
+    } else if (k == "host_zero_copy") {
+        if (value != 0.0 && value != 1.0) return fail(ctx, SCARF_EINVAL, "set_option: host_zero_copy must be 0 or 1");
+        ctx->host_zero_copy = (int)value;
     } else if (k == "grid_variant") {
         if (value != 0.0 && value != 1.0 && value != -1.0) return fail(ctx, SCARF_EINVAL, "set_option: grid_variant must be -1, 0 or 1");
         ctx->grid_variant = (int)value;
@@ -455,8 +474,8 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T)
         CU(cudaSetDevice(ctx->device), "set_transitions");
         cudaStream_t st = ctx->stream;
         const double* dT = T;
-        if (!is_device_ptr(T)) {
-            if (!all_finite(T, tsz)) return fail(ctx, SCARF_EINVAL, "set_transitions: NaN/Inf in T");
+        const bool T_host = !is_device_ptr(T);
+        if (T_host) {       // validated below, on the host, while the device already folds it
             CU(ctx->d_T.ensure(tsz * sizeof(double)), "set_transitions: alloc T");
             CU(cudaMemcpyAsync(ctx->d_T.p, T, tsz * sizeof(double), cudaMemcpyHostToDevice, st), "set_transitions: upload T");
             dT = static_cast<const double*>(ctx->d_T.p);
@@ -600,6 +619,13 @@ int scarf_set_transitions(scarf_ctx* ctx, int n_states, const double* T)
             float ms = 0.f;
             cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
             ctx->st.last_fold_ms = ms;
+        }
+        // Host T: NaN/Inf check (a pass over n_states nbf^2 doubles, 0.3 ms on config 3) AFTER the upload and the kernels have been
+        // queued, so that it overlaps them; a bad T still fails this very call, and nothing of it stays behind.
+        if (T_host && !all_finite(T, tsz)) {
+            cudaStreamSynchronize(st);
+            ctx->screen_pending = false;
+            return fail(ctx, SCARF_EINVAL, "set_transitions: NaN/Inf in T");
         }
         ctx->have_T = true;
         return SCARF_OK;
@@ -891,7 +917,10 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         }
         const long long ncol = (long long)nbx * BXs + (long long)nby * BYs + (long long)nbz * BZs;
         const long long n_rows = (long long)ctx->hs.pairs.size();    // prescreened pairs: an upper bound of the kept count
-        const int n_slabs = (out_host && nbx >= 4 && n_q >= 4 * 16384 && !has_high_classes(ctx->hs)) ? 4 : 1;
+        // Pinned host `out`: the last chunk of every box stores the finished values straight into it (a mapped alias), so the output
+        // crosses PCIe while the kernel runs and no copy follows it; partial sums of the chunks stay in the device scratch.
+        double* out_alias = (out_host && ctx->host_zero_copy && !has_high_classes(ctx->hs)) ? mapped_host_alias(out) : nullptr;
+        const int n_slabs = (out_host && !out_alias && nbx >= 4 && n_q >= 4 * 16384 && !has_high_classes(ctx->hs)) ? 4 : 1;
         if (n_slabs > 1) {
             if (!ctx->copy_stream) CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking), "form_factors_grid: copy stream");
             if (!ctx->ev_slice) CU(cudaEventCreateWithFlags(&ctx->ev_slice, cudaEventDisableTiming), "form_factors_grid: event");
@@ -913,6 +942,7 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
             a.v.n_tiles = (int)n_tiles;
             a.v.ns_real = t.ns_real;
             a.v.dst = dout + (size_t)t.s0 * n_q * 2;
+            a.v.dst_final = out_alias ? out_alias + (size_t)t.s0 * n_q * 2 : nullptr;
             a.qx = dax[0]; a.qy = dax[1]; a.qz = dax[2];
             a.nx = nx; a.ny = ny; a.nz = nz;
             a.nbx = nbx; a.nby = nby; a.nbz = nbz;
@@ -933,6 +963,18 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
                 a.bx0 = b0;
                 a.v.n_tiles = (int)tiles_s;
                 a.v.n_chunks = choose_chunks(ctx, tiles_s, ctr_g, t.ns_real, ctx->n_chunks_opt);
+                // Pinned host `out`: the CTAs are dispatched chunk-major inside groups of tiles, group after group, so that finished
+                // tiles leave for the host all along the kernel's run (chunk-major over all tiles would send everything in the last
+                // 1/n_chunks of it).  Measured on config 3 (ms per call, host `out`): groups of 128 tiles (3/7 of the CTA slots) and
+                // about 8 waves of CTAs (5 chunks) 6.60; 14 chunks 6.76; groups of 16 / 32 / 64 / 256 / 296 tiles (14 chunks) 7.27 /
+                // 6.96 / 6.89 / 7.01 / 7.15 (small groups: the chunks of a tile run side by side and queue at its ticket; large
+                // groups: a long tail); no groups 7.04; device `out` 6.46.
+                if (out_alias) {
+                    const long long slots = 2LL * ctx->sm_count;
+                    if (ctx->n_chunks_opt <= 0) a.v.n_chunks = (int)std::max<long long>(1, std::min<long long>(a.v.n_chunks, (8 * slots + tiles_s - 1) / tiles_s));
+                    a.v.tile_group = a.v.n_chunks > 1 ? (int)std::max<long long>(1, 3 * slots / 7) : 0;
+                    if (a.v.tile_group > 0 && ctx->host_tile_group > 0) a.v.tile_group = ctx->host_tile_group;
+                }
                 if (int rc = prepare_tickets(ctx, tiles_s, a.v.n_chunks, st, &a.v.tickets)) return n_slabs > 1 ? drain(rc) : rc;
                 CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, ctr_g, st, /*model=*/row ? 2 : 1), "form_factors_grid: chunk planning kernel");
                 if (ctx->timing) CU(cudaEventRecord(ctx->ev_m0, st), "form_factors_grid: event");
@@ -991,7 +1033,7 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         }
         if (out_host) {
             if (n_slabs > 1) CU(cudaStreamSynchronize(ctx->copy_stream), "form_factors_grid: sync copies");
-            else CU(cudaMemcpyAsync(out, dout, obytes, cudaMemcpyDeviceToHost, st), "form_factors_grid: download out");
+            else if (!out_alias) CU(cudaMemcpyAsync(out, dout, obytes, cudaMemcpyDeviceToHost, st), "form_factors_grid: download out");
             CU(cudaStreamSynchronize(st), "form_factors_grid: sync");
             if (harvest_screen(ctx, true) != SCARF_OK) return SCARF_ECUDA;
             if (ctx->T_bad) return fail(ctx, SCARF_EINVAL, std::string("form_factors_grid: ") + kBadT);
@@ -1090,6 +1132,8 @@ int scarf_form_factors_sph(scarf_ctx* ctx, int32_t n_r, const double* r, int32_t
             CU(ctx->d_out.ensure(obytes), "form_factors_sph: alloc out");
             dout = static_cast<double*>(ctx->d_out.p);
         }
+        // (No direct stores into a pinned host `out` here, unlike scarf_form_factors_grid: a lane owns a radius, so the kernel writes
+        // 16-byte pieces at a stride of n_theta n_phi 16 B; over PCIe that took 54 ms on config 5 against 34.8 ms with the copy.)
         if (ctx->timing) CU(cudaEventRecord(ctx->ev0, st), "form_factors_sph: event");
         int launches = 0;
         double main_ms = 0.0;

@@ -172,3 +172,59 @@ def test_row_kernel_q_adaptive_bound(oracle_mod, Scarf, torch_cuda):
         assert st["last_grid_variant"] == 1 and st["adaptive_bound"] > 0
         assert np.max(np.abs(f - exact)) <= st["adaptive_bound"] + 1e-12 * np.max(np.abs(exact))
         assert st["last_adaptive_work_fraction"] <= 1.0
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("shape,symmetric", [((6, 8, 64), True), ((5, 7, 70), False)])
+def test_pinned_host_output_written_by_the_kernel(oracle_mod, Scarf, torch_cuda, variant, shape, symmetric):
+    """Option host_zero_copy (default on): a PINNED host `out` receives the finished values from the last chunk of every box through
+    its mapped alias (no device->host copy); several chunks so that partial sums go through the device scratch.  Bit-identical to
+    the device-output call and to the copy path (host_zero_copy = 0, and a pageable numpy `out`); oracle on every point."""
+    torch = torch_cuda
+    b = all_class_basis()
+    rng = np.random.default_rng(sum(shape) + variant)
+    T = rng.normal(size=(13, b.nbf, b.nbf))
+    axes = [W.cartesian_axis(n, 3.0 + k) for k, n in enumerate(shape)] if symmetric else [rng.uniform(-4, 4, size=n) for n in shape]
+    n_q = int(np.prod(shape))
+    f_ref = oracle_mod.form_factors(b, T, expand(*axes))
+    with Scarf(0) as sc:
+        sc.set_basis(b)
+        sc.set_option("grid_variant", variant)
+        sc.set_option("n_chunks", 5)
+        sc.set_transitions(torch.as_tensor(T, device="cuda"))
+        f_dev = sc.form_factors_grid(*[torch.as_tensor(a, device="cuda") for a in axes])
+        torch.cuda.synchronize()
+        f_dev = f_dev.cpu().numpy()
+        assert sc.stats()["last_grid_symmetric"] == int(symmetric)
+        pinned = torch.full((13, n_q, 2), float("nan"), dtype=torch.float64).pin_memory()
+        f_pin = sc.form_factors_grid(*axes, out=pinned).numpy().copy()
+        sc.set_option("host_zero_copy", 0)
+        pinned2 = torch.full((13, n_q, 2), float("nan"), dtype=torch.float64).pin_memory()
+        f_copy = sc.form_factors_grid(*axes, out=pinned2).numpy().copy()
+        f_np = np.array(sc.form_factors_grid(*axes))
+    assert_parity(f_pin, f_ref)
+    assert np.array_equal(f_pin, f_dev) and np.array_equal(f_copy, f_dev) and np.array_equal(f_np, f_dev)
+
+
+@pytest.mark.parametrize("tile_group", [1, 3, 1000])
+def test_pinned_host_output_tile_groups(oracle_mod, Scarf, torch_cuda, tile_group):
+    """Option host_tile_group: with a pinned host `out` the CTAs are dispatched chunk-major inside groups of tiles; a group of one
+    tile, a ragged last group, one group for everything: same values as the device-output call, bit for bit."""
+    torch = torch_cuda
+    b = all_class_basis()
+    rng = np.random.default_rng(tile_group)
+    T = rng.normal(size=(12, b.nbf, b.nbf))
+    axes = [W.cartesian_axis(n, 3.0 + k) for k, n in enumerate((4, 14, 70))]          # 2 x 4 x 2 = 16 boxes of 1 x 4 x 64 (x halved)
+    n_q = 4 * 14 * 70
+    with Scarf(0) as sc:
+        sc.set_basis(b)
+        sc.set_option("grid_variant", 1)
+        sc.set_option("n_chunks", 4)
+        sc.set_option("host_tile_group", tile_group)
+        sc.set_transitions(torch.as_tensor(T, device="cuda"))
+        f_dev = sc.form_factors_grid(*[torch.as_tensor(a, device="cuda") for a in axes])
+        torch.cuda.synchronize()
+        pinned = torch.full((12, n_q, 2), float("nan"), dtype=torch.float64).pin_memory()
+        f_pin = sc.form_factors_grid(*axes, out=pinned).numpy().copy()
+    assert np.array_equal(f_pin, f_dev.cpu().numpy())
+    assert_parity(f_pin, oracle_mod.form_factors(b, T, expand(*axes)))

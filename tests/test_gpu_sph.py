@@ -213,3 +213,32 @@ def test_sph_high_classes_list_fallback_and_errors(oracle_mod, Scarf, torch_cuda
         bad[2] = np.inf
         with pytest.raises(Exception):
             sc.form_factors_sph(bad, ct, 4)
+
+
+@pytest.mark.parametrize("symmetric", [True, False])
+def test_sph_pinned_and_pageable_host_output(oracle_mod, Scarf, torch_cuda, symmetric):
+    """Host `out`, pinned or pageable (computed on the device, one copy; the kernel's strided 16-byte stores are not sent over PCIe):
+    bit-identical to the device-output call; oracle on every point."""
+    torch = torch_cuda
+    b = all_class_basis()
+    rng = np.random.default_rng(31 + symmetric)
+    T = rng.normal(size=(13, b.nbf, b.nbf))
+    n_r, n_t, n_p = 70, 5, 6
+    r = np.geomspace(0.05, 6.0, n_r)
+    ct = np.polynomial.legendre.leggauss(n_t)[0] if symmetric else rng.uniform(-1, 1, size=n_t)
+    n_q = n_r * n_t * n_p
+    f_ref = oracle_mod.form_factors(b, T, sph_points(r, ct, n_p))
+    with Scarf(0) as sc:
+        sc.set_basis(b)
+        sc.set_option("n_chunks", 5)
+        sc.set_transitions(torch.as_tensor(T, device="cuda"))
+        f_dev = sc.form_factors_sph(r, ct, n_p)
+        torch.cuda.synchronize()
+        f_dev = f_dev.cpu().numpy()
+        assert sc.stats()["last_grid_symmetric"] == int(symmetric)
+        pinned = torch.full((13, n_q, 2), float("nan"), dtype=torch.float64).pin_memory()
+        f_pin = sc.form_factors_sph(r, ct, n_p, out=pinned).numpy().copy()
+        sc.set_option("host_zero_copy", 0)
+        f_np = np.array(sc.form_factors_sph(r, ct, n_p, device=False))
+    assert_parity(f_pin, f_ref)
+    assert np.array_equal(f_pin, f_dev) and np.array_equal(f_np, f_dev)
