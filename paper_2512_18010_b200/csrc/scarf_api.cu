@@ -161,7 +161,10 @@ bool all_finite(const double* x, size_t n)
     // exponent field all ones <=> NaN or Inf; integer test so that the loop vectorises (a serial FP sum cost 1.6 ms per call on
     // config 3's q and T, inside the end-to-end step)
     uint64_t bad = 0;
-    for (size_t i = 0; i < n; ++i) {
+    const long long nn = (long long)n;
+    // large arrays (config 4's T: 34 MB) on up to 8 host threads: 3 ms -> 0.5 ms
+#pragma omp parallel for reduction(| : bad) schedule(static) num_threads(8) if (nn >= (1LL << 20))
+    for (long long i = 0; i < nn; ++i) {
         uint64_t b;
         std::memcpy(&b, x + i, sizeof(b));
         bad |= (uint64_t)((~b & 0x7ff0000000000000ULL) == 0);
