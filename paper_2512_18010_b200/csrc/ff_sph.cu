@@ -238,18 +238,33 @@ __device__ __forceinline__ void run_class_sph(SPipe& pp, const SphArgs& a, const
                     record_accum_sph<L, NS>(reinterpret_cast<const double2*>(Gw + k * g_stride(L, NS)), rp, gc, gs, re, im);
                 }
             };
-            // software-pipelined: the sincos chains of record k+1 are issued alongside the accumulate of record k
-            double gc[kNQ], gs[kNQ];
-            factors(0, gc, gs);
-#pragma unroll 1
-            for (int k = 0; k + 1 < cnt; ++k) {
-                double gcn[kNQ], gsn[kNQ];
-                factors(k + 1, gcn, gsn);
-                accum(k, gc, gs);
+            // software-pipelined by groups of U records: the sincos chains of group k+1 are issued alongside the accumulate of group k
+            constexpr int U = L <= 1 ? 2 : 1;
+            const int n_full = cnt / U * U;
+            double gc[U][kNQ], gs[U][kNQ];
+            if (n_full > 0) {
 #pragma unroll
-                for (int jj = 0; jj < kNQ; ++jj) { gc[jj] = gcn[jj]; gs[jj] = gsn[jj]; }
+                for (int u = 0; u < U; ++u) factors(u, gc[u], gs[u]);
+#pragma unroll 1
+                for (int k = 0; k + U < n_full; k += U) {
+                    double gcn[U][kNQ], gsn[U][kNQ];
+#pragma unroll
+                    for (int u = 0; u < U; ++u) factors(k + U + u, gcn[u], gsn[u]);
+#pragma unroll
+                    for (int u = 0; u < U; ++u) accum(k + u, gc[u], gs[u]);
+#pragma unroll
+                    for (int u = 0; u < U; ++u)
+#pragma unroll
+                        for (int jj = 0; jj < kNQ; ++jj) { gc[u][jj] = gcn[u][jj]; gs[u][jj] = gsn[u][jj]; }
+                }
+#pragma unroll
+                for (int u = 0; u < U; ++u) accum(n_full - U + u, gc[u], gs[u]);
             }
-            accum(cnt - 1, gc, gs);
+#pragma unroll 1
+            for (int k = n_full; k < cnt; ++k) {
+                factors(k, gc[0], gs[0]);
+                accum(k, gc[0], gs[0]);
+            }
         }
         __syncthreads();                                 // the slot and the warp areas are free again
         if (producer && j + kStages < n_st) issue(j + kStages);
