@@ -514,13 +514,13 @@ def run_ours(args):
                                             "frac_survey_model: the monomial-form count n_herm + 3 over the same time")
         alg_bytes = st["stream_bytes"] + 16.0 * w.n_states * w.n_q + 32.0 * st["n_pairs_kept"] * (n_eval_q ** (1 / 3))
     elif path == "sph":
-        slots = st["last_grid_kernel_slots"]        # the kernel's own count: W(L) = 2, 5, 6, 7 (+ the per-direction sums / 64), n_herm + 3 beyond L = 3; 22 per (q, pair)
+        slots = st["last_grid_kernel_slots"]        # the kernel's own count: W(L) = 2, 4, 5, 6 (+ the per-direction sums / 64), n_herm + 3 beyond L = 3; 24 per (q, pair)
         roofline = alu_roofline(slots, head["main_kernel_ms"], grid_kernel_name(st), poly_per_q * n_eval_q)
         survey_slots = n_eval_q * st["slots_per_q"]
         roofline["frac_survey_model"] = survey_slots / (head["main_kernel_ms"] * 1e-3) / peak_meas
         roofline["slots_model_note"] = ("frac: FP64 slots the kernel's algorithm needs (the 64 radii of a warp's direction share the phase slope "
-                                        "n.P and the per-degree sums of the polynomial: 5 / 6 / 7 slots per (q, pair, state) for L = 1 / 2 / 3 and "
-                                        "22 per (q, pair)); frac_survey_model: the list kernel's count (n_herm + 3, and 40 per (q, pair)) over "
+                                        "n.P and the per-degree sums of the polynomial: 4 / 5 / 6 slots per (q, pair, state) for L = 1 / 2 / 3 and "
+                                        "24 per (q, pair)); frac_survey_model: the list kernel's count (n_herm + 3, and 40 per (q, pair)) over "
                                         "the same time")
         alg_bytes = st["stream_bytes"] + 16.0 * w.n_states * w.n_q + 8.0 * st["n_pairs_kept"] * w.grid["n_r"]
     else:
@@ -555,7 +555,8 @@ def run_ours(args):
                     "job_seconds": e2e_s,
                     "note": ("host T (pinned) -> device copy and the pinned host `out` inside the timed region; on the product-grid paths the "
                              "kernel's last chunks store the finished values straight into the pinned buffer (option host_zero_copy), so the "
-                             "d2h bytes cross PCIe while the kernel runs" if path in ("grid", "sph") else
+                             "d2h bytes cross PCIe while the kernel runs" if path == "grid" else
+                             "host T (pinned) -> device copy; `out` computed on the device and copied once into the pinned host buffer" if path == "sph" else
                              "host T, q (pinned) -> device copies and the sliced device -> host download of `out` inside the timed region")},
             "gpu_launches": int(steps * (st["last_kernel_launches"] + st["last_fold_launches"])),
             "clocks": clocks, "roofline": roofline}

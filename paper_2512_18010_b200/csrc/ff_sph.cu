@@ -7,8 +7,9 @@
 // A WARP owns one direction and 64 radii (lane l: i = l and l + 32): d_P and every G_n are the same for the whole warp.  Per
 // stage of records the warp evaluates them once ("pre-pass": lane k takes d of record k; lane (k, s) the G of record k and
 // state s; results in a warp-private shared-memory area), then every lane needs, per record, one sincos of r d_P, E_P(r) from
-// a table, and per state the short polynomial in r: FP64 slots per (q, pair, state) 2, 5, 6, 7 for L = 0..3 (list kernel: 2,
-// 7, 13, 23) and 22 per (q, pair) instead of 40.  Classes L >= 4: the degree blocks of ff_common.cuh on q = r n.
+// a table, and per state the short polynomial in r (B = r (G_1 + G_3 r^2): the factor r is multiplied into the phase factor once
+// per record): FP64 slots per (q, pair, state) 2, 4, 5, 6 for L = 0..3 (list kernel: 2, 7, 13, 23) and 24 per (q, pair) instead
+// of 40.  Classes L >= 4: the degree blocks of ff_common.cuh on q = r n.
 //
 // Inversion symmetry.  f_s(-q) = conj f_s(q) (Eq. (19); real T, real orbitals).  When the theta nodes are
 // antisymmetric bit for bit (cos_theta[j] == -cos_theta[n_theta-1-j], e.g. Gauss-Legendre nodes) and n_phi is even, -q of grid
@@ -109,9 +110,12 @@ __device__ __forceinline__ void sph_prepass(const unsigned char* sp, int cnt, co
 }
 
 // ---- one record, L = 1..3: acc += (gc + i gs) (sum_{n even} r^n G_n + i sum_{n odd} r^n G_n), G from the warp's area -----------
+// B has odd powers of r only: B = r B', B' = G_1 + G_3 r^2; the factor r goes into g once per (point, record) — gcr = gc r,
+// gsr = gs r — instead of once per (point, record, state).
 template <int L, int NS>
 __device__ __forceinline__ void record_accum_sph(const double2* __restrict__ G2, const double (&rp)[kNQ][L + 1], const double (&gc)[kNQ],
-                                                 const double (&gs)[kNQ], double (&re)[kNQ][NS], double (&im)[kNQ][NS])
+                                                 const double (&gs)[kNQ], const double (&gcr)[kNQ], const double (&gsr)[kNQ],
+                                                 double (&re)[kNQ][NS], double (&im)[kNQ][NS])
 {
     constexpr int NG = L + 1, N = NS * NG;
     double G[NG];
@@ -127,13 +131,13 @@ __device__ __forceinline__ void record_accum_sph(const double2* __restrict__ G2,
                 if constexpr (g == NG - 1) {
 #pragma unroll
                     for (int j = 0; j < kNQ; ++j) {
-                        double A = G[0], B = G[1] * rp[j][1];
+                        double A = G[0], B = G[1];
                         if constexpr (L >= 2) A = fma(G[2], rp[j][2], A);
-                        if constexpr (L >= 3) B = fma(G[3], rp[j][3], B);
+                        if constexpr (L >= 3) B = fma(G[3], rp[j][2], B);
                         re[j][s] = fma(gc[j], A, re[j][s]);
                         im[j][s] = fma(gs[j], A, im[j][s]);
-                        re[j][s] = fma(-gs[j], B, re[j][s]);
-                        im[j][s] = fma(gc[j], B, im[j][s]);
+                        re[j][s] = fma(-gsr[j], B, re[j][s]);
+                        im[j][s] = fma(gcr[j], B, im[j][s]);
                     }
                 }
             }
@@ -201,15 +205,20 @@ __device__ __forceinline__ void run_class_sph(SPipe& pp, const SphArgs& a, const
             Dw[lane] = fma(nv[0], hdr[0], fma(nv[1], hdr[1], nv[2] * hdr[2]));
         }
         if constexpr (L == 0 || L >= 4) __syncwarp();
-        auto factors = [&](int k, double (&gc)[kNQ], double (&gs)[kNQ]) {      // g = E(r) (cos(r d) + i sin(r d)) for this lane's points
+        // g = E(r) (cos(r d) + i sin(r d)) for this lane's points: gq = {gc, gs, gc r, gs r}
+        auto factors = [&](int k, double (&gq)[4][kNQ]) {
             const double dP = Dw[k];
 #pragma unroll
             for (int jj = 0; jj < kNQ; ++jj) {
                 double sn, cs;
                 sincos_fast(rv[jj] * dP, sn, cs);
                 const double e = Es[k * kSphBR + 32 * jj];
-                gc[jj] = e * cs;
-                gs[jj] = e * sn;
+                gq[0][jj] = e * cs;
+                gq[1][jj] = e * sn;
+                if constexpr (L >= 1 && L <= 3) {
+                    gq[2][jj] = gq[0][jj] * rv[jj];
+                    gq[3][jj] = gq[1][jj] * rv[jj];
+                }
             }
         };
         if constexpr (L >= 4) {                         // degree blocks, both q-points together (ff_common.cuh)
@@ -219,7 +228,12 @@ __device__ __forceinline__ void run_class_sph(SPipe& pp, const SphArgs& a, const
                 double gcb[kBlkRec][kNQ], gsb[kBlkRec][kNQ];
                 static_for<kBlkRec>([&](auto rc) {
                     constexpr int r = decltype(rc)::value;
-                    if (r < nb) factors(k0 + r, gcb[r], gsb[r]);
+                    if (r < nb) {
+                        double gq[4][kNQ];
+                        factors(k0 + r, gq);
+#pragma unroll
+                        for (int jj = 0; jj < kNQ; ++jj) { gcb[r][jj] = gq[0][jj]; gsb[r][jj] = gq[1][jj]; }
+                    }
                 });
                 accum_blocks<L, NS>(sp + k0 * REC, nb, qv, gcb, gsb, re, im);
             }
@@ -228,42 +242,45 @@ __device__ __forceinline__ void run_class_sph(SPipe& pp, const SphArgs& a, const
                 sph_prepass<L, NS>(sp, cnt, dm, Gw, lane);
                 __syncwarp();
             }
-            auto accum = [&](int k, const double (&gc)[kNQ], const double (&gs)[kNQ]) {
+            auto accum = [&](int k, const double (&gq)[4][kNQ]) {
                 if constexpr (L == 0) {
                     double mono[kNQ][1];
 #pragma unroll
                     for (int jj = 0; jj < kNQ; ++jj) mono[jj][0] = 1.0;
-                    record_accum<0, NS, kNQ, 0>(reinterpret_cast<const double2*>(sp + k * REC), mono, gc, gs, re, im);
+                    record_accum<0, NS, kNQ, 0>(reinterpret_cast<const double2*>(sp + k * REC), mono, gq[0], gq[1], re, im);
                 } else {
-                    record_accum_sph<L, NS>(reinterpret_cast<const double2*>(Gw + k * g_stride(L, NS)), rp, gc, gs, re, im);
+                    record_accum_sph<L, NS>(reinterpret_cast<const double2*>(Gw + k * g_stride(L, NS)), rp, gq[0], gq[1], gq[2], gq[3], re, im);
                 }
             };
             // software-pipelined by groups of U records: the sincos chains of group k+1 are issued alongside the accumulate of group k
             constexpr int U = L <= 1 ? 2 : 1;
             const int n_full = cnt / U * U;
-            double gc[U][kNQ], gs[U][kNQ];
+            constexpr int NGQ = (L >= 1 && L <= 3) ? 4 : 2;       // components of gq that are live
+            double gq[U][4][kNQ];
             if (n_full > 0) {
 #pragma unroll
-                for (int u = 0; u < U; ++u) factors(u, gc[u], gs[u]);
+                for (int u = 0; u < U; ++u) factors(u, gq[u]);
 #pragma unroll 1
                 for (int k = 0; k + U < n_full; k += U) {
-                    double gcn[U][kNQ], gsn[U][kNQ];
+                    double gn[U][4][kNQ];
 #pragma unroll
-                    for (int u = 0; u < U; ++u) factors(k + U + u, gcn[u], gsn[u]);
+                    for (int u = 0; u < U; ++u) factors(k + U + u, gn[u]);
 #pragma unroll
-                    for (int u = 0; u < U; ++u) accum(k + u, gc[u], gs[u]);
+                    for (int u = 0; u < U; ++u) accum(k + u, gq[u]);
 #pragma unroll
                     for (int u = 0; u < U; ++u)
 #pragma unroll
-                        for (int jj = 0; jj < kNQ; ++jj) { gc[u][jj] = gcn[u][jj]; gs[u][jj] = gsn[u][jj]; }
+                        for (int c = 0; c < NGQ; ++c)
+#pragma unroll
+                            for (int jj = 0; jj < kNQ; ++jj) gq[u][c][jj] = gn[u][c][jj];
                 }
 #pragma unroll
-                for (int u = 0; u < U; ++u) accum(n_full - U + u, gc[u], gs[u]);
+                for (int u = 0; u < U; ++u) accum(n_full - U + u, gq[u]);
             }
 #pragma unroll 1
             for (int k = n_full; k < cnt; ++k) {
-                factors(k, gc[0], gs[0]);
-                accum(k, gc[0], gs[0]);
+                factors(k, gq[0]);
+                accum(k, gq[0]);
             }
         }
         __syncthreads();                                 // the slot and the warp areas are free again

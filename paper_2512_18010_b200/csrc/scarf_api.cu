@@ -44,11 +44,11 @@ const double kWGrid[kNClasses] = {2, 6, 10.5, 17, 38, 59, 87, 123, 168, 223, 289
 // (2, 7, 16 slots per (record, state)) spread over the 64 points of the row
 // ... and 4 slots per point for g = (X Y) Z, X Y once per (row, pair): 4 more, spread over the row's 64 points
 const double kCtrRow = 4.0 + 4.0 / 64.0;
-// spherical-grid kernel (ff_sph.cu): a warp's 64 radii share the direction: per point r d_P, sincos, E cos, E sin = 22 slots, d_P = n.P
-// once per (direction, pair); the polynomial in r: 5, 6, 7 slots per point for L = 1, 2, 3 plus the per-direction sums G_n
-// (3, 9, 19 slots per (direction, pair, state)); the E table: one exp (16 slots) per (pair, radius)
-const double kCtrSph = 22.0 + 3.0 / 64.0, kCtrSphTable = 16.0;
-const double kWSph[kNClasses] = {2, 5 + 3 / 64.0, 6 + 9 / 64.0, 7 + 19 / 64.0, 38, 59, 87, 123, 168, 223, 289, 367, 458};
+// spherical-grid kernel (ff_sph.cu): a warp's 64 radii share the direction: per point r d_P, sincos, E cos, E sin, and those two times r
+// = 24 slots, d_P = n.P once per (direction, pair); the polynomial in r: 4, 5, 6 slots per point for L = 1, 2, 3 plus the
+// per-direction sums G_n (3, 9, 19 slots per (direction, pair, state)); the E table: one exp (16 slots) per (pair, radius)
+const double kCtrSph = 24.0 + 3.0 / 64.0, kCtrSphTable = 16.0;
+const double kWSph[kNClasses] = {2, 4 + 3 / 64.0, 5 + 9 / 64.0, 6 + 19 / 64.0, 38, 59, 87, 123, 168, 223, 289, 367, 458};
 const double kWRow[kNClasses] = {2, 5 + 2 / 64.0, 7 + 7 / 64.0, 9 + 16 / 64.0, 38, 59, 87, 123, 168, 223, 289, 367, 458};
 
 }  // namespace
