@@ -154,6 +154,60 @@ __device__ __forceinline__ int active_prefix(const double* __restrict__ qc, long
     return (int)lo;
 }
 
+// ---- what a CTA of an S4 kernel has to do (all S4 kernels: grid = q tiles x stream chunks) -------------------------------------
+// Per class: the records of the CTA's chunk that its tile keeps, where they start in the stream and which table row they have —
+// worked out once by threads 0..6 and parked in shared memory, so that nothing of it stays live in registers across the class loops
+// (the kernels sit at the 255-register limit).  q-adaptive cut-off (option): of every class the tile keeps the records whose q_cut
+// exceeds its smallest |q|.  Ticket protocol over the chunks of the tile that have work (chunk 0 always takes part: it stores, zeros
+// if need be): a chunk without work leaves at once instead of holding an SM slot until its turn comes — with the cut-off the far-out
+// tiles keep only a prefix of every class, i.e. only their first chunks.
+struct CtaPlan {                                          // one per CTA, in shared memory
+    int nrec[kFastMaxClass + 1], nact[kFastMaxClass + 1];
+    unsigned long long off[kFastMaxClass + 1];            // byte offset of the first record from the stream base
+    long long row[kFastMaxClass + 1];                     // its stream-order index (row of the factor tables)
+    int turn, next;                                       // my turn at the tile's ticket (-1: no work), and the value I pass on
+    double sh_min[8];
+};
+// Whole-CTA call.  q2_min: the smallest |q|^2 over this thread's valid points (1e300 if it has none); read only with the cut-off on.
+template <int NS>
+__device__ __forceinline__ void plan_cta(const V1Args& v, int chunk, double q2_min, CtaPlan& p)
+{
+    double q_min = 0.0;
+    if (v.qcut != nullptr) q_min = sqrt(block_min(q2_min, p.sh_min));
+    if (threadIdx.x <= kFastMaxClass) {
+        const int L = threadIdx.x;
+        const StreamDesc& d = *v.desc;
+        const V1Chunk& ck = d.chunks[chunk];
+        int n = ck.n[L];
+        SCARF_CHECK(n >= 0 && ck.begin[L] >= 0 && (long long)ck.begin[L] + n <= d.cls_n[L]);
+        // records of the class this TILE keeps (all of them unless the q-adaptive cut-off is on)
+        const int n_act = v.qcut != nullptr ? active_prefix(v.qcut + d.cls_first[L], d.cls_n[L], q_min) : (int)d.cls_n[L];
+        p.nact[L] = n_act;
+        n = max(0, min(n, n_act - ck.begin[L]));
+        if (v.work != nullptr && n > 0) atomicAdd(v.work + L, (unsigned long long)n);
+        p.nrec[L] = n;
+        p.off[L] = d.cls_off[L] + (unsigned long long)ck.begin[L] * (unsigned long long)(rec_doubles(L, NS) * 8);
+        p.row[L] = d.cls_first[L] + ck.begin[L];
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const StreamDesc& d = *v.desc;
+        auto has_work = [&](int k) {
+            if (k == 0) return true;
+            for (int L = 0; L <= kFastMaxClass; ++L)
+                if (d.chunks[k].n[L] > 0 && p.nact[L] > d.chunks[k].begin[L]) return true;
+            return false;
+        };
+        int before = 0;
+        for (int k = 0; k < chunk; ++k) before += has_work(k) ? 1 : 0;
+        bool later = false;
+        for (int k = chunk + 1; k < v.n_chunks; ++k) later = later || has_work(k);
+        p.turn = has_work(chunk) ? before : -1;             // -1: nothing to do, nothing to add
+        p.next = later ? before + 1 : 0;                    // the last working chunk puts the ticket back to 0
+    }
+    __syncthreads();
+}
+
 // ---- one record = transcendental part (record_trans) + the (state, h) loop (record_accum) -------------------
 // The two are separate so that run_class can software-pipeline them: the exp/sincos chains of record k+1 (low
 // ILP: two dependent Horner chains per q-point) are issued in the same basic block as the 4 NS n_herm independent

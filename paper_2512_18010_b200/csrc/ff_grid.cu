@@ -236,63 +236,18 @@ __global__ void __launch_bounds__(kThreads, 2) ff_grid_kernel(const GridArgs a)
 #pragma unroll
         for (int s = 0; s < NS; ++s) re[j][s] = im[j][s] = 0.0;
 
-    // Per class: the records this CTA evaluates, where they start in the stream and in the tables — worked out once by
-    // threads 0..6 and parked in shared memory (nothing of it stays live in registers across the class loops).
-    // q-adaptive cut-off (option): of every class the box keeps the records whose q_cut exceeds its smallest |q|.
-    __shared__ int s_nrec[kFastMaxClass + 1], s_nact[kFastMaxClass + 1];
-    __shared__ int s_turn, s_next;                          // ticket protocol: my turn, and the value I pass on
-    __shared__ unsigned long long s_off[kFastMaxClass + 1];
-    __shared__ long long s_row[kFastMaxClass + 1];
+    __shared__ CtaPlan plan;                                // per class: the records this CTA evaluates; its ticket turn (ff_common.cuh)
     {
-        double q_min = 0.0;
-        if (a.v.qcut != nullptr) {
-            __shared__ double sh_min[kThreads / 32];
-            double m2 = 1e300;
+        double m2 = 1e300;
 #pragma unroll
-            for (int j = 0; j < kNQ; ++j)
-                if (bx * kGridBX + ixl + 2 * j < a.nx_eval && iy < a.ny && iz < a.nz)
-                    m2 = fmin(m2, qv[j][0] * qv[j][0] + qv[j][1] * qv[j][1] + qv[j][2] * qv[j][2]);
-            q_min = sqrt(block_min(m2, sh_min));
-        }
-        if (threadIdx.x <= kFastMaxClass) {
-            const int L = threadIdx.x;
-            const StreamDesc& d = *a.v.desc;
-            const V1Chunk& ck = d.chunks[chunk];
-            int n = ck.n[L];
-            SCARF_CHECK(n >= 0 && ck.begin[L] >= 0 && (long long)ck.begin[L] + n <= d.cls_n[L]);
-            // records of the class this TILE keeps (all of them unless the q-adaptive cut-off is on)
-            const int n_act = a.v.qcut != nullptr ? active_prefix(a.v.qcut + d.cls_first[L], d.cls_n[L], q_min) : (int)d.cls_n[L];
-            s_nact[L] = n_act;
-            n = max(0, min(n, n_act - ck.begin[L]));
-            if (a.v.work != nullptr && n > 0) atomicAdd(a.v.work + L, (unsigned long long)n);
-            s_nrec[L] = n;
-            s_off[L] = d.cls_off[L] + (unsigned long long)ck.begin[L] * (unsigned long long)(rec_doubles(L, NS) * 8);
-            s_row[L] = d.cls_first[L] + ck.begin[L];
-        }
-        __syncthreads();
-        // Ticket protocol over the chunks of this tile that have work (chunk 0 always takes part: it stores, zeros if need be).
-        // A chunk without work leaves at once instead of holding an SM slot until its turn comes — with the q-adaptive cut-off
-        // the far-out tiles keep only a prefix of every class, i.e. only their first chunks.
-        if (threadIdx.x == 0) {
-            const StreamDesc& d = *a.v.desc;
-            auto has_work = [&](int k) {
-                if (k == 0) return true;
-                for (int L = 0; L <= kFastMaxClass; ++L)
-                    if (d.chunks[k].n[L] > 0 && s_nact[L] > d.chunks[k].begin[L]) return true;
-                return false;
-            };
-            int before = 0;
-            for (int k = 0; k < chunk; ++k) before += has_work(k) ? 1 : 0;
-            bool later = false;
-            for (int k = chunk + 1; k < a.v.n_chunks; ++k) later = later || has_work(k);
-            s_turn = has_work(chunk) ? before : -1;           // -1: nothing to do, nothing to add
-            s_next = later ? before + 1 : 0;                  // the last working chunk puts the ticket back to 0
-        }
-        __syncthreads();
+        for (int j = 0; j < kNQ; ++j)
+            if (bx * kGridBX + ixl + 2 * j < a.nx_eval && iy < a.ny && iz < a.nz)
+                m2 = fmin(m2, qv[j][0] * qv[j][0] + qv[j][1] * qv[j][1] + qv[j][2] * qv[j][2]);
+        plan_cta<NS>(a.v, chunk, m2, plan);
     }
 #define SCARF_GRID_CLASS(LV)                                                                                        \
-    if (s_nrec[LV] > 0)                                                                                             \
-        run_class_grid<LV, NS>(pp, a, a.v.base + s_off[LV], s_row[LV], s_nrec[LV], bx, by, bz, ixl, iyl, izl, qv, re, im);
+    if (plan.nrec[LV] > 0)                                                                                          \
+        run_class_grid<LV, NS>(pp, a, a.v.base + plan.off[LV], plan.row[LV], plan.nrec[LV], bx, by, bz, ixl, iyl, izl, qv, re, im);
     SCARF_GRID_CLASS(0)
     SCARF_GRID_CLASS(1)
     SCARF_GRID_CLASS(2)
@@ -306,9 +261,9 @@ __global__ void __launch_bounds__(kThreads, 2) ff_grid_kernel(const GridArgs a)
     // also stores its conjugate at the mirror point when the grid is inversion-symmetric
     double2* dst = reinterpret_cast<double2*>(a.v.dst);
     double2* fin = a.v.dst_final != nullptr ? reinterpret_cast<double2*>(a.v.dst_final) : dst;    // finished values (last chunk)
-    const int turn = s_turn;
+    const int turn = plan.turn;
     if (turn < 0) return;                                   // a chunk without work (uniform over the CTA)
-    const bool first = turn == 0, last = s_next == 0;
+    const bool first = turn == 0, last = plan.next == 0;
     if (a.v.n_chunks > 1) ticket_wait(a.v.tickets + tile, turn);
 #pragma unroll
     for (int j = 0; j < kNQ; ++j) {
@@ -333,7 +288,7 @@ __global__ void __launch_bounds__(kThreads, 2) ff_grid_kernel(const GridArgs a)
                 }
         }
     }
-    if (a.v.n_chunks > 1) ticket_pass(a.v.tickets + tile, s_next);
+    if (a.v.n_chunks > 1) ticket_pass(a.v.tickets + tile, plan.next);
 }
 
 }  // namespace

@@ -322,56 +322,17 @@ __global__ void __launch_bounds__(kThreads, 2) ff_sph_kernel(const SphArgs a)
 #pragma unroll
         for (int s = 0; s < NS; ++s) re[j][s] = im[j][s] = 0.0;
 
-    // Per class: the records this CTA evaluates, where they start in the stream and in the table (ff_grid.cu has the same prologue)
-    __shared__ int s_nrec[kFastMaxClass + 1], s_nact[kFastMaxClass + 1];
-    __shared__ int s_turn, s_next;                          // ticket protocol: my turn, and the value I pass on
-    __shared__ unsigned long long s_off[kFastMaxClass + 1];
-    __shared__ long long s_row[kFastMaxClass + 1];
+    __shared__ CtaPlan plan;                                // per class: the records this CTA evaluates; its ticket turn (ff_common.cuh)
     {
-        double q_min = 0.0;
-        if (a.v.qcut != nullptr) {
-            __shared__ double sh_min[kThreads / 32];
-            double m = 1e300;
+        double m2 = 1e300;
 #pragma unroll
-            for (int j = 0; j < kNQ; ++j)
-                if (dir_ok && rbox * kSphBR + lane + 32 * j < a.n_r) m = fmin(m, fabs(rv[j]));     // |q| = |r| (n is a unit vector)
-            q_min = block_min(m, sh_min);
-        }
-        if (threadIdx.x <= kFastMaxClass) {
-            const int L = threadIdx.x;
-            const StreamDesc& dsc = *a.v.desc;
-            const V1Chunk& ck = dsc.chunks[chunk];
-            int n = ck.n[L];
-            SCARF_CHECK(n >= 0 && ck.begin[L] >= 0 && (long long)ck.begin[L] + n <= dsc.cls_n[L]);
-            const int n_act = a.v.qcut != nullptr ? active_prefix(a.v.qcut + dsc.cls_first[L], dsc.cls_n[L], q_min) : (int)dsc.cls_n[L];
-            s_nact[L] = n_act;
-            n = max(0, min(n, n_act - ck.begin[L]));
-            if (a.v.work != nullptr && n > 0) atomicAdd(a.v.work + L, (unsigned long long)n);
-            s_nrec[L] = n;
-            s_off[L] = dsc.cls_off[L] + (unsigned long long)ck.begin[L] * (unsigned long long)(rec_doubles(L, NS) * 8);
-            s_row[L] = dsc.cls_first[L] + ck.begin[L];
-        }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            const StreamDesc& dsc = *a.v.desc;
-            auto has_work = [&](int k) {
-                if (k == 0) return true;
-                for (int L = 0; L <= kFastMaxClass; ++L)
-                    if (dsc.chunks[k].n[L] > 0 && s_nact[L] > dsc.chunks[k].begin[L]) return true;
-                return false;
-            };
-            int before = 0;
-            for (int k = 0; k < chunk; ++k) before += has_work(k) ? 1 : 0;
-            bool later = false;
-            for (int k = chunk + 1; k < a.v.n_chunks; ++k) later = later || has_work(k);
-            s_turn = has_work(chunk) ? before : -1;           // -1: nothing to do, nothing to add
-            s_next = later ? before + 1 : 0;                  // the last working chunk puts the ticket back to 0
-        }
-        __syncthreads();
+        for (int j = 0; j < kNQ; ++j)
+            if (dir_ok && rbox * kSphBR + lane + 32 * j < a.n_r) m2 = fmin(m2, rv[j] * rv[j]);     // |q| = |r| (n is a unit vector)
+        plan_cta<NS>(a.v, chunk, m2, plan);
     }
 #define SCARF_SPH_CLASS(LV)                                                                                          \
-    if (s_nrec[LV] > 0)                                                                                              \
-        run_class_sph<LV, NS>(pp, a, a.v.base + s_off[LV], s_row[LV], s_nrec[LV], rbox, lane, Ww, nv, rv, re, im);
+    if (plan.nrec[LV] > 0)                                                                                           \
+        run_class_sph<LV, NS>(pp, a, a.v.base + plan.off[LV], plan.row[LV], plan.nrec[LV], rbox, lane, Ww, nv, rv, re, im);
     SCARF_SPH_CLASS(0)
     SCARF_SPH_CLASS(1)
     SCARF_SPH_CLASS(2)
@@ -385,9 +346,9 @@ __global__ void __launch_bounds__(kThreads, 2) ff_sph_kernel(const SphArgs a)
     // also stores its conjugate at the mirror point when the grid is inversion-symmetric
     double2* dst = reinterpret_cast<double2*>(a.v.dst);
     double2* fin = a.v.dst_final != nullptr ? reinterpret_cast<double2*>(a.v.dst_final) : dst;    // finished values (last chunk)
-    const int turn = s_turn;
+    const int turn = plan.turn;
     if (turn < 0) return;                                   // a chunk without work (uniform over the CTA)
-    const bool first = turn == 0, last = s_next == 0;
+    const bool first = turn == 0, last = plan.next == 0;
     if (a.v.n_chunks > 1) ticket_wait(a.v.tickets + tile, turn);
     const long long n_dir = (long long)a.n_theta * a.n_phi;
     long long d_mirror = -1;
@@ -418,7 +379,7 @@ __global__ void __launch_bounds__(kThreads, 2) ff_sph_kernel(const SphArgs a)
                 }
         }
     }
-    if (a.v.n_chunks > 1) ticket_pass(a.v.tickets + tile, s_next);
+    if (a.v.n_chunks > 1) ticket_pass(a.v.tickets + tile, plan.next);
 }
 
 template <int NS>
