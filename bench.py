@@ -285,13 +285,18 @@ def run_ours(args):
         step_grid()
         sc.set_option("grid_symmetry", 1)
 
-    def step_grid_box():                    # the box kernel (ff_grid.cu) where the row kernel (ff_row.cu) is the automatic choice
+    def step_grid_box():                    # the box kernel (ff_grid.cu) where another kernel is the automatic choice
         sc.set_option("grid_variant", 0)
         step_grid()
         sc.set_option("grid_variant", -1)
 
+    def step_grid_row():                    # the row kernel (ff_row.cu) where the mirror-pair kernel (ff_zrow.cu) is the automatic choice
+        sc.set_option("grid_variant", 1)
+        step_grid()
+        sc.set_option("grid_variant", -1)
+
     def grid_kernel_name(stats):
-        return {1: "ff_row_kernel<12>", 2: "ff_sph_kernel<12>"}.get(stats.get("last_grid_variant", 0), "ff_grid_kernel<12>")
+        return {1: "ff_row_kernel<12>", 2: "ff_zrow_kernel<12>", 3: "ff_sph_kernel<12>"}.get(stats.get("last_grid_variant", 0), "ff_grid_kernel<12>")
 
     def run_timed(step, steps, warmup, sample_clocks=False):
         """W untimed steps, then `steps` steps timed with CUDA events on the library's stream (L2 flushed before each,
@@ -359,7 +364,7 @@ def run_ours(args):
                 "kernel": grid_kernel_name(s2) if slots_key == "grid" else "ff_v1_kernel<12>",
                 "launches_per_step": int(s2["last_kernel_launches"] + s2["last_fold_launches"])}
 
-    list_path = grid_path = grid_plain = grid_box = sph_path = sph_plain = None
+    list_path = grid_path = grid_plain = grid_box = grid_row = sph_path = sph_plain = None
     if spherical:
         if path == "sph":
             list_path = dict(side(step_list, w.n_q, "list"), api="scarf_form_factors")
@@ -375,10 +380,14 @@ def run_ours(args):
             n_ax = w.grid["n_per_axis"]
             grid_path = dict(side(step_grid, ((n_ax + 1) // 2) * n_ax * n_ax, "grid"), api="scarf_form_factors_grid", symmetric=True)
         grid_plain = dict(side(step_grid_plain, w.n_q, "grid"), api="scarf_form_factors_grid", symmetric=False)
-        if st.get("last_grid_variant", 0) == 1 or (grid_path is not None and grid_path["kernel"].startswith("ff_row")):
+        head_variant = st.get("last_grid_variant", 0) if path == "grid" else {"ff_row_kernel<12>": 1, "ff_zrow_kernel<12>": 2}.get(grid_path["kernel"], 0)
+        if head_variant in (1, 2):
             n_ax = w.grid["n_per_axis"]
             grid_box = dict(side(step_grid_box, ((n_ax + 1) // 2) * n_ax * n_ax, "grid"), api="scarf_form_factors_grid", symmetric=True,
                             option="grid_variant = 0")
+        if head_variant == 2:
+            grid_row = dict(side(step_grid_row, ((n_ax + 1) // 2) * n_ax * n_ax, "grid"), api="scarf_form_factors_grid", symmetric=True,
+                            option="grid_variant = 1")
         (step_grid if path == "grid" else step_list)()        # leave the headline path's result in out_dev for the parity sample
         torch.cuda.synchronize()
 
@@ -503,7 +512,13 @@ def run_ours(args):
         # i.e. the slots this launch would have cost without sharing the (q_y, q_z) part between a thread's two points
         survey_slots = n_eval_q * (poly_per_q + 6.0 * st["n_pairs_kept"] * len(range(0, w.n_states, 12)))
         roofline["frac_survey_model"] = survey_slots / (head["main_kernel_ms"] * 1e-3) / peak_meas
-        if st.get("last_grid_variant", 0) == 1:
+        if st.get("last_grid_variant", 0) == 2:
+            roofline["slots_model_note"] = ("frac: FP64 slots the kernel's algorithm needs (a lane owns the points +z and -z of a row and accumulates "
+                                            "their half sum and half difference, whose polynomials in z^2 are shared by the pair and by the row: "
+                                            "4 / 5 / 6 slots per (q, pair, state) for L = 1 / 2 / 3, 2 per (q, pair), plus the per-row part, "
+                                            "14 / 23 / 36 slots per (row, pair, state)); frac_survey_model: the monomial-form count n_herm + 3 "
+                                            "over the same time")
+        elif st.get("last_grid_variant", 0) == 1:
             roofline["slots_model_note"] = ("frac: FP64 slots the kernel's algorithm needs (the 64 points of a warp's row share the (q_x, q_y) "
                                             "part of every polynomial: 5 / 7 / 9 slots per (q, pair, state) for L = 1 / 2 / 3 plus the "
                                             "per-row part, 2 / 7 / 16 slots per (row, pair, state)); frac_survey_model: the monomial-form "
@@ -562,7 +577,7 @@ def run_ours(args):
             "clocks": clocks, "roofline": roofline}
 
     for name, obj in (("list_path", list_path), ("grid_path", grid_path), ("grid_path_no_symmetry", grid_plain),
-                      ("grid_path_box_kernel", grid_box), ("sph_path", sph_path), ("sph_path_no_symmetry", sph_plain)):
+                      ("grid_path_box_kernel", grid_box), ("grid_path_row_kernel", grid_row), ("sph_path", sph_path), ("sph_path_no_symmetry", sph_plain)):
         if obj is not None:
             obj["roofline"] = alu_roofline(obj["slots_main_kernel"], obj["main_kernel_ms"], obj["kernel"])
             line[name] = obj

@@ -97,7 +97,7 @@ typedef struct scarf_stats {
     double last_grid_kernel_slots;             /* FP64 issue-slot model of the product-grid S4 kernel alone (no tables)*/
     double adaptive_bound;                     /* option adaptive_tol: |f_s(q) - exact| <= this for every q, s (0 when off) */
     double last_adaptive_work_fraction;        /* modelled work of the last S4 call / work without the cut-off (1 when off) */
-    int32_t last_grid_variant;                 /* kernel of the last product-grid call: 0 box, 1 row (option grid_variant), 2 scarf_form_factors_sph */
+    int32_t last_grid_variant;                 /* kernel of the last product-grid call: 0 box, 1 row, 2 mirror-pair row (option grid_variant), 3 scarf_form_factors_sph */
     int32_t reserved0;
 } scarf_stats;
 
@@ -143,8 +143,12 @@ int scarf_set_stream(scarf_ctx* ctx, void* cuda_stream);
  *           "grid_variant": default -1 (automatic).  Kernel of scarf_form_factors_grid: 0 = box kernel (a CTA owns a 4 x 8 x 8
  *                         box of the grid; the two points of a thread share (q_y, q_z)), 1 = row kernel (a warp owns 64
  *                         consecutive z-points of one (ix, iy) row, so the (q_x, q_y) part of every polynomial is evaluated
- *                         once per warp: fewer FP64 operations per point, but lanes beyond the end of a row idle), -1 = the
- *                         row kernel when its 4 (y) x 64 (z) boxes are at least 80 % full.  Same results to round-off.
+ *                         once per warp: fewer FP64 operations per point, but lanes beyond the end of a row idle), 2 = mirror-pair
+ *                         row kernel (needs a z axis with qz[i] == -qz[nz-1-i] bit for bit, else the choice is automatic: a lane
+ *                         owns the points +z and -z of its row and accumulates their half sum and half difference, whose
+ *                         polynomials in z^2 are shared by the pair), -1 = the mirror-pair kernel when the z axis allows it and
+ *                         its 4 (y) x 32 (pairs) boxes are at least 80 % full, else the row kernel when its 4 x 64 boxes are,
+ *                         else the box kernel.  Same results to round-off.
  *           "fft_density_variant": default 1 = FP64 tensor-core (DMMA) density kernel of scarf_fft_form_factors with the
  *                         orbital values evaluated per point tile in shared memory (falls back to 2 when the tile of a
  *                         very large basis does not fit), 2 = DMMA kernel reading orbital values tabulated in device
@@ -233,7 +237,7 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
  * negatives): its points agree with a caller's own list of the same grid to FP64 round-off of the trigonometric functions.
  * r, cos_theta: HOST pointers (r finite, |cos_theta| <= 1).  out: host or device; with a device `out` the call is asynchronous
  * on the context stream.  Results equal scarf_form_factors on the expanded point list up to FP64 round-off.  Bases with
- * g, h, i shells run that list path internally.  scarf_stats: last_grid_symmetric, last_grid_variant = 2, last_grid_kernel_slots. */
+ * g, h, i shells run that list path internally.  scarf_stats: last_grid_symmetric, last_grid_variant = 3, last_grid_kernel_slots. */
 int scarf_form_factors_sph(scarf_ctx* ctx, int32_t n_r, const double* r, int32_t n_theta, const double* cos_theta, int32_t n_phi,
                            double* out);
 

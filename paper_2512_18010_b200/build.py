@@ -15,7 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libscarf.so")
-SOURCES = ["host_setup.cpp", "fold.cu", "ff_v1.cu", "ff_grid.cu", "ff_row.cu", "ff_sph.cu", "ff_highl.cu", "angular.cu", "pure.cu", "fft_method.cu", "scarf_api.cu"]
+SOURCES = ["host_setup.cpp", "fold.cu", "ff_v1.cu", "ff_grid.cu", "ff_row.cu", "ff_zrow.cu", "ff_sph.cu", "ff_highl.cu", "angular.cu", "pure.cu", "fft_method.cu", "scarf_api.cu"]
 HEADERS = ["host_setup.hpp", "kernels.cuh", "ff_common.cuh", "ff_math.cuh", "math_coeffs.cuh", os.path.join("..", "..", "include", "scarf.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC,-O3,-fopenmp", "--expt-relaxed-constexpr"]

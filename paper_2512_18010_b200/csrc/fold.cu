@@ -390,7 +390,8 @@ __global__ void plan_chunks_kernel(StreamDesc* d, int K, int ns_real, double ctr
     // and the row kernel the (q_x, q_y) part between the 64 points of a warp
     const double kWl[kFastMaxClass + 1] = {2, 7, 13, 23, 38, 59, 87}, kWg[kFastMaxClass + 1] = {2, 6, 10.5, 17, 38, 59, 87},
                  kWr[kFastMaxClass + 1] = {2, 5.03, 7.11, 9.25, 38, 59, 87}, kWs[kFastMaxClass + 1] = {2, 4.05, 5.14, 6.3, 38, 59, 87};
-    const double* kW = model == 3 ? kWs : (model == 2 ? kWr : (model == 1 ? kWg : kWl));
+    const double kWz[kFastMaxClass + 1] = {2, 4.22, 5.36, 6.56, 38, 59, 87};
+    const double* kW = model == 4 ? kWz : (model == 3 ? kWs : (model == 2 ? kWr : (model == 1 ? kWg : kWl)));
     double w[kFastMaxClass + 1], total = 0.0;
     for (int c = 0; c <= kFastMaxClass; ++c) {
         w[c] = (double)ns_real * kW[c] + ctr;

@@ -121,7 +121,7 @@ cudaError_t launch_screen(const ScreenArgs& a, cudaStream_t st);
 cudaError_t launch_pack(const PackArgs& a, cudaStream_t st);
 // cost-balanced split of the FAST classes (0..kFastMaxClass) of the stream into exactly K chunks (K <= kMaxChunks);
 // w(c) = ns_real * W(c) + ctr.  One thread; ~2 us.
-// model: per-class slot counts of 0 the list kernel, 1 the box kernel (ff_grid.cu), 2 the row kernel (ff_row.cu), 3 the spherical-grid kernel (ff_sph.cu)
+// model: per-class slot counts of 0 the list kernel, 1 the box kernel (ff_grid.cu), 2 the row kernel (ff_row.cu), 3 the spherical-grid kernel (ff_sph.cu), 4 the mirror-pair row kernel (ff_zrow.cu)
 cudaError_t launch_plan_chunks(StreamDesc* desc, int K, int ns_real, double ctr, cudaStream_t st, int model = 0);
 
 // v1 (ff_v1.cu): the general-q kernel.  Grid = (n_tiles, n_chunks), dispatched chunk-major; the chunks of one q tile add
@@ -191,6 +191,12 @@ cudaError_t ff_grid_init_device();           // per-device function attributes (
 constexpr int kRowBX = 1, kRowBY = 4, kRowBZ = 64;
 cudaError_t launch_ff_row(int NS, const GridArgs& a, cudaStream_t st);
 cudaError_t ff_row_init_device();
+// mirror-pair row kernel (ff_zrow.cu): the row kernel on a grid whose z axis is antisymmetric bit for bit; a lane's two points are
+// (+z, -z).  GridArgs as for the row kernel except: nbz counts boxes of 32 mirror PAIRS and the Z table (box edge 32) covers the
+// first ceil(nz/2) points of the axis.
+constexpr int kZrowBX = 1, kZrowBY = 4, kZrowBZ = 32;
+cudaError_t launch_ff_zrow(int NS, const GridArgs& a, cudaStream_t st);
+cudaError_t ff_zrow_init_device();
 // spherical product grid (ff_sph.cu): q = r_i n_d, n_d = (sin t_j cos phi_k, sin t_j sin phi_k, cos t_j), d = j n_phi + k; point index
 // i * n_theta * n_phi + d (the layout of scarf_angular_moments' input).  A warp owns one direction and 64 radii.
 constexpr int kSphBD = 4, kSphBR = 64;

@@ -44,6 +44,10 @@ const double kWGrid[kNClasses] = {2, 6, 10.5, 17, 38, 59, 87, 123, 168, 223, 289
 // (2, 7, 16 slots per (record, state)) spread over the 64 points of the row
 // ... and 4 slots per point for g = (X Y) Z, X Y once per (row, pair): 4 more, spread over the row's 64 points
 const double kCtrRow = 4.0 + 4.0 / 64.0;
+// mirror-pair row kernel (ff_zrow.cu): E and O' are shared by the pair (+z, -z): 4, 5, 6 slots per point for L = 1, 2, 3 plus the
+// pre-pass (X Y, the sums, H = X Y G: 14, 23, 36 slots per (row, pair, state)); per (q, pair): c z, s z or the four products of L = 0
+const double kCtrZrow = 2.0;
+const double kWZrow[kNClasses] = {2, 4 + 14 / 64.0, 5 + 23 / 64.0, 6 + 36 / 64.0, 38, 59, 87, 123, 168, 223, 289, 367, 458};
 // spherical-grid kernel (ff_sph.cu): a warp's 64 radii share the direction: per point r d_P, sincos, E cos, E sin, and those two times r
 // = 24 slots, d_P = n.P once per (direction, pair); the polynomial in r: 4, 5, 6 slots per point for L = 1, 2, 3 plus the
 // per-direction sums G_n (3, 9, 19 slots per (direction, pair, state)); the E table: one exp (16 slots) per (pair, radius)
@@ -279,6 +283,7 @@ int scarf_create(scarf_ctx** out, int device)
         // per-device function attributes (idempotent; set for every context so that no process-wide flag is needed)
         if (e == cudaSuccess) e = ff_grid_init_device();
         if (e == cudaSuccess) e = ff_row_init_device();
+        if (e == cudaSuccess) e = ff_zrow_init_device();
         if (e == cudaSuccess) e = ff_sph_init_device();
         if (e == cudaSuccess) e = angular_init_device();
         if (e == cudaSuccess) e = density_fused_init_device();
@@ -352,7 +357,7 @@ int scarf_set_option(scarf_ctx* ctx, const char* key, double value)
         if (value != 0.0 && value != 1.0) return fail(ctx, SCARF_EINVAL, "set_option: host_zero_copy must be 0 or 1");
         ctx->host_zero_copy = (int)value;
     } else if (k == "grid_variant") {
-        if (value != 0.0 && value != 1.0 && value != -1.0) return fail(ctx, SCARF_EINVAL, "set_option: grid_variant must be -1, 0 or 1");
+        if (value != 0.0 && value != 1.0 && value != 2.0 && value != -1.0) return fail(ctx, SCARF_EINVAL, "set_option: grid_variant must be -1, 0, 1 or 2");
         ctx->grid_variant = (int)value;
     } else if (k == "n_chunks") {
         if (value < 0 || value > kMaxChunks) return fail(ctx, SCARF_EINVAL, "set_option: n_chunks outside 0..32");
@@ -878,7 +883,7 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
             if (!all_host)
                 CU(cudaMemcpyAsync(dax[k], ax_in[k], (size_t)ax_n[k] * sizeof(double), host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, st),
                    "form_factors_grid: copy axis");
-            if (ctx->grid_symmetry) {
+            {   // a host copy of every axis: the symmetry decisions below
                 hax[k].resize((size_t)ax_n[k]);
                 if (host) std::memcpy(hax[k].data(), ax_in[k], (size_t)ax_n[k] * sizeof(double));
                 else {
@@ -897,11 +902,19 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         // Kernel: the row kernel (a warp = 64 z-points of one (ix, iy) row, 4 rows per CTA) needs fewer FP64 slots per point but
         // wastes the lanes beyond the end of a row; it is taken when the 4 x 64 boxes are at least 80 % full.
         const double row_fill = ((double)ny * nz) / ((double)((ny + kRowBY - 1) / kRowBY * kRowBY) * (double)((nz + kRowBZ - 1) / kRowBZ * kRowBZ));
-        const bool row = ctx->grid_variant == 1 || (ctx->grid_variant < 0 && row_fill >= 0.8);
-        const int BXs = row ? kRowBX : kGridBX, BYs = row ? kRowBY : kGridBY, BZs = row ? kRowBZ : kGridBZ;
-        const double* kWg = row ? kWRow : kWGrid;
-        const double ctr_g = row ? kCtrRow : kCtrGrid;
-        const int nbx = (nx_eval + BXs - 1) / BXs, nby = (ny + BYs - 1) / BYs, nbz = (nz + BZs - 1) / BZs;
+        // Mirror-pair row kernel: needs a z axis that is antisymmetric bit for bit (a lane's two points are +z and -z of its row; this is
+        // independent of the inversion symmetry of the whole grid); its boxes are 4 (y) x 32 mirror pairs.
+        bool z_antisym = nz >= 2;
+        for (int i = 0; i < nz && z_antisym; ++i) z_antisym = hax[2][(size_t)i] == -hax[2][(size_t)(nz - 1 - i)];
+        const int nz_half = (nz + 1) / 2;
+        const double zrow_fill = ((double)ny * nz_half) / ((double)((ny + kZrowBY - 1) / kZrowBY * kZrowBY) * (double)((nz_half + kZrowBZ - 1) / kZrowBZ * kZrowBZ));
+        const bool zrow = z_antisym && (ctx->grid_variant == 2 || (ctx->grid_variant < 0 && zrow_fill >= 0.8));
+        const bool row = !zrow && (ctx->grid_variant == 1 || (ctx->grid_variant != 0 && row_fill >= 0.8));
+        const int BXs = zrow ? kZrowBX : (row ? kRowBX : kGridBX), BYs = zrow ? kZrowBY : (row ? kRowBY : kGridBY),
+                  BZs = zrow ? kZrowBZ : (row ? kRowBZ : kGridBZ);
+        const double* kWg = zrow ? kWZrow : (row ? kWRow : kWGrid);
+        const double ctr_g = zrow ? kCtrZrow : (row ? kCtrRow : kCtrGrid);
+        const int nbx = (nx_eval + BXs - 1) / BXs, nby = (ny + BYs - 1) / BYs, nbz = ((zrow ? nz_half : nz) + BZs - 1) / BZs;
         const long long n_tiles = (long long)nbx * nby * nbz;
         if (n_tiles > 0x7fffffffLL) return fail(ctx, SCARF_EINVAL, "form_factors_grid: grid too large for one call");
         const size_t obytes = (size_t)ctx->n_states * (size_t)n_q * 2 * sizeof(double);
@@ -955,7 +968,11 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
             a.n_rows = n_rows;
             a.v.qcut = ctx->qcut_dev;
             a.v.work = ctx->qcut_dev ? static_cast<unsigned long long*>(ctx->d_work.p) : nullptr;
-            CU(launch_grid_tables(a, tx, ty, tz, st), "form_factors_grid: table kernel");
+            {
+                GridArgs at = a;
+                if (zrow) at.nz = nz_half;              // the Z table of the mirror-pair kernel covers the first half of the axis
+                CU(launch_grid_tables(at, tx, ty, tz, st), "form_factors_grid: table kernel");
+            }
             ++launches;
             // Host output: the x boxes are cut into slabs; the device->host copies of a finished slab (and of its mirror slab on
             // a symmetric grid) run on a second stream while the next slab is being computed.
@@ -979,9 +996,9 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
                     if (a.v.tile_group > 0 && ctx->host_tile_group > 0) a.v.tile_group = ctx->host_tile_group;
                 }
                 if (int rc = prepare_tickets(ctx, tiles_s, a.v.n_chunks, st, &a.v.tickets)) return n_slabs > 1 ? drain(rc) : rc;
-                CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, ctr_g, st, /*model=*/row ? 2 : 1), "form_factors_grid: chunk planning kernel");
+                CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, ctr_g, st, /*model=*/zrow ? 4 : (row ? 2 : 1)), "form_factors_grid: chunk planning kernel");
                 if (ctx->timing) CU(cudaEventRecord(ctx->ev_m0, st), "form_factors_grid: event");
-                CU(row ? launch_ff_row(t.NS, a, st) : launch_ff_grid(t.NS, a, st), "form_factors_grid: kernel");
+                CU(zrow ? launch_ff_zrow(t.NS, a, st) : (row ? launch_ff_row(t.NS, a, st) : launch_ff_grid(t.NS, a, st)), "form_factors_grid: kernel");
                 if (ctx->timing) {
                     CU(cudaEventRecord(ctx->ev_m1, st), "form_factors_grid: event");
                     CU(cudaEventSynchronize(ctx->ev_m1), "form_factors_grid: event sync");
@@ -1024,7 +1041,7 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         ctx->last_grid_w = kWg;
         ctx->last_grid_ctr = ctr_g;
         ctx->last_table_ctr = kCtrTable;
-        ctx->st.last_grid_variant = row ? 1 : 0;
+        ctx->st.last_grid_variant = zrow ? 2 : (row ? 1 : 0);
         ctx->st.last_grid_slots = -1.0;            // filled by scarf_get_stats from the kept counts
         if (ctx->timing) {
             CU(cudaEventRecord(ctx->ev1, st), "form_factors_grid: event");
@@ -1186,7 +1203,7 @@ int scarf_form_factors_sph(scarf_ctx* ctx, int32_t n_r, const double* r, int32_t
         ctx->grid_eval_points = (double)n_dir_eval * n_r;
         ctx->grid_table_cols = (double)n_r;
         ctx->st.last_grid_symmetric = sym ? 1 : 0;
-        ctx->st.last_grid_variant = 2;
+        ctx->st.last_grid_variant = 3;
         ctx->last_grid_w = kWSph;
         ctx->last_grid_ctr = kCtrSph;
         ctx->last_table_ctr = kCtrSphTable;

@@ -137,8 +137,9 @@ def test_row_kernel_automatic_choice(oracle_mod, Scarf, torch_cuda):
 
 @pytest.mark.parametrize("config,n_sample", [(3, 160), (4, 40)])
 def test_row_kernel_full_size_sampled(oracle_mod, Scarf, torch_cuda, config, n_sample):
-    """Configs 3 and 4 (64^3, inversion-symmetric) in the launch configuration bench.py times — the row kernel is the automatic
-    choice there — against the oracle on a seeded sample of points from both halves, and against the list kernel on every point."""
+    """Configs 3 and 4 (64^3, inversion-symmetric) at full size with the row kernel (grid_variant = 1; the automatic choice on these
+    grids is the mirror-pair kernel, tests/test_gpu_grid_zrow.py) against the oracle on a seeded sample of points from both halves,
+    and against the list kernel on every point."""
     torch = torch_cuda
     w = W.make_workload(config, oracle_mod.overlap)
     ax = W.cartesian_axis(w.grid["n_per_axis"], w.grid["qmax"])
@@ -146,6 +147,7 @@ def test_row_kernel_full_size_sampled(oracle_mod, Scarf, torch_cuda, config, n_s
     f_ref = oracle_mod.form_factors(w.basis, w.T, w.q[idx])
     with Scarf(0) as sc:
         sc.set_basis(w.basis)
+        sc.set_option("grid_variant", 1)
         sc.set_transitions(torch.as_tensor(w.T, device="cuda"))
         axd = torch.as_tensor(ax, device="cuda")
         fg = sc.form_factors_grid(axd, axd, axd)

@@ -77,7 +77,7 @@ def test_sph_ragged_shapes_all_classes(oracle_mod, Scarf, torch_cuda, shape, n_s
     r = rng.uniform(-1.0, 6.0, size=n_r)
     ct = rng.uniform(-1.0, 1.0, size=n_t)
     f, st = sph_ff(Scarf, torch_cuda, b, T, r, ct, n_p)
-    assert st["last_grid_variant"] == 2 and st["last_grid_symmetric"] == 0
+    assert st["last_grid_variant"] == 3 and st["last_grid_symmetric"] == 0
     assert_parity(f, oracle_mod.form_factors(b, T, sph_points(r, ct, n_p)))
 
 
@@ -107,7 +107,7 @@ def test_sph_inversion_symmetry_both_halves(oracle_mod, Scarf, torch_cuda, shape
     assert np.array_equal(ct, -ct[::-1])
     f_ref = oracle_mod.form_factors(b, T, sph_points(r, ct, n_p))
     f, st = sph_ff(Scarf, torch_cuda, b, T, r, ct, n_p, device=device)
-    assert st["last_grid_symmetric"] == 1 and st["last_grid_variant"] == 2
+    assert st["last_grid_symmetric"] == 1 and st["last_grid_variant"] == 3
     assert_parity(f, f_ref)
     g = f.reshape(12, n_r, n_t, n_p)
     assert np.array_equal(np.roll(g[:, :, ::-1, :], n_p // 2, axis=3), np.conj(g))
@@ -161,7 +161,7 @@ def test_sph_config5_full_size_sampled_and_list_kernel(oracle_mod, Scarf, torch_
         sc.set_transitions(torch.as_tensor(w.T, device="cuda"))
         fs = sc.form_factors_sph(r, ct, g["n_phi"])
         st = sc.stats()
-        assert st["last_grid_symmetric"] == 1 and st["last_grid_variant"] == 2
+        assert st["last_grid_symmetric"] == 1 and st["last_grid_variant"] == 3
         fl = sc.form_factors(torch.as_tensor(w.q, device="cuda"))
         torch.cuda.synchronize()
         assert_parity(fs[:, torch.as_tensor(idx, device="cuda")].cpu().numpy(), f_ref)
