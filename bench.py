@@ -517,7 +517,10 @@ def run_ours(args):
                                             "their half sum and half difference, whose polynomials in z^2 are shared by the pair and by the row: "
                                             "4 / 5 / 6 slots per (q, pair, state) for L = 1 / 2 / 3, 2 per (q, pair), plus the per-row part, "
                                             "14 / 23 / 36 slots per (row, pair, state)); frac_survey_model: the monomial-form count n_herm + 3 "
-                                            "over the same time")
+                                            "over the same time.  With 12 (4, 8) states per tile the accumulates of classes L = 0..2 are "
+                                            "issued as mma.sync.m8n8k4.f64 (DMMA, the FP64 tensor pipe: a matrix product over the records "
+                                            "of a stage), the other classes and the per-row parts as DFMAs; peak stays the DFMA peak "
+                                            "(the DMMA rate is the same 64 FMA/clk/SM on a pipe of its own)")
         elif st.get("last_grid_variant", 0) == 1:
             roofline["slots_model_note"] = ("frac: FP64 slots the kernel's algorithm needs (the 64 points of a warp's row share the (q_x, q_y) "
                                             "part of every polynomial: 5 / 7 / 9 slots per (q, pair, state) for L = 1 / 2 / 3 plus the "

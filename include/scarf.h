@@ -140,6 +140,10 @@ int scarf_set_stream(scarf_ctx* ctx, void* cuda_stream);
  *                         Pageable host memory always takes the copy.  The call returns when `out` is complete either way.
  *           "host_tile_group": default 0 (automatic).  Tiles per dispatch group of the product-grid kernels when they write a
  *                         pinned host `out` (see host_zero_copy).  A tuning/testing knob; results do not depend on it.
+ *           "grid_tile_group": default -1 (automatic).  Tiles per dispatch group of the product-grid kernels when `out` is device
+ *                         memory: the CTAs run chunk-major inside groups of this many tiles, group after group, so that CTAs
+ *                         working on different pair classes (FP64-pipe loops, tensor-core loops) share an SM.  0 = chunk-major
+ *                         over all tiles.  A tuning/testing knob; results do not depend on it.
  *           "grid_variant": default -1 (automatic).  Kernel of scarf_form_factors_grid: 0 = box kernel (a CTA owns a 4 x 8 x 8
  *                         box of the grid; the two points of a thread share (q_y, q_z)), 1 = row kernel (a warp owns 64
  *                         consecutive z-points of one (ix, iy) row, so the (q_x, q_y) part of every polynomial is evaluated

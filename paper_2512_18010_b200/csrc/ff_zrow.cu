@@ -68,6 +68,16 @@ __host__ __device__ constexpr int h_warp_bytes(int NS)
 }
 template <int NS> constexpr int smem_bytes() { return kStages * kSlotBytes + kWarps * h_warp_bytes(NS) + 64; }
 
+// classes L = 1..kZrowMmaMaxL through mma.sync (zrow_mma) for state tiles that fill whole N tiles; the DFMA loops otherwise
+#ifndef SCARF_ZROW_MMA_MAXL
+#define SCARF_ZROW_MMA_MAXL 2
+#endif
+constexpr int kZrowMmaMaxL = SCARF_ZROW_MMA_MAXL;
+#ifndef SCARF_ZROW_MMA_MINL
+#define SCARF_ZROW_MMA_MINL 0
+#endif
+template <int L, int NS> constexpr bool kZrowMma = NS % 4 == 0 && L >= SCARF_ZROW_MMA_MINL && L <= kZrowMmaMaxL;
+
 struct ZPipe {
     unsigned char* buf;     // kStages slots of kSlotBytes: records | X slice | Y slice | Z slice (first half of the axis)
     uint64_t* full;
@@ -77,6 +87,248 @@ struct ZPipe {
 __device__ __forceinline__ double2 cmul(const double2 a, const double2 b)
 {
     return make_double2(fma(a.x, b.x, -(a.y * b.y)), fma(a.x, b.y, a.y * b.x));
+}
+
+// ---- L = 1 on the FP64 tensor cores -------------------------------------------------------------------------------------------
+// For L = 1 both polynomials are warp-uniform (E = H_0, O' = H_1), so the accumulate over the records k of a stage is a real matrix
+// product over (k, term):  S'[p][(s, re|im)] += [c | s z][p][k] . [H_0 | i H_1][k][(s, re|im)],  D' += [s | c z] . [i H_0 | H_1]
+// (p = the warp's 32 mirror pairs, 2 NS columns).  mma.sync.m8n8k4.f64: a k-tile = two records x two terms, four M tiles of eight
+// pairs, NS / 4 N tiles of four states; lane (g, t) = (lane / 4, lane % 4) holds A[g][t], B[t][g], C[g][2t, 2t + 1] = (re, im) of
+// pair 8 mt + g and state 4 nt + t.  Per record 8 FMAs per pair and state as with DFMAs, but the H of a k-tile is read once per
+// warp (NS / 4 loads of 16 distinct complex numbers) instead of broadcast to every lane for every state: the DFMA loop of this class
+// is bound by the shared-memory pipe (two wavefronts per broadcast LDS.128, 52 per record and warp against 96 DFMAs), this one is not.
+__device__ __forceinline__ void dmma884(double (&d)[2], double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ double flip_sign(double x, int mask) { return __hiloint2double(__double2hiint(x) ^ mask, __double2loint(x)); }
+constexpr int kFragStride(int NS) { return 2 * NS + 2; }   // doubles per pair row of the layout exchange (conflict-free 16-byte accesses)
+
+// per-lane sums (re[h][s], im[h][s]) of pair `lane` <-> C fragments, through the warp's private area (one half h at a time)
+template <int NS>
+__device__ __forceinline__ void zrow_to_frag(double* W, int lane, const double (&re)[kNQ][NS], const double (&im)[kNQ][NS],
+                                             double (&C)[2][4][NS / 4][2])
+{
+    constexpr int ST = kFragStride(NS);
+    static_assert(32 * ST * 8 <= h_warp_bytes(NS), "layout exchange larger than the warp's private area");
+    const int g = lane >> 2, t = lane & 3;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        __syncwarp();
+#pragma unroll
+        for (int s = 0; s < NS; ++s) *reinterpret_cast<double2*>(W + lane * ST + 2 * s) = make_double2(re[h][s], im[h][s]);
+        __syncwarp();
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NS / 4; ++nt) {
+                const double2 v = *reinterpret_cast<const double2*>(W + (8 * mt + g) * ST + 2 * (4 * nt + t));
+                C[h][mt][nt][0] = v.x;
+                C[h][mt][nt][1] = v.y;
+            }
+    }
+    __syncwarp();
+}
+template <int NS>
+__device__ __forceinline__ void zrow_from_frag(double* W, int lane, const double (&C)[2][4][NS / 4][2], double (&re)[kNQ][NS],
+                                               double (&im)[kNQ][NS])
+{
+    constexpr int ST = kFragStride(NS);
+    const int g = lane >> 2, t = lane & 3;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        __syncwarp();
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NS / 4; ++nt)
+                *reinterpret_cast<double2*>(W + (8 * mt + g) * ST + 2 * (4 * nt + t)) = make_double2(C[h][mt][nt][0], C[h][mt][nt][1]);
+        __syncwarp();
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            const double2 v = *reinterpret_cast<const double2*>(W + lane * ST + 2 * s);
+            re[h][s] = v.x;
+            im[h][s] = v.y;
+        }
+    }
+    __syncwarp();
+}
+
+// What a lane holds of the A and B fragments does not change along a segment: row rho = 4 j + t of the j-th k-tile of a period
+// is term v = rho % (L + 1) (the power of z, the index of H) of record rho / (L + 1) of the period's records.
+//   v even:  S' column c z^v with row H_v,    D' column s z^v with row i H_v
+//   v odd:   S' column s z^v with row i H_v,  D' column c z^v with row H_v          (i H = (-H_i, H_r))
+template <int L>
+struct ZMmaLane {
+    static constexpr int NV = L + 1;
+    static constexpr int P = NV == 3 ? 3 : 1;             // k-tiles per period (4 P rows = R records of NV rows)
+    static constexpr int R = 4 * P / NV;
+    static_assert(4 * P == R * NV, "a period holds whole records");
+    int zoff[P];        // doubles from (c, s)[first record of the period][pair 8 mt + g] to this lane's S' factor (the D' factor: ^ 1)
+    int odd[P];         // v & 1
+    int hoff[P];        // doubles from H[first record][state 4 nt][0] to this lane's H_v of state 4 nt + g / 2
+    int drec[P];        // record of the period
+    int o1[P];          // component of H_v the S' row holds (the D' row: the other)
+    int neg1[P], neg2[P];   // sign-bit masks of the S' / D' row
+    double sc[P][4];    // z^v of pair 8 mt + g
+};
+template <int L, int NS>
+__device__ __forceinline__ void zrow_mma_lane(double z, int lane, ZMmaLane<L>& m)
+{
+    constexpr int NV = L + 1;
+    const int g = lane >> 2, t = lane & 3, comp = g & 1;
+    double zq[4];
+#pragma unroll
+    for (int mt = 0; mt < 4; ++mt) zq[mt] = __shfl_sync(0xffffffffu, z, 8 * mt + g);
+#pragma unroll
+    for (int j = 0; j < ZMmaLane<L>::P; ++j) {
+        const int rho = 4 * j + t, v = rho % NV, dr = rho / NV, ty = v & 1;
+        m.drec[j] = dr;
+        m.odd[j] = ty;
+        m.zoff[j] = dr * kZrowBZ * 2 + g * 2 + ty;
+        m.hoff[j] = ((dr * NS + (g >> 1)) * NV + v) * 2;
+        m.o1[j] = ty ? 1 - comp : comp;
+        m.neg1[j] = (ty == 1 && comp == 0) ? (int)0x80000000 : 0;
+        m.neg2[j] = (ty == 0 && comp == 0) ? (int)0x80000000 : 0;
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt) {
+            double p = 1.0;
+#pragma unroll
+            for (int e = 1; e <= L; ++e)
+                if (e <= v) p *= zq[mt];
+            m.sc[j][mt] = p;
+        }
+    }
+}
+
+// the records of one stage: Hd = the pre-pass' H[record][state][v] (complex) as doubles, Zd = the stage's Z slice (c, s)[record][pair]
+// as doubles
+template <int L, int NS>
+__device__ __forceinline__ void zrow_mma(const double* __restrict__ Hd, const double* __restrict__ Zd, int cnt, const ZMmaLane<L>& m,
+                                         double (&C)[2][4][NS / 4][2])
+{
+    constexpr int NT = NS / 4, NV = L + 1, P = ZMmaLane<L>::P, R = ZMmaLane<L>::R;
+#pragma unroll(P == 1 ? 2 : 1)
+    for (int k0 = 0; k0 < cnt; k0 += R) {
+        const double* zb = Zd + k0 * kZrowBZ * 2;
+        const double* hb = Hd + k0 * NS * NV * 2;
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+            const bool valid = k0 + m.drec[j] < cnt;      // a short last period: the rows of the missing records are zero
+            double a1[4], a2[4], b1[NT], b2[NT];
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt) {
+                const double* zp = zb + m.zoff[j] + 16 * mt;
+                const double u = valid ? zp[0] : 0.0, v = valid ? zp[1 - 2 * m.odd[j]] : 0.0;
+                a1[mt] = u * m.sc[j][mt];                   // c z^v | s z^v
+                a2[mt] = v * m.sc[j][mt];                   // s z^v | c z^v
+            }
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+                const double* hp = hb + m.hoff[j] + 4 * nt * NV * 2;
+                b1[nt] = flip_sign(valid ? hp[m.o1[j]] : 0.0, m.neg1[j]);
+                b2[nt] = flip_sign(valid ? hp[1 - m.o1[j]] : 0.0, m.neg2[j]);
+            }
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                    dmma884(C[0][mt][nt], a1[mt], b1[nt]);
+                    dmma884(C[1][mt][nt], a2[mt], b2[nt]);
+                }
+        }
+    }
+}
+
+// ---- L = 0: S' += c (X Y D_s), D' += s (i X Y D_s).  A k-tile = four records, one row each; the B rows are formed in the loop
+// from the records themselves (no pre-pass): lane (g, t) holds component g & 1 of X Y D of record k0 + t and state 4 nt + g / 2.
+template <int NS>
+__device__ __forceinline__ void zrow_mma0(const unsigned char* __restrict__ sp, const double2* __restrict__ Xs, const double2* __restrict__ Ys,
+                                          const double* __restrict__ Zd, int cnt, int lane, double (&C)[2][4][NS / 4][2])
+{
+    constexpr int NT = NS / 4, REC = rec_doubles(0, NS) * 8;
+    const int g = lane >> 2, t = lane & 3, comp = g & 1;
+#pragma unroll 2
+    for (int k0 = 0; k0 < cnt; k0 += 4) {
+        const bool valid = k0 + t < cnt;                    // a short last k-tile: the rows of the missing records are zero
+        const int r = valid ? k0 + t : k0;
+        const double2 xy = cmul(Xs[r * kZrowBX], Ys[r * kZrowBY]);
+        const double p = valid ? (comp ? xy.y : xy.x) : 0.0;     // S' row:  X Y D       = (a D, b D)
+        const double q = valid ? (comp ? xy.x : -xy.y) : 0.0;    // D' row:  i X Y D     = (-b D, a D)
+        const double* D = reinterpret_cast<const double*>(sp + r * REC) + 4 + (g >> 1);
+        double a1[4], a2[4], b1[NT], b2[NT];
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt) {
+            const double2 zc = *reinterpret_cast<const double2*>(Zd + (r * kZrowBZ + 8 * mt + g) * 2);
+            a1[mt] = valid ? zc.x : 0.0;
+            a2[mt] = valid ? zc.y : 0.0;
+        }
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            const double d = D[4 * nt];
+            b1[nt] = p * d;
+            b2[nt] = q * d;
+        }
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+                dmma884(C[0][mt][nt], a1[mt], b1[nt]);
+                dmma884(C[1][mt][nt], a2[mt], b2[nt]);
+            }
+    }
+}
+
+// ---- L = 1 without a pre-pass: H_0 = X Y (D_0 + i (q_x D_x + q_y D_y)), H_1 = X Y (i D_z) formed in the loop.  A k-tile = two
+// records x (H_0, H_1); lane (g, t): record k0 + t / 2, v = t & 1, state 4 nt + g / 2, component g & 1.  With X Y = a + i b and
+// H = X Y (Ge + i Go): the row holding H is p Ge + q Go, the row holding i H is q Ge - p Go, (p, q) = (a, -b) for the real and
+// (b, a) for the imaginary component.  zq[mt] = z of pair 8 mt + g.
+template <int NS>
+__device__ __forceinline__ void zrow_mma1(const unsigned char* __restrict__ sp, const double2* __restrict__ Xs, const double2* __restrict__ Ys,
+                                          const double* __restrict__ Zd, int cnt, double qx, double qy, const double (&zq)[4], int lane,
+                                          double (&C)[2][4][NS / 4][2])
+{
+    constexpr int NT = NS / 4, REC = rec_doubles(1, NS) * 8, NH = nherm(1);
+    const int g = lane >> 2, t = lane & 3, comp = g & 1, ty = t & 1, dr = t >> 1;
+    // Ge = w0 D[0], Go = w1 D[o1] + w2 D[o2]
+    const double w0 = ty ? 0.0 : 1.0, w1 = ty ? 1.0 : qx, w2 = ty ? 0.0 : qy;
+    const int o1 = ty ? 3 : 1, o2 = ty ? 3 : 2;
+    double sc[4];
+#pragma unroll
+    for (int mt = 0; mt < 4; ++mt) sc[mt] = ty ? zq[mt] : 1.0;
+#pragma unroll 2
+    for (int k0 = 0; k0 < cnt; k0 += 2) {
+        const bool valid = k0 + dr < cnt;                   // an odd stage: the rows of the missing record are zero
+        const int r = valid ? k0 + dr : k0;
+        const double2 xy = cmul(Xs[r * kZrowBX], Ys[r * kZrowBY]);
+        const double p = valid ? (comp ? xy.y : xy.x) : 0.0, q = valid ? (comp ? xy.x : -xy.y) : 0.0;
+        // v even: S' row = H, D' row = i H;  v odd: S' row = i H, D' row = H
+        const double P1 = ty ? q : p, Q1 = ty ? -p : q, P2 = ty ? p : q, Q2 = ty ? q : -p;
+        const double* D = reinterpret_cast<const double*>(sp + r * REC) + 4 + (g >> 1) * NH;
+        double a1[4], a2[4], b1[NT], b2[NT];
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt) {
+            const double* zp = Zd + (r * kZrowBZ + 8 * mt + g) * 2;
+            const double u = valid ? zp[ty] : 0.0, v = valid ? zp[1 - ty] : 0.0;
+            a1[mt] = u * sc[mt];                            // c | s z
+            a2[mt] = v * sc[mt];                            // s | c z
+        }
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            const double* Ds = D + 4 * nt * NH;
+            const double ge = w0 * Ds[0];
+            const double go = fma(w2, Ds[o2], w1 * Ds[o1]);
+            b1[nt] = fma(P1, ge, Q1 * go);
+            b2[nt] = fma(P2, ge, Q2 * go);
+        }
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+                dmma884(C[0][mt][nt], a1[mt], b1[nt]);
+                dmma884(C[1][mt][nt], a2[mt], b2[nt]);
+            }
+    }
 }
 
 // ---- pre-pass: H[record][state][v] = X Y (Ge_v + i Go_v) of one stage for this warp's row --------------------------------------
@@ -192,6 +444,19 @@ __device__ __forceinline__ void run_class_zrow(ZPipe& pp, const GridArgs& a, con
     __syncthreads();                                     // all threads have left the previous segment's stages
     if (producer)
         for (int j = 0; j < min(kStages, n_st); ++j) issue(j);
+    // L = 1 on the tensor cores: the sums live in C fragments for the length of the segment
+    constexpr bool MMA = kZrowMma<L, NS>;
+    double Cf[2][4][MMA ? NS / 4 : 1][2];
+    ZMmaLane<(MMA && L >= 2) ? L : 1> ml;
+    double zq[4];
+    if constexpr (MMA) {
+        if constexpr (L >= 2) zrow_mma_lane<L, NS>(z, lane, ml);
+        if constexpr (L == 1) {
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt) zq[mt] = __shfl_sync(0xffffffffu, z, 8 * mt + (lane >> 2));
+        }
+        zrow_to_frag<NS>(Ww, lane, re, im, Cf);
+    }
     for (int j = 0; j < n_st; ++j) {
         const uint32_t g = pp.it + (uint32_t)j;
         const int slot = (int)(g % kStages);
@@ -203,7 +468,17 @@ __device__ __forceinline__ void run_class_zrow(ZPipe& pp, const GridArgs& a, con
         const double2* Zs = reinterpret_cast<const double2*>(sp + kStageBytes + kMaxRec * (kXB + kYB)) + lane;
         double2* XYw = reinterpret_cast<double2*>(Ww);
         double2* Hw = XYw + kMaxRec;
-        if constexpr (L >= 1 && L <= 3) {
+        if constexpr (MMA && L == 0) {
+            zrow_mma0<NS>(sp, Xs, Ys, reinterpret_cast<const double*>(sp + kStageBytes + kMaxRec * (kXB + kYB)), cnt, lane, Cf);
+        } else if constexpr (MMA && L == 1) {
+            zrow_mma1<NS>(sp, Xs, Ys, reinterpret_cast<const double*>(sp + kStageBytes + kMaxRec * (kXB + kYB)), cnt, qv[0][0], qv[0][1], zq,
+                          lane, Cf);
+        } else if constexpr (MMA) {
+            zrow_prepass<L, NS>(sp, cnt, Xs, Ys, xym, Hw, lane);
+            __syncwarp();
+            zrow_mma<L, NS>(reinterpret_cast<const double*>(Hw), reinterpret_cast<const double*>(sp + kStageBytes + kMaxRec * (kXB + kYB)),
+                            cnt, ml, Cf);
+        } else if constexpr (L >= 1 && L <= 3) {
             zrow_prepass<L, NS>(sp, cnt, Xs, Ys, xym, Hw, lane);
             __syncwarp();
             // {c, s, c z, s z} of record k; software-pipelined by groups of U records
@@ -302,6 +577,7 @@ __device__ __forceinline__ void run_class_zrow(ZPipe& pp, const GridArgs& a, con
         if (producer && j + kStages < n_st) issue(j + kStages);
     }
     pp.it += (uint32_t)n_st;
+    if constexpr (MMA) zrow_from_frag<NS>(Ww, lane, Cf, re, im);
 }
 
 template <int NS>

@@ -77,6 +77,7 @@ struct scarf_ctx {
     double last_ctr = 40.0;
     int grid_symmetry = 1;    // 1: use f(-q) = conj f(q) on inversion-symmetric product grids; 0: never
     int host_tile_group = 0;  // tiles per dispatch group when the kernel writes a pinned host `out` (0: automatic)
+    int grid_tile_group = -1; // tiles per dispatch group of the product-grid kernels with a device `out` (-1: automatic, 0: none)
     int host_zero_copy = 1;   // 1: a pinned host `out` of the product-grid calls is written by the kernel itself (no device->host copies)
     int grid_variant = -1;    // product-grid kernel: 0 box kernel (ff_grid.cu), 1 row kernel (ff_row.cu), -1 by the grid's shape
     const double* last_grid_w = nullptr;   // work model of the last product-grid call (kWGrid or kWRow)
@@ -350,6 +351,9 @@ int scarf_set_option(scarf_ctx* ctx, const char* key, double value)
     } else if (k == "grid_symmetry") {
         if (value != 0.0 && value != 1.0) return fail(ctx, SCARF_EINVAL, "set_option: grid_symmetry must be 0 or 1");
         ctx->grid_symmetry = (int)value;
+    } else if (k == "grid_tile_group") {
+        if (value < -1 || value > 1e6) return fail(ctx, SCARF_EINVAL, "set_option: grid_tile_group outside -1..1e6");
+        ctx->grid_tile_group = (int)value;
     } else if (k == "host_tile_group") {
         if (value < 0 || value > 1e6) return fail(ctx, SCARF_EINVAL, "set_option: host_tile_group outside 0..1e6");
         ctx->host_tile_group = (int)value;
@@ -994,6 +998,8 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
                     if (ctx->n_chunks_opt <= 0) a.v.n_chunks = (int)std::max<long long>(1, std::min<long long>(a.v.n_chunks, (8 * slots + tiles_s - 1) / tiles_s));
                     a.v.tile_group = a.v.n_chunks > 1 ? (int)std::max<long long>(1, 3 * slots / 7) : 0;
                     if (a.v.tile_group > 0 && ctx->host_tile_group > 0) a.v.tile_group = ctx->host_tile_group;
+                } else {
+                    a.v.tile_group = a.v.n_chunks > 1 && ctx->grid_tile_group > 0 ? ctx->grid_tile_group : 0;
                 }
                 if (int rc = prepare_tickets(ctx, tiles_s, a.v.n_chunks, st, &a.v.tickets)) return n_slabs > 1 ? drain(rc) : rc;
                 CU(launch_plan_chunks(t.desc, a.v.n_chunks, t.ns_real, ctr_g, st, /*model=*/zrow ? 4 : (row ? 2 : 1)), "form_factors_grid: chunk planning kernel");
