@@ -17,6 +17,9 @@
 // A warp owns one (ix, iy) row and 32 mirror pairs (lane l: iz = 32 zb + l and nz - 1 - iz); a CTA = 4 consecutive iy.  The Z table
 // covers the first half of the axis only (32 complex numbers per record and pair box).  Everything else — the TMA stage ring,
 // stream chunks with ordered fix-up tickets, the conjugate store for the inversion mirror, the q-adaptive prefix — as in ff_row.cu.
+//
+// For state tiles of 4, 8 or 12 states the accumulates of classes 1 and 2 are issued as FP64 tensor-core matrix products over the
+// records of a stage (mma.sync.m8n8k4.f64; "classes L = 0..3 on the FP64 tensor cores" below).
 #include "ff_common.cuh"
 
 namespace scarf {
@@ -68,15 +71,11 @@ __host__ __device__ constexpr int h_warp_bytes(int NS)
 }
 template <int NS> constexpr int smem_bytes() { return kStages * kSlotBytes + kWarps * h_warp_bytes(NS) + 64; }
 
-// classes L = 1..kZrowMmaMaxL through mma.sync (zrow_mma) for state tiles that fill whole N tiles; the DFMA loops otherwise
-#ifndef SCARF_ZROW_MMA_MAXL
-#define SCARF_ZROW_MMA_MAXL 2
-#endif
-constexpr int kZrowMmaMaxL = SCARF_ZROW_MMA_MAXL;
-#ifndef SCARF_ZROW_MMA_MINL
-#define SCARF_ZROW_MMA_MINL 0
-#endif
-template <int L, int NS> constexpr bool kZrowMma = NS % 4 == 0 && L >= SCARF_ZROW_MMA_MINL && L <= kZrowMmaMaxL;
+// classes kZrowMmaMinL..kZrowMmaMaxL through mma.sync (zrow_mma) for state tiles that fill whole N tiles; the DFMA loops otherwise.
+// Measured on config 3 (kernel, ms): no class 5.43; L = 1: 5.10; L = 1..2: 5.00; L = 1..3: 5.00; L = 0..2: 5.07 (B rows of class 0 formed
+// in the loop) / 5.25 (from a pre-pass); see DESIGN.md section 8.
+constexpr int kZrowMmaMinL = 1, kZrowMmaMaxL = 2;
+template <int L, int NS> constexpr bool kZrowMma = NS % 4 == 0 && L >= kZrowMmaMinL && L <= kZrowMmaMaxL;
 
 struct ZPipe {
     unsigned char* buf;     // kStages slots of kSlotBytes: records | X slice | Y slice | Z slice (first half of the axis)
@@ -89,14 +88,18 @@ __device__ __forceinline__ double2 cmul(const double2 a, const double2 b)
     return make_double2(fma(a.x, b.x, -(a.y * b.y)), fma(a.x, b.y, a.y * b.x));
 }
 
-// ---- L = 1 on the FP64 tensor cores -------------------------------------------------------------------------------------------
-// For L = 1 both polynomials are warp-uniform (E = H_0, O' = H_1), so the accumulate over the records k of a stage is a real matrix
-// product over (k, term):  S'[p][(s, re|im)] += [c | s z][p][k] . [H_0 | i H_1][k][(s, re|im)],  D' += [s | c z] . [i H_0 | H_1]
-// (p = the warp's 32 mirror pairs, 2 NS columns).  mma.sync.m8n8k4.f64: a k-tile = two records x two terms, four M tiles of eight
-// pairs, NS / 4 N tiles of four states; lane (g, t) = (lane / 4, lane % 4) holds A[g][t], B[t][g], C[g][2t, 2t + 1] = (re, im) of
-// pair 8 mt + g and state 4 nt + t.  Per record 8 FMAs per pair and state as with DFMAs, but the H of a k-tile is read once per
-// warp (NS / 4 loads of 16 distinct complex numbers) instead of broadcast to every lane for every state: the DFMA loop of this class
-// is bound by the shared-memory pipe (two wavefronts per broadcast LDS.128, 52 per record and warp against 96 DFMAs), this one is not.
+// ---- classes L = 0..3 on the FP64 tensor cores ---------------------------------------------------------------------------------
+// The polynomials E = sum_{v even} H_v z^v and z O' = sum_{v odd} H_v z^v have warp-uniform coefficients H_v (pre-pass), so the
+// accumulate over the records k of a stage is a real matrix product over (k, v):
+//   S'[p][(s, re|im)] += A_S[p][(k, v)] B_S[(k, v)][(s, re|im)],   A_S = c z^v (v even) | s z^v (v odd),   B_S = H_v | i H_v
+//   D'[p][(s, re|im)] += A_D[p][(k, v)] B_D[(k, v)][(s, re|im)],   A_D = s z^v (v even) | c z^v (v odd),   B_D = i H_v | H_v
+// (p = the warp's 32 mirror pairs).  mma.sync.m8n8k4.f64: four M tiles of eight pairs, N tiles of four states; lane (g, t) =
+// (lane / 4, lane % 4) holds A[g][t], B[t][g], C[g][2t, 2t + 1] = (re, im) of pair 8 mt + g and state 4 nt + t.  L + 1 rows per
+// record and product: 4 / 8 / 12 / 16 FMAs per mirror pair and state for L = 0..3 (the DFMA loops: 4 / 8 / 10 / 12), but the H of a
+// k-tile is read once per warp instead of broadcast to every lane for every state (the DFMA loops of L >= 1 are bound by the
+// shared-memory pipe: two wavefronts per broadcast LDS.128, 52 / 76 / 100 per record and warp against 96 / 120 / 144 DFMAs).
+// DMMA is counted on the tensor pipe and DFMA on the FP64 pipe, but the two share the FP64 units (64 FMA/clk/SM together): splitting
+// the states of a record between a DMMA and a DFMA part in one loop body was slower than either.
 __device__ __forceinline__ void dmma884(double (&d)[2], double a, double b)
 {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
@@ -240,97 +243,6 @@ __device__ __forceinline__ void zrow_mma(const double* __restrict__ Hd, const do
     }
 }
 
-// ---- L = 0: S' += c (X Y D_s), D' += s (i X Y D_s).  A k-tile = four records, one row each; the B rows are formed in the loop
-// from the records themselves (no pre-pass): lane (g, t) holds component g & 1 of X Y D of record k0 + t and state 4 nt + g / 2.
-template <int NS>
-__device__ __forceinline__ void zrow_mma0(const unsigned char* __restrict__ sp, const double2* __restrict__ Xs, const double2* __restrict__ Ys,
-                                          const double* __restrict__ Zd, int cnt, int lane, double (&C)[2][4][NS / 4][2])
-{
-    constexpr int NT = NS / 4, REC = rec_doubles(0, NS) * 8;
-    const int g = lane >> 2, t = lane & 3, comp = g & 1;
-#pragma unroll 2
-    for (int k0 = 0; k0 < cnt; k0 += 4) {
-        const bool valid = k0 + t < cnt;                    // a short last k-tile: the rows of the missing records are zero
-        const int r = valid ? k0 + t : k0;
-        const double2 xy = cmul(Xs[r * kZrowBX], Ys[r * kZrowBY]);
-        const double p = valid ? (comp ? xy.y : xy.x) : 0.0;     // S' row:  X Y D       = (a D, b D)
-        const double q = valid ? (comp ? xy.x : -xy.y) : 0.0;    // D' row:  i X Y D     = (-b D, a D)
-        const double* D = reinterpret_cast<const double*>(sp + r * REC) + 4 + (g >> 1);
-        double a1[4], a2[4], b1[NT], b2[NT];
-#pragma unroll
-        for (int mt = 0; mt < 4; ++mt) {
-            const double2 zc = *reinterpret_cast<const double2*>(Zd + (r * kZrowBZ + 8 * mt + g) * 2);
-            a1[mt] = valid ? zc.x : 0.0;
-            a2[mt] = valid ? zc.y : 0.0;
-        }
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-            const double d = D[4 * nt];
-            b1[nt] = p * d;
-            b2[nt] = q * d;
-        }
-#pragma unroll
-        for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt) {
-                dmma884(C[0][mt][nt], a1[mt], b1[nt]);
-                dmma884(C[1][mt][nt], a2[mt], b2[nt]);
-            }
-    }
-}
-
-// ---- L = 1 without a pre-pass: H_0 = X Y (D_0 + i (q_x D_x + q_y D_y)), H_1 = X Y (i D_z) formed in the loop.  A k-tile = two
-// records x (H_0, H_1); lane (g, t): record k0 + t / 2, v = t & 1, state 4 nt + g / 2, component g & 1.  With X Y = a + i b and
-// H = X Y (Ge + i Go): the row holding H is p Ge + q Go, the row holding i H is q Ge - p Go, (p, q) = (a, -b) for the real and
-// (b, a) for the imaginary component.  zq[mt] = z of pair 8 mt + g.
-template <int NS>
-__device__ __forceinline__ void zrow_mma1(const unsigned char* __restrict__ sp, const double2* __restrict__ Xs, const double2* __restrict__ Ys,
-                                          const double* __restrict__ Zd, int cnt, double qx, double qy, const double (&zq)[4], int lane,
-                                          double (&C)[2][4][NS / 4][2])
-{
-    constexpr int NT = NS / 4, REC = rec_doubles(1, NS) * 8, NH = nherm(1);
-    const int g = lane >> 2, t = lane & 3, comp = g & 1, ty = t & 1, dr = t >> 1;
-    // Ge = w0 D[0], Go = w1 D[o1] + w2 D[o2]
-    const double w0 = ty ? 0.0 : 1.0, w1 = ty ? 1.0 : qx, w2 = ty ? 0.0 : qy;
-    const int o1 = ty ? 3 : 1, o2 = ty ? 3 : 2;
-    double sc[4];
-#pragma unroll
-    for (int mt = 0; mt < 4; ++mt) sc[mt] = ty ? zq[mt] : 1.0;
-#pragma unroll 2
-    for (int k0 = 0; k0 < cnt; k0 += 2) {
-        const bool valid = k0 + dr < cnt;                   // an odd stage: the rows of the missing record are zero
-        const int r = valid ? k0 + dr : k0;
-        const double2 xy = cmul(Xs[r * kZrowBX], Ys[r * kZrowBY]);
-        const double p = valid ? (comp ? xy.y : xy.x) : 0.0, q = valid ? (comp ? xy.x : -xy.y) : 0.0;
-        // v even: S' row = H, D' row = i H;  v odd: S' row = i H, D' row = H
-        const double P1 = ty ? q : p, Q1 = ty ? -p : q, P2 = ty ? p : q, Q2 = ty ? q : -p;
-        const double* D = reinterpret_cast<const double*>(sp + r * REC) + 4 + (g >> 1) * NH;
-        double a1[4], a2[4], b1[NT], b2[NT];
-#pragma unroll
-        for (int mt = 0; mt < 4; ++mt) {
-            const double* zp = Zd + (r * kZrowBZ + 8 * mt + g) * 2;
-            const double u = valid ? zp[ty] : 0.0, v = valid ? zp[1 - ty] : 0.0;
-            a1[mt] = u * sc[mt];                            // c | s z
-            a2[mt] = v * sc[mt];                            // s | c z
-        }
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-            const double* Ds = D + 4 * nt * NH;
-            const double ge = w0 * Ds[0];
-            const double go = fma(w2, Ds[o2], w1 * Ds[o1]);
-            b1[nt] = fma(P1, ge, Q1 * go);
-            b2[nt] = fma(P2, ge, Q2 * go);
-        }
-#pragma unroll
-        for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt) {
-                dmma884(C[0][mt][nt], a1[mt], b1[nt]);
-                dmma884(C[1][mt][nt], a2[mt], b2[nt]);
-            }
-    }
-}
-
 // ---- pre-pass: H[record][state][v] = X Y (Ge_v + i Go_v) of one stage for this warp's row --------------------------------------
 // xym[yz_index(t, u)] = q_x^t q_y^u (1 <= t + u <= L).  One (record, state) pair per lane and trip.
 template <int L, int NS>
@@ -447,14 +359,9 @@ __device__ __forceinline__ void run_class_zrow(ZPipe& pp, const GridArgs& a, con
     // L = 1 on the tensor cores: the sums live in C fragments for the length of the segment
     constexpr bool MMA = kZrowMma<L, NS>;
     double Cf[2][4][MMA ? NS / 4 : 1][2];
-    ZMmaLane<(MMA && L >= 2) ? L : 1> ml;
-    double zq[4];
+    ZMmaLane<MMA ? L : 1> ml;
     if constexpr (MMA) {
-        if constexpr (L >= 2) zrow_mma_lane<L, NS>(z, lane, ml);
-        if constexpr (L == 1) {
-#pragma unroll
-            for (int mt = 0; mt < 4; ++mt) zq[mt] = __shfl_sync(0xffffffffu, z, 8 * mt + (lane >> 2));
-        }
+        zrow_mma_lane<L, NS>(z, lane, ml);
         zrow_to_frag<NS>(Ww, lane, re, im, Cf);
     }
     for (int j = 0; j < n_st; ++j) {
@@ -468,12 +375,7 @@ __device__ __forceinline__ void run_class_zrow(ZPipe& pp, const GridArgs& a, con
         const double2* Zs = reinterpret_cast<const double2*>(sp + kStageBytes + kMaxRec * (kXB + kYB)) + lane;
         double2* XYw = reinterpret_cast<double2*>(Ww);
         double2* Hw = XYw + kMaxRec;
-        if constexpr (MMA && L == 0) {
-            zrow_mma0<NS>(sp, Xs, Ys, reinterpret_cast<const double*>(sp + kStageBytes + kMaxRec * (kXB + kYB)), cnt, lane, Cf);
-        } else if constexpr (MMA && L == 1) {
-            zrow_mma1<NS>(sp, Xs, Ys, reinterpret_cast<const double*>(sp + kStageBytes + kMaxRec * (kXB + kYB)), cnt, qv[0][0], qv[0][1], zq,
-                          lane, Cf);
-        } else if constexpr (MMA) {
+        if constexpr (MMA) {
             zrow_prepass<L, NS>(sp, cnt, Xs, Ys, xym, Hw, lane);
             __syncwarp();
             zrow_mma<L, NS>(reinterpret_cast<const double*>(Hw), reinterpret_cast<const double*>(sp + kStageBytes + kMaxRec * (kXB + kYB)),
