@@ -151,7 +151,7 @@ int scarf_set_stream(scarf_ctx* ctx, void* cuda_stream);
  *                         row kernel (needs a z axis with qz[i] == -qz[nz-1-i] bit for bit, else the choice is automatic: a lane
  *                         owns the points +z and -z of its row and accumulates their half sum and half difference, whose
  *                         polynomials in z^2 are shared by the pair), -1 = the mirror-pair kernel when the z axis allows it and
- *                         its 4 (y) x 32 (pairs) boxes are at least 80 % full, else the row kernel when its 4 x 64 boxes are,
+ *                         its 4 (y) x 32 (pairs) boxes are at least 75 % full, else the row kernel when its 4 x 64 boxes are at least 80 % full,
  *                         else the box kernel.  Same results to round-off.
  *           "fft_density_variant": default 1 = FP64 tensor-core (DMMA) density kernel of scarf_fft_form_factors with the
  *                         orbital values evaluated per point tile in shared memory (falls back to 2 when the tile of a

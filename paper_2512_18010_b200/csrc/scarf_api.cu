@@ -912,7 +912,9 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
         for (int i = 0; i < nz && z_antisym; ++i) z_antisym = hax[2][(size_t)i] == -hax[2][(size_t)(nz - 1 - i)];
         const int nz_half = (nz + 1) / 2;
         const double zrow_fill = ((double)ny * nz_half) / ((double)((ny + kZrowBY - 1) / kZrowBY * kZrowBY) * (double)((nz_half + kZrowBZ - 1) / kZrowBZ * kZrowBZ));
-        const bool zrow = z_antisym && (ctx->grid_variant == 2 || (ctx->grid_variant < 0 && zrow_fill >= 0.8));
+        // Taken from 75 % full boxes on (a 24-pair row is three whole M tiles of its tensor-core classes): measured on config 2's 48-point
+        // rows, job 1.94 ms against 2.17 ms for the box kernel.
+        const bool zrow = z_antisym && (ctx->grid_variant == 2 || (ctx->grid_variant < 0 && zrow_fill >= 0.75));
         const bool row = !zrow && (ctx->grid_variant == 1 || (ctx->grid_variant != 0 && row_fill >= 0.8));
         const int BXs = zrow ? kZrowBX : (row ? kRowBX : kGridBX), BYs = zrow ? kZrowBY : (row ? kRowBY : kGridBY),
                   BZs = zrow ? kZrowBZ : (row ? kRowBZ : kGridBZ);
@@ -987,6 +989,9 @@ int scarf_form_factors_grid(scarf_ctx* ctx, int32_t nx, const double* qx, int32_
                 a.bx0 = b0;
                 a.v.n_tiles = (int)tiles_s;
                 a.v.n_chunks = choose_chunks(ctx, tiles_s, ctr_g, t.ns_real, ctx->n_chunks_opt);
+                // the mirror-pair kernel pays per chunk for its layout exchanges and short last k-tiles: measured flat from 6 to 14 chunks
+                // on configs 3 and 4, 1.90-1.94 ms for 3..12 chunks against 2.05 ms for 25 on config 2
+                if (zrow && ctx->n_chunks_opt <= 0) a.v.n_chunks = std::min(a.v.n_chunks, 12);
                 // Pinned host `out`: the CTAs are dispatched chunk-major inside groups of tiles, group after group, so that finished
                 // tiles leave for the host all along the kernel's run (chunk-major over all tiles would send everything in the last
                 // 1/n_chunks of it).  Measured on config 3 (ms per call, host `out`): groups of 128 tiles (3/7 of the CTA slots) and

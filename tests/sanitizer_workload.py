@@ -53,6 +53,17 @@ def main():
                 total += float(np.abs(sc.form_factors_grid(*ax)).sum())
                 ax[1] = np.linspace(-2, 3, 9)
                 total += float(np.abs(sc.form_factors_grid(*ax)).sum())
+                # the three product-grid kernels by name (box, row, mirror-pair row with its tensor-core classes) on rows long
+                # enough for the row kernels; 13 states = a tile of 12 (mma.sync path) and a tile of 1 (DFMA path)
+                axr = [W.cartesian_axis(3, 3.0), W.cartesian_axis(5, 2.5), W.cartesian_axis(66, 3.5)]
+                for variant in (0, 1, 2):
+                    sc.set_option("grid_variant", variant)
+                    total += float(np.abs(sc.form_factors_grid(*axr)).sum())
+                    assert sc.stats()["last_grid_variant"] == variant
+                sc.set_option("grid_variant", -1)
+                if lmax == 3:                           # the spherical-grid kernel (two radius boxes, inversion-symmetric directions)
+                    ct, _ = np.polynomial.legendre.leggauss(6)
+                    total += float(np.abs(sc.form_factors_sph(np.geomspace(0.1, 3.0, 70), ct, 8).cpu().numpy()).sum())
                 sc.stats()
             sc.set_option("n_chunks", 0); sc.set_option("adaptive_tol", 0.0)
             sc.set_transitions(T)
@@ -74,7 +85,7 @@ def main():
         for shape, l_max in (((2, 3, 10, 18), 6), ((1, 1, 150, 64), 31), ((1, 2, 5, 2048), 3)):
             f = rng.normal(size=shape) + 1j * rng.normal(size=shape)
             ct, wt = np.polynomial.legendre.leggauss(shape[2])
-            for variant in (1, 2, 0):
+            for variant in (1, 0):
                 sc.set_option("angular_variant", variant)
                 R, f2 = sc.angular_moments(torch.as_tensor(f, device="cuda"), ct, wt, shape[3], l_max, n_r=shape[1])
                 total += float(R.abs().sum().item()) + float(f2.sum().item())

@@ -158,13 +158,14 @@ def test_zrow_tensor_core_classes_full_stages(oracle_mod, Scarf, torch_cuda, n_s
 
 def test_zrow_kernel_choice(oracle_mod, Scarf, torch_cuda):
     """grid_variant = 2 on a z axis that is not antisymmetric falls back to the automatic choice; grid_variant = -1 picks the
-    mirror-pair kernel when the z axis allows it and the boxes are full enough; either way the oracle's values."""
+    mirror-pair kernel when the z axis allows it and the boxes are at least 75 % full; either way the oracle's values."""
     w = W.make_workload(1, oracle_mod.overlap)
     rng = np.random.default_rng(17)
     az = antisym_axis(64, rng)
     off = az.copy()
     off[3] = np.nextafter(off[3], 10.0)
-    for axes, variant, expect in (((az[:3], az[:8], az), -1, 2), ((az[:3], az[:8], off), -1, 1), ((az[:3], az[:8], off), 2, 1),
+    az48 = antisym_axis(48, rng)                      # 24 mirror pairs = 75 % of a box: three whole M tiles of the tensor-core classes
+    for axes, variant, expect in (((az[:3], az[:8], az), -1, 2), ((az[:3], az[:8], az48), -1, 2), ((az[:3], az[:8], off), -1, 1), ((az[:3], az[:8], off), 2, 1),
                                   ((az[:3], az[:8], az[16:48]), -1, 0), ((az[:3], az[:5], az), -1, 0), ((az[:3], az[:8], az), 1, 1)):
         f, st = grid_ff(Scarf, torch_cuda, w.basis, w.T, axes, variant)
         assert st["last_grid_variant"] == expect, (variant, expect)
