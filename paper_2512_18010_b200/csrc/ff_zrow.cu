@@ -76,6 +76,8 @@ template <int NS> constexpr int smem_bytes() { return kStages * kSlotBytes + kWa
 // in the loop) / 5.25 (from a pre-pass); see DESIGN.md section 8.
 constexpr int kZrowMmaMinL = 1, kZrowMmaMaxL = 2;
 template <int L, int NS> constexpr bool kZrowMma = NS % 4 == 0 && L >= kZrowMmaMinL && L <= kZrowMmaMaxL;
+// class 0 through mma.sync with its B rows from a per-record table {a, b, -b, a} (zrow_mma0)
+template <int NS> constexpr bool kZrowMma0 = NS % 4 == 0;
 
 struct ZPipe {
     unsigned char* buf;     // kStages slots of kSlotBytes: records | X slice | Y slice | Z slice (first half of the axis)
@@ -243,6 +245,44 @@ __device__ __forceinline__ void zrow_mma(const double* __restrict__ Hd, const do
     }
 }
 
+// ---- class 0 on the tensor cores: S' += c (X Y D_s), D' += s (i X Y D_s).  A k-tile = four records, one row each.  pq[record] =
+// {a, b, -b, a} with X Y = a + i b (written by lane `record` before the loop): the S' row of lane (g, t) is pq[g & 1] D_s, the D' row
+// pq[2 + (g & 1)] D_s, for record k0 + t and state 4 nt + g / 2; the A columns are c and s as they stand in the Z slice.
+template <int NS>
+__device__ __forceinline__ void zrow_mma0(const unsigned char* __restrict__ sp, const double* __restrict__ pq, const double* __restrict__ Zd,
+                                          int cnt, int lane, double (&C)[2][4][NS / 4][2])
+{
+    constexpr int NT = NS / 4, REC = rec_doubles(0, NS) * 8;
+    const int g = lane >> 2, t = lane & 3, comp = g & 1;
+#pragma unroll 2
+    for (int k0 = 0; k0 < cnt; k0 += 4) {
+        const bool valid = k0 + t < cnt;                    // a short last k-tile: the B rows of the missing records are zero
+        const int r = valid ? k0 + t : k0;                  // (their A columns: those of a record that exists, finite)
+        const double p = valid ? pq[r * 4 + comp] : 0.0, q = valid ? pq[r * 4 + 2 + comp] : 0.0;
+        const double* D = reinterpret_cast<const double*>(sp + r * REC) + 4 + (g >> 1);
+        double a1[4], a2[4], b1[NT], b2[NT];
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt) {
+            const double2 zc = *reinterpret_cast<const double2*>(Zd + (r * kZrowBZ + 8 * mt + g) * 2);
+            a1[mt] = zc.x;
+            a2[mt] = zc.y;
+        }
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            const double d = D[4 * nt];
+            b1[nt] = p * d;
+            b2[nt] = q * d;
+        }
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+                dmma884(C[0][mt][nt], a1[mt], b1[nt]);
+                dmma884(C[1][mt][nt], a2[mt], b2[nt]);
+            }
+    }
+}
+
 // ---- pre-pass: H[record][state][v] = X Y (Ge_v + i Go_v) of one stage for this warp's row --------------------------------------
 // xym[yz_index(t, u)] = q_x^t q_y^u (1 <= t + u <= L).  One (record, state) pair per lane and trip.
 template <int L, int NS>
@@ -357,13 +397,11 @@ __device__ __forceinline__ void run_class_zrow(ZPipe& pp, const GridArgs& a, con
     if (producer)
         for (int j = 0; j < min(kStages, n_st); ++j) issue(j);
     // L = 1 on the tensor cores: the sums live in C fragments for the length of the segment
-    constexpr bool MMA = kZrowMma<L, NS>;
-    double Cf[2][4][MMA ? NS / 4 : 1][2];
+    constexpr bool MMA0 = L == 0 && kZrowMma0<NS>, MMA = kZrowMma<L, NS>;
+    double Cf[2][4][(MMA || MMA0) ? NS / 4 : 1][2];
     ZMmaLane<MMA ? L : 1> ml;
-    if constexpr (MMA) {
-        zrow_mma_lane<L, NS>(z, lane, ml);
-        zrow_to_frag<NS>(Ww, lane, re, im, Cf);
-    }
+    if constexpr (MMA) zrow_mma_lane<L, NS>(z, lane, ml);
+    if constexpr (MMA || MMA0) zrow_to_frag<NS>(Ww, lane, re, im, Cf);
     for (int j = 0; j < n_st; ++j) {
         const uint32_t g = pp.it + (uint32_t)j;
         const int slot = (int)(g % kStages);
@@ -375,7 +413,16 @@ __device__ __forceinline__ void run_class_zrow(ZPipe& pp, const GridArgs& a, con
         const double2* Zs = reinterpret_cast<const double2*>(sp + kStageBytes + kMaxRec * (kXB + kYB)) + lane;
         double2* XYw = reinterpret_cast<double2*>(Ww);
         double2* Hw = XYw + kMaxRec;
-        if constexpr (MMA) {
+        if constexpr (MMA0) {
+            double* pq = reinterpret_cast<double*>(Hw);
+            if (lane < cnt) {
+                const double2 xy = cmul(Xs[lane * kZrowBX], Ys[lane * kZrowBY]);
+                *reinterpret_cast<double2*>(pq + lane * 4) = xy;
+                *reinterpret_cast<double2*>(pq + lane * 4 + 2) = make_double2(-xy.y, xy.x);
+            }
+            __syncwarp();
+            zrow_mma0<NS>(sp, pq, reinterpret_cast<const double*>(sp + kStageBytes + kMaxRec * (kXB + kYB)), cnt, lane, Cf);
+        } else if constexpr (MMA) {
             zrow_prepass<L, NS>(sp, cnt, Xs, Ys, xym, Hw, lane);
             __syncwarp();
             zrow_mma<L, NS>(reinterpret_cast<const double*>(Hw), reinterpret_cast<const double*>(sp + kStageBytes + kMaxRec * (kXB + kYB)),
@@ -479,7 +526,7 @@ __device__ __forceinline__ void run_class_zrow(ZPipe& pp, const GridArgs& a, con
         if (producer && j + kStages < n_st) issue(j + kStages);
     }
     pp.it += (uint32_t)n_st;
-    if constexpr (MMA) zrow_from_frag<NS>(Ww, lane, Cf, re, im);
+    if constexpr (MMA || MMA0) zrow_from_frag<NS>(Ww, lane, Cf, re, im);
 }
 
 template <int NS>
