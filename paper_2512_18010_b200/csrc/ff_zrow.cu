@@ -18,7 +18,7 @@
 // covers the first half of the axis only (32 complex numbers per record and pair box).  Everything else — the TMA stage ring,
 // stream chunks with ordered fix-up tickets, the conjugate store for the inversion mirror, the q-adaptive prefix — as in ff_row.cu.
 //
-// For state tiles of 4, 8 or 12 states the accumulates of classes 1 and 2 are issued as FP64 tensor-core matrix products over the
+// For state tiles of 4, 8 or 12 states the accumulates of classes 0, 1 and 2 are issued as FP64 tensor-core matrix products over the
 // records of a stage (mma.sync.m8n8k4.f64; "classes L = 0..3 on the FP64 tensor cores" below).
 #include "ff_common.cuh"
 
@@ -72,8 +72,8 @@ __host__ __device__ constexpr int h_warp_bytes(int NS)
 template <int NS> constexpr int smem_bytes() { return kStages * kSlotBytes + kWarps * h_warp_bytes(NS) + 64; }
 
 // classes kZrowMmaMinL..kZrowMmaMaxL through mma.sync (zrow_mma) for state tiles that fill whole N tiles; the DFMA loops otherwise.
-// Measured on config 3 (kernel, ms): no class 5.43; L = 1: 5.10; L = 1..2: 5.00; L = 1..3: 5.00; L = 0..2: 5.07 (B rows of class 0 formed
-// in the loop) / 5.25 (from a pre-pass); see DESIGN.md section 8.
+// Measured on config 3 (kernel, ms): no class 5.43; L = 1: 5.10; L = 1..2: 5.00; L = 1..3: 5.00; class 0 besides (zrow_mma0): 4.89; see
+// DESIGN.md section 8.
 constexpr int kZrowMmaMinL = 1, kZrowMmaMaxL = 2;
 template <int L, int NS> constexpr bool kZrowMma = NS % 4 == 0 && L >= kZrowMmaMinL && L <= kZrowMmaMaxL;
 // class 0 through mma.sync with its B rows from a per-record table {a, b, -b, a} (zrow_mma0)

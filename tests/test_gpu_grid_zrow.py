@@ -139,8 +139,8 @@ def test_zrow_kernel_chunk_counts_and_pinned_output(oracle_mod, Scarf, torch_cud
 
 @pytest.mark.parametrize("n_states,K", [(4, 1), (8, 3), (12, 1), (12, 5), (24, 2)])
 def test_zrow_tensor_core_classes_full_stages(oracle_mod, Scarf, torch_cuda, n_states, K):
-    """Classes 1 and 2 on the FP64 tensor cores (state tiles of 4, 8, 12 states: whole N tiles of mma.sync.m8n8k4.f64): config 2's
-    basis has thousands of records per class, so the stages are full (24 / 12 records), the last one of a segment is short (the
+    """Classes 0, 1 and 2 on the FP64 tensor cores (state tiles of 4, 8, 12 states: whole N tiles of mma.sync.m8n8k4.f64): config 2's
+    basis has thousands of records per class, so the stages are full (24 / 24 / 12 records), the last one of a segment is short (the
     zero rows of a missing record) and with K > 1 the chunks start and end inside a class.  Against the oracle on every point, and
     against the row kernel (DFMA loops, grid_variant = 1) at 1e-12."""
     w = W.make_workload(2, oracle_mod.overlap)
@@ -149,7 +149,7 @@ def test_zrow_tensor_core_classes_full_stages(oracle_mod, Scarf, torch_cuda, n_s
     axes = [rng.uniform(-6, 6, size=2), rng.uniform(-6, 6, size=5), antisym_axis(66, rng, qmax=7.0)]
     f, st = grid_ff(Scarf, torch_cuda, w.basis, T, axes, 2, n_chunks=K)
     assert st["last_grid_variant"] == 2 and st["last_n_chunks"] == K
-    assert st["pairs_kept_per_class"][1] > 1000 and st["pairs_kept_per_class"][2] > 500
+    assert st["pairs_kept_per_class"][0] > 1000 and st["pairs_kept_per_class"][1] > 1000 and st["pairs_kept_per_class"][2] > 500
     f_row, st_row = grid_ff(Scarf, torch_cuda, w.basis, T, axes, 1, n_chunks=K)
     assert st_row["last_grid_variant"] == 1
     assert_parity(f, f_row, tol=1e-12)
